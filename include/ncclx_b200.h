@@ -1,0 +1,188 @@
+/*
+ * ncclx_b200.h -- C ABI of libncclx_b200.so
+ *
+ * The on-device data path of two NCCLX collectives ("Collective Communication for 100k+
+ * GPUs", arxiv 2510.20171; cited as PAPER.md L<n>), hand-written for NVIDIA B200 (sm_100a),
+ * over R EMULATED ranks whose send and receive buffers all live in one GPU's HBM:
+ *
+ *   1. AllToAllv with device-resident split counts -- the paper's GPU-resident collective
+ *      AllToAllvDynamic (section 6.1): metadata is taken BY REFERENCE
+ *      (L401, L409), actual counts are moved instead of maxcounts padding (L387, L397), the
+ *      receive counts are returned to the user (L419), the call is CUDA-graph capturable.
+ *   2. The sum reduction behind AllReduce / ReduceScatter -- the Reduce / ReduceCopy kernel
+ *      step of the paper's FTAR ring (section 5.3, Fig. 9): fp32
+ *      accumulation in rank order 0..R-1, one rounding.
+ *
+ * Conventions common to every entry point
+ *   - Plain C, no CUDA or torch types.  A stream is passed as `ncclx_stream_t` = the value of
+ *     a `cudaStream_t` (NULL = the legacy default stream).
+ *   - "DEVICE" pointers must be dereferenceable by kernels on the device given to
+ *     ncclx_init; "HOST" pointers by the CPU.  The caller owns every buffer it passes; the
+ *     library owns only its workspace (allocated in ncclx_init, freed in ncclx_finalize).
+ *   - Device entry points (`*_dev`, `*_sum`) only ENQUEUE kernels on `stream`: no host
+ *     synchronisation, no allocation, no host<->device copy.  They may be captured into a
+ *     CUDA graph; a replay re-reads the device-resident metadata.  One workspace exists per
+ *     process: calls must be ordered on ONE stream at a time (or by events).
+ *   - Return value: 0 = NCCLX_OK, otherwise an ncclx_result_t; nothing is enqueued on error.
+ *     No exceptions, no abort, nothing printed.  ncclx_strerror() names a code.
+ *   - There is no CPU fallback: without a CUDA device ncclx_init fails with
+ *     NCCLX_ERR_CUDA and every other call fails with NCCLX_ERR_NOT_INITIALIZED.
+ */
+#ifndef NCCLX_B200_H
+#define NCCLX_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NCCLX_B200_VERSION 100 /* 0.1.0 */
+#define NCCLX_MAX_RANKS 1024   /* hard upper bound on R (ncclx_init max_ranks) */
+
+typedef void* ncclx_stream_t; /* a cudaStream_t */
+
+typedef enum {
+    NCCLX_BF16 = 0, /* bfloat16, 2 bytes  */
+    NCCLX_F32 = 1,  /* IEEE binary32      */
+    NCCLX_F16 = 2,  /* IEEE binary16      */
+    NCCLX_U8 = 3    /* raw bytes: AllToAllv only (reductions return NCCLX_ERR_DTYPE) */
+} ncclx_dtype_t;
+
+typedef enum {
+    NCCLX_OK = 0,
+    NCCLX_ERR_ARG = 1,             /* null pointer, R < 1, bad parameter id/value              */
+    NCCLX_ERR_DTYPE = 2,           /* dtype not supported by this call                         */
+    NCCLX_ERR_NOT_INITIALIZED = 3, /* ncclx_init not called, or R > max_ranks given to it      */
+    NCCLX_ERR_CUDA = 4,            /* a CUDA runtime call failed (see ncclx_last_cuda_error)   */
+    NCCLX_ERR_CAPTURE = 5          /* a host-synchronous call was made while `stream` captures */
+} ncclx_result_t;
+
+/* ---- lifetime ------------------------------------------------------------------------- */
+
+/* Allocates the workspace (offset matrices, segment descriptors, work counters, status word:
+ * about 64 * max_ranks^2 bytes) on `device`, sets kernel attributes and queries the SM count.
+ * Call OUTSIDE stream capture.  Calling it again re-initialises (after an implicit finalize).
+ * 1 <= max_ranks <= NCCLX_MAX_RANKS. */
+int ncclx_init(int max_ranks, int device);
+int ncclx_finalize(void);
+const char* ncclx_strerror(int code);
+/* cudaError_t value of the last failing CUDA call (0 if none), and its string. */
+int ncclx_last_cuda_error(void);
+const char* ncclx_last_cuda_error_string(void);
+int ncclx_version(void);
+
+/* ---- AllToAllv with device-resident counts (section 6.1) ---------------------- *
+ *
+ * For every ordered pair (s, d) of the R emulated ranks, with C = sendcounts_dev:
+ *     recvcounts_dev[d*R + s] = C[s*R + d]                                   (L419, L439)
+ *     soff[s][d] = sum_{d'<d} C[s][d']      roff[d][s] = sum_{s'<s} C[s'][d]
+ *     recv[d][roff[d][s] .. +C[s][d])  =  send[s][soff[s][d] .. +C[s][d])    bytes verbatim
+ * i.e. send[s] is one contiguous buffer split by row s of C (L429), and recv[d] is packed by
+ * source rank ascending with no padding (reading 4).  Bytes of recv[d] outside
+ * the packed range are NOT written.
+ *
+ *   send            DEVICE array of R DEVICE pointers, send[s] (>= 16-byte aligned bases)
+ *   sendcounts_dev  DEVICE int64[R*R], row-major C[s*R+d], in ELEMENTS of dtype.  Read when
+ *                   the kernels EXECUTE, not when this call returns (L401, L409): a kernel or
+ *                   memcpy ordered before the call on `stream` (or before a graph replay) may
+ *                   rewrite it.  A negative entry is treated as 0 and sets bit 0 of the
+ *                   device status word (ncclx_device_status).
+ *   recv            DEVICE array of R DEVICE pointers, recv[d]
+ *   recvcounts_dev  DEVICE int64[R*R], OUT.  Must not overlap sendcounts_dev.
+ *   R               1 <= R <= max_ranks.  R == 1 is a plain copy.
+ *   dtype           any ncclx_dtype_t; only its element size matters (pure data movement).
+ *
+ * Capacity: the caller guarantees send[s] holds sum_d C[s][d] and recv[d] holds
+ * sum_s C[s][d] elements; overflow is undefined (as in NCCL).  send and recv buffers must not
+ * overlap.  Segment addresses may have any element alignment; full speed is only promised
+ * when every segment's source address, destination address and byte length are multiples of
+ * 16 (the cp.async.bulk path); everything else takes the vector path.
+ * The inverse ("combine") is the same call with send := recv, sendcounts := recvcounts.   */
+int ncclx_alltoallv_dev(const void* const* send, const int64_t* sendcounts_dev, void* const* recv,
+                        int64_t* recvcounts_dev, int R, ncclx_dtype_t dtype, ncclx_stream_t stream);
+
+/* Copies the offset matrices of the LAST enqueued ncclx_alltoallv_dev to HOST int64[R*R]
+ * arrays (either may be NULL).  Synchronises `stream`; not capturable (NCCLX_ERR_CAPTURE). */
+int ncclx_alltoallv_last_offsets(int64_t* soff_host, int64_t* roff_host, int R, ncclx_stream_t stream);
+
+/* Reads and clears the device status word into *status_host (bit 0: a negative count was
+ * seen).  Synchronises `stream`; not capturable. */
+int ncclx_device_status(uint32_t* status_host, ncclx_stream_t stream);
+
+/* ---- sum reduction (section 5.3; numeric contract DESIGN.md section 3) -- *
+ *
+ *     acc = (float) x_0[i];  for k = 1..R-1: acc = acc + (float) x_k[i]     (binary32, RNE,
+ *     no FTZ, no reassociation);  out = one round-to-nearest-even conversion of acc to dtype.
+ *     A NaN result is canonical (bf16/f16 0x7FFF, f32 0x7FFFFFFF).
+ *
+ * AllReduce:      recv[r][i] = out[i] for every r, i in [0, count).
+ *   send  DEVICE array of R DEVICE pointers to `count` elements; recv likewise.
+ *   recv[r] == send[r] (in place) is allowed; any other overlap is undefined.
+ * ReduceScatter:  recv[r][j] = out[r*recvcount + j], j in [0, recvcount).
+ *   send[k] holds R*recvcount elements; rank r receives contiguous block r (NCCL convention).
+ *   recv[r] == send[r] + r*recvcount is allowed; any other overlap is undefined.
+ * count == 0 is a no-op.  dtype in {BF16, F32, F16}.  Full speed needs 16-byte aligned
+ * pointers (and recvcount*sizeof(dtype) % 16 == 0 for ReduceScatter); otherwise a scalar
+ * path with the same arithmetic runs. */
+int ncclx_allreduce_sum(const void* const* send, void* const* recv, size_t count, int R,
+                        ncclx_dtype_t dtype, ncclx_stream_t stream);
+int ncclx_reducescatter_sum(const void* const* send, void* const* recv, size_t recvcount, int R,
+                            ncclx_dtype_t dtype, ncclx_stream_t stream);
+
+/* ---- host-buffer forms (the end-to-end path: H2D + kernels + D2H inside the call) ------ *
+ *
+ * Same semantics, but every pointer is a HOST pointer (pinned memory gives full PCIe
+ * speed; pageable works).  `send`/`recv` are HOST arrays of R HOST pointers and the counts
+ * are HOST arrays.  The library stages through its own device buffers (grown on demand with
+ * cudaMalloc and kept until ncclx_finalize), runs the device path on `stream`, copies the
+ * results back and synchronises `stream` before returning.  Not capturable.
+ * AllToAllv: recv[d] receives exactly sum_s C[s][d] elements; recvcounts_host is filled. */
+int ncclx_alltoallv_host(const void* const* send, const int64_t* sendcounts_host, void* const* recv,
+                         int64_t* recvcounts_host, int R, ncclx_dtype_t dtype, ncclx_stream_t stream);
+int ncclx_allreduce_sum_host(const void* const* send, void* const* recv, size_t count, int R,
+                             ncclx_dtype_t dtype, ncclx_stream_t stream);
+int ncclx_reducescatter_sum_host(const void* const* send, void* const* recv, size_t recvcount, int R,
+                                 ncclx_dtype_t dtype, ncclx_stream_t stream);
+
+/* ---- tuning and measurement (not part of the paper's contract) -------------------------- */
+
+typedef enum {
+    NCCLX_PARAM_COPY_CTAS_PER_SM = 0, /* persistent segment-copy CTAs per SM (1..4), default 1        */
+    NCCLX_PARAM_BULK_MIN_BYTES = 1,   /* 16B-aligned segments >= this many bytes take cp.async.bulk;   */
+                                      /* smaller or unaligned ones take the vector path. default 1024  */
+    NCCLX_PARAM_REDUCE_CTAS_PER_SM = 2, /* reduce grid = this * SM count, default 8                    */
+    NCCLX_PARAM_SCAN_CTAS = 3,        /* upper bound on CTAs of the counts kernel, default 16          */
+    NCCLX_PARAM_PROFILE = 4,          /* 1: bracket each kernel with CUDA events (never while capturing) */
+    NCCLX_PARAM_FORCE_VECTOR = 5,     /* 1: send every segment down the vector path (for A/B runs)     */
+    NCCLX_PARAM_BULK_TILE_SHIFT = 6,  /* log2 bytes of a bulk tile = one smem ring stage (12..16), default 15 */
+    NCCLX_PARAM_VEC_TILE_SHIFT = 7,   /* log2 bytes of a vector-path tile (10..20), default 14          */
+    NCCLX_PARAM_COUNT_
+} ncclx_param_t;
+
+int ncclx_set_param(int param, int64_t value);
+int ncclx_get_param(int param, int64_t* value);
+
+typedef enum {
+    NCCLX_KERNEL_COUNTS = 0, /* counts transpose + offsets scan + work list   */
+    NCCLX_KERNEL_COPY = 1,   /* byte-balanced segment copy                    */
+    NCCLX_KERNEL_REDUCE = 2, /* rank-order sum                                */
+    NCCLX_KERNEL_COUNT_
+} ncclx_kernel_t;
+
+/* With NCCLX_PARAM_PROFILE = 1: total device time (ms, CUDA events on the launch stream) and
+ * number of launches of `kernel` since the last ncclx_profile_reset.  Synchronises the
+ * recorded events.  ncclx_launch_count works with profiling off (counts every kernel this
+ * library launched since init or reset, captured launches counted once at capture). */
+int ncclx_profile_read(int kernel, double* total_ms, int64_t* launches);
+int ncclx_profile_reset(void);
+int64_t ncclx_launch_count(void);
+
+/* Number of SMs of the device the library was initialised on (0 before init). */
+int ncclx_sm_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NCCLX_B200_H */

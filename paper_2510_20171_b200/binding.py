@@ -1,0 +1,216 @@
+"""Thin ctypes binding over libncclx_b200.so -- argument marshalling only.
+
+Same names as include/ncclx_b200.h.  Every step of the hot path runs in the library's CUDA
+kernels; PyTorch appears only as the owner of device memory and streams.  There is NO
+fallback: if the shared library is missing or fails to load, importing a symbol raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Sequence
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libncclx_b200.so")
+
+BF16, F32, F16, U8 = 0, 1, 2, 3
+DTYPE_ID = {"bf16": BF16, "f32": F32, "f16": F16, "u8": U8}
+
+PARAM_COPY_CTAS_PER_SM = 0
+PARAM_BULK_MIN_BYTES = 1
+PARAM_REDUCE_CTAS_PER_SM = 2
+PARAM_SCAN_CTAS = 3
+PARAM_PROFILE = 4
+PARAM_FORCE_VECTOR = 5
+PARAM_BULK_TILE_SHIFT = 6
+PARAM_VEC_TILE_SHIFT = 7
+
+KERNEL_COUNTS, KERNEL_COPY, KERNEL_REDUCE = 0, 1, 2
+
+# every symbol include/ncclx_b200.h declares (tests check the .so exports all of them)
+SYMBOLS = [
+    "ncclx_init", "ncclx_finalize", "ncclx_strerror", "ncclx_last_cuda_error", "ncclx_last_cuda_error_string",
+    "ncclx_version", "ncclx_alltoallv_dev", "ncclx_alltoallv_last_offsets", "ncclx_device_status",
+    "ncclx_allreduce_sum", "ncclx_reducescatter_sum", "ncclx_alltoallv_host", "ncclx_allreduce_sum_host",
+    "ncclx_reducescatter_sum_host", "ncclx_set_param", "ncclx_get_param", "ncclx_profile_read",
+    "ncclx_profile_reset", "ncclx_launch_count", "ncclx_sm_count",
+]
+
+
+class NcclxError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        L = lib()
+        msg = L.ncclx_strerror(code).decode()
+        if code == 4:
+            msg += f" ({L.ncclx_last_cuda_error()}: {L.ncclx_last_cuda_error_string().decode()})"
+        super().__init__(f"{where}: {msg} [code {code}]")
+        self.code = code
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Loads the CUDA library; fails loudly when it has not been built (no CPU fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                              "(nvcc, sm_100a). There is no CPU fallback.")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i64, i64p = ctypes.c_void_p, ctypes.c_int64, ctypes.POINTER(ctypes.c_int64)
+        L.ncclx_init.argtypes = [ctypes.c_int, ctypes.c_int]
+        L.ncclx_strerror.argtypes = [ctypes.c_int]
+        L.ncclx_strerror.restype = ctypes.c_char_p
+        L.ncclx_last_cuda_error_string.restype = ctypes.c_char_p
+        L.ncclx_alltoallv_dev.argtypes = [vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, vp]
+        L.ncclx_alltoallv_last_offsets.argtypes = [vp, vp, ctypes.c_int, vp]
+        L.ncclx_device_status.argtypes = [ctypes.POINTER(ctypes.c_uint32), vp]
+        for f in (L.ncclx_allreduce_sum, L.ncclx_reducescatter_sum, L.ncclx_allreduce_sum_host,
+                  L.ncclx_reducescatter_sum_host):
+            f.argtypes = [vp, vp, ctypes.c_size_t, ctypes.c_int, ctypes.c_int, vp]
+        L.ncclx_alltoallv_host.argtypes = [vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, vp]
+        L.ncclx_set_param.argtypes = [ctypes.c_int, i64]
+        L.ncclx_get_param.argtypes = [ctypes.c_int, i64p]
+        L.ncclx_profile_read.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double), i64p]
+        L.ncclx_launch_count.restype = i64
+        _lib = L
+    return _lib
+
+
+def _ck(code: int, where: str) -> None:
+    if code != 0:
+        raise NcclxError(code, where)
+
+
+def _dt(dtype) -> int:
+    return DTYPE_ID[dtype] if isinstance(dtype, str) else int(dtype)
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return int(getattr(stream, "cuda_stream", stream))
+
+
+def _ptr(x) -> int:
+    """Device/host address of a torch tensor, numpy array or raw int."""
+    if x is None:
+        return 0
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if hasattr(x, "ctypes"):
+        return x.ctypes.data
+    return int(x)
+
+
+# ---- lifetime ------------------------------------------------------------------------------
+
+def ncclx_init(max_ranks: int = 128, device: int = 0) -> None:
+    _ck(lib().ncclx_init(max_ranks, device), "ncclx_init")
+
+
+def ncclx_finalize() -> None:
+    _ck(lib().ncclx_finalize(), "ncclx_finalize")
+
+
+def ncclx_version() -> int:
+    return lib().ncclx_version()
+
+
+def ncclx_sm_count() -> int:
+    return lib().ncclx_sm_count()
+
+
+# ---- device entry points ---------------------------------------------------------------------
+
+def device_ptr_table(tensors: Sequence, device=None):
+    """DEVICE int64 tensor holding the data_ptr of each tensor (the `send` / `recv` tables)."""
+    import torch
+    dev = device if device is not None else tensors[0].device
+    return torch.tensor([t.data_ptr() for t in tensors], dtype=torch.int64, device=dev)
+
+
+def ncclx_alltoallv_dev(send_table, sendcounts_dev, recv_table, recvcounts_dev, R: int, dtype, stream=None) -> None:
+    _ck(lib().ncclx_alltoallv_dev(_ptr(send_table), _ptr(sendcounts_dev), _ptr(recv_table), _ptr(recvcounts_dev),
+                                  R, _dt(dtype), _stream(stream)), "ncclx_alltoallv_dev")
+
+
+def ncclx_alltoallv_last_offsets(R: int, stream=None):
+    import numpy as np
+    soff = np.empty((R, R), np.int64)
+    roff = np.empty((R, R), np.int64)
+    _ck(lib().ncclx_alltoallv_last_offsets(soff.ctypes.data, roff.ctypes.data, R, _stream(stream)),
+        "ncclx_alltoallv_last_offsets")
+    return soff, roff
+
+
+def ncclx_device_status(stream=None) -> int:
+    st = ctypes.c_uint32(0)
+    _ck(lib().ncclx_device_status(ctypes.byref(st), _stream(stream)), "ncclx_device_status")
+    return st.value
+
+
+def ncclx_allreduce_sum(send_table, recv_table, count: int, R: int, dtype, stream=None) -> None:
+    _ck(lib().ncclx_allreduce_sum(_ptr(send_table), _ptr(recv_table), count, R, _dt(dtype), _stream(stream)),
+        "ncclx_allreduce_sum")
+
+
+def ncclx_reducescatter_sum(send_table, recv_table, recvcount: int, R: int, dtype, stream=None) -> None:
+    _ck(lib().ncclx_reducescatter_sum(_ptr(send_table), _ptr(recv_table), recvcount, R, _dt(dtype), _stream(stream)),
+        "ncclx_reducescatter_sum")
+
+
+# ---- host-buffer entry points ------------------------------------------------------------------
+
+def _host_table(bufs: Sequence):
+    tab = (ctypes.c_void_p * len(bufs))()
+    for i, b in enumerate(bufs):
+        tab[i] = _ptr(b)
+    return tab
+
+
+def ncclx_alltoallv_host(send: Sequence, sendcounts_host, recv: Sequence, recvcounts_host, R: int, dtype,
+                         stream=None) -> None:
+    st, rt = _host_table(send), _host_table(recv)
+    _ck(lib().ncclx_alltoallv_host(ctypes.addressof(st), _ptr(sendcounts_host), ctypes.addressof(rt),
+                                   _ptr(recvcounts_host), R, _dt(dtype), _stream(stream)), "ncclx_alltoallv_host")
+
+
+def ncclx_allreduce_sum_host(send: Sequence, recv: Sequence, count: int, R: int, dtype, stream=None) -> None:
+    st, rt = _host_table(send), _host_table(recv)
+    _ck(lib().ncclx_allreduce_sum_host(ctypes.addressof(st), ctypes.addressof(rt), count, R, _dt(dtype),
+                                       _stream(stream)), "ncclx_allreduce_sum_host")
+
+
+def ncclx_reducescatter_sum_host(send: Sequence, recv: Sequence, recvcount: int, R: int, dtype, stream=None) -> None:
+    st, rt = _host_table(send), _host_table(recv)
+    _ck(lib().ncclx_reducescatter_sum_host(ctypes.addressof(st), ctypes.addressof(rt), recvcount, R, _dt(dtype),
+                                           _stream(stream)), "ncclx_reducescatter_sum_host")
+
+
+# ---- tuning / measurement -------------------------------------------------------------------------
+
+def ncclx_set_param(param: int, value: int) -> None:
+    _ck(lib().ncclx_set_param(param, value), "ncclx_set_param")
+
+
+def ncclx_get_param(param: int) -> int:
+    v = ctypes.c_int64(0)
+    _ck(lib().ncclx_get_param(param, ctypes.byref(v)), "ncclx_get_param")
+    return v.value
+
+
+def ncclx_profile_read(kernel: int):
+    ms, n = ctypes.c_double(0), ctypes.c_int64(0)
+    _ck(lib().ncclx_profile_read(kernel, ctypes.byref(ms), ctypes.byref(n)), "ncclx_profile_read")
+    return ms.value, n.value
+
+
+def ncclx_profile_reset() -> None:
+    _ck(lib().ncclx_profile_reset(), "ncclx_profile_reset")
+
+
+def ncclx_launch_count() -> int:
+    return lib().ncclx_launch_count()

@@ -1,0 +1,485 @@
+// ncclx_b200.cu -- host launch layer + C ABI of libncclx_b200.so (see include/ncclx_b200.h).
+// Host code only validates arguments and enqueues fixed-grid kernels: no allocation, no
+// synchronisation and no host<->device copy on the device entry points, so they are
+// CUDA-graph capturable.  There is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include "../../include/ncclx_b200.h"
+#include "common.cuh"
+#include "copy_kernel.cuh"
+#include "counts_kernel.cuh"
+#include "reduce_kernel.cuh"
+
+using namespace ncclx;
+
+namespace {
+
+struct EventPair { cudaEvent_t a, b; };
+
+struct Context {
+    bool ready = false;
+    int device = -1;
+    int maxRanks = 0;
+    int smCount = 0;
+    int maxSmemOptin = 0;
+    Workspace ws{};
+    void* wsBase = nullptr;
+    // tunables
+    int64_t params[NCCLX_PARAM_COUNT_] = {1, 1024, 8, 16, 0, 0, 15, 14};
+    // profiling
+    std::vector<EventPair> events[NCCLX_KERNEL_COUNT_];
+    std::atomic<int64_t> launches{0};
+    int64_t kernelLaunches[NCCLX_KERNEL_COUNT_] = {0, 0, 0};
+    // host-path staging (device memory, grown on demand)
+    void* stage[4] = {nullptr, nullptr, nullptr, nullptr};   // 0 send data, 1 recv data, 2 meta, 3 spare
+    size_t stageCap[4] = {0, 0, 0, 0};
+    int lastCuda = 0;
+    std::mutex mu;
+};
+
+Context g;
+
+constexpr size_t kMaxProfiledLaunches = 8192;
+
+int cudaFail(cudaError_t e) {
+    g.lastCuda = (int)e;
+    cudaGetLastError();
+    return NCCLX_ERR_CUDA;
+}
+#define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return cudaFail(e_); } while (0)
+
+int elemSizeOf(int dtype) {
+    switch (dtype) {
+    case NCCLX_BF16: return 2;
+    case NCCLX_F32: return 4;
+    case NCCLX_F16: return 2;
+    case NCCLX_U8: return 1;
+    default: return 0;
+    }
+}
+
+size_t alignUp(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+bool isCapturing(cudaStream_t s) {
+    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(s, &st) != cudaSuccess) { cudaGetLastError(); return false; }
+    return st != cudaStreamCaptureStatusNone;
+}
+
+// Brackets a launch with events when profiling is on and the stream is not capturing.
+struct LaunchScope {
+    int kernel;
+    cudaStream_t stream;
+    bool timed = false;
+    EventPair ev{};
+    LaunchScope(int k, cudaStream_t s) : kernel(k), stream(s) {
+        g.launches.fetch_add(1, std::memory_order_relaxed);
+        g.kernelLaunches[k]++;
+        if (g.params[NCCLX_PARAM_PROFILE] && g.events[k].size() < kMaxProfiledLaunches && !isCapturing(s)) {
+            if (cudaEventCreate(&ev.a) == cudaSuccess && cudaEventCreate(&ev.b) == cudaSuccess) {
+                timed = true;
+                cudaEventRecord(ev.a, s);
+            }
+        }
+    }
+    ~LaunchScope() {
+        if (timed) {
+            cudaEventRecord(ev.b, stream);
+            g.events[kernel].push_back(ev);
+        }
+    }
+};
+
+size_t copySmemBytes(int stages, int tileShiftB, int R) {
+    return ((size_t)stages << tileShiftB) + COPY_MAX_STAGES * (8 + 8 + 4) + 2 * (size_t)(R + 1) * 4 + 16;
+}
+
+int chooseStages(int ctasPerSm, int tileShiftB, int R) {
+    const size_t budget = (size_t)g.maxSmemOptin / ctasPerSm - (ctasPerSm > 1 ? 1024 : 0);
+    int s = COPY_MAX_STAGES;
+    while (s > 2 && copySmemBytes(s, tileShiftB, R) > budget) --s;
+    return s;
+}
+
+int countsW(int R) {
+    // columns per CTA: spread over at most SCAN_CTAS CTAs, at most 32 columns, and 2*R*(W+1)*8 <= smem
+    int W = (R + (int)g.params[NCCLX_PARAM_SCAN_CTAS] - 1) / (int)g.params[NCCLX_PARAM_SCAN_CTAS];
+    if (W < 1) W = 1;
+    if (W > 32) W = 32;
+    const size_t budget = (size_t)g.maxSmemOptin - 1024;
+    while (W > 1 && 2 * (size_t)R * (W + 1) * 8 > budget) --W;
+    return W;
+}
+
+int launchAllToAllv(const void* const* send, const int64_t* C, void* const* recv, int64_t* RC, int R, int es,
+                    cudaStream_t stream) {
+    CountsArgs ca{};
+    ca.send = send; ca.recv = recv;
+    ca.C = reinterpret_cast<const long long*>(C);
+    ca.RC = reinterpret_cast<long long*>(RC);
+    ca.ws = g.ws; ca.R = R; ca.W = countsW(R); ca.elemSize = es;
+    ca.tileShift[0] = (int)g.params[NCCLX_PARAM_BULK_TILE_SHIFT]; ca.tileShift[1] = (int)g.params[NCCLX_PARAM_VEC_TILE_SHIFT];
+    ca.bulkMinBytes = g.params[NCCLX_PARAM_BULK_MIN_BYTES] < 16 ? 16 : g.params[NCCLX_PARAM_BULK_MIN_BYTES];
+    ca.forceVector = (int)g.params[NCCLX_PARAM_FORCE_VECTOR];
+    const int G = (R + ca.W - 1) / ca.W;
+    const size_t csm = 2 * (size_t)R * (ca.W + 1) * 8;
+    {
+        LaunchScope ls(NCCLX_KERNEL_COUNTS, stream);
+        counts_kernel<<<G, COUNTS_THREADS, csm, stream>>>(ca);
+        CK(cudaGetLastError());
+    }
+    CopyArgs cp{};
+    cp.desc = g.ws.desc; cp.colTiles[0] = g.ws.colTiles[0]; cp.colTiles[1] = g.ws.colTiles[1];
+    cp.ctl = g.ws.ctl; cp.R = R;
+    cp.tileShift[0] = ca.tileShift[0]; cp.tileShift[1] = ca.tileShift[1];
+    const int cps = (int)g.params[NCCLX_PARAM_COPY_CTAS_PER_SM];
+    cp.stages = chooseStages(cps, cp.tileShift[0], R);
+    const size_t smem = copySmemBytes(cp.stages, cp.tileShift[0], R);
+    {
+        LaunchScope ls(NCCLX_KERNEL_COPY, stream);
+        segment_copy_kernel<<<g.smCount * cps, COPY_THREADS, smem, stream>>>(cp);
+        CK(cudaGetLastError());
+    }
+    return NCCLX_OK;
+}
+
+template <int DT>
+int launchReduceDT(const ReduceArgs& ra, int grid, size_t smem, cudaStream_t stream) {
+    LaunchScope ls(NCCLX_KERNEL_REDUCE, stream);
+    if (ra.R <= 4) reduce_kernel<DT, 4><<<grid, REDUCE_THREADS, smem, stream>>>(ra);
+    else if (ra.R <= 8) reduce_kernel<DT, 8><<<grid, REDUCE_THREADS, smem, stream>>>(ra);
+    else reduce_kernel<DT, 16><<<grid, REDUCE_THREADS, smem, stream>>>(ra);
+    CK(cudaGetLastError());
+    return NCCLX_OK;
+}
+
+int launchReduce(const void* const* send, void* const* recv, size_t blockElems, int R, int dtype, int scatter,
+                 cudaStream_t stream) {
+    if (blockElems == 0) return NCCLX_OK;
+    ReduceArgs ra{};
+    ra.send = send; ra.recv = recv; ra.blockElems = blockElems; ra.R = R; ra.scatter = scatter;
+    const int es = elemSizeOf(dtype);
+    const unsigned long long totalVec = ((unsigned long long)blockElems * (scatter ? R : 1) * es + 15) / 16;
+    unsigned long long tiles = (totalVec + REDUCE_THREADS - 1) / REDUCE_THREADS + (scatter ? R : 0);
+    unsigned long long grid = (unsigned long long)g.smCount * (unsigned long long)g.params[NCCLX_PARAM_REDUCE_CTAS_PER_SM];
+    if (grid > tiles) grid = tiles;
+    if (grid < 1) grid = 1;
+    const size_t smem = 2 * (size_t)R * sizeof(void*);
+    switch (dtype) {
+    case NCCLX_BF16: return launchReduceDT<RED_BF16>(ra, (int)grid, smem, stream);
+    case NCCLX_F32: return launchReduceDT<RED_F32>(ra, (int)grid, smem, stream);
+    case NCCLX_F16: return launchReduceDT<RED_F16>(ra, (int)grid, smem, stream);
+    default: return NCCLX_ERR_DTYPE;
+    }
+}
+
+int ensureStage(int i, size_t bytes) {
+    if (bytes <= g.stageCap[i]) return NCCLX_OK;
+    if (g.stage[i]) { CK(cudaFree(g.stage[i])); g.stage[i] = nullptr; g.stageCap[i] = 0; }
+    const size_t cap = alignUp(bytes, (size_t)2 << 20);
+    CK(cudaMalloc(&g.stage[i], cap));
+    g.stageCap[i] = cap;
+    return NCCLX_OK;
+}
+
+int checkCommon(int R) {
+    if (!g.ready) return NCCLX_ERR_NOT_INITIALIZED;
+    if (R < 1) return NCCLX_ERR_ARG;
+    if (R > g.maxRanks) return NCCLX_ERR_NOT_INITIALIZED;
+    return NCCLX_OK;
+}
+
+void freeAll() {
+    if (g.wsBase) { cudaFree(g.wsBase); g.wsBase = nullptr; }
+    for (int i = 0; i < 4; ++i) {
+        if (g.stage[i]) { cudaFree(g.stage[i]); g.stage[i] = nullptr; g.stageCap[i] = 0; }
+    }
+    for (auto& v : g.events) {
+        for (auto& e : v) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+        v.clear();
+    }
+    cudaGetLastError();
+    g.ready = false;
+}
+
+template <typename K>
+int optInSmem(K kernel, int bytes) {
+    CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    return NCCLX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ncclx_version(void) { return NCCLX_B200_VERSION; }
+
+const char* ncclx_strerror(int code) {
+    switch (code) {
+    case NCCLX_OK: return "ok";
+    case NCCLX_ERR_ARG: return "invalid argument";
+    case NCCLX_ERR_DTYPE: return "unsupported dtype for this call";
+    case NCCLX_ERR_NOT_INITIALIZED: return "not initialised, or R exceeds max_ranks";
+    case NCCLX_ERR_CUDA: return "CUDA runtime error";
+    case NCCLX_ERR_CAPTURE: return "host-synchronous call while the stream is capturing";
+    default: return "unknown error code";
+    }
+}
+
+int ncclx_last_cuda_error(void) { return g.lastCuda; }
+const char* ncclx_last_cuda_error_string(void) { return cudaGetErrorString((cudaError_t)g.lastCuda); }
+
+int ncclx_init(int max_ranks, int device) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    if (max_ranks < 1 || max_ranks > NCCLX_MAX_RANKS) return NCCLX_ERR_ARG;
+    if (g.ready) freeAll();
+    CK(cudaSetDevice(device));
+    cudaDeviceProp prop{};
+    CK(cudaGetDeviceProperties(&prop, device));
+    if (prop.major < 10) { g.lastCuda = (int)cudaErrorNoKernelImageForDevice; return NCCLX_ERR_CUDA; }
+    g.device = device;
+    g.smCount = prop.multiProcessorCount;
+    g.maxSmemOptin = (int)prop.sharedMemPerBlockOptin;
+    g.maxRanks = max_ranks;
+
+    const size_t rr = (size_t)max_ranks * max_ranks;
+    size_t off = 0;
+    const size_t oSoff = off; off = alignUp(off + rr * 8, 256);
+    const size_t oRoff = off; off = alignUp(off + rr * 8, 256);
+    const size_t oDesc = off; off = alignUp(off + rr * sizeof(SegDesc), 256);
+    const size_t oCt0 = off; off = alignUp(off + (size_t)max_ranks * 4, 256);
+    const size_t oCt1 = off; off = alignUp(off + (size_t)max_ranks * 4, 256);
+    const size_t oCtl = off; off = alignUp(off + sizeof(WorkCtl), 256);
+    CK(cudaMalloc(&g.wsBase, off));
+    CK(cudaMemset(g.wsBase, 0, off));
+    char* b = static_cast<char*>(g.wsBase);
+    g.ws.soff = reinterpret_cast<long long*>(b + oSoff);
+    g.ws.roff = reinterpret_cast<long long*>(b + oRoff);
+    g.ws.desc = reinterpret_cast<SegDesc*>(b + oDesc);
+    g.ws.colTiles[0] = reinterpret_cast<int*>(b + oCt0);
+    g.ws.colTiles[1] = reinterpret_cast<int*>(b + oCt1);
+    g.ws.ctl = reinterpret_cast<WorkCtl*>(b + oCtl);
+
+    int rc;
+    if ((rc = optInSmem(segment_copy_kernel, g.maxSmemOptin))) return rc;
+    if ((rc = optInSmem(counts_kernel, g.maxSmemOptin))) return rc;
+    CK(cudaDeviceSynchronize());
+    g.launches = 0;
+    for (auto& k : g.kernelLaunches) k = 0;
+    g.ready = true;
+    return NCCLX_OK;
+}
+
+int ncclx_finalize(void) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    if (!g.ready) return NCCLX_ERR_NOT_INITIALIZED;
+    cudaDeviceSynchronize();
+    freeAll();
+    return NCCLX_OK;
+}
+
+int ncclx_sm_count(void) { return g.ready ? g.smCount : 0; }
+
+int ncclx_alltoallv_dev(const void* const* send, const int64_t* sendcounts_dev, void* const* recv,
+                        int64_t* recvcounts_dev, int R, ncclx_dtype_t dtype, ncclx_stream_t stream) {
+    int rc = checkCommon(R);
+    if (rc) return rc;
+    if (!send || !sendcounts_dev || !recv || !recvcounts_dev) return NCCLX_ERR_ARG;
+    if (sendcounts_dev == recvcounts_dev) return NCCLX_ERR_ARG;
+    const int es = elemSizeOf((int)dtype);
+    if (!es) return NCCLX_ERR_DTYPE;
+    return launchAllToAllv(send, sendcounts_dev, recv, recvcounts_dev, R, es, static_cast<cudaStream_t>(stream));
+}
+
+int ncclx_alltoallv_last_offsets(int64_t* soff_host, int64_t* roff_host, int R, ncclx_stream_t stream) {
+    int rc = checkCommon(R);
+    if (rc) return rc;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (isCapturing(s)) return NCCLX_ERR_CAPTURE;
+    CK(cudaStreamSynchronize(s));
+    const size_t bytes = (size_t)R * R * 8;
+    if (soff_host) CK(cudaMemcpy(soff_host, g.ws.soff, bytes, cudaMemcpyDeviceToHost));
+    if (roff_host) CK(cudaMemcpy(roff_host, g.ws.roff, bytes, cudaMemcpyDeviceToHost));
+    return NCCLX_OK;
+}
+
+int ncclx_device_status(uint32_t* status_host, ncclx_stream_t stream) {
+    if (!g.ready) return NCCLX_ERR_NOT_INITIALIZED;
+    if (!status_host) return NCCLX_ERR_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (isCapturing(s)) return NCCLX_ERR_CAPTURE;
+    CK(cudaStreamSynchronize(s));
+    CK(cudaMemcpy(status_host, &g.ws.ctl->status, 4, cudaMemcpyDeviceToHost));
+    CK(cudaMemset(&g.ws.ctl->status, 0, 4));
+    return NCCLX_OK;
+}
+
+int ncclx_allreduce_sum(const void* const* send, void* const* recv, size_t count, int R, ncclx_dtype_t dtype,
+                        ncclx_stream_t stream) {
+    int rc = checkCommon(R);
+    if (rc) return rc;
+    if (!send || !recv) return NCCLX_ERR_ARG;
+    if (!(dtype == NCCLX_BF16 || dtype == NCCLX_F32 || dtype == NCCLX_F16)) return NCCLX_ERR_DTYPE;
+    return launchReduce(send, recv, count, R, (int)dtype, 0, static_cast<cudaStream_t>(stream));
+}
+
+int ncclx_reducescatter_sum(const void* const* send, void* const* recv, size_t recvcount, int R,
+                            ncclx_dtype_t dtype, ncclx_stream_t stream) {
+    int rc = checkCommon(R);
+    if (rc) return rc;
+    if (!send || !recv) return NCCLX_ERR_ARG;
+    if (!(dtype == NCCLX_BF16 || dtype == NCCLX_F32 || dtype == NCCLX_F16)) return NCCLX_ERR_DTYPE;
+    return launchReduce(send, recv, recvcount, R, (int)dtype, 1, static_cast<cudaStream_t>(stream));
+}
+
+// ---- host-buffer forms -----------------------------------------------------------------------
+
+int ncclx_alltoallv_host(const void* const* send, const int64_t* sendcounts_host, void* const* recv,
+                         int64_t* recvcounts_host, int R, ncclx_dtype_t dtype, ncclx_stream_t stream) {
+    int rc = checkCommon(R);
+    if (rc) return rc;
+    if (!send || !sendcounts_host || !recv || !recvcounts_host) return NCCLX_ERR_ARG;
+    const int es = elemSizeOf((int)dtype);
+    if (!es) return NCCLX_ERR_DTYPE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (isCapturing(s)) return NCCLX_ERR_CAPTURE;
+
+    std::vector<size_t> sBytes(R, 0), rBytes(R, 0), sOff(R), rOff(R);
+    for (int i = 0; i < R; ++i)
+        for (int j = 0; j < R; ++j) {
+            const int64_t c = sendcounts_host[(size_t)i * R + j];
+            if (c > 0) { sBytes[i] += (size_t)c * es; rBytes[j] += (size_t)c * es; }
+        }
+    size_t sTot = 0, rTot = 0;
+    for (int i = 0; i < R; ++i) { sOff[i] = sTot; sTot += alignUp(sBytes[i], 256); rOff[i] = rTot; rTot += alignUp(rBytes[i], 256); }
+    const size_t rr = (size_t)R * R * 8;
+    const size_t metaBytes = 2 * rr + 2 * (size_t)R * 8;
+    if ((rc = ensureStage(0, sTot + 256))) return rc;
+    if ((rc = ensureStage(1, rTot + 256))) return rc;
+    if ((rc = ensureStage(2, metaBytes))) return rc;
+    char* meta = static_cast<char*>(g.stage[2]);
+    int64_t* dC = reinterpret_cast<int64_t*>(meta);
+    int64_t* dRC = reinterpret_cast<int64_t*>(meta + rr);
+    void** dSend = reinterpret_cast<void**>(meta + 2 * rr);
+    void** dRecv = dSend + R;
+    std::vector<void*> tab(2 * (size_t)R);
+    for (int i = 0; i < R; ++i) {
+        tab[i] = static_cast<char*>(g.stage[0]) + sOff[i];
+        tab[R + i] = static_cast<char*>(g.stage[1]) + rOff[i];
+    }
+    CK(cudaMemcpyAsync(dC, sendcounts_host, rr, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(dSend, tab.data(), 2 * (size_t)R * 8, cudaMemcpyHostToDevice, s));
+    for (int i = 0; i < R; ++i)
+        if (sBytes[i]) {
+            if (!send[i]) return NCCLX_ERR_ARG;
+            CK(cudaMemcpyAsync(tab[i], send[i], sBytes[i], cudaMemcpyHostToDevice, s));
+        }
+    rc = launchAllToAllv(reinterpret_cast<const void* const*>(dSend), dC, dRecv, dRC, R, es, s);
+    if (rc) return rc;
+    for (int i = 0; i < R; ++i)
+        if (rBytes[i]) {
+            if (!recv[i]) return NCCLX_ERR_ARG;
+            CK(cudaMemcpyAsync(recv[i], tab[R + i], rBytes[i], cudaMemcpyDeviceToHost, s));
+        }
+    CK(cudaMemcpyAsync(recvcounts_host, dRC, rr, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    return NCCLX_OK;
+}
+
+static int reduceHost(const void* const* send, void* const* recv, size_t blockElems, int R, int dtype, int scatter,
+                      cudaStream_t s) {
+    int rc = checkCommon(R);
+    if (rc) return rc;
+    if (!send || !recv) return NCCLX_ERR_ARG;
+    if (!(dtype == NCCLX_BF16 || dtype == NCCLX_F32 || dtype == NCCLX_F16)) return NCCLX_ERR_DTYPE;
+    if (isCapturing(s)) return NCCLX_ERR_CAPTURE;
+    if (blockElems == 0) return NCCLX_OK;
+    const int es = elemSizeOf(dtype);
+    const size_t inBytes = blockElems * (scatter ? (size_t)R : 1) * es;
+    const size_t outBytes = blockElems * es;
+    const size_t inPitch = alignUp(inBytes, 256), outPitch = alignUp(outBytes, 256);
+    if ((rc = ensureStage(0, inPitch * R))) return rc;
+    if ((rc = ensureStage(1, outPitch * R))) return rc;
+    if ((rc = ensureStage(2, 2 * (size_t)R * 8))) return rc;
+    std::vector<void*> tab(2 * (size_t)R);
+    for (int i = 0; i < R; ++i) {
+        if (!send[i] || !recv[i]) return NCCLX_ERR_ARG;
+        tab[i] = static_cast<char*>(g.stage[0]) + inPitch * i;
+        tab[R + i] = static_cast<char*>(g.stage[1]) + outPitch * i;
+    }
+    void** dSend = static_cast<void**>(g.stage[2]);
+    CK(cudaMemcpyAsync(dSend, tab.data(), 2 * (size_t)R * 8, cudaMemcpyHostToDevice, s));
+    for (int i = 0; i < R; ++i) CK(cudaMemcpyAsync(tab[i], send[i], inBytes, cudaMemcpyHostToDevice, s));
+    rc = launchReduce(reinterpret_cast<const void* const*>(dSend), dSend + R, blockElems, R, dtype, scatter, s);
+    if (rc) return rc;
+    for (int i = 0; i < R; ++i) CK(cudaMemcpyAsync(recv[i], tab[R + i], outBytes, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    return NCCLX_OK;
+}
+
+int ncclx_allreduce_sum_host(const void* const* send, void* const* recv, size_t count, int R, ncclx_dtype_t dtype,
+                             ncclx_stream_t stream) {
+    return reduceHost(send, recv, count, R, (int)dtype, 0, static_cast<cudaStream_t>(stream));
+}
+
+int ncclx_reducescatter_sum_host(const void* const* send, void* const* recv, size_t recvcount, int R,
+                                 ncclx_dtype_t dtype, ncclx_stream_t stream) {
+    return reduceHost(send, recv, recvcount, R, (int)dtype, 1, static_cast<cudaStream_t>(stream));
+}
+
+// ---- tuning / measurement --------------------------------------------------------------------
+
+int ncclx_set_param(int param, int64_t value) {
+    if (param < 0 || param >= NCCLX_PARAM_COUNT_) return NCCLX_ERR_ARG;
+    switch (param) {
+    case NCCLX_PARAM_COPY_CTAS_PER_SM: if (value < 1 || value > 4) return NCCLX_ERR_ARG; break;
+    case NCCLX_PARAM_BULK_MIN_BYTES: if (value < 16) return NCCLX_ERR_ARG; break;
+    case NCCLX_PARAM_REDUCE_CTAS_PER_SM: if (value < 1 || value > 64) return NCCLX_ERR_ARG; break;
+    case NCCLX_PARAM_SCAN_CTAS: if (value < 1 || value > 1024) return NCCLX_ERR_ARG; break;
+    case NCCLX_PARAM_BULK_TILE_SHIFT: if (value < 12 || value > 16) return NCCLX_ERR_ARG; break;
+    case NCCLX_PARAM_VEC_TILE_SHIFT: if (value < 10 || value > 20) return NCCLX_ERR_ARG; break;
+    default: if (value < 0) return NCCLX_ERR_ARG; break;
+    }
+    g.params[param] = value;
+    return NCCLX_OK;
+}
+
+int ncclx_get_param(int param, int64_t* value) {
+    if (param < 0 || param >= NCCLX_PARAM_COUNT_ || !value) return NCCLX_ERR_ARG;
+    *value = g.params[param];
+    return NCCLX_OK;
+}
+
+int ncclx_profile_read(int kernel, double* total_ms, int64_t* launches) {
+    if (kernel < 0 || kernel >= NCCLX_KERNEL_COUNT_ || !total_ms || !launches) return NCCLX_ERR_ARG;
+    double tot = 0;
+    for (auto& e : g.events[kernel]) {
+        CK(cudaEventSynchronize(e.b));
+        float ms = 0;
+        CK(cudaEventElapsedTime(&ms, e.a, e.b));
+        tot += ms;
+    }
+    *total_ms = tot;
+    *launches = (int64_t)g.events[kernel].size();
+    return NCCLX_OK;
+}
+
+int ncclx_profile_reset(void) {
+    for (auto& v : g.events) {
+        for (auto& e : v) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+        v.clear();
+    }
+    g.launches = 0;
+    for (auto& k : g.kernelLaunches) k = 0;
+    return NCCLX_OK;
+}
+
+int64_t ncclx_launch_count(void) { return g.launches.load(); }
+
+}  // extern "C"

@@ -1,0 +1,217 @@
+// reduce_kernel.cuh -- steps r1 / r2 of the hot path: the in-kernel sum behind AllReduce and
+// ReduceScatter (the Reduce / ReduceCopy step of the paper's FTAR ring, section 5.3
+// L335-337, Fig. 9: "combine the reduction and forwarding copy ... avoids redundant HBM
+// load ... avoid unnecessary HBM stores ... enhance instruction level parallelism").
+//
+// Numeric contract (BASELINE.json north_star): acc = (float)x_0;
+// acc = acc + (float)x_k for k = 1..R-1 in binary32 round-to-nearest-even, no FTZ, no
+// reassociation; ONE rounding to the output type; NaN results canonical.
+//
+// B200 design: HBM-bound streaming kernel.  Each thread owns one 16-byte vector position
+// (bf16x8 / f16x8 / fp32x4) per tile and issues the loads of CH ranks back to back (CH
+// independent 16 B loads in flight per thread, L1 no-allocate) before the ordered fp32 adds;
+// inputs are read exactly once and the result is written straight to the R outputs
+// (AllReduce) or to the owning rank's block (ReduceScatter): no intermediate HBM round trip.
+// The device pointer tables are staged once per CTA into shared memory.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include "common.cuh"
+
+namespace ncclx {
+
+constexpr int REDUCE_THREADS = 256;
+enum { RED_BF16 = 0, RED_F32 = 1, RED_F16 = 2 };
+
+struct ReduceArgs {
+    const void* const* send;     // device table, R pointers
+    void* const* recv;           // device table, R pointers
+    unsigned long long blockElems; // AllReduce: count; ReduceScatter: recvcount
+    int R;
+    int scatter;                 // 0: AllReduce (1 block, R outputs), 1: ReduceScatter (R blocks)
+};
+
+template <int DT> struct Acc;    // accumulators for one 16-byte vector
+
+template <> struct Acc<RED_BF16> {
+    float v[8];
+    __device__ __forceinline__ void set(const uint4& u) {
+        const unsigned int w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { v[2 * i] = __uint_as_float(w[i] << 16); v[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u); }
+    }
+    __device__ __forceinline__ void add(const uint4& u) {
+        const unsigned int w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            v[2 * i] = __fadd_rn(v[2 * i], __uint_as_float(w[i] << 16));
+            v[2 * i + 1] = __fadd_rn(v[2 * i + 1], __uint_as_float(w[i] & 0xffff0000u));
+        }
+    }
+    __device__ __forceinline__ uint4 pack() const {
+        unsigned int w[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            __nv_bfloat162 h = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]);   // cvt.rn.bf16x2.f32, NaN -> 0x7FFF
+            w[i] = *reinterpret_cast<unsigned int*>(&h);
+        }
+        return make_uint4(w[0], w[1], w[2], w[3]);
+    }
+};
+
+template <> struct Acc<RED_F16> {
+    float v[8];
+    __device__ __forceinline__ static float2 up(unsigned int w) {
+        return __half22float2(*reinterpret_cast<const __half2*>(&w));
+    }
+    __device__ __forceinline__ void set(const uint4& u) {
+        const unsigned int w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { float2 f = up(w[i]); v[2 * i] = f.x; v[2 * i + 1] = f.y; }
+    }
+    __device__ __forceinline__ void add(const uint4& u) {
+        const unsigned int w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            float2 f = up(w[i]);
+            v[2 * i] = __fadd_rn(v[2 * i], f.x);
+            v[2 * i + 1] = __fadd_rn(v[2 * i + 1], f.y);
+        }
+    }
+    __device__ __forceinline__ uint4 pack() const {
+        unsigned int w[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            __half2 h = __floats2half2_rn(v[2 * i], v[2 * i + 1]);              // NaN -> 0x7FFF
+            w[i] = *reinterpret_cast<unsigned int*>(&h);
+        }
+        return make_uint4(w[0], w[1], w[2], w[3]);
+    }
+};
+
+__device__ __forceinline__ unsigned int canon_f32(float f) {
+    return (f != f) ? 0x7fffffffu : __float_as_uint(f);
+}
+
+template <> struct Acc<RED_F32> {
+    float v[4];
+    __device__ __forceinline__ void set(const uint4& u) {
+        v[0] = __uint_as_float(u.x); v[1] = __uint_as_float(u.y); v[2] = __uint_as_float(u.z); v[3] = __uint_as_float(u.w);
+    }
+    __device__ __forceinline__ void add(const uint4& u) {
+        v[0] = __fadd_rn(v[0], __uint_as_float(u.x)); v[1] = __fadd_rn(v[1], __uint_as_float(u.y));
+        v[2] = __fadd_rn(v[2], __uint_as_float(u.z)); v[3] = __fadd_rn(v[3], __uint_as_float(u.w));
+    }
+    __device__ __forceinline__ uint4 pack() const {
+        return make_uint4(canon_f32(v[0]), canon_f32(v[1]), canon_f32(v[2]), canon_f32(v[3]));
+    }
+};
+
+// scalar helpers (unaligned / ragged path), same arithmetic
+template <int DT> __device__ __forceinline__ float load_elem(const void* p, unsigned long long i);
+template <> __device__ __forceinline__ float load_elem<RED_BF16>(const void* p, unsigned long long i) {
+    return __uint_as_float((unsigned int)reinterpret_cast<const volatile unsigned short*>(p)[i] << 16);
+}
+template <> __device__ __forceinline__ float load_elem<RED_F16>(const void* p, unsigned long long i) {
+    unsigned short b = reinterpret_cast<const volatile unsigned short*>(p)[i];
+    return __half2float(*reinterpret_cast<const __half*>(&b));
+}
+template <> __device__ __forceinline__ float load_elem<RED_F32>(const void* p, unsigned long long i) {
+    return reinterpret_cast<const volatile float*>(p)[i];
+}
+template <int DT> __device__ __forceinline__ void store_elem(void* p, unsigned long long i, float acc);
+template <> __device__ __forceinline__ void store_elem<RED_BF16>(void* p, unsigned long long i, float acc) {
+    __nv_bfloat16 h = __float2bfloat16_rn(acc);
+    reinterpret_cast<unsigned short*>(p)[i] = *reinterpret_cast<unsigned short*>(&h);
+}
+template <> __device__ __forceinline__ void store_elem<RED_F16>(void* p, unsigned long long i, float acc) {
+    __half h = __float2half_rn(acc);
+    unsigned short b = *reinterpret_cast<unsigned short*>(&h);
+    if (acc != acc) b = 0x7fff;
+    reinterpret_cast<unsigned short*>(p)[i] = b;
+}
+template <> __device__ __forceinline__ void store_elem<RED_F32>(void* p, unsigned long long i, float acc) {
+    reinterpret_cast<unsigned int*>(p)[i] = canon_f32(acc);
+}
+
+// dynamic smem: const void* sp[R]; void* rp[R]
+template <int DT, int CH>
+__global__ void __launch_bounds__(REDUCE_THREADS) reduce_kernel(const ReduceArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const unsigned char** sp = reinterpret_cast<const unsigned char**>(smem_raw);
+    unsigned char** rp = reinterpret_cast<unsigned char**>(smem_raw) + a.R;
+    __shared__ int sMis;
+    const int R = a.R;
+    constexpr int ES = DT == RED_F32 ? 4 : 2;
+    constexpr int EPV = 16 / ES;
+
+    if (threadIdx.x == 0) sMis = 0;
+    __syncthreads();
+    int mis = 0;
+    for (int k = threadIdx.x; k < R; k += REDUCE_THREADS) {
+        const unsigned char* s = reinterpret_cast<const unsigned char*>(a.send[k]);
+        unsigned char* r = reinterpret_cast<unsigned char*>(a.recv[k]);
+        sp[k] = s; rp[k] = r;
+        mis |= (int)(((unsigned long long)s | (unsigned long long)r) & 15ull);
+    }
+    if (mis) atomicOr(&sMis, 1);
+    __syncthreads();
+    const unsigned long long n = a.blockElems;
+    const int nblocks = a.scatter ? R : 1;
+    const bool vec = (sMis == 0) && (!a.scatter || ((n * ES) & 15ull) == 0);
+
+    if (vec) {
+        const unsigned long long nvec = n / EPV;                       // full vectors per block
+        const unsigned int tpb = (unsigned int)((nvec + REDUCE_THREADS - 1) / REDUCE_THREADS);
+        const unsigned long long ntiles = (unsigned long long)tpb * nblocks;
+        for (unsigned long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
+            const unsigned int blk = a.scatter ? (unsigned int)(t / tpb) : 0u;
+            const unsigned int tb = (unsigned int)(t - (unsigned long long)blk * tpb);
+            const unsigned long long v = (unsigned long long)tb * REDUCE_THREADS + threadIdx.x;
+            if (v < nvec) {
+                const unsigned long long inOff = ((unsigned long long)blk * nvec + v) * 16ull;   // n*ES % 16 == 0 when scatter
+                Acc<DT> acc;
+                for (int k0 = 0; k0 < R; k0 += CH) {
+                    uint4 x[CH];
+#pragma unroll
+                    for (int j = 0; j < CH; ++j)
+                        if (k0 + j < R) x[j] = ld_stream(reinterpret_cast<const uint4*>(sp[k0 + j] + inOff));
+#pragma unroll
+                    for (int j = 0; j < CH; ++j)
+                        if (k0 + j < R) { if (k0 + j == 0) acc.set(x[j]); else acc.add(x[j]); }
+                }
+                const uint4 o = acc.pack();
+                if (a.scatter) {
+                    st_stream(reinterpret_cast<uint4*>(rp[blk] + v * 16ull), o);
+                } else {
+                    for (int r = 0; r < R; ++r) st_stream(reinterpret_cast<uint4*>(rp[r] + v * 16ull), o);
+                }
+            }
+        }
+        // ragged tail of an AllReduce (count % EPV elements), scalar
+        if (!a.scatter && blockIdx.x == 0) {
+            const unsigned long long i = nvec * EPV + threadIdx.x;
+            if (i < n) {
+                float acc = load_elem<DT>(sp[0], i);
+                for (int k = 1; k < R; ++k) acc = __fadd_rn(acc, load_elem<DT>(sp[k], i));
+                for (int r = 0; r < R; ++r) store_elem<DT>(rp[r], i, acc);
+            }
+        }
+    } else {
+        // scalar path: any alignment, same arithmetic, one element per thread
+        const unsigned long long total = n * nblocks;
+        for (unsigned long long i = (unsigned long long)blockIdx.x * REDUCE_THREADS + threadIdx.x; i < total;
+             i += (unsigned long long)gridDim.x * REDUCE_THREADS) {
+            float acc = load_elem<DT>(sp[0], i);
+            for (int k = 1; k < R; ++k) acc = __fadd_rn(acc, load_elem<DT>(sp[k], i));
+            if (a.scatter) {
+                const unsigned long long blk = i / n;
+                store_elem<DT>(rp[blk], i - blk * n, acc);
+            } else {
+                for (int r = 0; r < R; ++r) store_elem<DT>(rp[r], i, acc);
+            }
+        }
+    }
+}
+
+}  // namespace ncclx

@@ -1,0 +1,246 @@
+"""-m gpu parity: ncclx_alltoallv_dev (C ABI) vs the CPU oracle, byte for byte over the FULL
+receive capacity (so writes past the packed end are caught), plus RC and the offset matrices."""
+import json
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import paper_2510_20171_b200 as nx
+from paper_2510_20171_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+from gpu_util import ES, NP_OF, SENT8, assert_a2a_matches, back, oracle_a2a, run_a2a, sentinel, to_dev  # noqa: E402
+
+
+@pytest.fixture(scope="module", autouse=True)
+def ctx():
+    assert torch.cuda.is_available()
+    nx.ncclx_init(1024, 0)
+    yield
+    nx.ncclx_finalize()
+
+
+@pytest.fixture(autouse=True)
+def default_params():
+    yield
+    nx.ncclx_set_param(nx.PARAM_COPY_CTAS_PER_SM, 1)
+    nx.ncclx_set_param(nx.PARAM_BULK_MIN_BYTES, 1024)
+    nx.ncclx_set_param(nx.PARAM_FORCE_VECTOR, 0)
+    nx.ncclx_set_param(nx.PARAM_BULK_TILE_SHIFT, 15)
+    nx.ncclx_set_param(nx.PARAM_VEC_TILE_SHIFT, 14)
+    nx.ncclx_set_param(nx.PARAM_SCAN_CTAS, 16)
+
+
+def make_send(C, dtype, seed=0):
+    return [W.np_values(int(np.maximum(np.asarray(C)[s], 0).sum()), dtype, seed + s) for s in range(np.asarray(C).shape[0])]
+
+
+def test_handworked_example(golden_dir):
+    g = json.load(open(os.path.join(golden_dir, "handworked_alltoallv.json")))
+    names = sorted({x for row in g["send"] for x in row})
+    code = {n: i + 1000 for i, n in enumerate(names)}
+    send = [np.array([code[x] for x in row], np.uint16) for row in g["send"]]
+    got, RC, (soff, roff), _ = run_a2a(send, g["C"], "bf16", slack_elems=0)
+    assert RC.tolist() == g["RC"] and soff.tolist() == g["soff"] and roff.tolist() == g["roff"]
+    for d in range(2):
+        assert got[d].tolist() == [code[x] for x in g["recv"][d]]
+
+
+def test_cfg1_and_inverse():
+    cfg = W.a2a_config(1)
+    C = cfg.counts
+    send = make_send(C, "bf16", 10)
+    got, RC = assert_a2a_matches(send, C, "bf16")
+    packed = [got[d][: int(C[:, d].sum())] for d in range(cfg.R)]
+    back_, RC2 = assert_a2a_matches(packed, RC, "bf16")
+    assert (RC2 == C).all()
+    for s in range(cfg.R):
+        assert back_[s][: send[s].size].tobytes() == send[s].tobytes()
+
+
+@pytest.mark.parametrize("R", [1, 2, 3, 5, 8, 17, 33, 64, 100, 128])
+@pytest.mark.parametrize("dtype", ["u8", "bf16", "f32"])
+def test_random_counts_any_alignment(R, dtype):
+    """Element-granular counts: segments start at arbitrary element offsets, so source and
+    destination misalignment differ; zero rows/columns included; spans several tiles and tails."""
+    rng = np.random.default_rng(R * 7 + ES[dtype])
+    hi = max(2, 3_000_000 // (R * R))
+    C = rng.integers(0, hi, (R, R))
+    C[rng.random((R, R)) < 0.3] = 0
+    if R > 2:
+        C[R // 2, :] = 0
+        C[:, R // 3] = 0
+    send = make_send(C, dtype, 3)
+    assert_a2a_matches(send, C, dtype)
+
+
+@pytest.mark.parametrize("mis_send,mis_recv", [(0, 0), (2, 2), (2, 6), (16, 32), (4, 0), (1, 3)])
+def test_misaligned_base_pointers(mis_send, mis_recv):
+    dtype = "u8" if (mis_send | mis_recv) & 1 else "bf16"
+    R = 6
+    rng = np.random.default_rng(5)
+    C = rng.integers(0, 70_000, (R, R)) * 8          # multiples of 16 B so only the bases misalign
+    send = make_send(C, dtype, 9)
+    got, RC, offs, status = run_a2a(send, C, dtype, mis_send=mis_send, mis_recv=mis_recv)
+    exp, eRC, *_ = oracle_a2a(send, C, dtype)
+    assert all(g.tobytes() == e.tobytes() for g, e in zip(got, exp)) and (RC == eRC).all()
+
+
+@pytest.mark.parametrize("rowbytes", [16, 256, 1024, 10240, 14336])
+def test_aligned_rows_mixed_sizes_bulk_and_vector(rowbytes):
+    """16B-aligned rows: segments above BULK_MIN_BYTES take cp.async.bulk, the rest the vector path;
+    includes segments of many tiles, exactly one tile, and zero."""
+    R = 16
+    rng = np.random.default_rng(rowbytes)
+    rows = rng.integers(0, max(2, (1 << 20) // rowbytes), (R, R))
+    rows[rng.random((R, R)) < 0.25] = 0
+    rows[0, 0] = (3 << 20) // rowbytes + 1           # a long one
+    rows[1, 2] = max(1, 32768 // rowbytes)           # ~ one tile
+    rows[2, 1] = 1
+    C = rows * (rowbytes // 2)
+    send = make_send(C, "bf16", 1)
+    assert_a2a_matches(send, C, "bf16")
+
+
+def test_ragged_bulk_tail_and_tiny_segments():
+    """Aligned sources/destinations but byte lengths not multiple of 16 (u8): the bulk path moves
+    floor16 and the engine copies the < 16 B tail; later segments become unaligned -> vector."""
+    R = 4
+    C = np.array([[40000 + 5, 16, 1, 0], [7, 131072 + 15, 3, 32768], [0, 0, 0, 0], [65536, 15, 17, 100001]])
+    send = make_send(C, "u8", 2)
+    assert_a2a_matches(send, C, "u8")
+    # first segment of every destination is 16B-aligned with ragged length: exercise bulk tail on each
+    C2 = np.zeros((R, R), np.int64)
+    C2[0] = [32768 * 3 + 9, 2048 + 1, 1024 + 15, 5000]
+    send = make_send(C2, "u8", 3)
+    assert_a2a_matches(send, C2, "u8")
+
+
+@pytest.mark.parametrize("param,value", [("FORCE_VECTOR", 1), ("COPY_CTAS_PER_SM", 2), ("COPY_CTAS_PER_SM", 4),
+                                         ("BULK_TILE_SHIFT", 12), ("BULK_TILE_SHIFT", 16), ("VEC_TILE_SHIFT", 10),
+                                         ("BULK_MIN_BYTES", 16), ("BULK_MIN_BYTES", 1 << 20), ("SCAN_CTAS", 1),
+                                         ("SCAN_CTAS", 64)])
+def test_launch_configurations_agree(param, value):
+    nx.ncclx_set_param(getattr(nx, "PARAM_" + param), value)
+    cfg = W.scaled_a2a(W.a2a_config(3), 64)
+    C = cfg.counts
+    send = make_send(C, "bf16", 4)
+    assert_a2a_matches(send, C, "bf16")
+
+
+def test_cfg5_small_messages_full_compare():
+    cfg = W.a2a_config(5)
+    C = cfg.counts
+    send = make_send(C, "bf16", 40)
+    got, RC = assert_a2a_matches(send, C, "bf16")
+    # by-bytes accounting (padding-free): bytes moved == sum of counts
+    assert sum(int(C[:, d].sum()) for d in range(cfg.R)) * 2 == int(cfg.rows.sum()) * 14336
+
+
+def test_uniform_counts_block_transpose():
+    R, c = 32, 4096
+    send = make_send(np.full((R, R), c), "f32", 8)
+    got, RC, _, _ = run_a2a(send, np.full((R, R), c), "f32", slack_elems=0)
+    exp = np.stack(send).reshape(R, R, c).swapaxes(0, 1)
+    for d in range(R):
+        assert got[d].tobytes() == exp[d].tobytes()
+
+
+def test_tagged_payload_closed_form():
+    cfg = W.a2a_config(1)
+    C = cfg.rows * 64
+    send = [W.tagged_payload_u32(s, int(C[s].sum())).view(np.float32) for s in range(cfg.R)]
+    got, *_ = run_a2a(send, C, "f32", slack_elems=0)
+    excl = np.cumsum(C, axis=1) - C
+    for d in range(cfg.R):
+        exp = np.concatenate([(np.uint32(s) << np.uint32(24)) | (np.uint32(excl[s, d]) + np.arange(C[s, d], dtype=np.uint32))
+                              for s in range(cfg.R)])
+        assert (got[d].view(np.uint32) == exp).all()
+
+
+def test_zero_matrix_negative_counts_and_R_limits():
+    R = 5
+    send = [W.np_values(8, "bf16", s) for s in range(R)]
+    got, RC, (soff, roff), status = run_a2a(send, np.zeros((R, R), np.int64), "bf16")
+    assert status == 0 and (RC == 0).all() and (soff == 0).all() and (roff == 0).all()
+    assert all((g.view(np.uint8) == SENT8).all() for g in got)
+    C = np.array([[2, -5], [1, 1]])
+    send = [W.np_values(2, "bf16", 0), W.np_values(2, "bf16", 1)]
+    assert_a2a_matches(send, C, "bf16")              # status == 1, negative treated as 0
+    assert nx.ncclx_device_status() == 0             # cleared by the read
+    t = torch.zeros(4, dtype=torch.int64, device="cuda")
+    with pytest.raises(nx.binding.NcclxError) as e:
+        nx.ncclx_alltoallv_dev(t, t, t, t, 2, "bf16")  # same count buffer for in and out
+    assert e.value.code == 1
+    with pytest.raises(nx.binding.NcclxError) as e:
+        nx.ncclx_alltoallv_dev(t, t, t, t[1:], 2000, "bf16")
+    assert e.value.code == 3
+    with pytest.raises(nx.binding.NcclxError) as e:
+        nx.ncclx_alltoallv_dev(t, t, t, t[1:], 2, 9)
+    assert e.value.code == 2
+
+
+@pytest.mark.parametrize("R", [256, 1024])
+def test_large_R(R):
+    rng = np.random.default_rng(R)
+    C = rng.integers(0, 40, (R, R))
+    C[rng.random((R, R)) < 0.5] = 0
+    C[1, 2] = 300_000
+    send = make_send(C, "bf16", 6)
+    assert_a2a_matches(send, C, "bf16")
+
+
+def test_graph_capture_counts_by_reference():
+    """counts may change until the collective executes.  Capture once with one
+    count matrix, rewrite the device-resident counts between replays, outputs must follow."""
+    R, width = 8, 256
+    rng = np.random.default_rng(11)
+    rowsA = rng.integers(0, 300, (R, R))
+    rowsB = rng.integers(0, 300, (R, R)); rowsB[rng.random((R, R)) < 0.4] = 0
+    rowsC = np.zeros((R, R), np.int64); rowsC[3, 5] = 299
+    cap_rows = 300 * R
+    send_np = [W.np_values(cap_rows * width, "bf16", 50 + s) for s in range(R)]
+    send = [to_dev(a) for a in send_np]
+    recv = [sentinel(cap_rows * width * 2) for _ in range(R)]
+    Cd = torch.from_numpy(rowsA * width).cuda()
+    RCd = torch.zeros_like(Cd)
+    st, rt = nx.device_ptr_table(send), nx.device_ptr_table(recv)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        nx.ncclx_alltoallv_dev(st, Cd, rt, RCd, R, "bf16")   # warm-up outside capture
+    torch.cuda.current_stream().wait_stream(side)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        nx.ncclx_alltoallv_dev(st, Cd, rt, RCd, R, "bf16")
+    import oracle
+    for rows in (rowsA, rowsB, rowsC, rowsA):
+        C = (rows * width).astype(np.int64)
+        for r in recv:
+            r.fill_(SENT8)
+        Cd.copy_(torch.from_numpy(C), non_blocking=True)       # stream-ordered rewrite of the metadata
+        graph.replay()
+        torch.cuda.synchronize()
+        exp = [np.full(cap_rows * width, 0xA5A5, np.uint16) for _ in range(R)]
+        RC, *_ = oracle.alltoallv(send_np, C, exp, "bf16", nthreads=4)
+        assert (RCd.cpu().numpy() == RC).all()
+        for d in range(R):
+            assert back(recv[d], "bf16").tobytes() == exp[d].tobytes()
+
+
+def test_host_buffer_form():
+    cfg = W.scaled_a2a(W.a2a_config(3), 128)
+    C = cfg.counts
+    R = cfg.R
+    send_np = make_send(C, "bf16", 70)
+    pinned = [torch.from_numpy(a.view(np.int16)).pin_memory() for a in send_np]
+    out = [torch.empty(int(C[:, d].sum()), dtype=torch.int16).pin_memory() for d in range(R)]
+    RCh = np.zeros((R, R), np.int64)
+    nx.ncclx_alltoallv_host(pinned, np.ascontiguousarray(C), out, RCh, R, "bf16")
+    exp, eRC, *_ = oracle_a2a(send_np, C, "bf16", slack_elems=0)
+    assert (RCh == eRC).all()
+    for d in range(R):
+        assert out[d].numpy().view(np.uint16).tobytes() == exp[d].tobytes()

@@ -1,0 +1,164 @@
+"""-m gpu parity: ncclx_allreduce_sum / ncclx_reducescatter_sum (C ABI) vs the CPU oracle,
+bit for bit (tolerance 0: fixed-order fp32 accumulation has one correct result)."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2510_20171_b200 as nx
+from paper_2510_20171_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+from gpu_util import ES, NP_OF, back, to_dev  # noqa: E402
+
+
+@pytest.fixture(scope="module", autouse=True)
+def ctx():
+    assert torch.cuda.is_available()
+    nx.ncclx_init(1024, 0)
+    yield
+    nx.ncclx_finalize()
+
+
+def gpu_allreduce(xs_np, dtype, mis=0, inplace=False):
+    R, n = len(xs_np), xs_np[0].size
+    xs = [to_dev(a, mis) for a in xs_np]
+    outs = xs if inplace else [torch.zeros(n * ES[dtype] + 64, dtype=torch.uint8, device="cuda")[mis:mis + n * ES[dtype]]
+                               for _ in range(R)]
+    nx.ncclx_allreduce_sum(nx.device_ptr_table(xs), nx.device_ptr_table(outs), n, R, dtype)
+    torch.cuda.synchronize()
+    return [back(o, dtype) for o in outs]
+
+
+def gpu_reducescatter(xs_np, dtype, mis=0):
+    R, N = len(xs_np), xs_np[0].size
+    n = N // R
+    xs = [to_dev(a, mis) for a in xs_np]
+    outs = [torch.zeros(n * ES[dtype] + 64, dtype=torch.uint8, device="cuda")[mis:mis + n * ES[dtype]] for _ in range(R)]
+    nx.ncclx_reducescatter_sum(nx.device_ptr_table(xs), nx.device_ptr_table(outs), n, R, dtype)
+    torch.cuda.synchronize()
+    return [back(o, dtype) for o in outs]
+
+
+def inject_specials(a: np.ndarray, dtype: str, seed: int) -> np.ndarray:
+    """Sprinkle inf / nan / subnormal / signed-zero bit patterns (reading 13/14 of DESIGN.md)."""
+    rng = np.random.default_rng(seed)
+    a = a.copy()
+    idx = rng.integers(0, a.size, max(1, a.size // 50))
+    if dtype == "f32":
+        pats = np.array([0x7F800000, 0xFF800000, 0x7FC00001, 0xFFFFFFFF, 1, 0x80000001, 0x007FFFFF, 0x80000000, 0], np.uint32)
+        a.view(np.uint32)[idx] = rng.choice(pats, idx.size)
+    elif dtype == "bf16":
+        pats = np.array([0x7F80, 0xFF80, 0x7FC1, 0xFFFF, 1, 0x8001, 0x007F, 0x8000, 0, 0x7F7F, 0xFF7F], np.uint16)
+        a[idx] = rng.choice(pats, idx.size)
+    else:
+        pats = np.array([0x7C00, 0xFC00, 0x7E01, 0xFFFF, 1, 0x8001, 0x03FF, 0x8000, 0, 0x7BFF, 0xFBFF], np.uint16)
+        a[idx] = rng.choice(pats, idx.size)
+    return a
+
+
+def test_golden_vectors(golden_dir):
+    for line in open(os.path.join(golden_dir, "bf16_sum_vectors.txt")):
+        line = line.split("#")[0].strip()
+        if not line:
+            continue
+        lhs, rhs = line.split("->")
+        ins, exp = [int(t, 16) for t in lhs.split()], int(rhs, 16)
+        for n in (1, 8, 9):                           # scalar-tail, vector, vector + tail
+            outs = gpu_allreduce([np.full(n, v, np.uint16) for v in ins], "bf16")
+            assert all((o == exp).all() for o in outs), (line, n, [hex(int(o[0])) for o in outs])
+
+
+def test_cfg2_allreduce_full():
+    cfg = W.reduce_config(2)
+    xs = [W.np_values(cfg.count, "bf16", cfg.seed * 100 + k) for k in range(cfg.R)]
+    got = gpu_allreduce(xs, "bf16")
+    exp = oracle.allreduce_sum(xs, "bf16", nthreads=8)
+    for r in range(cfg.R):
+        assert got[r].tobytes() == exp[r].tobytes()
+
+
+@pytest.mark.parametrize("R", [1, 2, 3, 4, 5, 8, 9, 16, 17, 40, 64])
+@pytest.mark.parametrize("dtype", ["bf16", "f32", "f16"])
+def test_random_R_ragged_sizes_with_specials(R, dtype):
+    n = 8 * 256 * 5 + 8 * 77 + 3                      # several tiles + ragged tile + scalar tail
+    xs = [inject_specials(W.np_values(n, dtype, 100 * R + k, 1.0 if k % 2 else 1e-3), dtype, k) for k in range(R)]
+    got = gpu_allreduce(xs, dtype)
+    exp = oracle.allreduce_sum(xs, dtype, nthreads=4)
+    for r in range(R):
+        assert got[r].tobytes() == exp[r].tobytes(), (R, dtype, r)
+
+
+@pytest.mark.parametrize("dtype", ["bf16", "f32", "f16"])
+@pytest.mark.parametrize("R,n", [(4, 8 * 1000), (16, 8 * 300 + 8), (3, 1001), (16, 5)])
+def test_reducescatter_matches_oracle_and_allreduce_slices(dtype, R, n):
+    xs = [inject_specials(W.np_values(R * n, dtype, 7 * R + k), dtype, 50 + k) for k in range(R)]
+    rs = gpu_reducescatter(xs, dtype)
+    ers = oracle.reducescatter_sum(xs, dtype, nthreads=4)
+    ar = gpu_allreduce(xs, dtype)
+    for r in range(R):
+        assert rs[r].tobytes() == ers[r].tobytes()
+        assert rs[r].tobytes() == ar[0][r * n:(r + 1) * n].tobytes()   # cross-API invariant
+        assert ar[r].tobytes() == ar[0].tobytes()
+
+
+@pytest.mark.parametrize("mis", [2, 4, 8, 6])
+def test_misaligned_pointers_scalar_path(mis):
+    R, n = 5, 4099
+    xs = [W.np_values(n, "bf16", 900 + k) for k in range(R)]
+    assert all(g.tobytes() == e.tobytes() for g, e in zip(gpu_allreduce(xs, "bf16", mis=mis), oracle.allreduce_sum(xs, "bf16")))
+    xs = [W.np_values(R * 1003, "bf16", 950 + k) for k in range(R)]
+    assert all(g.tobytes() == e.tobytes() for g, e in zip(gpu_reducescatter(xs, "bf16", mis=mis), oracle.reducescatter_sum(xs, "bf16")))
+
+
+def test_inplace_allreduce_and_all_bf16_patterns():
+    R, n = 8, 8 * 4096 + 5
+    xs = [W.np_values(n, "bf16", 300 + k) for k in range(R)]
+    got = gpu_allreduce(xs, "bf16", inplace=True)
+    exp = oracle.allreduce_sum(xs, "bf16", nthreads=4)
+    assert all(g.tobytes() == e.tobytes() for g, e in zip(got, exp))
+    allb = np.arange(65536, dtype=np.uint16)
+    assert gpu_allreduce([allb], "bf16")[0].tobytes() == oracle.allreduce_sum([allb], "bf16")[0].tobytes()
+    assert gpu_allreduce([allb], "f16")[0].tobytes() == oracle.allreduce_sum([allb], "f16")[0].tobytes()
+    # every bf16 pattern plus every other pattern shifted: exercises the final RNE over many exponents
+    b = np.roll(allb, 12345)
+    assert gpu_allreduce([allb, b], "bf16")[0].tobytes() == oracle.allreduce_sum([allb, b], "bf16")[0].tobytes()
+    assert gpu_allreduce([allb, b], "f16")[0].tobytes() == oracle.allreduce_sum([allb, b], "f16")[0].tobytes()
+
+
+def test_small_integer_sums_exact():
+    R, n = 64, 8 * 513
+    rng = np.random.default_rng(0)
+    ints = rng.integers(-2, 3, (R, n))
+    xs = [torch.from_numpy(ints[k].astype(np.float32)).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16) for k in range(R)]
+    got = gpu_allreduce(xs, "bf16")[0]
+    val = (got.astype(np.uint32) << 16).view(np.float32)
+    assert (val == ints.sum(axis=0)).all()
+
+
+def test_errors_and_noop():
+    t = torch.zeros(8, dtype=torch.int64, device="cuda")
+    nx.ncclx_allreduce_sum(t, t, 0, 2, "bf16")         # count == 0: no-op
+    with pytest.raises(nx.binding.NcclxError) as e:
+        nx.ncclx_allreduce_sum(t, t, 8, 2, "u8")
+    assert e.value.code == 2
+    with pytest.raises(nx.binding.NcclxError) as e:
+        nx.ncclx_reducescatter_sum(t, t, 8, 0, "bf16")
+    assert e.value.code == 1
+
+
+def test_host_buffer_forms():
+    R, n = 4, 8 * 5000
+    xs = [W.np_values(R * n, "bf16", 600 + k) for k in range(R)]
+    pin = [torch.from_numpy(a.view(np.int16)).pin_memory() for a in xs]
+    out_ar = [torch.empty(R * n, dtype=torch.int16).pin_memory() for _ in range(R)]
+    out_rs = [torch.empty(n, dtype=torch.int16).pin_memory() for _ in range(R)]
+    nx.ncclx_allreduce_sum_host(pin, out_ar, R * n, R, "bf16")
+    nx.ncclx_reducescatter_sum_host(pin, out_rs, n, R, "bf16")
+    exp = oracle.allreduce_sum(xs, "bf16", nthreads=4)
+    for r in range(R):
+        assert out_ar[r].numpy().view(np.uint16).tobytes() == exp[r].tobytes()
+        assert out_rs[r].numpy().view(np.uint16).tobytes() == exp[0][r * n:(r + 1) * n].tobytes()
