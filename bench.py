@@ -1,0 +1,451 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of the NCCLX on-device data path on B200.
+
+    python bench.py --gpus N --steps K --warmup W            (N>1: launched by torchrun, one rank per GPU)
+    python bench.py --impl reference --steps K --warmup W    (the CPU oracle on the host cores)
+
+A STEP is one pass of the whole hot path (a1-a6, r1, r2) over one batch of
+synthetic input at BASELINE.json's full sizes:
+    config 3  MoE dispatch AllToAllv, R=64, 16384 tokens x 5120 bf16 per rank, Zipf(1.1) top-1   (a1-a5)
+    config 3  the inverse (combine) AllToAllv                                                    (a6)
+    config 2  AllReduce sum, R=8, 4,194,304 bf16 per rank                                        (r1)
+    config 4  ReduceScatter sum, R=16, 268,435,456 bf16 per rank                                 (r2)
+metric = achieved HBM GB/s = algorithmic bytes (read + written) of the step / device time.
+Inputs (48.6 GiB touched per step) are far larger than the 126 MB L2, so every step is cold.
+Multi-GPU: the path does not shard across GPUs (north_star: one GPU) -> "replicas only": every
+rank runs the same step on its own data, no data-path collective; value = sum over ranks / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_2510_20171_b200 import workloads as W  # noqa: E402
+
+METRIC = "achieved HBM GB/s, AllToAllv-dev + sum-reduce hot path (cfg3 dispatch+combine, cfg2, cfg4)"
+NOMINAL_HBM_GBS = 8000.0
+FALLBACK_HBM_GBS = 6650.0
+GiB = 1 << 30
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._pump, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------ workloads
+class A2A:
+    """Device-resident AllToAllv problem: send/recv/back buffers, count matrices, pointer tables."""
+
+    def __init__(self, cfg: W.A2AConfig, torch, nx, with_back=True):
+        self.cfg, self.R = cfg, cfg.R
+        C = cfg.counts
+        self.C_host = C
+        es = W.ELEM_SIZE[cfg.dtype]
+        self.send_elems = [int(C[s].sum()) for s in range(cfg.R)]
+        self.recv_elems = [int(C[:, d].sum()) for d in range(cfg.R)]
+        self.bytes_one_way = sum(self.send_elems) * es
+        self.send = [W.torch_values(max(n, 8), cfg.dtype, cfg.seed * 1000 + s) for s, n in enumerate(self.send_elems)]
+        td = W.torch_dtype(cfg.dtype)
+        self.recv = [torch.empty(max(n, 8), dtype=td, device="cuda") for n in self.recv_elems]
+        self.back = [torch.empty(max(n, 8), dtype=td, device="cuda") for n in self.send_elems] if with_back else None
+        self.C = torch.from_numpy(C).cuda()
+        self.RC = torch.empty_like(self.C)
+        self.C2 = torch.empty_like(self.C)
+        self.st, self.rt = nx.device_ptr_table(self.send), nx.device_ptr_table(self.recv)
+        self.bt = nx.device_ptr_table(self.back) if with_back else None
+        self.nx = nx
+
+    def dispatch(self):
+        self.nx.ncclx_alltoallv_dev(self.st, self.C, self.rt, self.RC, self.R, self.cfg.dtype)
+
+    def combine(self):
+        self.nx.ncclx_alltoallv_dev(self.rt, self.RC, self.bt, self.C2, self.R, self.cfg.dtype)
+
+
+class Reduce:
+    def __init__(self, cfg: W.ReduceConfig, torch, nx, sets: int = 1):
+        self.cfg, self.R, self.nx = cfg, cfg.R, nx
+        td = W.torch_dtype(cfg.dtype)
+        es = W.ELEM_SIZE[cfg.dtype]
+        self.sets = []
+        for i in range(sets):
+            x = [W.torch_values(cfg.count, cfg.dtype, cfg.seed * 1000 + 17 * i + k, cfg.std) for k in range(cfg.R)]
+            n_out = cfg.count if cfg.kind == "allreduce" else cfg.count // cfg.R
+            y = [torch.empty(n_out, dtype=td, device="cuda") for _ in range(cfg.R)]
+            self.sets.append((x, y, nx.device_ptr_table(x), nx.device_ptr_table(y)))
+        self.n_out = n_out
+        self.bytes = cfg.R * cfg.count * es + cfg.R * n_out * es     # read + written
+
+    def run(self, i: int = 0):
+        x, y, xt, yt = self.sets[i % len(self.sets)]
+        if self.cfg.kind == "allreduce":
+            self.nx.ncclx_allreduce_sum(xt, yt, self.cfg.count, self.R, self.cfg.dtype)
+        else:
+            self.nx.ncclx_reducescatter_sum(xt, yt, self.n_out, self.R, self.cfg.dtype)
+
+
+def event_times_ms(torch, fn, iters, warm=3):
+    for _ in range(warm):
+        fn()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(iters)]
+    torch.cuda.synchronize()
+    for a, b in ev:
+        a.record(); fn(); b.record()
+    torch.cuda.synchronize()
+    return np.array([a.elapsed_time(b) for a, b in ev])
+
+
+def frac(gbs, peak):
+    return {"GBps": round(gbs, 1), "frac_of_measured": round(gbs / peak, 4), "frac_of_nominal_8TBps": round(gbs / NOMINAL_HBM_GBS, 4)}
+
+
+# ------------------------------------------------------------------------------------ CPU oracle leg
+def oracle_sample_step(state, nthreads):
+    import oracle
+    a, ar, rs = state["a2a"], state["ar"], state["rs"]
+    oracle.alltoallv(a["send"], a["C"], a["recv"], "bf16", nthreads)
+    RC = np.ascontiguousarray(a["C"].T)
+    oracle.alltoallv(a["recv"], RC, a["back"], "bf16", nthreads)
+    oracle.allreduce_sum(ar["x"], "bf16", nthreads, out=ar["y"])
+    oracle.reducescatter_sum(rs["x"], "bf16", nthreads, out=rs["y"])
+
+
+def oracle_sample_state(div=4):
+    """Bounded sample of the step's workload: config 3 with every (src,dst) row count // div, config 2
+    in full, config 4 with count // div elements per rank.  Values: N(0,1)/N(0,1e-3) bf16 bit patterns
+    from numpy (timing does not depend on values)."""
+    rng = np.random.default_rng(0)
+
+    def vals(n, std=1.0):
+        return (rng.standard_normal(n, dtype=np.float32) * np.float32(std)).view(np.uint32).__rshift__(16).astype(np.uint16)
+
+    c3 = W.scaled_a2a(W.a2a_config(3), div)
+    C = c3.counts
+    R = c3.R
+    a = {"C": C, "send": [vals(int(C[s].sum())) for s in range(R)],
+         "recv": [np.empty(int(C[:, d].sum()), np.uint16) for d in range(R)],
+         "back": [np.empty(int(C[s].sum()), np.uint16) for s in range(R)]}
+    c2 = W.reduce_config(2)
+    ar = {"x": [vals(c2.count) for _ in range(c2.R)], "y": [np.empty(c2.count, np.uint16) for _ in range(c2.R)]}
+    c4 = W.reduce_config(4)
+    n4 = c4.count // div
+    rs = {"x": [vals(n4, 1e-3) for _ in range(c4.R)], "y": [np.empty(n4 // c4.R, np.uint16) for _ in range(c4.R)]}
+    nbytes = 2 * 2 * sum(x.nbytes for x in a["send"]) + 2 * c2.R * c2.count * 2 + (c4.R * n4 * 2 + n4 * 2)
+    sample = (f"config 3 dispatch+combine with row counts // {div} ({sum(x.nbytes for x in a['send']) / GiB:.2f} GiB each way), "
+              f"config 2 in full, config 4 with {n4} elements per rank (1/{div})")
+    return {"a2a": a, "ar": ar, "rs": rs}, nbytes, sample
+
+
+def run_oracle_leg(steps, warmup, div=4):
+    cores = os.cpu_count() or 1
+    state, nbytes, sample = oracle_sample_state(div)
+    for _ in range(max(0, warmup)):
+        oracle_sample_step(state, cores)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle_sample_step(state, cores)
+    dt = (time.perf_counter() - t0) / steps
+    return {"value": round(nbytes / dt / 1e9, 3), "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": sample,
+            "s_per_sample_step": round(dt, 3)}, dt
+
+
+# ------------------------------------------------------------------------------------ main
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the per-config table (cfg1/cfg5 latency, cfg2 warm/cold)")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--latency-replays", type=int, default=10000)
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    config = {"workload": "cfg3 MoE dispatch+combine AllToAllv (R=64, 16384 tok x 5120 bf16, Zipf 1.1) + cfg2 AllReduce "
+                          "(R=8, 4Mi bf16) + cfg4 ReduceScatter (R=16, 256Mi bf16/rank); BASELINE.json configs[2],[1],[3]",
+              "bytes_per_step_GiB": None, "l2": "inputs larger than L2 (48.6 GiB touched per step vs 126 MB)",
+              "parallelism": f"replicas x{world} (path does not shard across GPUs)"}
+
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        cb, dt = run_oracle_leg(args.steps, args.warmup)
+        line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": "GB/s", "n_gpus": args.gpus,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(dt * 1e3, 2), "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic", "config": config,
+                "cpu_baseline": cb,
+                "e2e": {"value": cb["value"], "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                "gpu_launches": 0}
+        print(json.dumps(line))
+        return 0
+
+    import torch
+    import paper_2510_20171_b200 as nx
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    nx.ncclx_init(128, local_rank)
+    peak, peak_src = measured_peak()
+
+    a3 = A2A(W.a2a_config(3), torch, nx)
+    r2 = Reduce(W.reduce_config(2), torch, nx)
+    r4 = Reduce(W.reduce_config(4), torch, nx)
+    step_bytes = 2 * 2 * a3.bytes_one_way + r2.bytes + r4.bytes
+    config["bytes_per_step_GiB"] = round(step_bytes / GiB, 3)
+
+    def step():
+        a3.dispatch(); a3.combine(); r2.run(); r4.run()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(warmup):
+        step()
+    barrier()
+    # sanity outside the timed region: the combine must have restored every send buffer (round trip = identity)
+    assert all(torch.equal(b[:n], s[:n]) for b, s, n in zip(a3.back, a3.send, a3.send_elems)), "round trip broken"
+    assert torch.equal(a3.C2, a3.C) and torch.equal(a3.RC, a3.C.t().contiguous())
+
+    nx.ncclx_profile_reset()
+    nx.ncclx_set_param(nx.PARAM_PROFILE, 1)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = nx.ncclx_launch_count()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    launches = nx.ncclx_launch_count() - l0
+    clocks = sampler.stop()
+    ms_total = e0.elapsed_time(e1)
+    nx.ncclx_set_param(nx.PARAM_PROFILE, 0)
+    copy_ms, copy_n = nx.ncclx_profile_read(nx.KERNEL_COPY)
+    red_ms, red_n = nx.ncclx_profile_read(nx.KERNEL_REDUCE)
+    cnt_ms, cnt_n = nx.ncclx_profile_read(nx.KERNEL_COUNTS)
+    nx.ncclx_profile_reset()
+
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * step_bytes / (ms_step * 1e-3) / 1e9
+
+    copy_avg_ms = copy_ms / max(copy_n, 1)
+    copy_gbs = 2 * a3.bytes_one_way / (copy_avg_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "segment_copy_kernel", "achieved": round(copy_gbs, 1), "peak": peak,
+                "unit": "GB/s", "frac": round(copy_gbs / peak, 4), "peak_source": peak_src,
+                "frac_of_nominal_8TBps": round(copy_gbs / NOMINAL_HBM_GBS, 4),
+                "algorithmic_bytes_per_launch": 2 * a3.bytes_one_way, "avg_launch_ms": round(copy_avg_ms, 4),
+                "launches_timed": copy_n, "share_of_step": round(copy_ms / ms_total, 4),
+                "traffic": None,
+                "other_kernels": {"reduce_kernel": {"avg_ms": round(red_ms / max(red_n, 1), 4), "launches": red_n,
+                                                    "share_of_step": round(red_ms / ms_total, 4)},
+                                  "counts_kernel": {"avg_ms": round(cnt_ms / max(cnt_n, 1), 5), "launches": cnt_n,
+                                                    "share_of_step": round(cnt_ms / ms_total, 5)}}}
+    tr = os.path.join(ROOT, "profiles", "traffic.json")       # dram bytes per launch from the committed ncu capture
+    if os.path.exists(tr):
+        try:
+            roofline["traffic"] = json.load(open(tr)).get("segment_copy_kernel_cfg3_bytes_per_launch")
+        except Exception:
+            pass
+
+    line = {"metric": METRIC, "value": round(value, 1), "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+            "warmup": warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16", "data": "synthetic", "config": config, "clocks": clocks,
+            "gpu_launches": int(launches), "roofline": roofline,
+            "frac_of_measured_peak": round(value / world / peak, 4),
+            "frac_of_nominal_8TBps": round(value / world / NOMINAL_HBM_GBS, 4)}
+
+    # ---- per-config table (rank 0, N=1 only): the five BASELINE.json configs one by one --------------------
+    if rank == 0 and world == 1 and not args.no_extras:
+        per = {}
+        t = event_times_ms(torch, a3.dispatch, 10)
+        per["cfg3_dispatch"] = {"ms_median": round(float(np.median(t)), 4), "ms_min": round(float(t.min()), 4),
+                                **frac(2 * a3.bytes_one_way / (np.median(t) * 1e-3) / 1e9, peak)}
+        t = event_times_ms(torch, a3.combine, 10)
+        per["cfg3_combine"] = {"ms_median": round(float(np.median(t)), 4), "ms_min": round(float(t.min()), 4),
+                               **frac(2 * a3.bytes_one_way / (np.median(t) * 1e-3) / 1e9, peak)}
+        t = event_times_ms(torch, r4.run, 10)
+        per["cfg4_reducescatter"] = {"ms_median": round(float(np.median(t)), 4), "ms_min": round(float(t.min()), 4),
+                                     **frac(r4.bytes / (np.median(t) * 1e-3) / 1e9, peak)}
+        r2c = Reduce(W.reduce_config(2), torch, nx, sets=6)     # 6 x 128 MiB rotating sets > L2: cold
+        it = [0]
+
+        def cold():
+            r2c.run(it[0]); it[0] += 1
+        t = event_times_ms(torch, cold, 120, warm=12)
+        per["cfg2_allreduce_cold"] = {"us_median": round(float(np.median(t)) * 1e3, 2), **frac(r2.bytes / (np.median(t) * 1e-3) / 1e9, peak)}
+        t = event_times_ms(torch, r2.run, 100, warm=10)
+        per["cfg2_allreduce_warm_L2"] = {"us_median": round(float(np.median(t)) * 1e3, 2), **frac(r2.bytes / (np.median(t) * 1e-3) / 1e9, peak)}
+        del r2c
+        for idx, reps in ((1, 1000), (5, args.latency_replays)):
+            a = A2A(W.a2a_config(idx), torch, nx, with_back=False)
+            a.dispatch(); torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                a.dispatch()
+            t = event_times_ms(torch, g.replay, reps, warm=20)
+            p50 = float(np.percentile(t, 50))
+            per[f"cfg{idx}_graph_replay"] = {"replays": reps, "p50_us": round(p50 * 1e3, 2), "p99_us": round(float(np.percentile(t, 99)) * 1e3, 2),
+                                             "mean_us": round(float(t.mean()) * 1e3, 2), "bytes_each_way": a.bytes_one_way,
+                                             **frac(2 * a.bytes_one_way / (p50 * 1e-3) / 1e9, peak)}
+            del a, g
+        line["per_config"] = per
+
+    # ---- e2e: same step through the host-buffer C ABI (H2D + kernels + D2H inside the timed region) --------
+    if not args.no_e2e:
+        line["e2e"] = run_e2e(torch, nx, a3, r2, r4, step_bytes, world, rank, min(args.steps, 3))
+
+    # ---- CPU oracle baseline on the host cores (rank 0, N=1 only) --------------------------------------------
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cb, _ = run_oracle_leg(2, 1)
+        line["cpu_baseline"] = cb
+
+    if rank == 0:
+        print(json.dumps(line))
+    nx.ncclx_finalize()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def run_e2e(torch, nx, a3, r2, r4, step_bytes, world, rank, steps):
+    """Host-buffer step: pinned host inputs -> ncclx_*_host (H2D, kernels, D2H, sync) -> pinned host outputs."""
+    import psutil
+    R3 = a3.R
+    need = 3 * a3.bytes_one_way + r4.cfg.R * r4.cfg.count * 2 + r4.n_out * r4.cfg.R * 2 + 2 * r2.cfg.R * r2.cfg.count * 2
+    avail = psutil.virtual_memory().available
+    try:
+        lim = int(open("/sys/fs/cgroup/memory.max").read())
+        cur = int(open("/sys/fs/cgroup/memory.current").read())
+        avail = min(avail, lim - cur)
+    except Exception:
+        pass
+    if need * world > 0.6 * avail:
+        return {"value": None, "unit": "GB/s", "skipped": f"needs {need * world / GiB:.0f} GiB pinned host memory, {avail / GiB:.0f} GiB available"}
+
+    def pin_like(ts, elems):
+        return [torch.empty(max(n, 8), dtype=t.dtype).pin_memory() for t, n in zip(ts, elems)]
+
+    h_send = pin_like(a3.send, a3.send_elems)
+    for h, d in zip(h_send, a3.send):
+        h.copy_(d)
+    h_recv = pin_like(a3.recv, a3.recv_elems)
+    h_back = pin_like(a3.back, a3.send_elems)
+    C = np.ascontiguousarray(a3.C_host)
+    RC = np.zeros_like(C)
+    C2 = np.zeros_like(C)
+    x2, y2 = r2.sets[0][0], r2.sets[0][1]
+    x4, y4 = r4.sets[0][0], r4.sets[0][1]
+    hx2 = [t.cpu().pin_memory() for t in x2]
+    hy2 = [torch.empty_like(t, device="cpu").pin_memory() for t in y2]
+    hx4 = [t.cpu().pin_memory() for t in x4]
+    hy4 = [torch.empty_like(t, device="cpu").pin_memory() for t in y4]
+    # free the device-resident copies: the host path stages through the library's own device buffers
+    h2d = 2 * a3.bytes_one_way + r2.cfg.R * r2.cfg.count * 2 + r4.cfg.R * r4.cfg.count * 2 + 2 * C.nbytes
+    d2h = 2 * a3.bytes_one_way + r2.cfg.R * r2.cfg.count * 2 + r4.cfg.R * r4.n_out * 2 + 2 * C.nbytes
+
+    def estep():
+        nx.ncclx_alltoallv_host(h_send, C, h_recv, RC, R3, "bf16")
+        nx.ncclx_alltoallv_host(h_recv, RC, h_back, C2, R3, "bf16")
+        nx.ncclx_allreduce_sum_host(hx2, hy2, r2.cfg.count, r2.cfg.R, "bf16")
+        nx.ncclx_reducescatter_sum_host(hx4, hy4, r4.n_out, r4.cfg.R, "bf16")
+
+    estep()
+    torch.cuda.synchronize()
+    ok = all(torch.equal(b[:n], s[:n]) for b, s, n in zip(h_back, h_send, a3.send_elems)) and (C2 == C).all()
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        estep()
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = float(t.item())
+    return {"value": round(world * step_bytes / (dt / steps) / 1e9, 2), "unit": "GB/s", "steps": steps,
+            "ms_per_step": round(dt / steps * 1e3, 2), "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+            "roundtrip_identity": bool(ok), "api": "ncclx_alltoallv_host x2 + ncclx_allreduce_sum_host + ncclx_reducescatter_sum_host"}
+
+
+if __name__ == "__main__":
+    sys.exit(main())
