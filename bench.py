@@ -212,7 +212,7 @@ def run_oracle_leg(steps, warmup, div=4):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
@@ -318,10 +318,13 @@ def main():
                                                     "share_of_step": round(red_ms / ms_total, 4)},
                                   "counts_kernel": {"avg_ms": round(cnt_ms / max(cnt_n, 1), 5), "launches": cnt_n,
                                                     "share_of_step": round(cnt_ms / ms_total, 5)}}}
-    tr = os.path.join(ROOT, "profiles", "traffic.json")       # dram bytes per launch from the committed ncu capture
+    tr = os.path.join(ROOT, "profiles", "traffic.csv")        # dram bytes per launch from the committed ncu capture
     if os.path.exists(tr):
         try:
-            roofline["traffic"] = json.load(open(tr)).get("segment_copy_kernel_cfg3_bytes_per_launch")
+            import csv
+            for row in csv.DictReader(open(tr)):
+                if row["kernel"] == "segment_copy_kernel" and row["workload"] == "cfg3_dispatch":
+                    roofline["traffic"] = int(row["bytes_per_launch"])
         except Exception:
             pass
 
