@@ -174,9 +174,14 @@ def oracle_sample_state(div=4):
     in full, config 4 with count // div elements per rank.  Values: N(0,1)/N(0,1e-3) bf16 bit patterns
     from numpy (timing does not depend on values)."""
     rng = np.random.default_rng(0)
+    block = {}
 
     def vals(n, std=1.0):
-        return (rng.standard_normal(n, dtype=np.float32) * np.float32(std)).view(np.uint32).__rshift__(16).astype(np.uint16)
+        # one 16 Mi-element N(0,std) bf16 block, tiled: the oracle's timing does not depend on the values
+        if std not in block:
+            f = rng.standard_normal(1 << 24, dtype=np.float32) * np.float32(std)
+            block[std] = (f.view(np.uint32) >> 16).astype(np.uint16)
+        return np.resize(block[std], n)
 
     c3 = W.scaled_a2a(W.a2a_config(3), div)
     C = c3.counts
@@ -206,6 +211,37 @@ def run_oracle_leg(steps, warmup, div=4):
     dt = (time.perf_counter() - t0) / steps
     return {"value": round(nbytes / dt / 1e9, 3), "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": sample,
             "s_per_sample_step": round(dt, 3)}, dt
+
+
+# ------------------------------------------------------------------------------------ multi-rank host logic
+def init_dist(world: int, local_rank: int, backend: str = "nccl"):
+    """One process per GPU; rendezvous on 127.0.0.1 (env MASTER_* / RANK / WORLD_SIZE from torchrun)."""
+    if world <= 1:
+        return None
+    import torch
+    import torch.distributed as dist
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    os.environ.setdefault("MASTER_PORT", "29517")
+    if backend == "nccl":
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    else:
+        dist.init_process_group(backend)
+    return dist
+
+
+def max_over_ranks(x: float, dist, device="cpu") -> float:
+    """Device time of the job = the slowest rank's."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, step_bytes: int, ms_step: float) -> float:
+    """Replicas only: every rank moves step_bytes per step; GB/s of the whole job."""
+    return world * step_bytes / (ms_step * 1e-3) / 1e9
 
 
 # ------------------------------------------------------------------------------------ main
@@ -249,10 +285,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     torch.cuda.set_device(local_rank)
-    if world > 1:
-        import torch.distributed as dist
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dist = init_dist(world, local_rank, "nccl")
     nx.ncclx_init(128, local_rank)
     peak, peak_src = measured_peak()
 
@@ -267,7 +300,7 @@ def main():
 
     def barrier():
         torch.cuda.synchronize()
-        if world > 1:
+        if dist is not None:
             dist.barrier()
             torch.cuda.synchronize()
 
@@ -299,12 +332,9 @@ def main():
     cnt_ms, cnt_n = nx.ncclx_profile_read(nx.KERNEL_COUNTS)
     nx.ncclx_profile_reset()
 
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, dist, "cuda")
     ms_step = ms_total / args.steps
-    value = world * step_bytes / (ms_step * 1e-3) / 1e9
+    value = whole_job_value(world, step_bytes, ms_step)
 
     copy_avg_ms = copy_ms / max(copy_n, 1)
     copy_gbs = 2 * a3.bytes_one_way / (copy_avg_ms * 1e-3) / 1e9
@@ -373,7 +403,7 @@ def main():
 
     # ---- e2e: same step through the host-buffer C ABI (H2D + kernels + D2H inside the timed region) --------
     if not args.no_e2e:
-        line["e2e"] = run_e2e(torch, nx, a3, r2, r4, step_bytes, world, rank, min(args.steps, 3))
+        line["e2e"] = run_e2e(torch, nx, a3, r2, r4, step_bytes, world, dist, min(args.steps, 3))
 
     # ---- CPU oracle baseline on the host cores (rank 0, N=1 only) --------------------------------------------
     if rank == 0 and world == 1 and not args.no_cpu:
@@ -383,12 +413,12 @@ def main():
     if rank == 0:
         print(json.dumps(line))
     nx.ncclx_finalize()
-    if world > 1:
+    if dist is not None:
         dist.destroy_process_group()
     return 0
 
 
-def run_e2e(torch, nx, a3, r2, r4, step_bytes, world, rank, steps):
+def run_e2e(torch, nx, a3, r2, r4, step_bytes, world, dist, steps):
     """Host-buffer step: pinned host inputs -> ncclx_*_host (H2D, kernels, D2H, sync) -> pinned host outputs."""
     import psutil
     R3 = a3.R
@@ -433,19 +463,14 @@ def run_e2e(torch, nx, a3, r2, r4, step_bytes, world, rank, steps):
     estep()
     torch.cuda.synchronize()
     ok = all(torch.equal(b[:n], s[:n]) for b, s, n in zip(h_back, h_send, a3.send_elems)) and (C2 == C).all()
-    if world > 1:
-        import torch.distributed as dist
+    if dist is not None:
         dist.barrier()
     t0 = time.perf_counter()
     for _ in range(steps):
         estep()
     torch.cuda.synchronize()
-    dt = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dt = float(t.item())
-    return {"value": round(world * step_bytes / (dt / steps) / 1e9, 2), "unit": "GB/s", "steps": steps,
+    dt = max_over_ranks(time.perf_counter() - t0, dist, "cuda")
+    return {"value": round(whole_job_value(world, step_bytes, dt / steps * 1e3), 2), "unit": "GB/s", "steps": steps,
             "ms_per_step": round(dt / steps * 1e3, 2), "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
             "roundtrip_identity": bool(ok), "api": "ncclx_alltoallv_host x2 + ncclx_allreduce_sum_host + ncclx_reducescatter_sum_host"}
 
