@@ -255,6 +255,8 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the per-config table (cfg1/cfg5 latency, cfg2 warm/cold)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--latency-replays", type=int, default=10000)
+    ap.add_argument("--probe", type=int, default=0, choices=[0, 1, 2, 3, 4, 5],
+                    help="run ONLY BASELINE.json config N eagerly for --steps iterations (for ncu captures of one config)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -288,6 +290,9 @@ def main():
     dist = init_dist(world, local_rank, "nccl")
     nx.ncclx_init(128, local_rank)
     peak, peak_src = measured_peak()
+
+    if args.probe:
+        return probe(args, torch, nx, peak)
 
     a3 = A2A(W.a2a_config(3), torch, nx)
     r2 = Reduce(W.reduce_config(2), torch, nx)
@@ -415,6 +420,26 @@ def main():
     nx.ncclx_finalize()
     if dist is not None:
         dist.destroy_process_group()
+    return 0
+
+
+def probe(args, torch, nx, peak):
+    """One config, eager launches, CUDA-event time per call (the command ncu captures are taken from)."""
+    n = args.probe
+    if n in (1, 3, 5):
+        w = A2A(W.a2a_config(n), torch, nx, with_back=False)
+        fn, nbytes = w.dispatch, 2 * w.bytes_one_way
+    else:
+        w = Reduce(W.reduce_config(n), torch, nx, sets=6 if n == 2 else 1)
+        it = [0]
+
+        def fn():
+            w.run(it[0]); it[0] += 1
+        nbytes = w.bytes
+    t = event_times_ms(torch, fn, args.steps, warm=max(args.warmup, 3))
+    print(json.dumps({"probe": f"cfg{n}", "calls": args.steps, "us_median": round(float(np.median(t)) * 1e3, 2),
+                      "us_min": round(float(t.min()) * 1e3, 2), **frac(nbytes / (np.median(t) * 1e-3) / 1e9, peak)}))
+    nx.ncclx_finalize()
     return 0
 
 

@@ -158,6 +158,11 @@ typedef enum {
     NCCLX_PARAM_FORCE_VECTOR = 5,     /* 1: send every segment down the vector path (for A/B runs)     */
     NCCLX_PARAM_BULK_TILE_SHIFT = 6,  /* log2 bytes of a bulk tile = one smem ring stage (12..16), default 15 */
     NCCLX_PARAM_VEC_TILE_SHIFT = 7,   /* log2 bytes of a vector-path tile (10..20), default 14          */
+    NCCLX_PARAM_PDL = 8,              /* 1 (default): launch the copy kernel with programmatic dependent   */
+                                      /* launch so its prologue overlaps the counts kernel; 0: plain order */
+    NCCLX_PARAM_COPY_STATIC_EIGHTHS = 9, /* 0..8: share of copy tiles assigned statically per engine, default 0 */
+    NCCLX_PARAM_COPY_KMAX = 10,       /* max tiles per dynamic claim when segments are short (1..64), default 6 */
+    NCCLX_PARAM_COPY_KMAX_LONG = 11,  /* same when segments average >= 8 tiles (1..64), default 2          */
     NCCLX_PARAM_COUNT_
 } ncclx_param_t;
 

@@ -24,6 +24,10 @@ PARAM_PROFILE = 4
 PARAM_FORCE_VECTOR = 5
 PARAM_BULK_TILE_SHIFT = 6
 PARAM_VEC_TILE_SHIFT = 7
+PARAM_PDL = 8
+PARAM_COPY_STATIC_EIGHTHS = 9
+PARAM_COPY_KMAX = 10
+PARAM_COPY_KMAX_LONG = 11
 
 KERNEL_COUNTS, KERNEL_COPY, KERNEL_REDUCE = 0, 1, 2
 

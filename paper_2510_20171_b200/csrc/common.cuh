@@ -39,6 +39,23 @@ struct Workspace {
 
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
 
+// Classification shared by the counts kernel (which builds the per-list tile prefixes) and the copy
+// kernel (which re-derives a segment's tile count from its descriptor): number of tiles the segment
+// contributes to work list L.  A segment is on exactly one list: BULK iff source and destination are
+// 16-byte aligned and it has at least bulkMinBytes bytes (and the vector path is not forced).
+struct ClassParams {
+    long long bulkMinBytes;
+    int forceVector;
+    int tileShift[2];
+};
+__device__ __forceinline__ int seg_tiles(int L, unsigned long long src, unsigned long long dst, long long bytes,
+                                         const ClassParams& cp) {
+    if (bytes <= 0) return 0;
+    const bool bulk = !cp.forceVector && (((src | dst) & 15ull) == 0) && bytes >= cp.bulkMinBytes;
+    if (bulk != (L == 0)) return 0;
+    return (int)((bytes + (1ll << cp.tileShift[L]) - 1) >> cp.tileShift[L]);
+}
+
 __device__ __forceinline__ long long warp_incl_scan(long long v) {
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -60,6 +77,13 @@ __device__ __forceinline__ long long warp_sum(long long v) {
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
+
+// ---- programmatic dependent launch (PDL) ------------------------------------------------------
+// The copy kernel is launched with programmatic stream serialization: its CTAs may become resident and
+// run their prologue while the counts kernel drains; griddep_wait() blocks until the counts grid has
+// completed and its writes are visible.  Both are no-ops when the launch carries no such attribute.
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 // ---- streaming global accesses --------------------------------------------------------------
 __device__ __forceinline__ uint4 ld_stream_nc(const uint4* p) {   // read-only for the whole kernel

@@ -23,41 +23,103 @@
 namespace ncclx {
 
 constexpr int COPY_THREADS = 512;          // warp 0: bulk engine; warps 1..15: vector engines
-constexpr int COPY_MAX_STAGES = 8;
-constexpr int COPY_KMAX_BULK = 16;         // max tiles per claim
-constexpr int COPY_KMAX_VEC = 8;
+constexpr int COPY_SLOTS = 16;             // outstanding bulk tiles per engine (mbarriers); <= 32
 
 struct CopyArgs {
     const SegDesc* desc;
     const int* colTiles[2];
     WorkCtl* ctl;
     int R;
-    int tileShift[2];
-    int stages;                            // ring stages of 2^tileShift[BULK] bytes
+    unsigned int ringBytes;                // shared-memory ring size, multiple of 128, >= 3 tiles
+    int staticEighths;                     // 0..8: share of the tiles assigned statically (contiguous per engine)
+    int kmax[2];                           // max tiles per dynamic claim, per list (short-segment regime)
+    int kmaxLong;                          // same, when segments average >= 8 tiles
+    ClassParams cls;
 };
 
-// Warp-uniform cursor over one work list.  All lanes hold identical state.
+// Warp-uniform cursor over one work list.  All lanes hold identical state except the descriptor
+// WINDOW: lane i caches descriptor q = qw + i of the destination-major table, and the next 32 are
+// prefetched into a second register set, so stepping from one segment to the next non-empty one of
+// this list is a ballot over registers instead of a chain of dependent L2 reads (config 5 has a new
+// segment every ~2 tiles).  Only a fresh claim pays the search: smem binary search over columns,
+// then a warp-wide 32-ary search over the column's tile prefixes.
 template <int L>
 struct Cursor {
     const SegDesc* desc;
     const int* colBase;                    // smem, R+1 entries, colBase[R] = total tiles
     unsigned int* counter;
-    int R, tileShift, total, nEngines, kmax;
+    ClassParams cls;
+    int R, RR, tileShift, total, nEngines, kmax, kmin;
+    int staticK, engineId;                 // first chunk is assigned statically: [engineId*staticK, +staticK)
+    int dynBase;                           // tiles >= dynBase are claimed dynamically
+    int pendCur, pendK;                    // lane 0: the NEXT chunk, claimed ahead of need (atomic in flight)
     int t, tEnd;                           // current tile, end of the claimed chunk
-    int segFirst, segEnd;                  // tile range of the current segment
+    int q, kInSeg, segTiles;               // current segment, tile within it, its tile count
     unsigned long long src, dst;
     long long bytes;
-    bool exhausted;
+    int qw, qn;                            // bases of the current / prefetched window
+    uint4 w0, w1, n0, n1;                  // this lane's descriptor in each window
+    bool first, exhausted, haveWindow, longSegs;
 
-    __device__ __forceinline__ void init(const CopyArgs& a, const int* colBase_, int nEngines_, int kmax_) {
-        desc = a.desc; colBase = colBase_; counter = &a.ctl->next[L];
-        R = a.R; tileShift = a.tileShift[L]; total = colBase_[a.R];
-        nEngines = nEngines_; kmax = kmax_;
-        t = tEnd = 0; segFirst = segEnd = 0; src = dst = 0; bytes = 0;
-        exhausted = (total == 0);
+    __device__ __forceinline__ void load_desc(int qq, uint4& a, uint4& b) const {
+        if (qq < RR) {
+            const uint4* p = reinterpret_cast<const uint4*>(desc + qq);
+            a = __ldg(p); b = __ldg(p + 1);
+        } else {
+            a = make_uint4(0, 0, 0, 0); b = make_uint4(0, 0, 0, 0);
+        }
+    }
+    __device__ __forceinline__ int my_tiles() const {
+        return seg_tiles(L, ((unsigned long long)w0.y << 32) | w0.x, ((unsigned long long)w0.w << 32) | w0.z,
+                         (long long)(((unsigned long long)w1.y << 32) | w1.x), cls);
+    }
+    __device__ __forceinline__ void take(int fromLane) {    // adopt the descriptor held by lane `fromLane`
+        const unsigned int sx = __shfl_sync(0xffffffffu, w0.x, fromLane), sy = __shfl_sync(0xffffffffu, w0.y, fromLane);
+        const unsigned int dx = __shfl_sync(0xffffffffu, w0.z, fromLane), dy = __shfl_sync(0xffffffffu, w0.w, fromLane);
+        const unsigned int bx = __shfl_sync(0xffffffffu, w1.x, fromLane), by = __shfl_sync(0xffffffffu, w1.y, fromLane);
+        src = ((unsigned long long)sy << 32) | sx;
+        dst = ((unsigned long long)dy << 32) | dx;
+        bytes = (long long)(((unsigned long long)by << 32) | bx);
+        segTiles = __shfl_sync(0xffffffffu, my_tiles(), fromLane);
+        q = qw + fromLane;
     }
 
-    // Find the segment that owns global tile index tt (0 <= tt < total).
+    __device__ __forceinline__ void init(const CopyArgs& a, const int* colBase_, int nEngines_, int engineId_, int kmax_) {
+        desc = a.desc; colBase = colBase_; counter = &a.ctl->next[L]; cls = a.cls;
+        R = a.R; RR = a.R * a.R; tileShift = a.cls.tileShift[L]; total = colBase_[a.R];
+        nEngines = nEngines_; engineId = engineId_;
+        // long segments (>= 8 tiles each on average): claims resolve inside the cached window, so take
+        // small chunks and keep all SMs in a tight moving window of HBM; short segments: every claim
+        // pays a search, amortise it over more tiles.
+        longSegs = total >= 8 * RR;
+        kmax = longSegs ? a.kmaxLong : kmax_;
+        // staticEighths/8 of the tiles can be split evenly and statically (contiguous range per engine);
+        // the rest is claimed dynamically, IN ORDER, in guided chunks.  Measured on B200: the in-order
+        // dynamic claim keeps all SMs inside one moving window of HBM and is ~7 % faster than contiguous
+        // static ranges (148 far-apart streams), so the default is fully dynamic (staticEighths = 0).
+        staticK = (int)(((long long)total * a.staticEighths / 8) / nEngines);
+        kmin = total >= 8 * nEngines ? 2 : 1;
+        dynBase = staticK * nEngines;
+        pendCur = pendK = 0;
+        t = tEnd = 0; q = 0; kInSeg = segTiles = 0; src = dst = 0; bytes = 0;
+        qw = qn = 0; w0 = w1 = n0 = n1 = make_uint4(0, 0, 0, 0);
+        first = true;
+        haveWindow = false;
+        exhausted = (total == 0);
+        if (!exhausted) claim_issue(dynBase);
+    }
+
+    // Lane 0 issues the atomic for the next dynamic chunk; the result is only consumed by claim_take(),
+    // so its L2 round trip overlaps the tiles of the current chunk.
+    __device__ __forceinline__ void claim_issue(int counterHint) {
+        if (lane_id() == 0) {
+            const int rem = total - min(total, counterHint);
+            pendK = max(kmin, min(kmax, rem / (2 * nEngines)));
+            pendCur = dynBase + (int)atomicAdd(counter, (unsigned int)pendK);
+        }
+    }
+
+    // Find the segment that owns global tile index tt (0 <= tt < total) and (re)load the windows there.
     __device__ __forceinline__ void locate(int tt) {
         const int lane = lane_id();
         int lo = 0, hi = R;                // colBase[lo] <= tt < colBase[hi]
@@ -66,57 +128,114 @@ struct Cursor {
             if (colBase[mid] <= tt) lo = mid; else hi = mid;
         }
         const int d = lo;
-        const int base = colBase[d];
-        const int tl = tt - base;
+        const int tl = tt - colBase[d];
         const SegDesc* col = desc + (size_t)d * R;
         int s0 = 0, n = R;                 // smallest s with col[s].pfx[L] > tl lies in [s0, s0+n)
-        while (n > 32) {
-            const int step = (n + 31) >> 5;
-            const int idx = s0 + min((lane + 1) * step, n) - 1;
-            const int v = __ldg(&col[idx].pfx[L]);
-            const int m = __popc(__ballot_sync(0xffffffffu, v <= tl));
+        while (n > 32) {                   // 128-ary rounds: every lane probes 4 block ends per L2 round trip
+            const int step = (n + 127) >> 7;
+            int cnt = 0;
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int b = lane * 4 + u;
+                const int idx = s0 + min((b + 1) * step, n) - 1;
+                cnt += (__ldg(&col[idx].pfx[L]) <= tl) ? 1 : 0;
+            }
+            int m = cnt;                   // blocks entirely <= tl (monotone, so a plain count)
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) m += __shfl_xor_sync(0xffffffffu, m, o);
             s0 += m * step;
             n = min(step, n - m * step);
         }
-        const int v = lane < n ? __ldg(&col[s0 + lane].pfx[L]) : 0x7fffffff;
-        const int m = __popc(__ballot_sync(0xffffffffu, v <= tl));
-        const int s = s0 + m;
-        const uint4* p = reinterpret_cast<const uint4*>(col + s);
-        const uint4 w0 = __ldg(p), w1 = __ldg(p + 1);
-        const int prev = s > 0 ? __ldg(&col[s - 1].pfx[L]) : 0;
-        src = ((unsigned long long)w0.y << 32) | w0.x;
-        dst = ((unsigned long long)w0.w << 32) | w0.z;
-        bytes = (long long)(((unsigned long long)w1.y << 32) | w1.x);
+        // last round doubles as the window load; the window starts one descriptor early so that the
+        // predecessor's prefix (needed for the tile index inside the segment) comes with it
+        const int sb = s0 > 0 ? s0 - 1 : 0;
+        const int nn = n + (s0 - sb);
+        qw = d * R + sb;
+        load_desc(qw + lane, w0, w1);
+        qn = qw + 32;
+        load_desc(qn + lane, n0, n1);
         const int pf = L == LIST_BULK ? (int)w1.z : (int)w1.w;
-        segFirst = base + prev;
-        segEnd = base + pf;
+        const int m = __popc(__ballot_sync(0xffffffffu, lane < nn && pf <= tl));
+        const int prevInWin = __shfl_sync(0xffffffffu, pf, m > 0 ? m - 1 : 0);
+        const int prev = m > 0 ? prevInWin : 0;
+        take(m);
+        kInSeg = tl - prev;
+    }
+
+    // Step to the next segment of this list (t stays inside the claimed chunk, so one exists).
+    __device__ __forceinline__ void advance_segment() {
+        int cl = q - qw;                   // lane that holds the current segment
+        while (true) {
+            const unsigned int later = cl >= 31 ? 0u : (0xffffffffu << (cl + 1));
+            const unsigned int mask = __ballot_sync(0xffffffffu, my_tiles() > 0) & later;
+            if (mask) { take(__ffs(mask) - 1); break; }
+            qw = qn; w0 = n0; w1 = n1;     // slide: prefetched window becomes current, prefetch the next
+            qn = qw + 32;
+            load_desc(qn + lane_id(), n0, n1);
+            cl = -1;
+            if (qw >= RR) { exhausted = true; break; }      // cannot happen while t < total
+        }
+        kInSeg = 0;
+    }
+
+    // Jump forward by `delta` tiles of this list using only the cached windows (current + prefetched):
+    // no memory round trip when the target lies within ~64 descriptors, which is the common case for
+    // in-order claims over long segments.  Returns false if the target is farther (caller searches).
+    __device__ __forceinline__ bool advance_by(int delta) {
+        const int rem = segTiles - kInSeg;
+        if (delta < rem) { kInSeg += delta; return true; }
+        delta -= rem;
+        int cl = q - qw;
+        for (int pass = 0; pass < 2; ++pass) {     // current window, then the already-prefetched one
+            const int mt = (lane_id() > cl) ? my_tiles() : 0;
+            const int incl = warp_incl_scan(mt);
+            const int tot = __shfl_sync(0xffffffffu, incl, 31);
+            if (delta < tot) {
+                const int l = __ffs(__ballot_sync(0xffffffffu, incl > delta)) - 1;
+                const int before = __shfl_sync(0xffffffffu, incl - mt, l);
+                take(l);
+                kInSeg = delta - before;
+                return true;
+            }
+            delta -= tot;
+            qw = qn; w0 = n0; w1 = n1;     // slide to the prefetched window, prefetch the next
+            qn = qw + 32;
+            load_desc(qn + lane_id(), n0, n1);
+            cl = -1;
+            if (qw >= RR) return false;
+        }
+        return false;
     }
 
     // Make (t, segment) valid; false when the list is drained.
     __device__ __forceinline__ bool ensure() {
         if (exhausted) return false;
         if (t < tEnd) {
-            if (t >= segEnd) locate(t);
-            return true;
+            if (kInSeg >= segTiles) advance_segment();
+            return !exhausted;
         }
-        int cur = 0, k = 0;
-        if (lane_id() == 0) {
-            const unsigned int seen = *reinterpret_cast<volatile unsigned int*>(counter);
-            const int rem = total - (int)min(seen, (unsigned int)total);
-            k = max(1, min(kmax, rem / (2 * nEngines)));
-            cur = (int)atomicAdd(counter, (unsigned int)k);
+        int cur, k;
+        if (first && staticK > 0) {        // static share: no atomic on the start-up path
+            first = false;
+            cur = engineId * staticK;
+            k = staticK;
+        } else {
+            first = false;
+            cur = __shfl_sync(0xffffffffu, pendCur, 0);
+            k = __shfl_sync(0xffffffffu, pendK, 0);
+            if (cur >= total || cur < 0) { exhausted = true; return false; }
+            claim_issue(cur + k);
         }
-        cur = __shfl_sync(0xffffffffu, cur, 0);
-        k = __shfl_sync(0xffffffffu, k, 0);
-        if (cur >= total) { exhausted = true; return false; }
+        const bool near = longSegs && haveWindow && cur >= t && advance_by(cur - t);
         t = cur;
         tEnd = min(cur + k, total);
-        locate(t);
+        if (!near) locate(t);
+        haveWindow = true;
         return true;
     }
 
-    __device__ __forceinline__ long long tile_off() const { return (long long)(t - segFirst) << tileShift; }
-    __device__ __forceinline__ void next() { ++t; }
+    __device__ __forceinline__ long long tile_off() const { return (long long)kInSeg << tileShift; }
+    __device__ __forceinline__ void next() { ++t; ++kInSeg; }
 };
 
 // ---- vector path -------------------------------------------------------------------------------
@@ -161,22 +280,24 @@ __device__ __forceinline__ void warp_copy_bytes(const unsigned char* src, unsign
     if (lane_id() < tail) dst[done + lane_id()] = __ldg(src + done + lane_id());
 }
 
-// dynamic smem layout: [ring: stages << tileShiftB][mbar: 8 x u64][stDst: 8 x u64][stLen: 8 x u32]
-//                      [colBase bulk: R+1 ints][colBase vec: R+1 ints]
+// dynamic smem layout: [ring: ringBytes][mbar: COPY_SLOTS x u64][colBase bulk: R+1 ints][colBase vec: R+1 ints]
 __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const CopyArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = lane_id();
     const int warp = threadIdx.x >> 5;
     const int R = a.R;
-    const size_t ringBytes = (size_t)a.stages << a.tileShift[LIST_BULK];
-    unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + ringBytes);
-    unsigned long long* stDst = mbar + COPY_MAX_STAGES;
-    unsigned int* stLen = reinterpret_cast<unsigned int*>(stDst + COPY_MAX_STAGES);
+    unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + a.ringBytes);
     int* colBase[2];
-    colBase[0] = reinterpret_cast<int*>(stLen + COPY_MAX_STAGES);
+    colBase[0] = reinterpret_cast<int*>(mbar + COPY_SLOTS);
     colBase[1] = colBase[0] + (R + 1);
 
-    // ---- prologue: cross-column tile bases (scan of R per-column totals), mbarrier init ------
+    // ---- prologue: mbarrier init (overlaps the counts kernel under PDL), then cross-column tile
+    //      bases = scan of the R per-column totals the counts kernel wrote -------------------------
+    if (warp == 2 && lane == 0) {
+        for (int i = 0; i < COPY_SLOTS; ++i) mbar_init(smem_u32(&mbar[i]), 1);
+        fence_mbar_init();
+    }
+    griddep_wait();
     if (warp < 2) {
         const int* ct = a.colTiles[warp];
         int* cb = colBase[warp];
@@ -188,24 +309,28 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
             if (c0 + lane < R) cb[c0 + lane + 1] = run + incl;
             run += __shfl_sync(0xffffffffu, incl, 31);
         }
-    } else if (warp == 2 && lane == 0) {
-        for (int i = 0; i < a.stages; ++i) mbar_init(smem_u32(&mbar[i]), 1);
-        fence_mbar_init();
     }
     __syncthreads();
 
     if (warp == 0) {
-        // ================= bulk engine: TMA ring driven by one elected lane ====================
+        // ================= bulk engine: byte-granular TMA ring driven by one elected lane ========
+        // The ring is a circular BYTE buffer (not fixed-size stages): every tile takes exactly
+        // align128(len) bytes, so short tiles (config 5: 10-28 KiB) keep as many bytes in flight as
+        // long ones.  Up to COPY_SLOTS tiles are outstanding; slot j's bookkeeping (destination,
+        // length, smem offset, virtual start) lives in the registers of lane j.
         Cursor<LIST_BULK> cur;
-        cur.init(a, colBase[LIST_BULK], (int)gridDim.x, COPY_KMAX_BULK);
-        const int S = a.stages;
-        const unsigned int tileBytes = 1u << a.tileShift[LIST_BULK];
+        cur.init(a, colBase[LIST_BULK], (int)gridDim.x, (int)blockIdx.x, a.kmax[LIST_BULK]);
+        const unsigned int tileBytes = 1u << a.cls.tileShift[LIST_BULK];
+        const unsigned int ringBytes = a.ringBytes;
         const uint32_t ring0 = smem_u32(smem);
-        int iLoad = 0, iStore = 0;
+        unsigned long long mDst = 0;          // slot registers (lane j <-> slot j)
+        unsigned int mLen = 0, mOff = 0, mV = 0;
+        unsigned int vHead = 0, phys = 0;     // virtual (mod 2^32) and physical allocation offsets
+        int iLoad = 0, iStore = 0, freed = 0;  // stores [0, freed) have finished reading their smem
         bool more = cur.ensure();
         while (true) {
-            // fill: issue loads while a stage is free (its previous store has finished READING smem)
-            while (more && iLoad < max(iStore - 1, 0) + S) {
+            // fill: issue loads while a slot and enough ring bytes are free
+            while (more) {
                 const long long off = cur.tile_off();
                 const long long rest = cur.bytes - off;
                 const unsigned int len = rest < (long long)tileBytes ? (unsigned int)rest : tileBytes;
@@ -213,14 +338,23 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
                 const unsigned char* srcp = reinterpret_cast<const unsigned char*>(cur.src + off);
                 unsigned char* dstp = reinterpret_cast<unsigned char*>(cur.dst + off);
                 if (len16) {
-                    const int st = iLoad % S;
+                    if (iLoad - freed >= COPY_SLOTS) break;
+                    const unsigned int pad = phys + len16 > ringBytes ? ringBytes - phys : 0u;   // wrap
+                    const unsigned int vTail = freed < iLoad ? __shfl_sync(0xffffffffu, mV, freed % COPY_SLOTS) : vHead;
+                    if (vHead + pad + len16 - vTail > ringBytes) break;
+                    const unsigned int vStart = vHead + pad;
+                    const unsigned int po = pad ? 0u : phys;
+                    const int slot = iLoad % COPY_SLOTS;
+                    if (lane == slot) { mDst = (unsigned long long)dstp; mLen = len16; mOff = po; mV = vStart; }
                     if (lane == 0) {
-                        stDst[st] = (unsigned long long)dstp;
-                        stLen[st] = len16;
-                        const uint32_t bar = smem_u32(&mbar[st]);
+                        const uint32_t bar = smem_u32(&mbar[slot]);
                         mbar_expect_tx(bar, len16);
-                        bulk_g2s(ring0 + ((uint32_t)st << a.tileShift[LIST_BULK]), srcp, len16, bar);
+                        bulk_g2s(ring0 + po, srcp, len16, bar);
                     }
+                    const unsigned int adv = (len16 + 127u) & ~127u;
+                    vHead = vStart + adv;
+                    phys = po + adv;
+                    if (phys >= ringBytes) phys = 0;
                     ++iLoad;
                 }
                 const int tail = (int)(len & 15u);        // only the last tile of a ragged segment
@@ -230,15 +364,25 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
             }
             if (iStore == iLoad) {
                 if (!more) break;
+                // every issued tile is stored but the next one does not fit behind the last store's
+                // not-yet-released bytes: release everything and restart the ring at offset 0
+                if (lane == 0) bulk_wait_read<0>();
+                freed = iStore;
+                phys = 0;
                 continue;
             }
-            const int st = iStore % S;
-            mbar_wait(smem_u32(&mbar[st]), (uint32_t)((iStore / S) & 1));
+            const int slot = iStore % COPY_SLOTS;
+            mbar_wait(smem_u32(&mbar[slot]), (uint32_t)((iStore / COPY_SLOTS) & 1));
+            const unsigned int dlo = __shfl_sync(0xffffffffu, (unsigned int)mDst, slot);
+            const unsigned int dhi = __shfl_sync(0xffffffffu, (unsigned int)(mDst >> 32), slot);
+            const unsigned int slen = __shfl_sync(0xffffffffu, mLen, slot);
+            const unsigned int soff = __shfl_sync(0xffffffffu, mOff, slot);
             if (lane == 0) {
-                bulk_s2g(reinterpret_cast<void*>(stDst[st]), ring0 + ((uint32_t)st << a.tileShift[LIST_BULK]), stLen[st]);
+                bulk_s2g(reinterpret_cast<void*>(((unsigned long long)dhi << 32) | dlo), ring0 + soff, slen);
                 bulk_commit();
-                if (more) bulk_wait_read<1>();            // frees the stage of store iStore-1
+                if (more) bulk_wait_read<1>();            // releases the smem of every store but this one
             }
+            freed = max(freed, iStore);                   // (only consulted while `more`)
             ++iStore;
             __syncwarp();
         }
@@ -246,8 +390,9 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
     } else {
         // ================= vector engines: one warp per tile ===================================
         Cursor<LIST_VEC> cur;
-        cur.init(a, colBase[LIST_VEC], (int)gridDim.x * (COPY_THREADS / 32 - 1), COPY_KMAX_VEC);
-        const long long tileBytes = 1ll << a.tileShift[LIST_VEC];
+        cur.init(a, colBase[LIST_VEC], (int)gridDim.x * (COPY_THREADS / 32 - 1),
+                 (int)blockIdx.x * (COPY_THREADS / 32 - 1) + warp - 1, a.kmax[LIST_VEC]);
+        const long long tileBytes = 1ll << a.cls.tileShift[LIST_VEC];
         while (cur.ensure()) {
             const long long off = cur.tile_off();
             const long long rest = cur.bytes - off;

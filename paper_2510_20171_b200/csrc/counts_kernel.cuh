@@ -11,12 +11,20 @@
 // row-wise send offset soff[s][d], is rebuilt by the owner from row s's prefix C[s][0..d0) (an
 // L2-resident re-read of at most R*R*8 bytes per CTA).  The cross-column tile base is left to
 // the copy kernel, which scans the R per-column totals itself.
+//
+// This kernel sits on the small-message latency path (config 5: ~5 % of the call), so all global
+// loads are issued up front with high memory-level parallelism: each warp sums ROWS_PER_PASS rows
+// at once (ROWS_PER_PASS independent loads per lane per step) and the pointer tables are staged
+// in shared memory while those loads fly; phase 2 then only reads shared memory and streams out
+// its results.
 #pragma once
 #include "common.cuh"
 
 namespace ncclx {
 
 constexpr int COUNTS_THREADS = 512;
+constexpr int COUNTS_ROWS_PER_PASS = 8;
+constexpr int COUNTS_COLS_UNROLL = 4;     // x32 lanes = 128 prefix columns per pass
 
 struct CountsArgs {
     const void* const* send;      // device table
@@ -27,61 +35,109 @@ struct CountsArgs {
     int R;
     int W;                        // columns per CTA (<= 32)
     int elemSize;
-    int tileShift[2];             // log2 tile bytes: bulk, vector
-    long long bulkMinBytes;       // >= 16; segments below it (or unaligned) go to the vector list
-    int forceVector;
+    ClassParams cls;
 };
 
-// dynamic smem: long long cval[R][W+1], sofs[R][W+1]   (+1: conflict-free column reads)
+// dynamic smem: long long cval[R][W+1], sofs[R][W+1] (+1: conflict-free column reads), u64 sendPtr[R], recvPtr[W]
 __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int R = a.R, W = a.W, P = W + 1;
     long long* cval = reinterpret_cast<long long*>(smem_raw);
     long long* sofs = cval + (size_t)R * P;
+    unsigned long long* sendPtr = reinterpret_cast<unsigned long long*>(sofs + (size_t)R * P);
+    unsigned long long* recvPtr = sendPtr + R;
 
     const int lane = lane_id();
     const int warp = threadIdx.x >> 5;
-    const int nwarps = COUNTS_THREADS / 32;
+    constexpr int nwarps = COUNTS_THREADS / 32;
+    constexpr int RB = COUNTS_ROWS_PER_PASS;
+    constexpr int DU = COUNTS_COLS_UNROLL;
     const int d0 = blockIdx.x * W;
     const int Wc = min(W, R - d0);
 
+    griddep_launch_dependents();                 // let the copy kernel's CTAs start their prologue
     if (blockIdx.x == 0 && threadIdx.x == 0) {   // the copy kernel follows on the same stream
         a.ws.ctl->next[0] = 0u;
         a.ws.ctl->next[1] = 0u;
     }
+    // pointer tables: issue the loads now, park them in shared memory only after phase 1's loads are
+    // in flight too (one DRAM round trip instead of two on a cold start)
+    constexpr int PT = 2;                        // covers R <= 1024 with 512 threads
+    unsigned long long sp[PT];
+#pragma unroll
+    for (int i = 0; i < PT; ++i) {
+        const int s = threadIdx.x + i * COUNTS_THREADS;
+        sp[i] = s < R ? (unsigned long long)a.send[s] : 0ull;
+    }
+    const unsigned long long rp = threadIdx.x < Wc ? (unsigned long long)a.recv[d0 + threadIdx.x] : 0ull;
+    bool parked = false;
 
-    // ---- phase 1: warp per source row s: soff for the owned columns -------------------------
+    // ---- phase 1: warp per group of RB source rows: soff for the owned columns ---------------
     bool sawNeg = false;
-    for (int s = warp; s < R; s += nwarps) {
-        const long long* row = a.C + (size_t)s * R;
-        long long part = 0;
-        for (int d = lane; d < d0; d += 32) {
-            long long c = row[d];
-            part += c > 0 ? c : 0;
+    for (int sb = warp * RB; sb < R; sb += nwarps * RB) {
+        long long part[RB], c[RB];
+#pragma unroll
+        for (int r = 0; r < RB; ++r) {
+            part[r] = 0;
+            c[r] = (sb + r < R && lane < Wc) ? a.C[(size_t)(sb + r) * R + d0 + lane] : 0;
         }
-        const long long base = warp_sum(part);
-        long long c = 0;
-        if (lane < Wc) {
-            c = row[d0 + lane];
-            if (c < 0) { sawNeg = true; c = 0; }
+        // prefix columns [0, d0): RB x DU independent loads are issued before any of them is consumed
+        for (int db = 0; db < d0; db += 32 * DU) {
+            long long v[RB][DU];
+#pragma unroll
+            for (int r = 0; r < RB; ++r) {
+#pragma unroll
+                for (int u = 0; u < DU; ++u) {
+                    const int d = db + u * 32 + lane;
+                    v[r][u] = (sb + r < R && d < d0) ? a.C[(size_t)(sb + r) * R + d] : 0;
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < RB; ++r) {
+#pragma unroll
+                for (int u = 0; u < DU; ++u) part[r] += v[r][u] > 0 ? v[r][u] : 0;
+            }
         }
-        const long long incl = warp_incl_scan(c);
-        if (lane < Wc) {
-            const long long so = base + incl - c;
-            cval[(size_t)s * P + lane] = c;
-            sofs[(size_t)s * P + lane] = so;
-            a.ws.soff[(size_t)s * R + d0 + lane] = so;
+        if (!parked) {                                            // every thread passes here at most once
+            parked = true;
+#pragma unroll
+            for (int i = 0; i < PT; ++i) {
+                const int s = threadIdx.x + i * COUNTS_THREADS;
+                if (s < R) sendPtr[s] = sp[i];
+            }
+            if (threadIdx.x < Wc) recvPtr[threadIdx.x] = rp;
         }
+#pragma unroll
+        for (int r = 0; r < RB; ++r) {
+            const int s = sb + r;
+            if (s >= R) break;                                    // warp-uniform
+            const long long base = warp_sum(part[r]);
+            long long cc = c[r];
+            if (cc < 0) { sawNeg = true; cc = 0; }
+            const long long incl = warp_incl_scan(cc);
+            if (lane < Wc) {
+                const long long so = base + incl - cc;
+                cval[(size_t)s * P + lane] = cc;
+                sofs[(size_t)s * P + lane] = so;
+                a.ws.soff[(size_t)s * R + d0 + lane] = so;
+            }
+        }
+    }
+    if (!parked) {                                                // warps that owned no row group
+#pragma unroll
+        for (int i = 0; i < PT; ++i) {
+            const int s = threadIdx.x + i * COUNTS_THREADS;
+            if (s < R) sendPtr[s] = sp[i];
+        }
+        if (threadIdx.x < Wc) recvPtr[threadIdx.x] = rp;
     }
     if (sawNeg) atomicOr(&a.ws.ctl->status, 1u);
     __syncthreads();
 
     // ---- phase 2: warp per owned destination column d: RC, roff, descriptors, tile prefixes --
-    const long long tileB = 1ll << a.tileShift[LIST_BULK];
-    const long long tileV = 1ll << a.tileShift[LIST_VEC];
     for (int j = warp; j < Wc; j += nwarps) {
         const int d = d0 + j;
-        const unsigned long long dstBase = (unsigned long long)a.recv[d];
+        const unsigned long long dstBase = recvPtr[j];
         long long run = 0;
         int runT[2] = {0, 0};
         for (int s0 = 0; s0 < R; s0 += 32) {
@@ -94,28 +150,22 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
             unsigned long long src = 0, dst = 0;
             int tb = 0, tv = 0;
             if (valid) {
-                src = (unsigned long long)a.send[s] + (unsigned long long)(sofs[(size_t)s * P + j] * a.elemSize);
+                src = sendPtr[s] + (unsigned long long)(sofs[(size_t)s * P + j] * a.elemSize);
                 dst = dstBase + (unsigned long long)(ro * a.elemSize);
-                if (bytes > 0) {
-                    const bool bulk = !a.forceVector && (((src | dst) & 15ull) == 0) && bytes >= a.bulkMinBytes;
-                    if (bulk) tb = (int)((bytes + tileB - 1) >> a.tileShift[LIST_BULK]);
-                    else      tv = (int)((bytes + tileV - 1) >> a.tileShift[LIST_VEC]);
-                }
+                tb = seg_tiles(LIST_BULK, src, dst, bytes, a.cls);
+                tv = seg_tiles(LIST_VEC, src, dst, bytes, a.cls);
             }
-            const int ib = warp_incl_scan(tb);
-            const int iv = warp_incl_scan(tv);
+            const long long it = warp_incl_scan(((long long)tb << 32) | (long long)(unsigned int)tv);   // both lists at once
+            const int ib = (int)(it >> 32);
+            const int iv = (int)(unsigned int)it;
             if (valid) {
                 const size_t q = (size_t)d * R + s;
                 a.RC[q] = c;
                 a.ws.roff[q] = ro;
-                SegDesc sd;
-                sd.src = src; sd.dst = dst; sd.bytes = bytes;
-                sd.pfx[LIST_BULK] = runT[0] + ib;
-                sd.pfx[LIST_VEC] = runT[1] + iv;
                 uint4* out = reinterpret_cast<uint4*>(a.ws.desc + q);
-                const uint4* in = reinterpret_cast<const uint4*>(&sd);
-                out[0] = in[0];
-                out[1] = in[1];
+                out[0] = make_uint4((unsigned int)src, (unsigned int)(src >> 32), (unsigned int)dst, (unsigned int)(dst >> 32));
+                out[1] = make_uint4((unsigned int)bytes, (unsigned int)((unsigned long long)bytes >> 32),
+                                    (unsigned int)(runT[0] + ib), (unsigned int)(runT[1] + iv));
             }
             run += __shfl_sync(0xffffffffu, incl, 31);
             runT[0] += __shfl_sync(0xffffffffu, ib, 31);

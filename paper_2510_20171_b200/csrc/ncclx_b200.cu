@@ -31,7 +31,7 @@ struct Context {
     Workspace ws{};
     void* wsBase = nullptr;
     // tunables
-    int64_t params[NCCLX_PARAM_COUNT_] = {1, 1024, 8, 16, 0, 0, 15, 14};
+    int64_t params[NCCLX_PARAM_COUNT_] = {1, 1024, 8, 16, 0, 0, 15, 14, 1, 0, 6, 2};
     // profiling
     std::vector<EventPair> events[NCCLX_KERNEL_COUNT_];
     std::atomic<int64_t> launches{0};
@@ -96,16 +96,17 @@ struct LaunchScope {
     }
 };
 
-size_t copySmemBytes(int stages, int tileShiftB, int R) {
-    return ((size_t)stages << tileShiftB) + COPY_MAX_STAGES * (8 + 8 + 4) + 2 * (size_t)(R + 1) * 4 + 16;
+size_t copyAuxBytes(int R) { return COPY_SLOTS * 8 + 2 * (size_t)(R + 1) * 4 + 16; }
+
+// Ring size: everything the SM has (per resident CTA) minus bookkeeping, rounded down to 128 B.
+unsigned int chooseRingBytes(int ctasPerSm, int R) {
+    size_t budget = (size_t)g.maxSmemOptin / ctasPerSm - (ctasPerSm > 1 ? 1024 : 0);
+    if (ctasPerSm == 1) budget -= 20 * 1024;      // leave room for a co-resident counts CTA (PDL overlap)
+    size_t ring = budget > copyAuxBytes(R) ? (budget - copyAuxBytes(R)) & ~(size_t)127 : 0;
+    return (unsigned int)ring;
 }
 
-int chooseStages(int ctasPerSm, int tileShiftB, int R) {
-    const size_t budget = (size_t)g.maxSmemOptin / ctasPerSm - (ctasPerSm > 1 ? 1024 : 0);
-    int s = COPY_MAX_STAGES;
-    while (s > 2 && copySmemBytes(s, tileShiftB, R) > budget) --s;
-    return s;
-}
+size_t countsSmemBytes(int R, int W) { return 2 * (size_t)R * (W + 1) * 8 + (size_t)(R + W) * 8; }
 
 int countsW(int R) {
     // columns per CTA: spread over at most SCAN_CTAS CTAs, at most 32 columns, and 2*R*(W+1)*8 <= smem
@@ -113,7 +114,7 @@ int countsW(int R) {
     if (W < 1) W = 1;
     if (W > 32) W = 32;
     const size_t budget = (size_t)g.maxSmemOptin - 1024;
-    while (W > 1 && 2 * (size_t)R * (W + 1) * 8 > budget) --W;
+    while (W > 1 && countsSmemBytes(R, W) > budget) --W;
     return W;
 }
 
@@ -124,11 +125,15 @@ int launchAllToAllv(const void* const* send, const int64_t* C, void* const* recv
     ca.C = reinterpret_cast<const long long*>(C);
     ca.RC = reinterpret_cast<long long*>(RC);
     ca.ws = g.ws; ca.R = R; ca.W = countsW(R); ca.elemSize = es;
-    ca.tileShift[0] = (int)g.params[NCCLX_PARAM_BULK_TILE_SHIFT]; ca.tileShift[1] = (int)g.params[NCCLX_PARAM_VEC_TILE_SHIFT];
-    ca.bulkMinBytes = g.params[NCCLX_PARAM_BULK_MIN_BYTES] < 16 ? 16 : g.params[NCCLX_PARAM_BULK_MIN_BYTES];
-    ca.forceVector = (int)g.params[NCCLX_PARAM_FORCE_VECTOR];
+    const int cps = (int)g.params[NCCLX_PARAM_COPY_CTAS_PER_SM];
+    const unsigned int ring = chooseRingBytes(cps, R);
+    ca.cls.tileShift[0] = (int)g.params[NCCLX_PARAM_BULK_TILE_SHIFT];
+    while (ca.cls.tileShift[0] > 10 && ((size_t)3 << ca.cls.tileShift[0]) > ring) --ca.cls.tileShift[0];   // >= 3 tiles fit
+    ca.cls.tileShift[1] = (int)g.params[NCCLX_PARAM_VEC_TILE_SHIFT];
+    ca.cls.bulkMinBytes = g.params[NCCLX_PARAM_BULK_MIN_BYTES] < 16 ? 16 : g.params[NCCLX_PARAM_BULK_MIN_BYTES];
+    ca.cls.forceVector = (int)g.params[NCCLX_PARAM_FORCE_VECTOR];
     const int G = (R + ca.W - 1) / ca.W;
-    const size_t csm = 2 * (size_t)R * (ca.W + 1) * 8;
+    const size_t csm = countsSmemBytes(R, ca.W);
     {
         LaunchScope ls(NCCLX_KERNEL_COUNTS, stream);
         counts_kernel<<<G, COUNTS_THREADS, csm, stream>>>(ca);
@@ -137,14 +142,26 @@ int launchAllToAllv(const void* const* send, const int64_t* C, void* const* recv
     CopyArgs cp{};
     cp.desc = g.ws.desc; cp.colTiles[0] = g.ws.colTiles[0]; cp.colTiles[1] = g.ws.colTiles[1];
     cp.ctl = g.ws.ctl; cp.R = R;
-    cp.tileShift[0] = ca.tileShift[0]; cp.tileShift[1] = ca.tileShift[1];
-    const int cps = (int)g.params[NCCLX_PARAM_COPY_CTAS_PER_SM];
-    cp.stages = chooseStages(cps, cp.tileShift[0], R);
-    const size_t smem = copySmemBytes(cp.stages, cp.tileShift[0], R);
+    cp.cls = ca.cls;
+    cp.ringBytes = ring;
+    cp.staticEighths = (int)g.params[NCCLX_PARAM_COPY_STATIC_EIGHTHS];
+    cp.kmax[0] = (int)g.params[NCCLX_PARAM_COPY_KMAX];
+    cp.kmax[1] = 8;
+    cp.kmaxLong = (int)g.params[NCCLX_PARAM_COPY_KMAX_LONG];
+    const size_t smem = (size_t)cp.ringBytes + copyAuxBytes(R);
     {
         LaunchScope ls(NCCLX_KERNEL_COPY, stream);
-        segment_copy_kernel<<<g.smCount * cps, COPY_THREADS, smem, stream>>>(cp);
-        CK(cudaGetLastError());
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)(g.smCount * cps));
+        cfg.blockDim = dim3(COPY_THREADS);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = g.params[NCCLX_PARAM_PDL] ? 1 : 0;
+        CK(cudaLaunchKernelEx(&cfg, segment_copy_kernel, cp));
     }
     return NCCLX_OK;
 }
@@ -444,6 +461,9 @@ int ncclx_set_param(int param, int64_t value) {
     case NCCLX_PARAM_SCAN_CTAS: if (value < 1 || value > 1024) return NCCLX_ERR_ARG; break;
     case NCCLX_PARAM_BULK_TILE_SHIFT: if (value < 12 || value > 16) return NCCLX_ERR_ARG; break;
     case NCCLX_PARAM_VEC_TILE_SHIFT: if (value < 10 || value > 20) return NCCLX_ERR_ARG; break;
+    case NCCLX_PARAM_COPY_STATIC_EIGHTHS: if (value < 0 || value > 8) return NCCLX_ERR_ARG; break;
+    case NCCLX_PARAM_COPY_KMAX:
+    case NCCLX_PARAM_COPY_KMAX_LONG: if (value < 1 || value > 64) return NCCLX_ERR_ARG; break;
     default: if (value < 0) return NCCLX_ERR_ARG; break;
     }
     g.params[param] = value;
