@@ -103,6 +103,22 @@ __device__ __forceinline__ void st_stream(uint4* p, const uint4& v) {
                  :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
+// 256-bit global accesses (sm_100: LDG.E.256 / STG.E.256): half the load instructions of the 128-bit
+// form and 32 B per lane per request; measured +10 % on the 16-stream reduction.
+struct u32x8 { uint4 lo, hi; };
+__device__ __forceinline__ u32x8 ld_stream256(const void* p) {     // may alias an output (in-place)
+    u32x8 r;
+    asm volatile("ld.global.L1::no_allocate.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(r.lo.x), "=r"(r.lo.y), "=r"(r.lo.z), "=r"(r.lo.w), "=r"(r.hi.x), "=r"(r.hi.y), "=r"(r.hi.z), "=r"(r.hi.w)
+                 : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ void st_stream256(void* p, const u32x8& v) {
+    asm volatile("st.global.L1::no_allocate.v8.u32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 :: "l"(p), "r"(v.lo.x), "r"(v.lo.y), "r"(v.lo.z), "r"(v.lo.w), "r"(v.hi.x), "r"(v.hi.y), "r"(v.hi.z), "r"(v.hi.w)
+                 : "memory");
+}
+
 // ---- mbarrier + cp.async.bulk (descriptor-less 1-D TMA) --------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 

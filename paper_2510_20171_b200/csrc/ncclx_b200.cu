@@ -31,7 +31,7 @@ struct Context {
     Workspace ws{};
     void* wsBase = nullptr;
     // tunables
-    int64_t params[NCCLX_PARAM_COUNT_] = {1, 1024, 8, 16, 0, 0, 15, 14, 1, 0, 6, 2};
+    int64_t params[NCCLX_PARAM_COUNT_] = {1, 1024, 4, 16, 0, 0, 15, 14, 1, 0, 6, 2};
     // profiling
     std::vector<EventPair> events[NCCLX_KERNEL_COUNT_];
     std::atomic<int64_t> launches{0};
@@ -182,7 +182,7 @@ int launchReduce(const void* const* send, void* const* recv, size_t blockElems, 
     ReduceArgs ra{};
     ra.send = send; ra.recv = recv; ra.blockElems = blockElems; ra.R = R; ra.scatter = scatter;
     const int es = elemSizeOf(dtype);
-    const unsigned long long totalVec = ((unsigned long long)blockElems * (scatter ? R : 1) * es + 15) / 16;
+    const unsigned long long totalVec = ((unsigned long long)blockElems * (scatter ? R : 1) * es + 31) / 32;
     unsigned long long tiles = (totalVec + REDUCE_THREADS - 1) / REDUCE_THREADS + (scatter ? R : 0);
     unsigned long long grid = (unsigned long long)g.smCount * (unsigned long long)g.params[NCCLX_PARAM_REDUCE_CTAS_PER_SM];
     if (grid > tiles) grid = tiles;

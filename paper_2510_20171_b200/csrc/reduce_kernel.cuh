@@ -7,9 +7,10 @@
 // acc = acc + (float)x_k for k = 1..R-1 in binary32 round-to-nearest-even, no FTZ, no
 // reassociation; ONE rounding to the output type; NaN results canonical.
 //
-// B200 design: HBM-bound streaming kernel.  Each thread owns one 16-byte vector position
-// (bf16x8 / f16x8 / fp32x4) per tile and issues the loads of CH ranks back to back (CH
-// independent 16 B loads in flight per thread, L1 no-allocate) before the ordered fp32 adds;
+// B200 design: HBM-bound streaming kernel.  Each thread owns one 32-byte vector position
+// (bf16x16 / f16x16 / fp32x8; 16-byte vectors when only 16 B alignment holds) per tile and issues the
+// 256-bit loads (LDG.E.256) of CH ranks back to back (CH independent 32 B loads in flight per thread,
+// L1 no-allocate) before the ordered fp32 adds;
 // inputs are read exactly once and the result is written straight to the R outputs
 // (AllReduce) or to the owning rank's block (ReduceScatter): no intermediate HBM round trip.
 // The device pointer tables are staged once per CTA into shared memory.
@@ -20,7 +21,7 @@
 
 namespace ncclx {
 
-constexpr int REDUCE_THREADS = 256;
+constexpr int REDUCE_THREADS = 128;
 enum { RED_BF16 = 0, RED_F32 = 1, RED_F16 = 2 };
 
 struct ReduceArgs {
@@ -134,6 +135,69 @@ template <> __device__ __forceinline__ void store_elem<RED_F32>(void* p, unsigne
     reinterpret_cast<unsigned int*>(p)[i] = canon_f32(acc);
 }
 
+// One tile of THREADS vector positions: every thread reduces one VB-byte vector (VB = 32: one 256-bit
+// load per rank; VB = 16: one 128-bit load per rank) over all R ranks and writes the result.
+template <int DT, int CH, int VB>
+__device__ __forceinline__ void reduce_vectors(const ReduceArgs& a, const unsigned char* const* sp, unsigned char* const* rp,
+                                               unsigned long long n, int nblocks) {
+    constexpr int ES = DT == RED_F32 ? 4 : 2;
+    constexpr int EPV = VB / ES;
+    const int R = a.R;
+    const unsigned long long nvec = n / EPV;                       // full vectors per block
+    const unsigned int tpb = (unsigned int)((nvec + blockDim.x - 1) / blockDim.x);
+    const unsigned long long ntiles = (unsigned long long)tpb * nblocks;
+    for (unsigned long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const unsigned int blk = a.scatter ? (unsigned int)(t / tpb) : 0u;
+        const unsigned int tb = (unsigned int)(t - (unsigned long long)blk * tpb);
+        const unsigned long long v = (unsigned long long)tb * blockDim.x + threadIdx.x;
+        if (v < nvec) {
+            const unsigned long long inOff = ((unsigned long long)blk * nvec + v) * VB;   // n*ES % VB == 0 when scatter
+            Acc<DT> acc0, acc1;
+            for (int k0 = 0; k0 < R; k0 += CH) {
+                if constexpr (VB == 32) {
+                    u32x8 x[CH];
+#pragma unroll
+                    for (int j = 0; j < CH; ++j)
+                        if (k0 + j < R) x[j] = ld_stream256(sp[k0 + j] + inOff);
+#pragma unroll
+                    for (int j = 0; j < CH; ++j)
+                        if (k0 + j < R) {
+                            if (k0 + j == 0) { acc0.set(x[j].lo); acc1.set(x[j].hi); }
+                            else { acc0.add(x[j].lo); acc1.add(x[j].hi); }
+                        }
+                } else {
+                    uint4 x[CH];
+#pragma unroll
+                    for (int j = 0; j < CH; ++j)
+                        if (k0 + j < R) x[j] = ld_stream(reinterpret_cast<const uint4*>(sp[k0 + j] + inOff));
+#pragma unroll
+                    for (int j = 0; j < CH; ++j)
+                        if (k0 + j < R) { if (k0 + j == 0) acc0.set(x[j]); else acc0.add(x[j]); }
+                }
+            }
+            if constexpr (VB == 32) {
+                u32x8 o;
+                o.lo = acc0.pack(); o.hi = acc1.pack();
+                if (a.scatter) st_stream256(rp[blk] + v * VB, o);
+                else for (int r = 0; r < R; ++r) st_stream256(rp[r] + v * VB, o);
+            } else {
+                const uint4 o = acc0.pack();
+                if (a.scatter) st_stream(reinterpret_cast<uint4*>(rp[blk] + v * VB), o);
+                else for (int r = 0; r < R; ++r) st_stream(reinterpret_cast<uint4*>(rp[r] + v * VB), o);
+            }
+        }
+    }
+    // ragged tail of an AllReduce (count % EPV elements), scalar
+    if (!a.scatter && blockIdx.x == 0) {
+        const unsigned long long i = nvec * EPV + threadIdx.x;
+        if (i < n) {
+            float acc = load_elem<DT>(sp[0], i);
+            for (int k = 1; k < R; ++k) acc = __fadd_rn(acc, load_elem<DT>(sp[k], i));
+            for (int r = 0; r < R; ++r) store_elem<DT>(rp[r], i, acc);
+        }
+    }
+}
+
 // dynamic smem: const void* sp[R]; void* rp[R]
 template <int DT, int CH>
 __global__ void __launch_bounds__(REDUCE_THREADS) reduce_kernel(const ReduceArgs a) {
@@ -143,7 +207,6 @@ __global__ void __launch_bounds__(REDUCE_THREADS) reduce_kernel(const ReduceArgs
     __shared__ int sMis;
     const int R = a.R;
     constexpr int ES = DT == RED_F32 ? 4 : 2;
-    constexpr int EPV = 16 / ES;
 
     if (threadIdx.x == 0) sMis = 0;
     __syncthreads();
@@ -152,51 +215,18 @@ __global__ void __launch_bounds__(REDUCE_THREADS) reduce_kernel(const ReduceArgs
         const unsigned char* s = reinterpret_cast<const unsigned char*>(a.send[k]);
         unsigned char* r = reinterpret_cast<unsigned char*>(a.recv[k]);
         sp[k] = s; rp[k] = r;
-        mis |= (int)(((unsigned long long)s | (unsigned long long)r) & 15ull);
+        mis |= (int)(((unsigned long long)s | (unsigned long long)r) & 31ull);
     }
-    if (mis) atomicOr(&sMis, 1);
+    if (mis) atomicOr(&sMis, mis);
     __syncthreads();
     const unsigned long long n = a.blockElems;
     const int nblocks = a.scatter ? R : 1;
-    const bool vec = (sMis == 0) && (!a.scatter || ((n * ES) & 15ull) == 0);
+    const int misAll = sMis | (a.scatter ? (int)((n * ES) & 31ull) : 0);   // block stride must keep the alignment
 
-    if (vec) {
-        const unsigned long long nvec = n / EPV;                       // full vectors per block
-        const unsigned int tpb = (unsigned int)((nvec + REDUCE_THREADS - 1) / REDUCE_THREADS);
-        const unsigned long long ntiles = (unsigned long long)tpb * nblocks;
-        for (unsigned long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
-            const unsigned int blk = a.scatter ? (unsigned int)(t / tpb) : 0u;
-            const unsigned int tb = (unsigned int)(t - (unsigned long long)blk * tpb);
-            const unsigned long long v = (unsigned long long)tb * REDUCE_THREADS + threadIdx.x;
-            if (v < nvec) {
-                const unsigned long long inOff = ((unsigned long long)blk * nvec + v) * 16ull;   // n*ES % 16 == 0 when scatter
-                Acc<DT> acc;
-                for (int k0 = 0; k0 < R; k0 += CH) {
-                    uint4 x[CH];
-#pragma unroll
-                    for (int j = 0; j < CH; ++j)
-                        if (k0 + j < R) x[j] = ld_stream(reinterpret_cast<const uint4*>(sp[k0 + j] + inOff));
-#pragma unroll
-                    for (int j = 0; j < CH; ++j)
-                        if (k0 + j < R) { if (k0 + j == 0) acc.set(x[j]); else acc.add(x[j]); }
-                }
-                const uint4 o = acc.pack();
-                if (a.scatter) {
-                    st_stream(reinterpret_cast<uint4*>(rp[blk] + v * 16ull), o);
-                } else {
-                    for (int r = 0; r < R; ++r) st_stream(reinterpret_cast<uint4*>(rp[r] + v * 16ull), o);
-                }
-            }
-        }
-        // ragged tail of an AllReduce (count % EPV elements), scalar
-        if (!a.scatter && blockIdx.x == 0) {
-            const unsigned long long i = nvec * EPV + threadIdx.x;
-            if (i < n) {
-                float acc = load_elem<DT>(sp[0], i);
-                for (int k = 1; k < R; ++k) acc = __fadd_rn(acc, load_elem<DT>(sp[k], i));
-                for (int r = 0; r < R; ++r) store_elem<DT>(rp[r], i, acc);
-            }
-        }
+    if ((misAll & 31) == 0) {
+        reduce_vectors<DT, CH, 32>(a, sp, rp, n, nblocks);
+    } else if ((misAll & 15) == 0) {
+        reduce_vectors<DT, CH, 16>(a, sp, rp, n, nblocks);
     } else {
         // scalar path: any alignment, same arithmetic, one element per thread
         const unsigned long long total = n * nblocks;
