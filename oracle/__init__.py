@@ -37,6 +37,9 @@ def lib() -> ctypes.CDLL:
             f.restype = ctypes.c_int
         L.oracle_reduce_samples.argtypes = [vp, vp, ctypes.c_size_t, ctypes.c_int, ctypes.c_int]
         L.oracle_reduce_samples.restype = ctypes.c_int
+        L.oracle_alltoallv_dynamic.argtypes = [vp, i64p, ctypes.c_int, i64p, ctypes.c_int, i64p, ctypes.c_int, vp, i64p,
+                                               ctypes.c_int, ctypes.c_int]
+        L.oracle_alltoallv_dynamic.restype = ctypes.c_int
         L.oracle_f32_to_bf16_rne.argtypes = [ctypes.c_uint32]
         L.oracle_f32_to_bf16_rne.restype = ctypes.c_uint16
         L.oracle_f32_to_f16_rne.argtypes = [ctypes.c_uint32]
@@ -99,6 +102,34 @@ def alltoallv(send: Sequence[np.ndarray], C: np.ndarray, recv: Sequence[np.ndarr
     neg = lib().oracle_alltoallv(st, _i64p(C), rt, _i64p(RC), _i64p(soff), _i64p(roff), R, dt, nthreads)
     assert neg >= 0
     return RC, soff, roff, neg
+
+
+def alltoallv_dynamic(send: Sequence[np.ndarray], split_lengths: np.ndarray, indices: np.ndarray, block_lens: np.ndarray,
+                      max_block_len: int, recvbuffs: Sequence[Sequence[np.ndarray]], dtype):
+    """The paper's AllToAllvDynamic.  split_lengths (R, n), indices (R, maxIndices),
+    block_lens (R, R); recvbuffs[d][s] are written IN PLACE at the sender's split offsets.
+    -> (recvAllSplitLengths (R, R, n), status bits)."""
+    dt = _dt(dtype)
+    Ls = np.ascontiguousarray(split_lengths, dtype=np.int64)
+    idx = np.ascontiguousarray(indices, dtype=np.int64)
+    bl = np.ascontiguousarray(block_lens, dtype=np.int64)
+    R, n = Ls.shape
+    assert bl.shape == (R, R) and idx.shape[0] == R and len(send) == R and len(recvbuffs) == R
+    e = lib().oracle_elem_size(dt)
+    tot = np.maximum(Ls, 0).sum(axis=1)
+    flat = []
+    for d in range(R):
+        assert len(recvbuffs[d]) == R
+        for s in range(R):
+            assert recvbuffs[d][s].itemsize == e and recvbuffs[d][s].size >= int(tot[s]), "recvbuff too small"
+            flat.append(recvbuffs[d][s])
+    for s in range(R):
+        assert send[s].itemsize == e and send[s].size >= int(tot[s])
+    out = np.empty((R, R, n), np.int64)
+    st = lib().oracle_alltoallv_dynamic(_ptr_table(send), _i64p(Ls), n, _i64p(idx), idx.shape[1], _i64p(bl), max_block_len,
+                                        _ptr_table(flat), _i64p(out), R, dt)
+    assert st >= 0
+    return out, st
 
 
 def allreduce_sum(send: Sequence[np.ndarray], dtype, nthreads: int = 1, out: Sequence[np.ndarray] | None = None):

@@ -170,6 +170,57 @@ int oracle_alltoallv(const void* const* send, const int64_t* C, void* const* rec
     return neg;
 }
 
+/* ---- AllToAllvDynamic: the paper's full metadata interface (section 6.1.2) ----
+ *
+ * Per sending rank s (L429): sendbuff = one contiguous buffer; sendSplitLengths L_s[0..n) split it into
+ * n pieces, piece i at element offset O_s[i] = sum_{i'<i} L_s[i']; sendIndices = the flattened 2-D list
+ * "which splits go to which rank" (sub-list of rank d = blockLens[s][d] consecutive entries, sub-lists in
+ * rank order; entries need not be contiguous and a split may appear in several sub-lists: duplicated
+ * experts, L437).  Receive side (L439): recvbuffs[d][s] is rank d's array for source s; "the paddings
+ * are reserved": a received split keeps the offset it had in the sender's buffer (Fig. 17: rank 1's data
+ * from rank 0 = splits {0,2,3} "contains the padding of index 1"), so
+ *     recvbuffs[d][s][O_s[idx] .. +L_s[idx]) = send[s][O_s[idx] .. +L_s[idx])   for every idx in s's
+ *     sub-list for d;  everything else in recvbuffs[d][s] keeps its pre-call bytes;
+ * recvAllSplitLengths[d][s][i] = L_s[i]: every rank receives ALL ranks' split lengths (L439).
+ * Readings: negative lengths count as 0 (status bit 0); an index outside [0,n) is
+ * skipped (bit 1); a block length < 0 or > maxBlockLen is clamped (bit 2).
+ * Arrays: L = R*n, indices = R*maxIndices (row stride), blockLens = R*R, recvbuffs = R*R host pointers
+ * [d*R+s], recvAll = R*R*n.  Returns the status bits. */
+int oracle_alltoallv_dynamic(const void* const* send, const int64_t* L, int n, const int64_t* indices,
+                             int maxIndices, const int64_t* blockLens, int maxBlockLen, void* const* recvbuffs,
+                             int64_t* recvAll, int R, int dtype) {
+    int e = elem_size(dtype);
+    if (e == 0 || R < 1 || n < 1) return -1;
+    int status = 0;
+    for (int d = 0; d < R; d++)
+        for (int s = 0; s < R; s++)
+            for (int i = 0; i < n; i++) {
+                int64_t l = L[(size_t)s * n + i];
+                if (l < 0) { status |= 1; l = 0; }
+                recvAll[((size_t)d * R + s) * n + i] = l;
+            }
+    for (int s = 0; s < R; s++) {
+        int64_t pos = 0;                                   /* read position in s's index list */
+        for (int d = 0; d < R; d++) {
+            int64_t bl = blockLens[(size_t)s * R + d];
+            if (bl < 0) { status |= 4; bl = 0; }
+            if (bl > maxBlockLen) { status |= 4; bl = maxBlockLen; }
+            for (int64_t j = 0; j < bl; j++) {
+                if (pos + j >= maxIndices) { status |= 4; break; }
+                int64_t idx = indices[(size_t)s * maxIndices + pos + j];
+                if (idx < 0 || idx >= n) { status |= 2; continue; }
+                int64_t off = 0;
+                for (int64_t i = 0; i < idx; i++) { int64_t l = L[(size_t)s * n + i]; off += l > 0 ? l : 0; }
+                int64_t len = L[(size_t)s * n + idx];
+                if (len > 0)
+                    memcpy((char*)recvbuffs[(size_t)d * R + s] + off * e, (const char*)send[s] + off * e, (size_t)len * e);
+            }
+            pos += bl;
+        }
+    }
+    return status;
+}
+
 /* ---- sum reduction ------------------------------------------------------------------ */
 
 static float load_as_f32(const void* p, size_t i, int dtype) {
