@@ -411,6 +411,7 @@ def main():
                                              "mean_us": round(float(t.mean()) * 1e3, 2), "bytes_each_way": a.bytes_one_way,
                                              **frac(2 * a.bytes_one_way / (p50 * 1e-3) / 1e9, peak)}
             del a, g
+        per["next1_alltoallv_dynamic_R64_tok256"] = dynamic_extra(torch, nx, peak, min(args.latency_replays, 2000))
         line["per_config"] = per
 
     # ---- e2e: same step through the host-buffer C ABI (H2D + kernels + D2H inside the timed region) --------
@@ -428,6 +429,37 @@ def main():
     if dist is not None:
         dist.destroy_process_group()
     return 0
+
+
+def dynamic_extra(torch, nx, peak, reps):
+    """the paper's full AllToAllvDynamic interface on an inference-shaped MoE dispatch
+    (R=64, 256 tokens x 5120 bf16 per rank, 128 experts + one redundant hot expert), CUDA-graph replays."""
+    Ls, idx, bl, J = W.dynamic_moe_metadata()
+    R, n = Ls.shape
+    nx.ncclx_init_dynamic(n, R * R * J)
+    tot = Ls.sum(axis=1)
+    send = [W.torch_values(int(t), "bf16", 5000 + s) for s, t in enumerate(tot)]
+    recv = [torch.empty(int(tot[s]), dtype=torch.bfloat16, device="cuda") for d in range(R) for s in range(R)]
+    st, rt = nx.device_ptr_table(send), nx.device_ptr_table(recv)
+    Ld, Id, Bd = (torch.from_numpy(np.ascontiguousarray(x)).cuda() for x in (Ls, idx, bl))
+    allL = torch.empty((R, R, n), dtype=torch.int64, device="cuda")
+
+    def call():
+        nx.ncclx_alltoallv_dynamic_dev(st, Ld, n, Id, idx.shape[1], Bd, J, rt, allL, R, "bf16")
+    call(); torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        call()
+    t = event_times_ms(torch, g.replay, reps, warm=20)
+    moved = 0
+    for s_ in range(R):
+        pos = 0
+        for d in range(R):
+            moved += int(Ls[s_, idx[s_, pos:pos + bl[s_, d]]].sum()) * 2
+            pos += int(bl[s_, d])
+    p50 = float(np.percentile(t, 50))
+    return {"replays": reps, "p50_us": round(p50 * 1e3, 2), "p99_us": round(float(np.percentile(t, 99)) * 1e3, 2),
+            "bytes_each_way": moved, "segments": int(bl.sum()), **frac(2 * moved / (p50 * 1e-3) / 1e9, peak)}
 
 
 def probe(args, torch, nx, peak):

@@ -111,6 +111,32 @@ int ncclx_alltoallv_last_offsets(int64_t* soff_host, int64_t* roff_host, int R, 
  * seen).  Synchronises `stream`; not capturable. */
 int ncclx_device_status(uint32_t* status_host, ncclx_stream_t stream);
 
+/* ---- AllToAllvDynamic: the paper's full metadata interface (section 6.1.2) ---- *
+ *
+ * Per sending rank s: send[s] is one contiguous buffer that sendSplitLengths row s cuts into `nsplits`
+ * pieces (piece i at element offset O_s[i] = sum_{i'<i} L_s[i']); sendIndices row s is the flattened
+ * list of split indices to send, sub-list for rank d = sendIndicesBlockLens[s*R+d] consecutive entries,
+ * sub-lists in rank order; a sub-list need not be contiguous and one split may go to several ranks
+ * (duplicated experts, L437).  Receive side (L439): recvbuffs[d*R+s] is rank d's array for source s and
+ * "the paddings are reserved": every received split lands at the offset it had in the sender's buffer,
+ *     recvbuffs[d][s][O_s[idx] .. +L_s[idx]) = send[s][O_s[idx] .. +L_s[idx])  for each idx in s's
+ *     sub-list for d;   all other bytes of recvbuffs[d][s] are NOT written;
+ *     recvAllSplitLengths[(d*R+s)*nsplits + i] = L_s[i]  (every rank receives all split lengths).
+ * All metadata is DEVICE-resident and read when the kernels execute (L401, L409); capturable.
+ *
+ *   maxIndices    row stride of sendIndices_dev (>= sum_d blockLens[s][d] for every s)
+ *   maxBlockLen   upper bound on any block length (= experts per rank incl. redundant ones); sizes the
+ *                 work list: R*R*maxBlockLen <= the capacity given to ncclx_init_dynamic
+ * Device status bits (ncclx_device_status): 0 negative split length (treated as 0), 1 split index outside
+ * [0,nsplits) (skipped), 2 block length < 0 or > maxBlockLen or list overrun (clamped).
+ * Each recvbuffs[d][s] must hold sum_i L_s[i] elements and must not overlap any send buffer.
+ * Call ncclx_init_dynamic(max_splits, max_segments) once after ncclx_init, outside capture. */
+int ncclx_init_dynamic(int max_splits, int64_t max_segments);
+int ncclx_alltoallv_dynamic_dev(const void* const* send, const int64_t* sendSplitLengths_dev, int nsplits,
+                                const int64_t* sendIndices_dev, int maxIndices,
+                                const int64_t* sendIndicesBlockLens_dev, int maxBlockLen, void* const* recvbuffs,
+                                int64_t* recvAllSplitLengths_dev, int R, ncclx_dtype_t dtype, ncclx_stream_t stream);
+
 /* ---- sum reduction (section 5.3; numeric contract DESIGN.md section 3) -- *
  *
  *     acc = (float) x_0[i];  for k = 1..R-1: acc = acc + (float) x_k[i]     (binary32, RNE,
@@ -173,6 +199,7 @@ typedef enum {
     NCCLX_KERNEL_COUNTS = 0, /* counts transpose + offsets scan + work list   */
     NCCLX_KERNEL_COPY = 1,   /* byte-balanced segment copy                    */
     NCCLX_KERNEL_REDUCE = 2, /* rank-order sum                                */
+    NCCLX_KERNEL_DYN = 3,    /* AllToAllvDynamic metadata kernels (prep + desc) */
     NCCLX_KERNEL_COUNT_
 } ncclx_kernel_t;
 

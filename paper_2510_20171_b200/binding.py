@@ -29,7 +29,7 @@ PARAM_COPY_STATIC_EIGHTHS = 9
 PARAM_COPY_KMAX = 10
 PARAM_COPY_KMAX_LONG = 11
 
-KERNEL_COUNTS, KERNEL_COPY, KERNEL_REDUCE = 0, 1, 2
+KERNEL_COUNTS, KERNEL_COPY, KERNEL_REDUCE, KERNEL_DYN = 0, 1, 2, 3
 
 # every symbol include/ncclx_b200.h declares (tests check the .so exports all of them)
 SYMBOLS = [
@@ -37,7 +37,7 @@ SYMBOLS = [
     "ncclx_version", "ncclx_alltoallv_dev", "ncclx_alltoallv_last_offsets", "ncclx_device_status",
     "ncclx_allreduce_sum", "ncclx_reducescatter_sum", "ncclx_alltoallv_host", "ncclx_allreduce_sum_host",
     "ncclx_reducescatter_sum_host", "ncclx_set_param", "ncclx_get_param", "ncclx_profile_read",
-    "ncclx_profile_reset", "ncclx_launch_count", "ncclx_sm_count",
+    "ncclx_profile_reset", "ncclx_launch_count", "ncclx_sm_count", "ncclx_init_dynamic", "ncclx_alltoallv_dynamic_dev",
 ]
 
 
@@ -74,6 +74,9 @@ def lib() -> ctypes.CDLL:
                   L.ncclx_reducescatter_sum_host):
             f.argtypes = [vp, vp, ctypes.c_size_t, ctypes.c_int, ctypes.c_int, vp]
         L.ncclx_alltoallv_host.argtypes = [vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, vp]
+        L.ncclx_init_dynamic.argtypes = [ctypes.c_int, i64]
+        L.ncclx_alltoallv_dynamic_dev.argtypes = [vp, vp, ctypes.c_int, vp, ctypes.c_int, vp, ctypes.c_int, vp, vp,
+                                                  ctypes.c_int, ctypes.c_int, vp]
         L.ncclx_set_param.argtypes = [ctypes.c_int, i64]
         L.ncclx_get_param.argtypes = [ctypes.c_int, i64p]
         L.ncclx_profile_read.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double), i64p]
@@ -154,6 +157,19 @@ def ncclx_device_status(stream=None) -> int:
     st = ctypes.c_uint32(0)
     _ck(lib().ncclx_device_status(ctypes.byref(st), _stream(stream)), "ncclx_device_status")
     return st.value
+
+
+def ncclx_init_dynamic(max_splits: int, max_segments: int) -> None:
+    _ck(lib().ncclx_init_dynamic(max_splits, max_segments), "ncclx_init_dynamic")
+
+
+def ncclx_alltoallv_dynamic_dev(send_table, split_lengths_dev, nsplits: int, indices_dev, max_indices: int, block_lens_dev,
+                                max_block_len: int, recvbuffs_table, recv_all_split_lengths_dev, R: int, dtype,
+                                stream=None) -> None:
+    _ck(lib().ncclx_alltoallv_dynamic_dev(_ptr(send_table), _ptr(split_lengths_dev), nsplits, _ptr(indices_dev), max_indices,
+                                          _ptr(block_lens_dev), max_block_len, _ptr(recvbuffs_table),
+                                          _ptr(recv_all_split_lengths_dev), R, _dt(dtype), _stream(stream)),
+        "ncclx_alltoallv_dynamic_dev")
 
 
 def ncclx_allreduce_sum(send_table, recv_table, count: int, R: int, dtype, stream=None) -> None:

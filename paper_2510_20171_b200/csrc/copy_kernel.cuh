@@ -29,7 +29,8 @@ struct CopyArgs {
     const SegDesc* desc;
     const int* colTiles[2];
     WorkCtl* ctl;
-    int R;
+    int ncols;                             // destination columns of the descriptor table (= R)
+    int colLen;                            // descriptor slots per column (R for the plain call, R*maxBlockLen for the dynamic one)
     unsigned int ringBytes;                // shared-memory ring size, multiple of 128, >= 3 tiles
     int staticEighths;                     // 0..8: share of the tiles assigned statically (contiguous per engine)
     int kmax[2];                           // max tiles per dynamic claim, per list (short-segment regime)
@@ -46,10 +47,10 @@ struct CopyArgs {
 template <int L>
 struct Cursor {
     const SegDesc* desc;
-    const int* colBase;                    // smem, R+1 entries, colBase[R] = total tiles
+    const int* colBase;                    // smem, ncols+1 entries, colBase[ncols] = total tiles
     unsigned int* counter;
     ClassParams cls;
-    int R, RR, tileShift, total, nEngines, kmax, kmin;
+    int ncols, colLen, RR, tileShift, total, nEngines, kmax, kmin;
     int staticK, engineId;                 // first chunk is assigned statically: [engineId*staticK, +staticK)
     int dynBase;                           // tiles >= dynBase are claimed dynamically
     int pendCur, pendK;                    // lane 0: the NEXT chunk, claimed ahead of need (atomic in flight)
@@ -86,7 +87,7 @@ struct Cursor {
 
     __device__ __forceinline__ void init(const CopyArgs& a, const int* colBase_, int nEngines_, int engineId_, int kmax_) {
         desc = a.desc; colBase = colBase_; counter = &a.ctl->next[L]; cls = a.cls;
-        R = a.R; RR = a.R * a.R; tileShift = a.cls.tileShift[L]; total = colBase_[a.R];
+        ncols = a.ncols; colLen = a.colLen; RR = a.ncols * a.colLen; tileShift = a.cls.tileShift[L]; total = colBase_[a.ncols];
         nEngines = nEngines_; engineId = engineId_;
         // long segments (>= 8 tiles each on average): claims resolve inside the cached window, so take
         // small chunks and keep all SMs in a tight moving window of HBM; short segments: every claim
@@ -122,15 +123,15 @@ struct Cursor {
     // Find the segment that owns global tile index tt (0 <= tt < total) and (re)load the windows there.
     __device__ __forceinline__ void locate(int tt) {
         const int lane = lane_id();
-        int lo = 0, hi = R;                // colBase[lo] <= tt < colBase[hi]
+        int lo = 0, hi = ncols;            // colBase[lo] <= tt < colBase[hi]
         while (hi - lo > 1) {
             const int mid = (lo + hi) >> 1;
             if (colBase[mid] <= tt) lo = mid; else hi = mid;
         }
         const int d = lo;
         const int tl = tt - colBase[d];
-        const SegDesc* col = desc + (size_t)d * R;
-        int s0 = 0, n = R;                 // smallest s with col[s].pfx[L] > tl lies in [s0, s0+n)
+        const SegDesc* col = desc + (size_t)d * colLen;
+        int s0 = 0, n = colLen;                 // smallest s with col[s].pfx[L] > tl lies in [s0, s0+n)
         while (n > 32) {                   // 128-ary rounds: every lane probes 4 block ends per L2 round trip
             const int step = (n + 127) >> 7;
             int cnt = 0;
@@ -150,7 +151,7 @@ struct Cursor {
         // predecessor's prefix (needed for the tile index inside the segment) comes with it
         const int sb = s0 > 0 ? s0 - 1 : 0;
         const int nn = n + (s0 - sb);
-        qw = d * R + sb;
+        qw = d * colLen + sb;
         load_desc(qw + lane, w0, w1);
         qn = qw + 32;
         load_desc(qn + lane, n0, n1);
@@ -285,7 +286,7 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = lane_id();
     const int warp = threadIdx.x >> 5;
-    const int R = a.R;
+    const int R = a.ncols;
     unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + a.ringBytes);
     int* colBase[2];
     colBase[0] = reinterpret_cast<int*>(mbar + COPY_SLOTS);

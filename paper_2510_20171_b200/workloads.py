@@ -155,3 +155,28 @@ def tagged_payload_u32(s: int, n: int) -> np.ndarray:
     (SURVEY.md section 8(c.4)).  A label, not arithmetic of the method."""
     assert n < (1 << 24) and s < 256
     return (np.uint32(s) << np.uint32(24)) | np.arange(n, dtype=np.uint32)
+
+
+def dynamic_moe_metadata(R: int = 64, tokens: int = 256, experts: int = 128, width: int = 5120, s: float = 1.1,
+                         seed: int = 5, redundant_hot_expert: bool = True):
+    """Metadata of an inference-shaped AllToAllvDynamic call (Table 3: batch
+    128/256 tokens per rank): per source rank one multinomial(tokens, Zipf(s)) over the experts gives
+    sendSplitLengths (rows x width elements, sorted by expert id, MetaShuffling L699); rank d hosts experts
+    [d*E/R, (d+1)*E/R) and, if asked, the last rank also hosts a redundant copy of the hottest expert 0
+    (duplicated experts, L437).  -> (split_lengths (R,E), indices (R,maxIndices), block_lens (R,R), maxBlockLen)."""
+    p = (np.arange(experts) + 1.0) ** (-s)
+    p /= p.sum()
+    rng = np.random.default_rng(seed)
+    rows = np.stack([rng.multinomial(tokens, p) for _ in range(R)]).astype(np.int64)
+    per = experts // R
+    J = per + (1 if redundant_hot_expert else 0)
+    bl = np.full((R, R), per, np.int64)
+    if redundant_hot_expert:
+        bl[:, R - 1] = per + 1
+    lst = []
+    for d in range(R):
+        lst += list(range(d * per, (d + 1) * per))
+        if redundant_hot_expert and d == R - 1:
+            lst.append(0)
+    idx = np.tile(np.array(lst, np.int64), (R, 1))
+    return rows * width, idx, bl, J
