@@ -412,6 +412,7 @@ def main():
                                              **frac(2 * a.bytes_one_way / (p50 * 1e-3) / 1e9, peak)}
             del a, g
         per["next1_alltoallv_dynamic_R64_tok256"] = dynamic_extra(torch, nx, peak, min(args.latency_replays, 2000))
+        per["next2_reducecopy_cta_sweep"] = reducecopy_extra(torch, nx, peak)
         line["per_config"] = per
 
     # ---- e2e: same step through the host-buffer C ABI (H2D + kernels + D2H inside the timed region) --------
@@ -460,6 +461,22 @@ def dynamic_extra(torch, nx, peak, reps):
     p50 = float(np.percentile(t, 50))
     return {"replays": reps, "p50_us": round(p50 * 1e3, 2), "p99_us": round(float(np.percentile(t, 99)) * 1e3, 2),
             "bytes_each_way": moved, "segments": int(bl.sum()), **frac(2 * moved / (p50 * 1e-3) / 1e9, peak)}
+
+
+def reducecopy_extra(torch, nx, peak):
+    """FTAR-style ReduceCopy step: 512 MiB bf16 message, 8 MiB chunks,
+    out + fwd written (4 x message bytes of traffic), GB/s as a function of the number of 512-thread CTAs."""
+    n = 256 << 20
+    a = W.torch_values(n, "bf16", 6001)
+    b = W.torch_values(n, "bf16", 6002, 1e-3)
+    out, fwd = torch.empty_like(a), torch.empty_like(a)
+    res = {"message_MiB": n * 2 >> 20, "chunk_MiB": 8, "threads_per_cta": 512, "by_ctas": {}}
+    for ctas in (1, 2, 4, 8, 16, 32, 64, 148):
+        t = event_times_ms(torch, lambda: nx.ncclx_reducecopy_sum(a, b, out, fwd, n, "bf16", 8 << 20, ctas), 5, warm=2)
+        m = float(np.median(t))
+        res["by_ctas"][str(ctas)] = {"ms": round(m, 3), "traffic_GBps": round(4 * n * 2 / (m * 1e-3) / 1e9, 1),
+                                     "message_GBps": round(n * 2 / (m * 1e-3) / 1e9, 1)}
+    return res
 
 
 def probe(args, torch, nx, peak):

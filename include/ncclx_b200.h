@@ -157,6 +157,22 @@ int ncclx_allreduce_sum(const void* const* send, void* const* recv, size_t count
 int ncclx_reducescatter_sum(const void* const* send, void* const* recv, size_t recvcount, int R,
                             ncclx_dtype_t dtype, ncclx_stream_t stream);
 
+/* ---- FTAR-style ReduceCopy step (section 5.3, Fig. 9: Reduce / ReduceCopy) ---------- *
+ *
+ * One pipeline step of the paper's ring AllReduce on local memory: the incoming chunk `a` (from the previous
+ * peer) is summed with the local chunk `b`,  r[i] = rn_dtype((float)a[i] + (float)b[i])  (same arithmetic as
+ * ncclx_allreduce_sum with R = 2, NaN canonical), and r is written to `out` (local result; Reduce), to
+ * `fwd` (the buffer forwarded to the next peer; ReduceCopy, "combine the reduction and forwarding copy"), or
+ * to both; either may be NULL but not both ("avoid unnecessary HBM stores in the intermediate forwarding
+ * steps").  The message is walked in fixed chunks of `chunk_bytes` (paper: S = 8 MB; 0 selects 8 MiB) by a
+ * FIXED grid of `num_ctas` CTAs x 512 threads (paper: 2 CTAs suffice to stay hidden under the network;
+ * 0 selects 2) -- the SM-frugal regime, as opposed to the full-chip ncclx_allreduce_sum.
+ * a, b, out, fwd: DEVICE pointers to `count` elements; out/fwd may alias a or b exactly (in place), other
+ * overlap is undefined.  dtype in {BF16, F32, F16}.  32-byte aligned pointers and chunk size take the
+ * 256-bit vector path, anything else a scalar path with the same arithmetic.  Capturable. */
+int ncclx_reducecopy_sum(const void* a, const void* b, void* out, void* fwd, size_t count, ncclx_dtype_t dtype,
+                         size_t chunk_bytes, int num_ctas, ncclx_stream_t stream);
+
 /* ---- host-buffer forms (the end-to-end path: H2D + kernels + D2H inside the call) ------ *
  *
  * Same semantics, but every pointer is a HOST pointer (pinned memory gives full PCIe

@@ -38,6 +38,7 @@ SYMBOLS = [
     "ncclx_allreduce_sum", "ncclx_reducescatter_sum", "ncclx_alltoallv_host", "ncclx_allreduce_sum_host",
     "ncclx_reducescatter_sum_host", "ncclx_set_param", "ncclx_get_param", "ncclx_profile_read",
     "ncclx_profile_reset", "ncclx_launch_count", "ncclx_sm_count", "ncclx_init_dynamic", "ncclx_alltoallv_dynamic_dev",
+    "ncclx_reducecopy_sum",
 ]
 
 
@@ -77,6 +78,7 @@ def lib() -> ctypes.CDLL:
         L.ncclx_init_dynamic.argtypes = [ctypes.c_int, i64]
         L.ncclx_alltoallv_dynamic_dev.argtypes = [vp, vp, ctypes.c_int, vp, ctypes.c_int, vp, ctypes.c_int, vp, vp,
                                                   ctypes.c_int, ctypes.c_int, vp]
+        L.ncclx_reducecopy_sum.argtypes = [vp, vp, vp, vp, ctypes.c_size_t, ctypes.c_int, ctypes.c_size_t, ctypes.c_int, vp]
         L.ncclx_set_param.argtypes = [ctypes.c_int, i64]
         L.ncclx_get_param.argtypes = [ctypes.c_int, i64p]
         L.ncclx_profile_read.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double), i64p]
@@ -175,6 +177,11 @@ def ncclx_alltoallv_dynamic_dev(send_table, split_lengths_dev, nsplits: int, ind
 def ncclx_allreduce_sum(send_table, recv_table, count: int, R: int, dtype, stream=None) -> None:
     _ck(lib().ncclx_allreduce_sum(_ptr(send_table), _ptr(recv_table), count, R, _dt(dtype), _stream(stream)),
         "ncclx_allreduce_sum")
+
+
+def ncclx_reducecopy_sum(a, b, out, fwd, count: int, dtype, chunk_bytes: int = 0, num_ctas: int = 0, stream=None) -> None:
+    _ck(lib().ncclx_reducecopy_sum(_ptr(a), _ptr(b), _ptr(out), _ptr(fwd), count, _dt(dtype), chunk_bytes, num_ctas,
+                                   _stream(stream)), "ncclx_reducecopy_sum")
 
 
 def ncclx_reducescatter_sum(send_table, recv_table, recvcount: int, R: int, dtype, stream=None) -> None:

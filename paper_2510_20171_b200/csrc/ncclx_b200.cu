@@ -443,6 +443,31 @@ int ncclx_reducescatter_sum(const void* const* send, void* const* recv, size_t r
     return launchReduce(send, recv, recvcount, R, (int)dtype, 1, static_cast<cudaStream_t>(stream));
 }
 
+int ncclx_reducecopy_sum(const void* a, const void* b, void* out, void* fwd, size_t count, ncclx_dtype_t dtype,
+                         size_t chunk_bytes, int num_ctas, ncclx_stream_t stream) {
+    if (!g.ready) return NCCLX_ERR_NOT_INITIALIZED;
+    if (!a || !b || (!out && !fwd) || num_ctas < 0 || num_ctas > 65535) return NCCLX_ERR_ARG;
+    if (!(dtype == NCCLX_BF16 || dtype == NCCLX_F32 || dtype == NCCLX_F16)) return NCCLX_ERR_DTYPE;
+    if (count == 0) return NCCLX_OK;
+    const int es = elemSizeOf((int)dtype);
+    if (chunk_bytes == 0) chunk_bytes = (size_t)8 << 20;
+    if (chunk_bytes % es) return NCCLX_ERR_ARG;
+    if (num_ctas == 0) num_ctas = 2;
+    ReduceCopyArgs ra{};
+    ra.a = static_cast<const unsigned char*>(a); ra.b = static_cast<const unsigned char*>(b);
+    ra.out = static_cast<unsigned char*>(out); ra.fwd = static_cast<unsigned char*>(fwd);
+    ra.count = count; ra.chunkElems = chunk_bytes / es;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    LaunchScope ls(NCCLX_KERNEL_REDUCE, s);
+    switch (dtype) {
+    case NCCLX_BF16: reducecopy_kernel<RED_BF16><<<num_ctas, RC_THREADS, 0, s>>>(ra); break;
+    case NCCLX_F32: reducecopy_kernel<RED_F32><<<num_ctas, RC_THREADS, 0, s>>>(ra); break;
+    default: reducecopy_kernel<RED_F16><<<num_ctas, RC_THREADS, 0, s>>>(ra); break;
+    }
+    CK(cudaGetLastError());
+    return NCCLX_OK;
+}
+
 // ---- host-buffer forms -----------------------------------------------------------------------
 
 int ncclx_alltoallv_host(const void* const* send, const int64_t* sendcounts_host, void* const* recv,

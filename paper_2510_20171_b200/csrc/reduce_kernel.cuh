@@ -244,4 +244,78 @@ __global__ void __launch_bounds__(REDUCE_THREADS) reduce_kernel(const ReduceArgs
     }
 }
 
+// ---- FTAR-style ReduceCopy step (section 5.3, Fig. 9) ---------
+// One pipeline step of the paper's ring: an incoming chunk `a` (what the previous peer sent) is summed
+// with the local chunk `b`; the result goes to the local output `out` (Reduce), to the forward buffer
+// `fwd` that the next peer will receive (ReduceCopy: "combine the reduction and forwarding copy ... avoids
+// redundant HBM load"; `out` may be NULL in the intermediate steps: "avoid unnecessary HBM stores"), or
+// both.  The message is processed in fixed chunks of S bytes (paper: 8 MB) by a FIXED, small number of
+// CTAs x 512 threads (paper: 2 CTAs suffice against the network): throughput per CTA comes from
+// instruction-level parallelism (L335), here RC_UNROLL independent 256-bit loads per input per thread.
+constexpr int RC_THREADS = 512;
+constexpr int RC_UNROLL = 4;
+
+struct ReduceCopyArgs {
+    const unsigned char* a;
+    const unsigned char* b;
+    unsigned char* out;          // may be null
+    unsigned char* fwd;          // may be null
+    unsigned long long count;    // elements
+    unsigned long long chunkElems;
+};
+
+template <int DT>
+__global__ void __launch_bounds__(RC_THREADS) reducecopy_kernel(const ReduceCopyArgs p) {
+    constexpr int ES = DT == RED_F32 ? 4 : 2;
+    constexpr int EPV = 32 / ES;
+    const bool vec = ((((unsigned long long)p.a | (unsigned long long)p.b | (unsigned long long)p.out |
+                        (unsigned long long)p.fwd) & 31ull) == 0) && ((p.chunkElems * ES) & 31ull) == 0;
+    for (unsigned long long c0 = 0; c0 < p.count; c0 += p.chunkElems) {        // chunk by chunk, in order
+        const unsigned long long cn = min(p.chunkElems, p.count - c0);
+        if (vec) {
+            const unsigned long long nvec = cn / EPV;
+            const unsigned long long base = c0 * ES;
+            // a CTA's tile = RC_UNROLL x 512 vectors, interleaved so that every load instruction is coalesced
+            for (unsigned long long t = (unsigned long long)blockIdx.x * RC_THREADS * RC_UNROLL; t < nvec;
+                 t += (unsigned long long)gridDim.x * RC_THREADS * RC_UNROLL) {
+                u32x8 xa[RC_UNROLL], xb[RC_UNROLL];
+#pragma unroll
+                for (int u = 0; u < RC_UNROLL; ++u) {
+                    const unsigned long long v = t + (unsigned long long)u * RC_THREADS + threadIdx.x;
+                    if (v < nvec) { xa[u] = ld_stream256(p.a + base + v * 32); xb[u] = ld_stream256(p.b + base + v * 32); }
+                }
+#pragma unroll
+                for (int u = 0; u < RC_UNROLL; ++u) {
+                    const unsigned long long v = t + (unsigned long long)u * RC_THREADS + threadIdx.x;
+                    if (v < nvec) {
+                        Acc<DT> lo, hi;
+                        lo.set(xa[u].lo); hi.set(xa[u].hi);
+                        lo.add(xb[u].lo); hi.add(xb[u].hi);
+                        u32x8 o;
+                        o.lo = lo.pack(); o.hi = hi.pack();
+                        if (p.out) st_stream256(p.out + base + v * 32, o);
+                        if (p.fwd) st_stream256(p.fwd + base + v * 32, o);
+                    }
+                }
+            }
+            // ragged tail of the chunk (only the last chunk can have one)
+            if (blockIdx.x == 0) {
+                const unsigned long long i = c0 + nvec * EPV + threadIdx.x;
+                if (i < c0 + cn) {
+                    const float acc = __fadd_rn(load_elem<DT>(p.a, i), load_elem<DT>(p.b, i));
+                    if (p.out) store_elem<DT>(p.out, i, acc);
+                    if (p.fwd) store_elem<DT>(p.fwd, i, acc);
+                }
+            }
+        } else {
+            for (unsigned long long i = c0 + (unsigned long long)blockIdx.x * RC_THREADS + threadIdx.x; i < c0 + cn;
+                 i += (unsigned long long)gridDim.x * RC_THREADS) {
+                const float acc = __fadd_rn(load_elem<DT>(p.a, i), load_elem<DT>(p.b, i));
+                if (p.out) store_elem<DT>(p.out, i, acc);
+                if (p.fwd) store_elem<DT>(p.fwd, i, acc);
+            }
+        }
+    }
+}
+
 }  // namespace ncclx

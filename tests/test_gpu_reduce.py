@@ -162,3 +162,42 @@ def test_host_buffer_forms():
     for r in range(R):
         assert out_ar[r].numpy().view(np.uint16).tobytes() == exp[r].tobytes()
         assert out_rs[r].numpy().view(np.uint16).tobytes() == exp[0][r * n:(r + 1) * n].tobytes()
+
+
+# ---- NEXT-2: FTAR-style ReduceCopy step -------------------------------------------------
+
+@pytest.mark.parametrize("dtype", ["bf16", "f32", "f16"])
+@pytest.mark.parametrize("n,chunk,ctas", [(8 * 1024 * 1024 // 2 * 3 + 8 * 100 + 5, 8 << 20, 2), (100_003, 4096, 1),
+                                          (16 * 512 * 4 * 3, 16 * 512 * 4 * 2, 3), (777, 0, 0)])
+def test_reducecopy_matches_two_rank_oracle(dtype, n, chunk, ctas):
+    a = inject_specials(W.np_values(n, dtype, 1), dtype, 1)
+    b = inject_specials(W.np_values(n, dtype, 2, 1e-3), dtype, 2)
+    exp = oracle.allreduce_sum([a, b], dtype, nthreads=4)[0]
+    da, db = to_dev(a), to_dev(b)
+    nb = n * ES[dtype]
+    out = torch.zeros(nb + 64, dtype=torch.uint8, device="cuda")[:nb]
+    fwd = torch.zeros(nb + 64, dtype=torch.uint8, device="cuda")[:nb]
+    nx.ncclx_reducecopy_sum(da, db, out, fwd, n, dtype, chunk, ctas)            # ReduceCopy with local result
+    torch.cuda.synchronize()
+    assert back(out, dtype).tobytes() == exp.tobytes() and back(fwd, dtype).tobytes() == exp.tobytes()
+    fwd.zero_()
+    nx.ncclx_reducecopy_sum(da, db, None, fwd, n, dtype, chunk, ctas)           # intermediate step: forward only
+    nx.ncclx_reducecopy_sum(da, db, db, None, n, dtype, chunk, ctas)            # Reduce, in place on the local chunk
+    torch.cuda.synchronize()
+    assert back(fwd, dtype).tobytes() == exp.tobytes() and back(db, dtype).tobytes() == exp.tobytes()
+
+
+def test_reducecopy_misaligned_and_errors():
+    n = 5001
+    a, b = W.np_values(n, "bf16", 3), W.np_values(n, "bf16", 4)
+    da, db = to_dev(a, 2), to_dev(b, 6)
+    out = torch.zeros(2 * n + 64, dtype=torch.uint8, device="cuda")[10:10 + 2 * n]
+    nx.ncclx_reducecopy_sum(da, db, out, None, n, "bf16", 1000, 2)
+    torch.cuda.synchronize()
+    assert back(out, "bf16").tobytes() == oracle.allreduce_sum([a, b], "bf16")[0].tobytes()
+    with pytest.raises(nx.binding.NcclxError) as e:
+        nx.ncclx_reducecopy_sum(da, db, None, None, n, "bf16")
+    assert e.value.code == 1
+    with pytest.raises(nx.binding.NcclxError) as e:
+        nx.ncclx_reducecopy_sum(da, db, out, None, n, "u8")
+    assert e.value.code == 2
