@@ -40,6 +40,11 @@ def lib() -> ctypes.CDLL:
         L.oracle_alltoallv_dynamic.argtypes = [vp, i64p, ctypes.c_int, i64p, ctypes.c_int, i64p, ctypes.c_int, vp, i64p,
                                                ctypes.c_int, ctypes.c_int]
         L.oracle_alltoallv_dynamic.restype = ctypes.c_int
+        i32p = ctypes.POINTER(ctypes.c_int32)
+        L.oracle_moe_dispatch_topk.argtypes = [vp, i32p, i64p, vp, i64p, i64p, i64p] + [ctypes.c_int] * 5
+        L.oracle_moe_dispatch_topk.restype = ctypes.c_int
+        L.oracle_moe_combine_topk_sum.argtypes = [vp, i32p, i64p, vp] + [ctypes.c_int] * 5
+        L.oracle_moe_combine_topk_sum.restype = ctypes.c_int
         L.oracle_f32_to_bf16_rne.argtypes = [ctypes.c_uint32]
         L.oracle_f32_to_bf16_rne.restype = ctypes.c_uint16
         L.oracle_f32_to_f16_rne.argtypes = [ctypes.c_uint32]
@@ -128,6 +133,42 @@ def alltoallv_dynamic(send: Sequence[np.ndarray], split_lengths: np.ndarray, ind
     out = np.empty((R, R, n), np.int64)
     st = lib().oracle_alltoallv_dynamic(_ptr_table(send), _i64p(Ls), n, _i64p(idx), idx.shape[1], _i64p(bl), max_block_len,
                                         _ptr_table(flat), _i64p(out), R, dt)
+    assert st >= 0
+    return out, st
+
+
+def _i32p(a: np.ndarray):
+    assert a.dtype == np.int32 and a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_int32))
+
+
+def moe_dispatch_topk(tokens: Sequence[np.ndarray], pos: np.ndarray, Crows: np.ndarray, recv: Sequence[np.ndarray], width: int, dtype):
+    """Top-k dispatch (virtual sorted send buffer, see ncclx_oracle.c).  tokens[s]: (T*width,), pos: (R, T, k) int32,
+    Crows: (R, R) rows; recv[d] written in place.  -> (RC rows, status)."""
+    dt = _dt(dtype)
+    pos = np.ascontiguousarray(pos, dtype=np.int32)
+    C = np.ascontiguousarray(Crows, dtype=np.int64)
+    R, T, k = pos.shape
+    assert C.shape == (R, R)
+    for s in range(R):
+        assert tokens[s].size >= T * width
+    for d in range(R):
+        assert recv[d].size >= int(np.maximum(C[:, d], 0).sum()) * width
+    RC, soff, roff = (np.empty((R, R), np.int64) for _ in range(3))
+    st = lib().oracle_moe_dispatch_topk(_ptr_table(tokens), _i32p(pos), _i64p(C), _ptr_table(recv), _i64p(RC), _i64p(soff),
+                                        _i64p(roff), R, T, k, width, dt)
+    assert st >= 0
+    return RC, st
+
+
+def moe_combine_topk_sum(Y: Sequence[np.ndarray], pos: np.ndarray, Crows: np.ndarray, width: int, dtype):
+    """Top-k combine fused with the fixed-order fp32 sum.  -> (list of R arrays (T*width,), status)."""
+    dt = _dt(dtype)
+    pos = np.ascontiguousarray(pos, dtype=np.int32)
+    C = np.ascontiguousarray(Crows, dtype=np.int64)
+    R, T, k = pos.shape
+    out = [np.zeros(T * width, NP_DTYPE[dt]) for _ in range(R)]
+    st = lib().oracle_moe_combine_topk_sum(_ptr_table(Y), _i32p(pos), _i64p(C), _ptr_table(out), R, T, k, width, dt)
     assert st >= 0
     return out, st
 

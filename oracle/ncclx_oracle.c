@@ -40,6 +40,7 @@
  */
 #include <stddef.h>
 #include <stdint.h>
+#include <stdlib.h>
 #include <string.h>
 
 enum { ORACLE_BF16 = 0, ORACLE_F32 = 1, ORACLE_F16 = 2, ORACLE_U8 = 3 };
@@ -120,6 +121,9 @@ static uint32_t canon_nan_f32(float f) {
     if ((u & 0x7FFFFFFFu) > 0x7F800000u) return 0x7FFFFFFFu;
     return u;
 }
+
+static float load_as_f32(const void* p, size_t i, int dtype);
+static void store_from_f32(void* p, size_t i, int dtype, float acc);
 
 /* ---- AllToAllv --------------------------------------------------------------------- */
 
@@ -218,6 +222,71 @@ int oracle_alltoallv_dynamic(const void* const* send, const int64_t* L, int n, c
             pos += bl;
         }
     }
+    return status;
+}
+
+/* ---- top-k MoE dispatch / combine (Table 3) -----
+ *
+ * The router sends every token to k experts (L383); MetaShuffling then sorts the k*T token COPIES by
+ * expert into the AllToAllv send buffer (L699).  Here that sorted buffer is VIRTUAL: pos[s][t*k+j] = p
+ * says "the j-th copy (router order j = 0..k-1) of rank s's token t sits at row p of rank s's sorted
+ * send buffer", and C[s][d] (in ROWS) splits that buffer by destination exactly as in the plain call.
+ *   dispatch: recv[d][roff[d][s] + (p - soff[s][d])] = X_s[t]       for the d with soff[s][d] <= p < soff[s][d+1]
+ *             (the plain AllToAllv of the virtual buffer; the token row is duplicated on the way)
+ *   combine:  Z_s[t] = rn_dtype( (..((float)y_0 + y_1) + ..) + y_{k-1} ),  y_j = Y[d_j][that same row],
+ *             fp32 accumulation in router order j, ONE rounding -- the inverse AllToAllv fused with the
+ *             fixed-order sum of this build's reduction (no weights: scaling is the caller's, reading 11).
+ * A position outside [0, sum_d C[s][d]) is skipped (status bit 1); a token with no valid copy gets +0.
+ * tokens[s] / out[s]: T rows of `width` elements; recv[d] / Y[d]: packed like the plain call. */
+static int locate_row(const int64_t* soff, const int64_t* roff, const int64_t* RC, int R, int s, int64_t p,
+                      int* d_out, int64_t* row_out) {
+    for (int d = 0; d < R; d++) {
+        int64_t lo = soff[(size_t)s * R + d], c = RC[(size_t)d * R + s];
+        if (p >= lo && p < lo + c) { *d_out = d; *row_out = roff[(size_t)d * R + s] + (p - lo); return 1; }
+    }
+    return 0;
+}
+
+int oracle_moe_dispatch_topk(const void* const* tokens, const int32_t* pos, const int64_t* Crows, void* const* recv,
+                             int64_t* RC, int64_t* soff, int64_t* roff, int R, int T, int k, int width, int dtype) {
+    int e = elem_size(dtype);
+    if (e == 0 || R < 1 || T < 0 || k < 1 || width < 1) return -1;
+    int status = oracle_alltoallv_offsets(Crows, R, RC, soff, roff) ? 1 : 0;
+    size_t row = (size_t)width * e;
+    for (int s = 0; s < R; s++)
+        for (int t = 0; t < T; t++)
+            for (int j = 0; j < k; j++) {
+                int64_t p = pos[((size_t)s * T + t) * k + j];
+                int d; int64_t r;
+                if (p < 0 || !locate_row(soff, roff, RC, R, s, p, &d, &r)) { status |= 2; continue; }
+                memcpy((char*)recv[d] + (size_t)r * row, (const char*)tokens[s] + (size_t)t * row, row);
+            }
+    return status;
+}
+
+int oracle_moe_combine_topk_sum(const void* const* Y, const int32_t* pos, const int64_t* Crows, void* const* out,
+                                int R, int T, int k, int width, int dtype) {
+    if (R < 1 || T < 0 || k < 1 || width < 1 || !(dtype == ORACLE_BF16 || dtype == ORACLE_F32 || dtype == ORACLE_F16)) return -1;
+    size_t rr = (size_t)R * R;
+    int64_t* RC = (int64_t*)malloc(3 * rr * sizeof(int64_t));
+    int64_t* soff = RC + rr; int64_t* roff = soff + rr;
+    int status = oracle_alltoallv_offsets(Crows, R, RC, soff, roff) ? 1 : 0;
+    for (int s = 0; s < R; s++)
+        for (int t = 0; t < T; t++)
+            for (int c = 0; c < width; c++) {
+                float acc = 0.0f;
+                int have = 0;
+                for (int j = 0; j < k; j++) {
+                    int64_t p = pos[((size_t)s * T + t) * k + j];
+                    int d; int64_t r;
+                    if (p < 0 || !locate_row(soff, roff, RC, R, s, p, &d, &r)) { status |= 2; continue; }
+                    float y = load_as_f32(Y[d], (size_t)r * width + c, dtype);
+                    acc = have ? acc + y : y;
+                    have = 1;
+                }
+                store_from_f32(out[s], (size_t)t * width + c, dtype, acc);
+            }
+    free(RC);
     return status;
 }
 

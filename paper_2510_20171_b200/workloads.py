@@ -180,3 +180,26 @@ def dynamic_moe_metadata(R: int = 64, tokens: int = 256, experts: int = 128, wid
             lst.append(0)
     idx = np.tile(np.array(lst, np.int64), (R, 1))
     return rows * width, idx, bl, J
+
+
+def topk_routing(R: int, T: int, k: int, experts: int, seed: int, s: float = 1.1):
+    """Synthetic top-k router + MetaShuffling order: every token of every rank draws k
+    DISTINCT experts (Zipf(s) popularity, Gumbel top-k), copies are sorted by (expert id, token id) into the
+    virtual send buffer.  -> (pos (R, T, k) int32: row of copy j of token t in rank s's sorted buffer;
+    Crows (R, R) int64: rows sent s -> d, expert e living on rank e // (experts // R)).
+    A labelling of the input, not arithmetic of the method (no offsets, no sums of payload)."""
+    rng = np.random.default_rng(seed)
+    logp = -s * np.log(np.arange(experts) + 1.0)
+    per = experts // R
+    pos = np.empty((R, T, k), np.int32)
+    C = np.zeros((R, R), np.int64)
+    for r in range(R):
+        g = rng.gumbel(size=(T, experts)) + logp
+        top = np.argsort(-g, axis=1)[:, :k]                       # router order j = 0..k-1
+        flat_e = top.reshape(-1)
+        order = np.argsort(flat_e * (T * k) + np.arange(T * k), kind="stable")   # by expert, then (token, j)
+        p = np.empty(T * k, np.int64)
+        p[order] = np.arange(T * k)
+        pos[r] = p.reshape(T, k).astype(np.int32)
+        C[r] = np.bincount(flat_e // per, minlength=R)
+    return pos, C
