@@ -413,6 +413,7 @@ def main():
             del a, g
         per["next1_alltoallv_dynamic_R64_tok256"] = dynamic_extra(torch, nx, peak, min(args.latency_replays, 2000))
         per["next2_reducecopy_cta_sweep"] = reducecopy_extra(torch, nx, peak)
+        per["next3_topk_R64_T4096_k4"] = topk_extra(torch, nx, peak)
         line["per_config"] = per
 
     # ---- e2e: same step through the host-buffer C ABI (H2D + kernels + D2H inside the timed region) --------
@@ -461,6 +462,29 @@ def dynamic_extra(torch, nx, peak, reps):
     p50 = float(np.percentile(t, 50))
     return {"replays": reps, "p50_us": round(p50 * 1e3, 2), "p99_us": round(float(np.percentile(t, 99)) * 1e3, 2),
             "bytes_each_way": moved, "segments": int(bl.sum()), **frac(2 * moved / (p50 * 1e-3) / 1e9, peak)}
+
+
+def topk_extra(torch, nx, peak, R=64, T=4096, k=4, width=5120):
+    """top-k dispatch with duplication on the way + combine fused with the fixed-order sum,
+    at config-3 scale (k*T = 16384 virtual rows per rank): dispatch reads T rows and writes k*T, combine the reverse."""
+    pos, C = W.topk_routing(R, T, k, 128, seed=7)
+    X = [W.torch_values(T * width, "bf16", 7000 + s) for s in range(R)]
+    recv = [torch.empty(max(int(C[:, d].sum()), 1) * width, dtype=torch.bfloat16, device="cuda") for d in range(R)]
+    Z = [torch.empty(T * width, dtype=torch.bfloat16, device="cuda") for _ in range(R)]
+    dpos, dC = torch.from_numpy(pos).cuda(), torch.from_numpy(C).cuda()
+    dRC = torch.empty_like(dC)
+    xt, rt, zt = nx.device_ptr_table(X), nx.device_ptr_table(recv), nx.device_ptr_table(Z)
+    rows = R * T * width * 2
+    t = event_times_ms(torch, lambda: nx.ncclx_moe_dispatch_topk_dev(xt, dpos, dC, rt, dRC, R, T, k, width, "bf16"), 10)
+    td = float(np.median(t))
+    t = event_times_ms(torch, lambda: nx.ncclx_moe_combine_topk_sum_dev(rt, dpos, dC, zt, R, T, k, width, "bf16"), 10)
+    tc = float(np.median(t))
+    nbytes = (1 + k) * rows
+    ok = all(torch.equal(z.float(), k * x.float()) for z, x in zip(Z[:4], X[:4]))    # identity experts: Z = k * X exactly
+    return {"dispatch": {"ms": round(td, 4), **frac(nbytes / (td * 1e-3) / 1e9, peak)},
+            "combine": {"ms": round(tc, 4), **frac(nbytes / (tc * 1e-3) / 1e9, peak)},
+            "algorithmic_bytes_each": nbytes, "combine_of_dispatch_equals_k_times_x": bool(ok),
+            "note": "unfused path would move 2*k*rows per direction plus the shuffle / the separate k-way sum"}
 
 
 def reducecopy_extra(torch, nx, peak):

@@ -173,6 +173,30 @@ int ncclx_reducescatter_sum(const void* const* send, void* const* recv, size_t r
 int ncclx_reducecopy_sum(const void* a, const void* b, void* out, void* fwd, size_t count, ncclx_dtype_t dtype,
                          size_t chunk_bytes, int num_ctas, ncclx_stream_t stream);
 
+/* ---- top-k MoE dispatch / combine ("which k experts a given token should go to"; Table 3) ---- *
+ *
+ * Rank s holds T token rows X_s (T x width elements).  The router picked k experts per token and the
+ * shuffle (MetaShuffling, L699) ordered the k*T token COPIES by expert; that sorted send buffer stays
+ * VIRTUAL here.  Device-resident metadata, read when the kernels execute:
+ *   pos_dev          int32[R*T*k]: pos[(s*T+t)*k+j] = row of copy j (router order) of token t in rank s's
+ *                    virtual sorted buffer, a permutation of [0, k*T)
+ *   sendcounts_rows  int64[R*R]: C[s*R+d] = ROWS of that buffer going to rank d (sum_d = k*T)
+ * ncclx_moe_dispatch_topk_dev: the AllToAllv of the virtual buffer with the duplication done on the way --
+ *   recv[d][roff[d][s] + (p - soff[s][d])] = X_s[t]  for p = pos[s][t][j] in [soff[s][d], soff[s][d+1]);
+ *   recv[d] is packed exactly as by ncclx_alltoallv_dev (rows of width elements); recvcounts_rows_dev = C^T.
+ * ncclx_moe_combine_topk_sum_dev: the inverse AllToAllv fused with the fixed-order sum --
+ *   out[s][t] = rn_dtype( (..((float)y_0 + y_1) + ..) + y_{k-1} ),  y_j = the row of expert_out[d_j] that
+ *   dispatch wrote copy j to; fp32 accumulation in router order j, one rounding, NaN canonical.
+ * A position outside [0, sum_d C[s][d]) is skipped (device status bit 1); a token with no valid copy
+ * yields +0.  Duplicate positions are undefined.  1 <= k <= 32.  dtype: dispatch any, combine BF16/F32/F16.
+ * Rows and bases that are multiples of 32 bytes take the 256-bit path.  Capturable. */
+int ncclx_moe_dispatch_topk_dev(const void* const* tokens, const int32_t* pos_dev, const int64_t* sendcounts_rows_dev,
+                                void* const* recv, int64_t* recvcounts_rows_dev, int R, int T, int k, int width,
+                                ncclx_dtype_t dtype, ncclx_stream_t stream);
+int ncclx_moe_combine_topk_sum_dev(const void* const* expert_out, const int32_t* pos_dev,
+                                   const int64_t* sendcounts_rows_dev, void* const* out, int R, int T, int k,
+                                   int width, ncclx_dtype_t dtype, ncclx_stream_t stream);
+
 /* ---- host-buffer forms (the end-to-end path: H2D + kernels + D2H inside the call) ------ *
  *
  * Same semantics, but every pointer is a HOST pointer (pinned memory gives full PCIe
@@ -216,6 +240,7 @@ typedef enum {
     NCCLX_KERNEL_COPY = 1,   /* byte-balanced segment copy                    */
     NCCLX_KERNEL_REDUCE = 2, /* rank-order sum                                */
     NCCLX_KERNEL_DYN = 3,    /* AllToAllvDynamic metadata kernels (prep + desc) */
+    NCCLX_KERNEL_TOPK = 4,   /* top-k dispatch / combine kernels               */
     NCCLX_KERNEL_COUNT_
 } ncclx_kernel_t;
 

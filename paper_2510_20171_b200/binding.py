@@ -29,7 +29,7 @@ PARAM_COPY_STATIC_EIGHTHS = 9
 PARAM_COPY_KMAX = 10
 PARAM_COPY_KMAX_LONG = 11
 
-KERNEL_COUNTS, KERNEL_COPY, KERNEL_REDUCE, KERNEL_DYN = 0, 1, 2, 3
+KERNEL_COUNTS, KERNEL_COPY, KERNEL_REDUCE, KERNEL_DYN, KERNEL_TOPK = 0, 1, 2, 3, 4
 
 # every symbol include/ncclx_b200.h declares (tests check the .so exports all of them)
 SYMBOLS = [
@@ -38,7 +38,7 @@ SYMBOLS = [
     "ncclx_allreduce_sum", "ncclx_reducescatter_sum", "ncclx_alltoallv_host", "ncclx_allreduce_sum_host",
     "ncclx_reducescatter_sum_host", "ncclx_set_param", "ncclx_get_param", "ncclx_profile_read",
     "ncclx_profile_reset", "ncclx_launch_count", "ncclx_sm_count", "ncclx_init_dynamic", "ncclx_alltoallv_dynamic_dev",
-    "ncclx_reducecopy_sum",
+    "ncclx_reducecopy_sum", "ncclx_moe_dispatch_topk_dev", "ncclx_moe_combine_topk_sum_dev",
 ]
 
 
@@ -79,6 +79,8 @@ def lib() -> ctypes.CDLL:
         L.ncclx_alltoallv_dynamic_dev.argtypes = [vp, vp, ctypes.c_int, vp, ctypes.c_int, vp, ctypes.c_int, vp, vp,
                                                   ctypes.c_int, ctypes.c_int, vp]
         L.ncclx_reducecopy_sum.argtypes = [vp, vp, vp, vp, ctypes.c_size_t, ctypes.c_int, ctypes.c_size_t, ctypes.c_int, vp]
+        L.ncclx_moe_dispatch_topk_dev.argtypes = [vp, vp, vp, vp, vp] + [ctypes.c_int] * 5 + [vp]
+        L.ncclx_moe_combine_topk_sum_dev.argtypes = [vp, vp, vp, vp] + [ctypes.c_int] * 5 + [vp]
         L.ncclx_set_param.argtypes = [ctypes.c_int, i64]
         L.ncclx_get_param.argtypes = [ctypes.c_int, i64p]
         L.ncclx_profile_read.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double), i64p]
@@ -177,6 +179,20 @@ def ncclx_alltoallv_dynamic_dev(send_table, split_lengths_dev, nsplits: int, ind
 def ncclx_allreduce_sum(send_table, recv_table, count: int, R: int, dtype, stream=None) -> None:
     _ck(lib().ncclx_allreduce_sum(_ptr(send_table), _ptr(recv_table), count, R, _dt(dtype), _stream(stream)),
         "ncclx_allreduce_sum")
+
+
+def ncclx_moe_dispatch_topk_dev(tokens_table, pos_dev, sendcounts_rows_dev, recv_table, recvcounts_rows_dev, R: int, T: int,
+                                k: int, width: int, dtype, stream=None) -> None:
+    _ck(lib().ncclx_moe_dispatch_topk_dev(_ptr(tokens_table), _ptr(pos_dev), _ptr(sendcounts_rows_dev), _ptr(recv_table),
+                                          _ptr(recvcounts_rows_dev), R, T, k, width, _dt(dtype), _stream(stream)),
+        "ncclx_moe_dispatch_topk_dev")
+
+
+def ncclx_moe_combine_topk_sum_dev(expert_out_table, pos_dev, sendcounts_rows_dev, out_table, R: int, T: int, k: int,
+                                   width: int, dtype, stream=None) -> None:
+    _ck(lib().ncclx_moe_combine_topk_sum_dev(_ptr(expert_out_table), _ptr(pos_dev), _ptr(sendcounts_rows_dev),
+                                             _ptr(out_table), R, T, k, width, _dt(dtype), _stream(stream)),
+        "ncclx_moe_combine_topk_sum_dev")
 
 
 def ncclx_reducecopy_sum(a, b, out, fwd, count: int, dtype, chunk_bytes: int = 0, num_ctas: int = 0, stream=None) -> None:

@@ -34,7 +34,7 @@ struct CountsArgs {
     Workspace ws;
     int R;
     int W;                        // columns per CTA (<= 32)
-    int elemSize;
+    long long elemSize;               // bytes per count unit (an element, or a whole row for the top-k calls)
     ClassParams cls;
 };
 
