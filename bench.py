@@ -255,7 +255,7 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the per-config table (cfg1/cfg5 latency, cfg2 warm/cold)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--latency-replays", type=int, default=10000)
-    ap.add_argument("--probe", type=int, default=0, choices=[0, 1, 2, 3, 4, 5],
+    ap.add_argument("--probe", type=int, default=0, choices=[0, 1, 2, 3, 4, 5, 6],
                     help="run ONLY BASELINE.json config N eagerly for --steps iterations (for ncu captures of one config)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -414,6 +414,7 @@ def main():
         per["next1_alltoallv_dynamic_R64_tok256"] = dynamic_extra(torch, nx, peak, min(args.latency_replays, 2000))
         per["next2_reducecopy_cta_sweep"] = reducecopy_extra(torch, nx, peak)
         per["next3_topk_R64_T4096_k4"] = topk_extra(torch, nx, peak)
+        per["next4_latency"] = latency_extra(torch, nx, peak, min(args.latency_replays, 2000))
         line["per_config"] = per
 
     # ---- e2e: same step through the host-buffer C ABI (H2D + kernels + D2H inside the timed region) --------
@@ -503,9 +504,69 @@ def reducecopy_extra(torch, nx, peak):
     return res
 
 
+def graph_p50(torch, enqueue, reps, warm=20):
+    """Capture `enqueue` once (after one eager run on a side stream), time `reps` replays with CUDA events."""
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        enqueue()
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        enqueue()
+    t = event_times_ms(torch, g.replay, reps, warm=warm)
+    return {"p50_us": round(float(np.percentile(t, 50)) * 1e3, 2), "p99_us": round(float(np.percentile(t, 99)) * 1e3, 2)}
+
+
+def latency_extra(torch, nx, peak, reps):
+    """SURVEY 8(f) NEXT-4 (PAPER.md L447-483): (a) config 1 as ONE fused kernel vs the two-kernel path;
+    (b) dispatch + combine back to back (the MoE layer's two consecutive AllToAlls): plain stream order vs the
+    split-phase form with two plan slots, where the combine's metadata phase runs beside the dispatch's payload."""
+    res = {}
+    a1 = A2A(W.a2a_config(1), torch, nx, with_back=True)
+
+    def pair1():
+        a1.dispatch(); a1.combine()
+    res["cfg1_one_kernel"] = graph_p50(torch, a1.dispatch, reps)
+    res["cfg1_pair_one_kernel_each"] = graph_p50(torch, pair1, reps)
+    nx.ncclx_set_param(nx.PARAM_FUSED_MAX_RANKS, 0)
+    res["cfg1_two_kernels"] = graph_p50(torch, a1.dispatch, reps)
+    res["cfg1_pair_two_kernels_each"] = graph_p50(torch, pair1, reps)
+    nx.ncclx_set_param(nx.PARAM_FUSED_MAX_RANKS, 32)
+    del a1
+    a5 = A2A(W.a2a_config(5), torch, nx, with_back=True)
+    side = torch.cuda.Stream()
+
+    def pair_plain():
+        a5.dispatch(); a5.combine()
+
+    def pair_double_buffered():
+        main = torch.cuda.current_stream()
+        nx.ncclx_alltoallv_prepare_dev(0, a5.st, a5.C, a5.rt, a5.RC, a5.R, a5.cfg.dtype)
+        side.wait_stream(main)
+        with torch.cuda.stream(side):
+            nx.ncclx_alltoallv_prepare_dev(1, a5.rt, a5.RC, a5.bt, a5.C2, a5.R, a5.cfg.dtype)
+        nx.ncclx_alltoallv_execute_dev(0)
+        main.wait_stream(side)
+        nx.ncclx_alltoallv_execute_dev(1)
+    res["cfg5_pair_stream_order"] = graph_p50(torch, pair_plain, reps)
+    res["cfg5_pair_double_buffered"] = graph_p50(torch, pair_double_buffered, reps)
+    ok = all(bool((a5.back[s][:n] == a5.send[s][:n]).all()) for s, n in enumerate(a5.send_elems) if n)
+    res["cfg5_pair_roundtrip_identity"] = ok
+    res["cfg5_pair_bytes"] = 4 * a5.bytes_one_way
+    for k in ("cfg5_pair_stream_order", "cfg5_pair_double_buffered"):
+        res[k].update(frac(4 * a5.bytes_one_way / (res[k]["p50_us"] * 1e-6) / 1e9, peak))
+    return res
+
+
 def probe(args, torch, nx, peak):
     """One config, eager launches, CUDA-event time per call (the command ncu captures are taken from)."""
     n = args.probe
+    if n == 6:
+        print(json.dumps({"probe": "next4_latency", **latency_extra(torch, nx, peak, args.steps)}))
+        nx.ncclx_finalize()
+        return 0
     if n in (1, 3, 5):
         w = A2A(W.a2a_config(n), torch, nx, with_back=False)
         fn, nbytes = w.dispatch, 2 * w.bytes_one_way

@@ -99,16 +99,42 @@ int ncclx_version(void);
  * overlap.  Segment addresses may have any element alignment; full speed is only promised
  * when every segment's source address, destination address and byte length are multiples of
  * 16 (the cp.async.bulk path); everything else takes the vector path.
- * The inverse ("combine") is the same call with send := recv, sendcounts := recvcounts.   */
+ * The inverse ("combine") is the same call with send := recv, sendcounts := recvcounts.
+ * For R <= 32 (NCCLX_PARAM_FUSED_MAX_RANKS) the call is ONE kernel launch (the small-message fast path,
+ * PAPER.md L483): every CTA rebuilds offsets and work list from the <= 8 KB count matrix in shared memory
+ * and picks the tile size from the byte total; results are identical to the two-kernel path.          */
 int ncclx_alltoallv_dev(const void* const* send, const int64_t* sendcounts_dev, void* const* recv,
                         int64_t* recvcounts_dev, int R, ncclx_dtype_t dtype, ncclx_stream_t stream);
+
+/* ---- split-phase form and plan slots (section 6.2) ---------- *
+ *
+ * The paper splits a small-message AllToAll into the control exchange (~50 % of the latency, Table 2)
+ * and the payload puts, and removes the exchange from the critical path: handles are exchanged once, and
+ * "double buffering" lets "two consecutive AllToAlls ... always use different receive buffers" so that no
+ * barrier separates them (L483).  Here the control exchange is steps a1-a3 (transpose, offsets, work list)
+ * and the payload is step a4, and the library's workspace is the shared resource that would serialise two
+ * calls; so it exists NCCLX_NUM_PLANS times:
+ *   ncclx_alltoallv_prepare_dev(plan, ...)  enqueues ONLY a1-a3 into plan slot `plan`: recvcounts_dev is
+ *       written, offsets and the work list stay in the slot.  Counts are read when it EXECUTES (L401).
+ *   ncclx_alltoallv_execute_dev(plan)       enqueues ONLY a4 for the slot's work list (buffers = the ones given
+ *       to prepare).  It may run any number of times per prepare (the claim counters reset themselves).
+ * prepare(p) must be ordered before execute(p), and execute(p) before the next prepare(p), by stream order
+ * or events; different slots are independent, so the combine's prepare (whose counts are the dispatch's
+ * recvcounts, complete as soon as the dispatch's prepare is) can run on a second stream WHILE the dispatch's
+ * payload moves.  ncclx_alltoallv_dev == prepare(0) + execute(0) for R > 32, one fused kernel otherwise;
+ * the dynamic and top-k calls also use slot 0.  Arguments as for ncclx_alltoallv_dev; 0 <= plan <
+ * NCCLX_NUM_PLANS; execute returns NCCLX_ERR_ARG for a slot that was never prepared.  Both capturable. */
+#define NCCLX_NUM_PLANS 4
+int ncclx_alltoallv_prepare_dev(int plan, const void* const* send, const int64_t* sendcounts_dev, void* const* recv,
+                                int64_t* recvcounts_dev, int R, ncclx_dtype_t dtype, ncclx_stream_t stream);
+int ncclx_alltoallv_execute_dev(int plan, ncclx_stream_t stream);
 
 /* Copies the offset matrices of the LAST enqueued ncclx_alltoallv_dev to HOST int64[R*R]
  * arrays (either may be NULL).  Synchronises `stream`; not capturable (NCCLX_ERR_CAPTURE). */
 int ncclx_alltoallv_last_offsets(int64_t* soff_host, int64_t* roff_host, int R, ncclx_stream_t stream);
 
-/* Reads and clears the device status word into *status_host (bit 0: a negative count was
- * seen).  Synchronises `stream`; not capturable. */
+/* Reads and clears the device status word (the OR over all plan slots) into *status_host (bit 0: a
+ * negative count was seen).  Synchronises `stream`; not capturable. */
 int ncclx_device_status(uint32_t* status_host, ncclx_stream_t stream);
 
 /* ---- AllToAllvDynamic: the paper's full metadata interface (section 6.1.2) ---- *
@@ -229,6 +255,8 @@ typedef enum {
     NCCLX_PARAM_COPY_STATIC_EIGHTHS = 9, /* 0..8: share of copy tiles assigned statically per engine, default 0 */
     NCCLX_PARAM_COPY_KMAX = 10,       /* max tiles per dynamic claim when segments are short (1..64), default 6 */
     NCCLX_PARAM_COPY_KMAX_LONG = 11,  /* same when segments average >= 8 tiles (1..64), default 2          */
+    NCCLX_PARAM_FUSED_MAX_RANKS = 12, /* ncclx_alltoallv_dev runs as ONE kernel for R <= this (0..32; 0 = never), default 32 */
+    NCCLX_PARAM_FUSED_MIN_TILE_SHIFT = 13, /* smallest bulk tile the single-launch path may choose (log2 bytes, 10..16), default 12 */
     NCCLX_PARAM_COUNT_
 } ncclx_param_t;
 
@@ -241,6 +269,7 @@ typedef enum {
     NCCLX_KERNEL_REDUCE = 2, /* rank-order sum                                */
     NCCLX_KERNEL_DYN = 3,    /* AllToAllvDynamic metadata kernels (prep + desc) */
     NCCLX_KERNEL_TOPK = 4,   /* top-k dispatch / combine kernels               */
+    NCCLX_KERNEL_FUSED = 5,  /* single-launch AllToAllv (scan + work list + copy in one kernel) */
     NCCLX_KERNEL_COUNT_
 } ncclx_kernel_t;
 

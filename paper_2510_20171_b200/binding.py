@@ -28,8 +28,11 @@ PARAM_PDL = 8
 PARAM_COPY_STATIC_EIGHTHS = 9
 PARAM_COPY_KMAX = 10
 PARAM_COPY_KMAX_LONG = 11
+PARAM_FUSED_MAX_RANKS = 12
+PARAM_FUSED_MIN_TILE_SHIFT = 13
+NUM_PLANS = 4
 
-KERNEL_COUNTS, KERNEL_COPY, KERNEL_REDUCE, KERNEL_DYN, KERNEL_TOPK = 0, 1, 2, 3, 4
+KERNEL_COUNTS, KERNEL_COPY, KERNEL_REDUCE, KERNEL_DYN, KERNEL_TOPK, KERNEL_FUSED = 0, 1, 2, 3, 4, 5
 
 # every symbol include/ncclx_b200.h declares (tests check the .so exports all of them)
 SYMBOLS = [
@@ -39,6 +42,7 @@ SYMBOLS = [
     "ncclx_reducescatter_sum_host", "ncclx_set_param", "ncclx_get_param", "ncclx_profile_read",
     "ncclx_profile_reset", "ncclx_launch_count", "ncclx_sm_count", "ncclx_init_dynamic", "ncclx_alltoallv_dynamic_dev",
     "ncclx_reducecopy_sum", "ncclx_moe_dispatch_topk_dev", "ncclx_moe_combine_topk_sum_dev",
+    "ncclx_alltoallv_prepare_dev", "ncclx_alltoallv_execute_dev",
 ]
 
 
@@ -69,6 +73,8 @@ def lib() -> ctypes.CDLL:
         L.ncclx_strerror.restype = ctypes.c_char_p
         L.ncclx_last_cuda_error_string.restype = ctypes.c_char_p
         L.ncclx_alltoallv_dev.argtypes = [vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, vp]
+        L.ncclx_alltoallv_prepare_dev.argtypes = [ctypes.c_int, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, vp]
+        L.ncclx_alltoallv_execute_dev.argtypes = [ctypes.c_int, vp]
         L.ncclx_alltoallv_last_offsets.argtypes = [vp, vp, ctypes.c_int, vp]
         L.ncclx_device_status.argtypes = [ctypes.POINTER(ctypes.c_uint32), vp]
         for f in (L.ncclx_allreduce_sum, L.ncclx_reducescatter_sum, L.ncclx_allreduce_sum_host,
@@ -146,6 +152,16 @@ def device_ptr_table(tensors: Sequence, device=None):
 def ncclx_alltoallv_dev(send_table, sendcounts_dev, recv_table, recvcounts_dev, R: int, dtype, stream=None) -> None:
     _ck(lib().ncclx_alltoallv_dev(_ptr(send_table), _ptr(sendcounts_dev), _ptr(recv_table), _ptr(recvcounts_dev),
                                   R, _dt(dtype), _stream(stream)), "ncclx_alltoallv_dev")
+
+
+def ncclx_alltoallv_prepare_dev(plan: int, send_table, sendcounts_dev, recv_table, recvcounts_dev, R: int, dtype,
+                                stream=None) -> None:
+    _ck(lib().ncclx_alltoallv_prepare_dev(plan, _ptr(send_table), _ptr(sendcounts_dev), _ptr(recv_table),
+                                          _ptr(recvcounts_dev), R, _dt(dtype), _stream(stream)), "ncclx_alltoallv_prepare_dev")
+
+
+def ncclx_alltoallv_execute_dev(plan: int, stream=None) -> None:
+    _ck(lib().ncclx_alltoallv_execute_dev(plan, _stream(stream)), "ncclx_alltoallv_execute_dev")
 
 
 def ncclx_alltoallv_last_offsets(R: int, stream=None):

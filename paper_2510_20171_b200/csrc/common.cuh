@@ -22,11 +22,12 @@ static_assert(sizeof(SegDesc) == 32, "SegDesc must be 32 bytes");
 
 enum { LIST_BULK = 0, LIST_VEC = 1 };
 
-// Device-resident control block (zeroed by the counts kernel before every copy kernel).
+// Device-resident control block.  The claim counters are zero between kernels: the copy kernel's last
+// CTA resets them on its way out (workctl_checkout), and the counts kernel zeroes them as well.
 struct WorkCtl {
     unsigned int next[2];     // dynamic tile-claim counters, one per work list
     unsigned int status;      // sticky: bit 0 = negative count seen
-    unsigned int pad;
+    unsigned int done;        // CTAs of the running copy kernel that have drained their engines
 };
 
 struct Workspace {
@@ -128,6 +129,8 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 __device__ __forceinline__ void fence_mbar_init() {
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
+// orders this thread's generic-proxy accesses to shared memory before later async-proxy (TMA) accesses
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
 }

@@ -44,7 +44,8 @@ struct CopyArgs {
 // this list is a ballot over registers instead of a chain of dependent L2 reads (config 5 has a new
 // segment every ~2 tiles).  Only a fresh claim pays the search: smem binary search over columns,
 // then a warp-wide 32-ary search over the column's tile prefixes.
-template <int L>
+// SM = true: the descriptor table lives in SHARED memory (single-launch path, fused_kernel.cuh).
+template <int L, bool SM = false>
 struct Cursor {
     const SegDesc* desc;
     const int* colBase;                    // smem, ncols+1 entries, colBase[ncols] = total tiles
@@ -65,7 +66,7 @@ struct Cursor {
     __device__ __forceinline__ void load_desc(int qq, uint4& a, uint4& b) const {
         if (qq < RR) {
             const uint4* p = reinterpret_cast<const uint4*>(desc + qq);
-            a = __ldg(p); b = __ldg(p + 1);
+            if constexpr (SM) { a = p[0]; b = p[1]; } else { a = __ldg(p); b = __ldg(p + 1); }
         } else {
             a = make_uint4(0, 0, 0, 0); b = make_uint4(0, 0, 0, 0);
         }
@@ -85,30 +86,34 @@ struct Cursor {
         q = qw + fromLane;
     }
 
-    __device__ __forceinline__ void init(const CopyArgs& a, const int* colBase_, int nEngines_, int engineId_, int kmax_) {
-        desc = a.desc; colBase = colBase_; counter = &a.ctl->next[L]; cls = a.cls;
-        ncols = a.ncols; colLen = a.colLen; RR = a.ncols * a.colLen; tileShift = a.cls.tileShift[L]; total = colBase_[a.ncols];
+    // staticK_ tiles per engine are assigned statically ([engineId*staticK, +staticK): no atomic on the
+    // start-up path); tiles >= staticK*nEngines are claimed dynamically, IN ORDER, in guided chunks.
+    // Measured on B200: the in-order dynamic claim keeps all SMs inside one moving window of HBM and is
+    // ~7 % faster than contiguous static ranges (148 far-apart streams), so the two-kernel path defaults
+    // to fully dynamic (staticK = 0); the single-launch path takes one static tile per engine.
+    __device__ __forceinline__ void init(const SegDesc* desc_, const int* colBase_, unsigned int* counter_,
+                                         const ClassParams& cls_, int ncols_, int colLen_, int nEngines_, int engineId_,
+                                         int kmax_, int kmaxLong_, int staticK_) {
+        desc = desc_; colBase = colBase_; counter = counter_; cls = cls_;
+        ncols = ncols_; colLen = colLen_; RR = ncols_ * colLen_; tileShift = cls_.tileShift[L]; total = colBase_[ncols_];
         nEngines = nEngines_; engineId = engineId_;
         // long segments (>= 8 tiles each on average): claims resolve inside the cached window, so take
         // small chunks and keep all SMs in a tight moving window of HBM; short segments: every claim
         // pays a search, amortise it over more tiles.
         longSegs = total >= 8 * RR;
-        kmax = longSegs ? a.kmaxLong : kmax_;
-        // staticEighths/8 of the tiles can be split evenly and statically (contiguous range per engine);
-        // the rest is claimed dynamically, IN ORDER, in guided chunks.  Measured on B200: the in-order
-        // dynamic claim keeps all SMs inside one moving window of HBM and is ~7 % faster than contiguous
-        // static ranges (148 far-apart streams), so the default is fully dynamic (staticEighths = 0).
-        staticK = (int)(((long long)total * a.staticEighths / 8) / nEngines);
+        kmax = longSegs ? kmaxLong_ : kmax_;
+        staticK = staticK_;
         kmin = total >= 8 * nEngines ? 2 : 1;
         dynBase = staticK * nEngines;
-        pendCur = pendK = 0;
+        pendCur = total; pendK = 0;        // reads as "drained" unless a claim is issued
         t = tEnd = 0; q = 0; kInSeg = segTiles = 0; src = dst = 0; bytes = 0;
         qw = qn = 0; w0 = w1 = n0 = n1 = make_uint4(0, 0, 0, 0);
         first = true;
         haveWindow = false;
         exhausted = (total == 0);
-        if (!exhausted) claim_issue(dynBase);
+        if (total > dynBase) claim_issue(dynBase);
     }
+    __device__ __forceinline__ bool uses_counter() const { return total > dynBase; }
 
     // Lane 0 issues the atomic for the next dynamic chunk; the result is only consumed by claim_take(),
     // so its L2 round trip overlaps the tiles of the current chunk.
@@ -139,7 +144,8 @@ struct Cursor {
             for (int u = 0; u < 4; ++u) {
                 const int b = lane * 4 + u;
                 const int idx = s0 + min((b + 1) * step, n) - 1;
-                cnt += (__ldg(&col[idx].pfx[L]) <= tl) ? 1 : 0;
+                const int pv = SM ? col[idx].pfx[L] : __ldg(&col[idx].pfx[L]);
+                cnt += (pv <= tl) ? 1 : 0;
             }
             int m = cnt;                   // blocks entirely <= tl (monotone, so a plain count)
 #pragma unroll
@@ -220,6 +226,7 @@ struct Cursor {
             first = false;
             cur = engineId * staticK;
             k = staticK;
+            if (cur >= total) { exhausted = true; return false; }
         } else {
             first = false;
             cur = __shfl_sync(0xffffffffu, pendCur, 0);
@@ -281,6 +288,112 @@ __device__ __forceinline__ void warp_copy_bytes(const unsigned char* src, unsign
     if (lane_id() < tail) dst[done + lane_id()] = __ldg(src + done + lane_id());
 }
 
+// ================= bulk engine: byte-granular TMA ring driven by one elected lane (one warp) ========
+// The ring is a circular BYTE buffer (not fixed-size stages): every tile takes exactly
+// align128(len) bytes, so short tiles (config 5: 10-28 KiB) keep as many bytes in flight as
+// long ones.  Up to COPY_SLOTS tiles are outstanding; slot j's bookkeeping (destination,
+// length, smem offset, virtual start) lives in the registers of lane j.
+template <bool SM>
+__device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned char* ring, unsigned long long* mbar,
+                                            const unsigned int ringBytes) {
+    const int lane = lane_id();
+    const unsigned int tileBytes = 1u << cur.tileShift;
+    const uint32_t ring0 = smem_u32(ring);
+    unsigned long long mDst = 0;          // slot registers (lane j <-> slot j)
+    unsigned int mLen = 0, mOff = 0, mV = 0;
+    unsigned int vHead = 0, phys = 0;     // virtual (mod 2^32) and physical allocation offsets
+    int iLoad = 0, iStore = 0, freed = 0;  // stores [0, freed) have finished reading their smem
+    bool more = cur.ensure();
+    while (true) {
+        // fill: issue loads while a slot and enough ring bytes are free
+        while (more) {
+            const long long off = cur.tile_off();
+            const long long rest = cur.bytes - off;
+            const unsigned int len = rest < (long long)tileBytes ? (unsigned int)rest : tileBytes;
+            const unsigned int len16 = len & ~15u;
+            const unsigned char* srcp = reinterpret_cast<const unsigned char*>(cur.src + off);
+            unsigned char* dstp = reinterpret_cast<unsigned char*>(cur.dst + off);
+            if (len16) {
+                if (iLoad - freed >= COPY_SLOTS) break;
+                const unsigned int pad = phys + len16 > ringBytes ? ringBytes - phys : 0u;   // wrap
+                const unsigned int vTail = freed < iLoad ? __shfl_sync(0xffffffffu, mV, freed % COPY_SLOTS) : vHead;
+                if (vHead + pad + len16 - vTail > ringBytes) break;
+                const unsigned int vStart = vHead + pad;
+                const unsigned int po = pad ? 0u : phys;
+                const int slot = iLoad % COPY_SLOTS;
+                if (lane == slot) { mDst = (unsigned long long)dstp; mLen = len16; mOff = po; mV = vStart; }
+                if (lane == 0) {
+                    const uint32_t bar = smem_u32(&mbar[slot]);
+                    mbar_expect_tx(bar, len16);
+                    bulk_g2s(ring0 + po, srcp, len16, bar);
+                }
+                const unsigned int adv = (len16 + 127u) & ~127u;
+                vHead = vStart + adv;
+                phys = po + adv;
+                if (phys >= ringBytes) phys = 0;
+                ++iLoad;
+            }
+            const int tail = (int)(len & 15u);        // only the last tile of a ragged segment
+            if (lane < tail) dstp[len16 + lane] = __ldg(srcp + len16 + lane);
+            cur.next();
+            more = cur.ensure();
+        }
+        if (iStore == iLoad) {
+            if (!more) break;
+            // every issued tile is stored but the next one does not fit behind the last store's
+            // not-yet-released bytes: release everything and restart the ring at offset 0
+            if (lane == 0) bulk_wait_read<0>();
+            freed = iStore;
+            phys = 0;
+            continue;
+        }
+        const int slot = iStore % COPY_SLOTS;
+        mbar_wait(smem_u32(&mbar[slot]), (uint32_t)((iStore / COPY_SLOTS) & 1));
+        const unsigned int dlo = __shfl_sync(0xffffffffu, (unsigned int)mDst, slot);
+        const unsigned int dhi = __shfl_sync(0xffffffffu, (unsigned int)(mDst >> 32), slot);
+        const unsigned int slen = __shfl_sync(0xffffffffu, mLen, slot);
+        const unsigned int soff = __shfl_sync(0xffffffffu, mOff, slot);
+        if (lane == 0) {
+            bulk_s2g(reinterpret_cast<void*>(((unsigned long long)dhi << 32) | dlo), ring0 + soff, slen);
+            bulk_commit();
+            if (more) bulk_wait_read<1>();            // releases the smem of every store but this one
+        }
+        freed = max(freed, iStore);                   // (only consulted while `more`)
+        ++iStore;
+        __syncwarp();
+    }
+    if (lane == 0) bulk_wait_all<0>();
+}
+
+// ================= vector engine: one warp per tile ===========================================
+template <bool SM>
+__device__ __forceinline__ void vector_engine(Cursor<LIST_VEC, SM>& cur) {
+    const long long tileBytes = 1ll << cur.tileShift;
+    while (cur.ensure()) {
+        const long long off = cur.tile_off();
+        const long long rest = cur.bytes - off;
+        const long long len = rest < tileBytes ? rest : tileBytes;
+        warp_copy_bytes(reinterpret_cast<const unsigned char*>(cur.src + off),
+                        reinterpret_cast<unsigned char*>(cur.dst + off), len);
+        cur.next();
+    }
+}
+
+// The claim counters reset themselves: every CTA checks out once all its engines are drained (each
+// engine has consumed every atomic it issued by then), and the last one out zeroes the counters, so the
+// same work list can be executed again (ncclx_alltoallv_execute_dev) and the single-launch path needs
+// no preceding kernel to clear them.  `used` must be grid-uniform.
+__device__ __forceinline__ void workctl_checkout(WorkCtl* ctl, bool used) {
+    __syncthreads();
+    if (threadIdx.x == 0 && used) {
+        __threadfence();
+        if (atomicAdd(&ctl->done, 1u) == gridDim.x - 1) {
+            ctl->next[0] = 0u; ctl->next[1] = 0u; ctl->done = 0u;
+            __threadfence();
+        }
+    }
+}
+
 // dynamic smem layout: [ring: ringBytes][mbar: COPY_SLOTS x u64][colBase bulk: R+1 ints][colBase vec: R+1 ints]
 __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const CopyArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -313,96 +426,22 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
     }
     __syncthreads();
 
+    constexpr int NV = COPY_THREADS / 32 - 1;          // vector engines per CTA
+    const int nB = (int)gridDim.x, nV = (int)gridDim.x * NV;
+    const int stB = (int)(((long long)colBase[LIST_BULK][R] * a.staticEighths / 8) / nB);
+    const int stV = (int)(((long long)colBase[LIST_VEC][R] * a.staticEighths / 8) / nV);
     if (warp == 0) {
-        // ================= bulk engine: byte-granular TMA ring driven by one elected lane ========
-        // The ring is a circular BYTE buffer (not fixed-size stages): every tile takes exactly
-        // align128(len) bytes, so short tiles (config 5: 10-28 KiB) keep as many bytes in flight as
-        // long ones.  Up to COPY_SLOTS tiles are outstanding; slot j's bookkeeping (destination,
-        // length, smem offset, virtual start) lives in the registers of lane j.
         Cursor<LIST_BULK> cur;
-        cur.init(a, colBase[LIST_BULK], (int)gridDim.x, (int)blockIdx.x, a.kmax[LIST_BULK]);
-        const unsigned int tileBytes = 1u << a.cls.tileShift[LIST_BULK];
-        const unsigned int ringBytes = a.ringBytes;
-        const uint32_t ring0 = smem_u32(smem);
-        unsigned long long mDst = 0;          // slot registers (lane j <-> slot j)
-        unsigned int mLen = 0, mOff = 0, mV = 0;
-        unsigned int vHead = 0, phys = 0;     // virtual (mod 2^32) and physical allocation offsets
-        int iLoad = 0, iStore = 0, freed = 0;  // stores [0, freed) have finished reading their smem
-        bool more = cur.ensure();
-        while (true) {
-            // fill: issue loads while a slot and enough ring bytes are free
-            while (more) {
-                const long long off = cur.tile_off();
-                const long long rest = cur.bytes - off;
-                const unsigned int len = rest < (long long)tileBytes ? (unsigned int)rest : tileBytes;
-                const unsigned int len16 = len & ~15u;
-                const unsigned char* srcp = reinterpret_cast<const unsigned char*>(cur.src + off);
-                unsigned char* dstp = reinterpret_cast<unsigned char*>(cur.dst + off);
-                if (len16) {
-                    if (iLoad - freed >= COPY_SLOTS) break;
-                    const unsigned int pad = phys + len16 > ringBytes ? ringBytes - phys : 0u;   // wrap
-                    const unsigned int vTail = freed < iLoad ? __shfl_sync(0xffffffffu, mV, freed % COPY_SLOTS) : vHead;
-                    if (vHead + pad + len16 - vTail > ringBytes) break;
-                    const unsigned int vStart = vHead + pad;
-                    const unsigned int po = pad ? 0u : phys;
-                    const int slot = iLoad % COPY_SLOTS;
-                    if (lane == slot) { mDst = (unsigned long long)dstp; mLen = len16; mOff = po; mV = vStart; }
-                    if (lane == 0) {
-                        const uint32_t bar = smem_u32(&mbar[slot]);
-                        mbar_expect_tx(bar, len16);
-                        bulk_g2s(ring0 + po, srcp, len16, bar);
-                    }
-                    const unsigned int adv = (len16 + 127u) & ~127u;
-                    vHead = vStart + adv;
-                    phys = po + adv;
-                    if (phys >= ringBytes) phys = 0;
-                    ++iLoad;
-                }
-                const int tail = (int)(len & 15u);        // only the last tile of a ragged segment
-                if (lane < tail) dstp[len16 + lane] = __ldg(srcp + len16 + lane);
-                cur.next();
-                more = cur.ensure();
-            }
-            if (iStore == iLoad) {
-                if (!more) break;
-                // every issued tile is stored but the next one does not fit behind the last store's
-                // not-yet-released bytes: release everything and restart the ring at offset 0
-                if (lane == 0) bulk_wait_read<0>();
-                freed = iStore;
-                phys = 0;
-                continue;
-            }
-            const int slot = iStore % COPY_SLOTS;
-            mbar_wait(smem_u32(&mbar[slot]), (uint32_t)((iStore / COPY_SLOTS) & 1));
-            const unsigned int dlo = __shfl_sync(0xffffffffu, (unsigned int)mDst, slot);
-            const unsigned int dhi = __shfl_sync(0xffffffffu, (unsigned int)(mDst >> 32), slot);
-            const unsigned int slen = __shfl_sync(0xffffffffu, mLen, slot);
-            const unsigned int soff = __shfl_sync(0xffffffffu, mOff, slot);
-            if (lane == 0) {
-                bulk_s2g(reinterpret_cast<void*>(((unsigned long long)dhi << 32) | dlo), ring0 + soff, slen);
-                bulk_commit();
-                if (more) bulk_wait_read<1>();            // releases the smem of every store but this one
-            }
-            freed = max(freed, iStore);                   // (only consulted while `more`)
-            ++iStore;
-            __syncwarp();
-        }
-        if (lane == 0) bulk_wait_all<0>();
+        cur.init(a.desc, colBase[LIST_BULK], &a.ctl->next[LIST_BULK], a.cls, a.ncols, a.colLen, nB, (int)blockIdx.x,
+                 a.kmax[LIST_BULK], a.kmaxLong, stB);
+        bulk_engine<false>(cur, smem, mbar, a.ringBytes);
     } else {
-        // ================= vector engines: one warp per tile ===================================
         Cursor<LIST_VEC> cur;
-        cur.init(a, colBase[LIST_VEC], (int)gridDim.x * (COPY_THREADS / 32 - 1),
-                 (int)blockIdx.x * (COPY_THREADS / 32 - 1) + warp - 1, a.kmax[LIST_VEC]);
-        const long long tileBytes = 1ll << a.cls.tileShift[LIST_VEC];
-        while (cur.ensure()) {
-            const long long off = cur.tile_off();
-            const long long rest = cur.bytes - off;
-            const long long len = rest < tileBytes ? rest : tileBytes;
-            warp_copy_bytes(reinterpret_cast<const unsigned char*>(cur.src + off),
-                            reinterpret_cast<unsigned char*>(cur.dst + off), len);
-            cur.next();
-        }
+        cur.init(a.desc, colBase[LIST_VEC], &a.ctl->next[LIST_VEC], a.cls, a.ncols, a.colLen, nV,
+                 (int)blockIdx.x * NV + warp - 1, a.kmax[LIST_VEC], a.kmaxLong, stV);
+        vector_engine<false>(cur);
     }
+    workctl_checkout(a.ctl, colBase[LIST_BULK][R] > stB * nB || colBase[LIST_VEC][R] > stV * nV);
 }
 
 }  // namespace ncclx

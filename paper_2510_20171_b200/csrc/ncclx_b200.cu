@@ -15,6 +15,7 @@
 #include "copy_kernel.cuh"
 #include "counts_kernel.cuh"
 #include "dynamic_kernel.cuh"
+#include "fused_kernel.cuh"
 #include "reduce_kernel.cuh"
 #include "topk_kernel.cuh"
 
@@ -30,14 +31,17 @@ struct Context {
     int maxRanks = 0;
     int smCount = 0;
     int maxSmemOptin = 0;
-    Workspace ws{};
+    Workspace ws{};                       // plan 0: the workspace of the one-call entry points
+    Workspace wsPlan[NCCLX_NUM_PLANS]{};  // wsPlan[0] == ws; plans 1.. serve the split-phase calls (double buffering)
+    struct PlanState { bool prepared = false; int R = 0; ClassParams cls{}; unsigned int ring = 0; } plan[NCCLX_NUM_PLANS];
+    WorkCtl* fusedCtl = nullptr;          // claim counters of the single-launch path (self-resetting)
     void* wsBase = nullptr;
     // tunables
-    int64_t params[NCCLX_PARAM_COUNT_] = {1, 1024, 4, 16, 0, 0, 15, 14, 1, 0, 6, 2};
+    int64_t params[NCCLX_PARAM_COUNT_] = {1, 1024, 4, 16, 0, 0, 15, 14, 1, 0, 6, 2, 32, 12};
     // profiling
     std::vector<EventPair> events[NCCLX_KERNEL_COUNT_];
     std::atomic<int64_t> launches{0};
-    int64_t kernelLaunches[NCCLX_KERNEL_COUNT_] = {0, 0, 0, 0, 0};
+    int64_t kernelLaunches[NCCLX_KERNEL_COUNT_] = {0, 0, 0, 0, 0, 0};
     long long* rcScratch = nullptr;   // R*R, RC sink for calls that do not return it
     // AllToAllvDynamic workspace (ncclx_init_dynamic)
     void* dynBase = nullptr;
@@ -142,10 +146,11 @@ ClassParams classParams(unsigned int* ringOut) {
     return c;
 }
 
-int launchCopy(const SegDesc* desc, int ncols, int colLen, const ClassParams& cls, unsigned int ring, cudaStream_t stream) {
+int launchCopy(const Workspace& ws, const SegDesc* desc, int ncols, int colLen, const ClassParams& cls, unsigned int ring,
+               cudaStream_t stream) {
     CopyArgs cp{};
-    cp.desc = desc; cp.colTiles[0] = g.ws.colTiles[0]; cp.colTiles[1] = g.ws.colTiles[1];
-    cp.ctl = g.ws.ctl; cp.ncols = ncols; cp.colLen = colLen;
+    cp.desc = desc; cp.colTiles[0] = ws.colTiles[0]; cp.colTiles[1] = ws.colTiles[1];
+    cp.ctl = ws.ctl; cp.ncols = ncols; cp.colLen = colLen;
     cp.cls = cls;
     cp.ringBytes = ring;
     cp.staticEighths = (int)g.params[NCCLX_PARAM_COPY_STATIC_EIGHTHS];
@@ -169,25 +174,67 @@ int launchCopy(const SegDesc* desc, int ncols, int colLen, const ClassParams& cl
     return NCCLX_OK;
 }
 
+int launchCounts(const Workspace& ws, const void* const* send, const int64_t* C, void* const* recv, int64_t* RC, int R,
+                 long long es, const ClassParams& cls, cudaStream_t stream);
 int launchCounts(const void* const* send, const int64_t* C, void* const* recv, int64_t* RC, int R, long long es,
-                 const ClassParams& cls, cudaStream_t stream);
+                 const ClassParams& cls, cudaStream_t stream) {
+    return launchCounts(g.ws, send, C, recv, RC, R, es, cls, stream);
+}
+
+// Single-launch path (fused_kernel.cuh): ring = what is left of the SM's shared memory after the R*R
+// descriptors; the maximum bulk tile still has to fit three times.
+int launchFused(const void* const* send, const int64_t* C, void* const* recv, int64_t* RC, int R, int es,
+                cudaStream_t stream) {
+    FusedArgs fa{};
+    unsigned int ringStd = 0;
+    fa.cls = classParams(&ringStd);
+    const size_t budget = (size_t)g.maxSmemOptin - 1024;
+    const size_t aux = fused_aux_bytes(R);
+    fa.ringBytes = (unsigned int)((budget - aux) & ~(size_t)127);
+    while (fa.cls.tileShift[0] > 10 && ((size_t)3 << fa.cls.tileShift[0]) > fa.ringBytes) --fa.cls.tileShift[0];
+    fa.send = send; fa.recv = recv;
+    fa.C = reinterpret_cast<const long long*>(C);
+    fa.RC = reinterpret_cast<long long*>(RC);
+    fa.soff = g.ws.soff; fa.roff = g.ws.roff;
+    fa.ctl = g.fusedCtl; fa.status = &g.ws.ctl->status;
+    fa.R = R; fa.elemSize = es;
+    fa.kmax[0] = (int)g.params[NCCLX_PARAM_COPY_KMAX]; fa.kmax[1] = 8;
+    fa.kmaxLong = (int)g.params[NCCLX_PARAM_COPY_KMAX_LONG];
+    const int minShift = (int)g.params[NCCLX_PARAM_FUSED_MIN_TILE_SHIFT];
+    fa.minTileShift[0] = minShift < fa.cls.tileShift[0] ? minShift : fa.cls.tileShift[0];
+    fa.minTileShift[1] = 10 < fa.cls.tileShift[1] ? 10 : fa.cls.tileShift[1];
+    LaunchScope ls(NCCLX_KERNEL_FUSED, stream);
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)g.smCount);
+    cfg.blockDim = dim3(COPY_THREADS);
+    cfg.dynamicSmemBytes = (size_t)fa.ringBytes + aux;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = g.params[NCCLX_PARAM_PDL] ? 1 : 0;
+    CK(cudaLaunchKernelEx(&cfg, alltoallv_fused_kernel, fa));
+    return NCCLX_OK;
+}
 
 int launchAllToAllv(const void* const* send, const int64_t* C, void* const* recv, int64_t* RC, int R, int es,
                     cudaStream_t stream) {
+    if (R <= FUSED_MAX_R && R <= (int)g.params[NCCLX_PARAM_FUSED_MAX_RANKS]) return launchFused(send, C, recv, RC, R, es, stream);
     unsigned int ring = 0;
     const ClassParams cls = classParams(&ring);
-    int rc = launchCounts(send, C, recv, RC, R, es, cls, stream);
+    int rc = launchCounts(g.ws, send, C, recv, RC, R, es, cls, stream);
     if (rc) return rc;
-    return launchCopy(g.ws.desc, R, R, cls, ring, stream);
+    return launchCopy(g.ws, g.ws.desc, R, R, cls, ring, stream);
 }
 
-int launchCounts(const void* const* send, const int64_t* C, void* const* recv, int64_t* RC, int R, long long es,
-                 const ClassParams& cls, cudaStream_t stream) {
+int launchCounts(const Workspace& ws, const void* const* send, const int64_t* C, void* const* recv, int64_t* RC, int R,
+                 long long es, const ClassParams& cls, cudaStream_t stream) {
     CountsArgs ca{};
     ca.send = send; ca.recv = recv;
     ca.C = reinterpret_cast<const long long*>(C);
     ca.RC = reinterpret_cast<long long*>(RC);
-    ca.ws = g.ws; ca.R = R; ca.W = countsW(R); ca.elemSize = es;
+    ca.ws = ws; ca.R = R; ca.W = countsW(R); ca.elemSize = es;
     ca.cls = cls;
     const int G = (R + ca.W - 1) / ca.W;
     const size_t csm = countsSmemBytes(R, ca.W);
@@ -331,27 +378,39 @@ int ncclx_init(int max_ranks, int device) {
 
     const size_t rr = (size_t)max_ranks * max_ranks;
     size_t off = 0;
-    const size_t oSoff = off; off = alignUp(off + rr * 8, 256);
-    const size_t oRoff = off; off = alignUp(off + rr * 8, 256);
-    const size_t oDesc = off; off = alignUp(off + rr * sizeof(SegDesc), 256);
-    const size_t oCt0 = off; off = alignUp(off + (size_t)max_ranks * 4, 256);
-    const size_t oCt1 = off; off = alignUp(off + (size_t)max_ranks * 4, 256);
-    const size_t oCtl = off; off = alignUp(off + sizeof(WorkCtl), 256);
+    size_t oSoff[NCCLX_NUM_PLANS], oRoff[NCCLX_NUM_PLANS], oDesc[NCCLX_NUM_PLANS], oCt0[NCCLX_NUM_PLANS],
+        oCt1[NCCLX_NUM_PLANS], oCtl[NCCLX_NUM_PLANS];
+    for (int p = 0; p < NCCLX_NUM_PLANS; ++p) {
+        oSoff[p] = off; off = alignUp(off + rr * 8, 256);
+        oRoff[p] = off; off = alignUp(off + rr * 8, 256);
+        oDesc[p] = off; off = alignUp(off + rr * sizeof(SegDesc), 256);
+        oCt0[p] = off; off = alignUp(off + (size_t)max_ranks * 4, 256);
+        oCt1[p] = off; off = alignUp(off + (size_t)max_ranks * 4, 256);
+        oCtl[p] = off; off = alignUp(off + sizeof(WorkCtl), 256);
+    }
+    const size_t oFctl = off; off = alignUp(off + sizeof(WorkCtl), 256);
     const size_t oRcs = off; off = alignUp(off + rr * 8, 256);
     CK(cudaMalloc(&g.wsBase, off));
     CK(cudaMemset(g.wsBase, 0, off));
     char* b = static_cast<char*>(g.wsBase);
-    g.ws.soff = reinterpret_cast<long long*>(b + oSoff);
-    g.ws.roff = reinterpret_cast<long long*>(b + oRoff);
-    g.ws.desc = reinterpret_cast<SegDesc*>(b + oDesc);
-    g.ws.colTiles[0] = reinterpret_cast<int*>(b + oCt0);
-    g.ws.colTiles[1] = reinterpret_cast<int*>(b + oCt1);
-    g.ws.ctl = reinterpret_cast<WorkCtl*>(b + oCtl);
+    for (int p = 0; p < NCCLX_NUM_PLANS; ++p) {
+        Workspace& w = g.wsPlan[p];
+        w.soff = reinterpret_cast<long long*>(b + oSoff[p]);
+        w.roff = reinterpret_cast<long long*>(b + oRoff[p]);
+        w.desc = reinterpret_cast<SegDesc*>(b + oDesc[p]);
+        w.colTiles[0] = reinterpret_cast<int*>(b + oCt0[p]);
+        w.colTiles[1] = reinterpret_cast<int*>(b + oCt1[p]);
+        w.ctl = reinterpret_cast<WorkCtl*>(b + oCtl[p]);
+        g.plan[p] = Context::PlanState{};
+    }
+    g.ws = g.wsPlan[0];
+    g.fusedCtl = reinterpret_cast<WorkCtl*>(b + oFctl);
     g.rcScratch = reinterpret_cast<long long*>(b + oRcs);
 
     int rc;
     if ((rc = optInSmem(segment_copy_kernel, g.maxSmemOptin))) return rc;
     if ((rc = optInSmem(counts_kernel, g.maxSmemOptin))) return rc;
+    if ((rc = optInSmem(alltoallv_fused_kernel, g.maxSmemOptin))) return rc;
     CK(cudaDeviceSynchronize());
     g.launches = 0;
     for (auto& k : g.kernelLaunches) k = 0;
@@ -380,6 +439,30 @@ int ncclx_alltoallv_dev(const void* const* send, const int64_t* sendcounts_dev, 
     return launchAllToAllv(send, sendcounts_dev, recv, recvcounts_dev, R, es, static_cast<cudaStream_t>(stream));
 }
 
+int ncclx_alltoallv_prepare_dev(int plan, const void* const* send, const int64_t* sendcounts_dev, void* const* recv,
+                                int64_t* recvcounts_dev, int R, ncclx_dtype_t dtype, ncclx_stream_t stream) {
+    int rc = checkCommon(R);
+    if (rc) return rc;
+    if (plan < 0 || plan >= NCCLX_NUM_PLANS) return NCCLX_ERR_ARG;
+    if (!send || !sendcounts_dev || !recv || !recvcounts_dev) return NCCLX_ERR_ARG;
+    if (sendcounts_dev == recvcounts_dev) return NCCLX_ERR_ARG;
+    const int es = elemSizeOf((int)dtype);
+    if (!es) return NCCLX_ERR_DTYPE;
+    Context::PlanState& ps = g.plan[plan];
+    ps.cls = classParams(&ps.ring);
+    ps.R = R;
+    rc = launchCounts(g.wsPlan[plan], send, sendcounts_dev, recv, recvcounts_dev, R, es, ps.cls, static_cast<cudaStream_t>(stream));
+    ps.prepared = rc == NCCLX_OK;
+    return rc;
+}
+
+int ncclx_alltoallv_execute_dev(int plan, ncclx_stream_t stream) {
+    if (!g.ready) return NCCLX_ERR_NOT_INITIALIZED;
+    if (plan < 0 || plan >= NCCLX_NUM_PLANS || !g.plan[plan].prepared) return NCCLX_ERR_ARG;
+    const Context::PlanState& ps = g.plan[plan];
+    return launchCopy(g.wsPlan[plan], g.wsPlan[plan].desc, ps.R, ps.R, ps.cls, ps.ring, static_cast<cudaStream_t>(stream));
+}
+
 int ncclx_alltoallv_last_offsets(int64_t* soff_host, int64_t* roff_host, int R, ncclx_stream_t stream) {
     int rc = checkCommon(R);
     if (rc) return rc;
@@ -398,8 +481,14 @@ int ncclx_device_status(uint32_t* status_host, ncclx_stream_t stream) {
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     if (isCapturing(s)) return NCCLX_ERR_CAPTURE;
     CK(cudaStreamSynchronize(s));
-    CK(cudaMemcpy(status_host, &g.ws.ctl->status, 4, cudaMemcpyDeviceToHost));
-    CK(cudaMemset(&g.ws.ctl->status, 0, 4));
+    uint32_t all = 0;
+    for (int p = 0; p < NCCLX_NUM_PLANS; ++p) {
+        uint32_t v = 0;
+        CK(cudaMemcpy(&v, &g.wsPlan[p].ctl->status, 4, cudaMemcpyDeviceToHost));
+        if (v) CK(cudaMemset(&g.wsPlan[p].ctl->status, 0, 4));
+        all |= v;
+    }
+    *status_host = all;
     return NCCLX_OK;
 }
 
@@ -467,7 +556,7 @@ int ncclx_alltoallv_dynamic_dev(const void* const* send, const int64_t* sendSpli
         cfg.numAttrs = g.params[NCCLX_PARAM_PDL] ? 1 : 0;
         CK(cudaLaunchKernelEx(&cfg, dyn_desc_kernel, da));
     }
-    return launchCopy(g.dynDesc, R, R * maxBlockLen, da.cls, ring, s);
+    return launchCopy(g.ws, g.dynDesc, R, R * maxBlockLen, da.cls, ring, s);
 }
 
 int ncclx_allreduce_sum(const void* const* send, void* const* recv, size_t count, int R, ncclx_dtype_t dtype,
@@ -674,6 +763,8 @@ int ncclx_set_param(int param, int64_t value) {
     case NCCLX_PARAM_COPY_STATIC_EIGHTHS: if (value < 0 || value > 8) return NCCLX_ERR_ARG; break;
     case NCCLX_PARAM_COPY_KMAX:
     case NCCLX_PARAM_COPY_KMAX_LONG: if (value < 1 || value > 64) return NCCLX_ERR_ARG; break;
+    case NCCLX_PARAM_FUSED_MAX_RANKS: if (value < 0 || value > FUSED_MAX_R) return NCCLX_ERR_ARG; break;
+    case NCCLX_PARAM_FUSED_MIN_TILE_SHIFT: if (value < 10 || value > 16) return NCCLX_ERR_ARG; break;
     default: if (value < 0) return NCCLX_ERR_ARG; break;
     }
     g.params[param] = value;
