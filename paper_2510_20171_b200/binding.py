@@ -30,6 +30,8 @@ PARAM_COPY_KMAX = 10
 PARAM_COPY_KMAX_LONG = 11
 PARAM_FUSED_MAX_RANKS = 12
 PARAM_FUSED_MIN_TILE_SHIFT = 13
+PARAM_COPY_PENDING_STORES = 14
+PARAM_COPY_BULK_ENGINES = 15
 NUM_PLANS = 4
 
 KERNEL_COUNTS, KERNEL_COPY, KERNEL_REDUCE, KERNEL_DYN, KERNEL_TOPK, KERNEL_FUSED = 0, 1, 2, 3, 4, 5

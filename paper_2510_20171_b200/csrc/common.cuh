@@ -35,6 +35,7 @@ struct Workspace {
     long long* roff;          // R*R, roff[d*R+s]
     SegDesc* desc;            // R*R, desc[d*R+s]
     int* colTiles[2];         // R each: tiles of list L in column d
+    int* coarse[2];           // R*ceil(colLen/32) each: tiles of list L in column d before its descriptor 32*j
     WorkCtl* ctl;
 };
 

@@ -23,45 +23,73 @@
 namespace ncclx {
 
 constexpr int COPY_THREADS = 512;          // warp 0: bulk engine; warps 1..15: vector engines
-constexpr int COPY_SLOTS = 16;             // outstanding bulk tiles per engine (mbarriers); <= 32
+constexpr int COPY_SLOTS = 32;             // outstanding bulk tiles per engine (mbarriers; slot j lives in lane j): <= 32
+constexpr int COPY_MAX_ENGINES = 4;        // bulk engines (warps 0..E-1) per CTA, each with its own share of the ring
+constexpr int COPY_MBAR_BYTES = COPY_MAX_ENGINES * COPY_SLOTS * 8;
 
 struct CopyArgs {
     const SegDesc* desc;
     const int* colTiles[2];
+    const int* coarse[2];                  // per list: tiles of column d before its descriptor 32*j, [d*nb + j] (counts kernel)
     WorkCtl* ctl;
     int ncols;                             // destination columns of the descriptor table (= R)
     int colLen;                            // descriptor slots per column (R for the plain call, R*maxBlockLen for the dynamic one)
+    int useCoarse;                         // 1: stage both coarse indexes in shared memory (2*ncols*nb ints)
     unsigned int ringBytes;                // shared-memory ring size, multiple of 128, >= 3 tiles
     int staticEighths;                     // 0..8: share of the tiles assigned statically (contiguous per engine)
     int kmax[2];                           // max tiles per dynamic claim, per list (short-segment regime)
     int kmaxLong;                          // same, when segments average >= 8 tiles
+    int maxPendingStores;                  // 1..8: stores whose shared-memory read may be outstanding before the engine waits
+    int bulkEngines;                       // E = 1, 2 or 4 bulk engine warps per CTA (ring split E ways); warps E..15 are vector engines
     ClassParams cls;
 };
 
+#ifdef NCCLX_EXPERIMENTS
+__device__ int g_exp_mode = 0;             // _work probes only: 1 = skip stores, 2 = skip loads (results invalid)
+__device__ long long g_exp_cycles[256 * 8];
+#define EXP_T0() const long long t0_ = clock64()
+#define EXP_ACC(i) do { expc[i] += clock64() - t0_; } while (0)
+#else
+#define EXP_T0() do {} while (0)
+#define EXP_ACC(i) do {} while (0)
+#endif
+
+__host__ __device__ inline int coarse_blocks(int colLen) { return (colLen + 31) >> 5; }
+
 // Warp-uniform cursor over one work list.  All lanes hold identical state except the descriptor
-// WINDOW: lane i caches descriptor q = qw + i of the destination-major table, and the next 32 are
+// WINDOWS: lane i caches descriptor q = qw + i of the destination-major table, and the next 32 are
 // prefetched into a second register set, so stepping from one segment to the next non-empty one of
 // this list is a ballot over registers instead of a chain of dependent L2 reads (config 5 has a new
-// segment every ~2 tiles).  Only a fresh claim pays the search: smem binary search over columns,
-// then a warp-wide 32-ary search over the column's tile prefixes.
+// segment every ~2 tiles).
+// Finding the segment that owns a freshly claimed tile index: binary search over the column bases,
+// then over the column's COARSE index (tiles before every 32nd descriptor) -- both in shared memory --
+// which names the one 32-descriptor block to load; the final position is a ballot over that window.
+// Short-segment regime (config 5: a claim of 6 tiles is ~150 KB, the next one lies ~2000 descriptors
+// ahead): the search and the window load of the NEXT chunk are issued while the current chunk is being
+// copied (claims run two chunks ahead, windows one), so the engine never waits for metadata after
+// start-up.  Long-segment regime (config 3): small in-order claims resolve inside the cached windows.
+// Without a coarse index (table too large for shared memory) the block is found by a 128-ary search in L2.
 // SM = true: the descriptor table lives in SHARED memory (single-launch path, fused_kernel.cuh).
 template <int L, bool SM = false>
 struct Cursor {
     const SegDesc* desc;
     const int* colBase;                    // smem, ncols+1 entries, colBase[ncols] = total tiles
+    const int* coarse;                     // smem, ncols*nb entries, or null
     unsigned int* counter;
     ClassParams cls;
-    int ncols, colLen, RR, tileShift, total, nEngines, kmax, kmin;
+    int ncols, colLen, nb, RR, tileShift, total, nEngines, kmax, kmin;
     int staticK, engineId;                 // first chunk is assigned statically: [engineId*staticK, +staticK)
     int dynBase;                           // tiles >= dynBase are claimed dynamically
-    int pendCur, pendK;                    // lane 0: the NEXT chunk, claimed ahead of need (atomic in flight)
+    int pendCur, pendK;                    // lane 0: a chunk claimed ahead of need (atomic in flight)
     int t, tEnd;                           // current tile, end of the claimed chunk
     int q, kInSeg, segTiles;               // current segment, tile within it, its tile count
     unsigned long long src, dst;
     long long bytes;
     int qw, qn;                            // bases of the current / prefetched window
     uint4 w0, w1, n0, n1;                  // this lane's descriptor in each window
-    bool first, exhausted, haveWindow, longSegs;
+    int cCur, cK, cQw, cEnd, cPrev, cTl;   // pipelined mode: the staged NEXT chunk and where it starts
+    uint4 c0, c1;                          // its window (load in flight until adopt())
+    bool first, exhausted, haveWindow, longSegs, indexed, pipelined, cHave, needPrefetch;
 
     __device__ __forceinline__ void load_desc(int qq, uint4& a, uint4& b) const {
         if (qq < RR) {
@@ -89,34 +117,48 @@ struct Cursor {
     // staticK_ tiles per engine are assigned statically ([engineId*staticK, +staticK): no atomic on the
     // start-up path); tiles >= staticK*nEngines are claimed dynamically, IN ORDER, in guided chunks.
     // Measured on B200: the in-order dynamic claim keeps all SMs inside one moving window of HBM and is
-    // ~7 % faster than contiguous static ranges (148 far-apart streams), so the two-kernel path defaults
-    // to fully dynamic (staticK = 0); the single-launch path takes one static tile per engine.
-    __device__ __forceinline__ void init(const SegDesc* desc_, const int* colBase_, unsigned int* counter_,
+    // ~7 % faster than contiguous static ranges (148 far-apart streams), so only the FIRST chunk of each
+    // engine is static (chunk e to engine e, which is also what in-order claims would hand out).
+    __device__ __forceinline__ void init(const SegDesc* desc_, const int* colBase_, const int* coarse_, unsigned int* counter_,
                                          const ClassParams& cls_, int ncols_, int colLen_, int nEngines_, int engineId_,
                                          int kmax_, int kmaxLong_, int staticK_) {
-        desc = desc_; colBase = colBase_; counter = counter_; cls = cls_;
-        ncols = ncols_; colLen = colLen_; RR = ncols_ * colLen_; tileShift = cls_.tileShift[L]; total = colBase_[ncols_];
+        desc = desc_; colBase = colBase_; coarse = coarse_; counter = counter_; cls = cls_;
+        ncols = ncols_; colLen = colLen_; nb = coarse_blocks(colLen_); RR = ncols_ * colLen_;
+        tileShift = cls_.tileShift[L]; total = colBase_[ncols_];
         nEngines = nEngines_; engineId = engineId_;
         // long segments (>= 8 tiles each on average): claims resolve inside the cached window, so take
-        // small chunks and keep all SMs in a tight moving window of HBM; short segments: every claim
-        // pays a search, amortise it over more tiles.
+        // small chunks and keep all SMs in a tight moving window of HBM; short segments: amortise the
+        // per-claim work over a few tiles and hide it behind the previous chunk.
         longSegs = total >= 8 * RR;
+        indexed = coarse_ != nullptr || nb == 1;
+        pipelined = indexed && !longSegs;
         kmax = longSegs ? kmaxLong_ : kmax_;
         staticK = staticK_;
         kmin = total >= 8 * nEngines ? 2 : 1;
         dynBase = staticK * nEngines;
         pendCur = total; pendK = 0;        // reads as "drained" unless a claim is issued
         t = tEnd = 0; q = 0; kInSeg = segTiles = 0; src = dst = 0; bytes = 0;
-        qw = qn = 0; w0 = w1 = n0 = n1 = make_uint4(0, 0, 0, 0);
+        qw = qn = 0; w0 = w1 = n0 = n1 = c0 = c1 = make_uint4(0, 0, 0, 0);
+        cCur = cK = cQw = cEnd = cPrev = cTl = 0;
         first = true;
         haveWindow = false;
+        cHave = needPrefetch = false;
         exhausted = (total == 0);
-        if (total > dynBase) claim_issue(dynBase);
+        if (exhausted) return;
+        if (!pipelined) {
+            if (total > dynBase) claim_issue(dynBase);
+        } else if (staticK > 0) {
+            const int c = engineId * staticK;
+            if (c < total) stage_next(c, staticK);             // else: nothing for this engine (then total <= dynBase)
+            if (total > dynBase) claim_issue(dynBase);
+        } else {
+            claim_issue(dynBase);
+            prefetch_next();                                   // waits for the atomic once, at start-up
+        }
     }
-    __device__ __forceinline__ bool uses_counter() const { return total > dynBase; }
 
-    // Lane 0 issues the atomic for the next dynamic chunk; the result is only consumed by claim_take(),
-    // so its L2 round trip overlaps the tiles of the current chunk.
+    // Lane 0 issues the atomic for a later dynamic chunk; the result is consumed one chunk (pipelined:
+    // two chunks) later, so its L2 round trip overlaps the copying.
     __device__ __forceinline__ void claim_issue(int counterHint) {
         if (lane_id() == 0) {
             const int rem = total - min(total, counterHint);
@@ -125,9 +167,50 @@ struct Cursor {
         }
     }
 
+    // Shared-memory search: column d that owns global tile tt, tile index tl inside the column, the
+    // 32-descriptor block j of the column that holds it and the tiles of the column before that block.
+    __device__ __forceinline__ void find_block(int tt, int& d, int& tl, int& j, int& prev) const {
+        int lo = 0, hi = ncols;            // colBase[lo] <= tt < colBase[hi]
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (colBase[mid] <= tt) lo = mid; else hi = mid;
+        }
+        d = lo;
+        tl = tt - colBase[d];
+        j = 0; prev = 0;
+        if (nb > 1) {
+            const int* cr = coarse + d * nb;
+            int a = 0, b = nb;             // cr[a] <= tl < cr[b]  (cr[nb] = +inf)
+            while (b - a > 1) {
+                const int mid = (a + b) >> 1;
+                if (cr[mid] <= tl) a = mid; else b = mid;
+            }
+            j = a; prev = cr[a];
+        }
+    }
+    // The current window holds the segment that owns tile tl of its column (prev tiles lie before the
+    // window, colEnd = first descriptor index of the next column): select it.
+    __device__ __forceinline__ void position(int tl, int prev, int colEnd) {
+        const int pf = L == LIST_BULK ? (int)w1.z : (int)w1.w;
+        const int m = __popc(__ballot_sync(0xffffffffu, qw + lane_id() < colEnd && pf <= tl));
+        const int before = __shfl_sync(0xffffffffu, pf, m > 0 ? m - 1 : 0);
+        take(m);
+        kInSeg = tl - (m > 0 ? before : prev);
+    }
+
     // Find the segment that owns global tile index tt (0 <= tt < total) and (re)load the windows there.
     __device__ __forceinline__ void locate(int tt) {
         const int lane = lane_id();
+        if (indexed) {
+            int d, tl, j, prev;
+            find_block(tt, d, tl, j, prev);
+            qw = d * colLen + 32 * j;
+            load_desc(qw + lane, w0, w1);
+            qn = qw + 32;
+            load_desc(qn + lane, n0, n1);
+            position(tl, prev, (d + 1) * colLen);
+            return;
+        }
         int lo = 0, hi = ncols;            // colBase[lo] <= tt < colBase[hi]
         while (hi - lo > 1) {
             const int mid = (lo + hi) >> 1;
@@ -156,17 +239,41 @@ struct Cursor {
         // last round doubles as the window load; the window starts one descriptor early so that the
         // predecessor's prefix (needed for the tile index inside the segment) comes with it
         const int sb = s0 > 0 ? s0 - 1 : 0;
-        const int nn = n + (s0 - sb);
         qw = d * colLen + sb;
         load_desc(qw + lane, w0, w1);
         qn = qw + 32;
         load_desc(qn + lane, n0, n1);
-        const int pf = L == LIST_BULK ? (int)w1.z : (int)w1.w;
-        const int m = __popc(__ballot_sync(0xffffffffu, lane < nn && pf <= tl));
-        const int prevInWin = __shfl_sync(0xffffffffu, pf, m > 0 ? m - 1 : 0);
-        const int prev = m > 0 ? prevInWin : 0;
-        take(m);
-        kInSeg = tl - prev;
+        position(tl, 0, (d + 1) * colLen);
+    }
+
+    // ---- pipelined mode ------------------------------------------------------------------------
+    __device__ __forceinline__ void stage_next(int cur, int k) {   // chunk [cur, cur+k): find its block, start the window load
+        int d, j;
+        find_block(cur, d, cTl, j, cPrev);
+        cCur = cur; cK = k;
+        cQw = d * colLen + 32 * j;
+        cEnd = (d + 1) * colLen;
+        load_desc(cQw + lane_id(), c0, c1);
+        cHave = true;
+    }
+    __device__ __forceinline__ void prefetch_next() {      // consume the pending claim, stage it, claim one more
+        needPrefetch = false;
+        const int pc = __shfl_sync(0xffffffffu, pendCur, 0);
+        const int pk = __shfl_sync(0xffffffffu, pendK, 0);
+        if (pc >= total || pc < 0) { cHave = false; return; }
+        stage_next(pc, pk);
+        claim_issue(pc + pk);
+    }
+    __device__ __forceinline__ void adopt() {              // the staged chunk becomes the current one
+        t = cCur;
+        tEnd = min(cCur + cK, total);
+        qw = cQw; w0 = c0; w1 = c1;
+        qn = qw + 32;
+        load_desc(qn + lane_id(), n0, n1);
+        position(cTl, cPrev, cEnd);
+        haveWindow = true;
+        cHave = false;
+        needPrefetch = true;
     }
 
     // Step to the next segment of this list (t stays inside the claimed chunk, so one exists).
@@ -218,8 +325,15 @@ struct Cursor {
     __device__ __forceinline__ bool ensure() {
         if (exhausted) return false;
         if (t < tEnd) {
+            if (needPrefetch) prefetch_next();     // (pipelined) after the chunk's first tile is on its way
             if (kInSeg >= segTiles) advance_segment();
             return !exhausted;
+        }
+        if (pipelined) {
+            if (needPrefetch) prefetch_next();
+            if (!cHave) { exhausted = true; return false; }
+            adopt();
+            return true;
         }
         int cur, k;
         if (first && staticK > 0) {        // static share: no atomic on the start-up path
@@ -293,16 +407,36 @@ __device__ __forceinline__ void warp_copy_bytes(const unsigned char* src, unsign
 // align128(len) bytes, so short tiles (config 5: 10-28 KiB) keep as many bytes in flight as
 // long ones.  Up to COPY_SLOTS tiles are outstanding; slot j's bookkeeping (destination,
 // length, smem offset, virtual start) lives in the registers of lane j.
+// A store's ring bytes are reclaimed with cp.async.bulk.wait_group.read: after a store is issued the engine
+// waits until at most maxPending (1..8) stores still read shared memory.
+__device__ __forceinline__ void bulk_release_oldest(int pending) {   // lane 0; pending = stores not yet known to be read (1..8)
+    switch (pending) {
+    case 1: bulk_wait_read<0>(); break;
+    case 2: bulk_wait_read<1>(); break;
+    case 3: bulk_wait_read<2>(); break;
+    case 4: bulk_wait_read<3>(); break;
+    case 5: bulk_wait_read<4>(); break;
+    case 6: bulk_wait_read<5>(); break;
+    case 7: bulk_wait_read<6>(); break;
+    default: bulk_wait_read<7>(); break;
+    }
+}
+
 template <bool SM>
 __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned char* ring, unsigned long long* mbar,
-                                            const unsigned int ringBytes) {
+                                            const unsigned int ringBytes, const int maxPending) {
     const int lane = lane_id();
+#ifdef NCCLX_EXPERIMENTS
+    const int expMode = g_exp_mode;
+    long long expc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    const long long tStart = clock64();
+#endif
     const unsigned int tileBytes = 1u << cur.tileShift;
     const uint32_t ring0 = smem_u32(ring);
     unsigned long long mDst = 0;          // slot registers (lane j <-> slot j)
     unsigned int mLen = 0, mOff = 0, mV = 0;
     unsigned int vHead = 0, phys = 0;     // virtual (mod 2^32) and physical allocation offsets
-    int iLoad = 0, iStore = 0, freed = 0;  // stores [0, freed) have finished reading their smem
+    int iLoad = 0, iStore = 0, freed = 0;  // stores [0, freed) have finished reading their smem; freed <= iStore <= iLoad
     bool more = cur.ensure();
     while (true) {
         // fill: issue loads while a slot and enough ring bytes are free
@@ -314,18 +448,22 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
             const unsigned char* srcp = reinterpret_cast<const unsigned char*>(cur.src + off);
             unsigned char* dstp = reinterpret_cast<unsigned char*>(cur.dst + off);
             if (len16) {
-                if (iLoad - freed >= COPY_SLOTS) break;
                 const unsigned int pad = phys + len16 > ringBytes ? ringBytes - phys : 0u;   // wrap
                 const unsigned int vTail = freed < iLoad ? __shfl_sync(0xffffffffu, mV, freed % COPY_SLOTS) : vHead;
-                if (vHead + pad + len16 - vTail > ringBytes) break;
+                if (iLoad - freed >= COPY_SLOTS || vHead + pad + len16 - vTail > ringBytes) break;   // store a landed tile first
                 const unsigned int vStart = vHead + pad;
                 const unsigned int po = pad ? 0u : phys;
                 const int slot = iLoad % COPY_SLOTS;
                 if (lane == slot) { mDst = (unsigned long long)dstp; mLen = len16; mOff = po; mV = vStart; }
                 if (lane == 0) {
                     const uint32_t bar = smem_u32(&mbar[slot]);
-                    mbar_expect_tx(bar, len16);
-                    bulk_g2s(ring0 + po, srcp, len16, bar);
+#ifdef NCCLX_EXPERIMENTS
+                    if (expMode == 2) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory"); } else
+#endif
+                    {
+                        mbar_expect_tx(bar, len16);
+                        bulk_g2s(ring0 + po, srcp, len16, bar);
+                    }
                 }
                 const unsigned int adv = (len16 + 127u) & ~127u;
                 vHead = vStart + adv;
@@ -336,33 +474,48 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
             const int tail = (int)(len & 15u);        // only the last tile of a ragged segment
             if (lane < tail) dstp[len16 + lane] = __ldg(srcp + len16 + lane);
             cur.next();
-            more = cur.ensure();
+            { EXP_T0(); more = cur.ensure(); EXP_ACC(0); }
         }
         if (iStore == iLoad) {
             if (!more) break;
-            // every issued tile is stored but the next one does not fit behind the last store's
-            // not-yet-released bytes: release everything and restart the ring at offset 0
+            // nothing in flight and nothing left to reclaim, yet the next tile does not fit behind the
+            // allocation point: restart the ring at offset 0
             if (lane == 0) bulk_wait_read<0>();
             freed = iStore;
             phys = 0;
             continue;
         }
         const int slot = iStore % COPY_SLOTS;
-        mbar_wait(smem_u32(&mbar[slot]), (uint32_t)((iStore / COPY_SLOTS) & 1));
+        { EXP_T0(); mbar_wait(smem_u32(&mbar[slot]), (uint32_t)((iStore / COPY_SLOTS) & 1)); EXP_ACC(1); }
+#ifdef NCCLX_EXPERIMENTS
+        expc[5] += 1;
+#endif
         const unsigned int dlo = __shfl_sync(0xffffffffu, (unsigned int)mDst, slot);
         const unsigned int dhi = __shfl_sync(0xffffffffu, (unsigned int)(mDst >> 32), slot);
         const unsigned int slen = __shfl_sync(0xffffffffu, mLen, slot);
         const unsigned int soff = __shfl_sync(0xffffffffu, mOff, slot);
         if (lane == 0) {
+#ifdef NCCLX_EXPERIMENTS
+            if (expMode != 1)
+#endif
             bulk_s2g(reinterpret_cast<void*>(((unsigned long long)dhi << 32) | dlo), ring0 + soff, slen);
             bulk_commit();
-            if (more) bulk_wait_read<1>();            // releases the smem of every store but this one
         }
-        freed = max(freed, iStore);                   // (only consulted while `more`)
         ++iStore;
-        __syncwarp();
+        { EXP_T0();
+        while (iStore - freed > maxPending) {                     // at most maxPending stores keep ring bytes
+            if (lane == 0) bulk_release_oldest(iStore - freed);
+            ++freed;
+        }
+        __syncwarp(); EXP_ACC(2); }
     }
-    if (lane == 0) bulk_wait_all<0>();
+    { EXP_T0(); if (lane == 0) bulk_wait_all<0>(); EXP_ACC(3); }
+#ifdef NCCLX_EXPERIMENTS
+    if (lane == 0) {
+        expc[4] = clock64() - tStart;
+        for (int i = 0; i < 8; ++i) g_exp_cycles[(blockIdx.x & 255) * 8 + i] = expc[i];
+    }
+#endif
 }
 
 // ================= vector engine: one warp per tile ===========================================
@@ -394,7 +547,16 @@ __device__ __forceinline__ void workctl_checkout(WorkCtl* ctl, bool used) {
     }
 }
 
-// dynamic smem layout: [ring: ringBytes][mbar: COPY_SLOTS x u64][colBase bulk: R+1 ints][colBase vec: R+1 ints]
+// First chunk of every engine is static (chunk e to engine e; see Cursor::init); a positive staticEighths
+// instead assigns that share of ALL tiles as contiguous static ranges (kept for A/B runs).
+__device__ __forceinline__ int static_first_chunk(int total, int nEngines, int kmax, int kmaxLong, int RR, int eighths) {
+    if (eighths > 0) return (int)(((long long)total * eighths / 8) / nEngines);
+    const int km = total >= 8 * RR ? kmaxLong : kmax;
+    return max(1, min(km, total / (4 * nEngines)));
+}
+
+// dynamic smem layout: [ring: ringBytes][mbar: COPY_MAX_ENGINES x COPY_SLOTS x u64][colBase bulk: R+1 ints][colBase vec: R+1 ints]
+//                      [coarse bulk: R*nb ints][coarse vec: R*nb ints]   (the last two only if useCoarse)
 __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const CopyArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = lane_id();
@@ -402,19 +564,28 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
     const int R = a.ncols;
     unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + a.ringBytes);
     int* colBase[2];
-    colBase[0] = reinterpret_cast<int*>(mbar + COPY_SLOTS);
+    colBase[0] = reinterpret_cast<int*>(mbar + COPY_MAX_ENGINES * COPY_SLOTS);
     colBase[1] = colBase[0] + (R + 1);
+    const int E = a.bulkEngines;
+    const int nbR = R * coarse_blocks(a.colLen);
+    int* coarse[2] = {nullptr, nullptr};
+    if (a.useCoarse) { coarse[0] = colBase[1] + (R + 1); coarse[1] = coarse[0] + nbR; }
 
     // ---- prologue: mbarrier init (overlaps the counts kernel under PDL), then cross-column tile
-    //      bases = scan of the R per-column totals the counts kernel wrote -------------------------
-    if (warp == 2 && lane == 0) {
-        for (int i = 0; i < COPY_SLOTS; ++i) mbar_init(smem_u32(&mbar[i]), 1);
+    //      bases = scan of the R per-column totals the counts kernel wrote, and the coarse indexes ----
+    griddep_launch_dependents();           // the next call's metadata kernel may become resident (it waits for us)
+    if (threadIdx.x >= 64 && threadIdx.x < 64 + E * COPY_SLOTS) {
+        mbar_init(smem_u32(&mbar[threadIdx.x - 64]), 1);
         fence_mbar_init();
     }
     griddep_wait();
+    if (a.useCoarse && warp >= 2) {
+        for (int i = threadIdx.x - 64; i < 2 * nbR; i += COPY_THREADS - 64)
+            coarse[0][i] = i < nbR ? __ldg(a.coarse[0] + i) : __ldg(a.coarse[1] + (i - nbR));
+    }
     if (warp < 2) {
-        const int* ct = a.colTiles[warp];
-        int* cb = colBase[warp];
+        const int* ct = warp ? a.colTiles[1] : a.colTiles[0];
+        int* cb = warp ? colBase[1] : colBase[0];
         int run = 0;
         if (lane == 0) cb[0] = 0;
         for (int c0 = 0; c0 < R; c0 += 32) {
@@ -426,19 +597,21 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
     }
     __syncthreads();
 
-    constexpr int NV = COPY_THREADS / 32 - 1;          // vector engines per CTA
-    const int nB = (int)gridDim.x, nV = (int)gridDim.x * NV;
-    const int stB = (int)(((long long)colBase[LIST_BULK][R] * a.staticEighths / 8) / nB);
-    const int stV = (int)(((long long)colBase[LIST_VEC][R] * a.staticEighths / 8) / nV);
-    if (warp == 0) {
+    const int NV = COPY_THREADS / 32 - E;              // vector engines per CTA
+    const int nB = (int)gridDim.x * E, nV = (int)gridDim.x * NV;
+    const unsigned int subRing = (a.ringBytes / (unsigned int)E) & ~127u;
+    const int RR = a.ncols * a.colLen;
+    const int stB = static_first_chunk(colBase[LIST_BULK][R], nB, a.kmax[LIST_BULK], a.kmaxLong, RR, a.staticEighths);
+    const int stV = static_first_chunk(colBase[LIST_VEC][R], nV, a.kmax[LIST_VEC], a.kmaxLong, RR, a.staticEighths);
+    if (warp < E) {
         Cursor<LIST_BULK> cur;
-        cur.init(a.desc, colBase[LIST_BULK], &a.ctl->next[LIST_BULK], a.cls, a.ncols, a.colLen, nB, (int)blockIdx.x,
-                 a.kmax[LIST_BULK], a.kmaxLong, stB);
-        bulk_engine<false>(cur, smem, mbar, a.ringBytes);
+        cur.init(a.desc, colBase[LIST_BULK], coarse[LIST_BULK], &a.ctl->next[LIST_BULK], a.cls, a.ncols, a.colLen, nB,
+                 (int)blockIdx.x * E + warp, a.kmax[LIST_BULK], a.kmaxLong, stB);
+        bulk_engine<false>(cur, smem + (size_t)warp * subRing, mbar + warp * COPY_SLOTS, subRing, a.maxPendingStores);
     } else {
         Cursor<LIST_VEC> cur;
-        cur.init(a.desc, colBase[LIST_VEC], &a.ctl->next[LIST_VEC], a.cls, a.ncols, a.colLen, nV,
-                 (int)blockIdx.x * NV + warp - 1, a.kmax[LIST_VEC], a.kmaxLong, stV);
+        cur.init(a.desc, colBase[LIST_VEC], coarse[LIST_VEC], &a.ctl->next[LIST_VEC], a.cls, a.ncols, a.colLen, nV,
+                 (int)blockIdx.x * NV + warp - E, a.kmax[LIST_VEC], a.kmaxLong, stV);
         vector_engine<false>(cur);
     }
     workctl_checkout(a.ctl, colBase[LIST_BULK][R] > stB * nB || colBase[LIST_VEC][R] > stV * nV);

@@ -56,10 +56,7 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
     const int Wc = min(W, R - d0);
 
     griddep_launch_dependents();                 // let the copy kernel's CTAs start their prologue
-    if (blockIdx.x == 0 && threadIdx.x == 0) {   // the copy kernel follows on the same stream
-        a.ws.ctl->next[0] = 0u;
-        a.ws.ctl->next[1] = 0u;
-    }
+    griddep_wait();                              // (launched with PDL itself: the stream's previous kernel must be complete)
     // pointer tables: issue the loads now, park them in shared memory only after phase 1's loads are
     // in flight too (one DRAM round trip instead of two on a cold start)
     constexpr int PT = 2;                        // covers R <= 1024 with 512 threads
@@ -140,7 +137,9 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
         const unsigned long long dstBase = recvPtr[j];
         long long run = 0;
         int runT[2] = {0, 0};
+        const int nb = (R + 31) >> 5;
         for (int s0 = 0; s0 < R; s0 += 32) {
+            if (lane < 2) a.ws.coarse[lane][(size_t)d * nb + (s0 >> 5)] = lane ? runT[1] : runT[0];     // coarse index for the copy kernel's search
             const int s = s0 + lane;
             const bool valid = s < R;
             const long long c = valid ? cval[(size_t)s * P + j] : 0;

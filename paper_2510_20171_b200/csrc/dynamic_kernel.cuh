@@ -36,7 +36,6 @@ __global__ void __launch_bounds__(DYN_PREP_THREADS) dyn_prep_kernel(const DynArg
     const int s = blockIdx.x, lane = lane_id(), warp = threadIdx.x >> 5;
     const int R = a.R, n = a.n;
     griddep_launch_dependents();
-    if (s == 0 && threadIdx.x == 0) { a.ws.ctl->next[0] = 0u; a.ws.ctl->next[1] = 0u; }
     const long long* Ls = a.L + (size_t)s * n;
     if (warp == 0) {                                       // exclusive scan of the split lengths
         long long run = 0;
@@ -79,7 +78,9 @@ __global__ void __launch_bounds__(32) dyn_desc_kernel(const DynArgs a) {
     griddep_wait();                                        // O / ioff come from dyn_prep_kernel
     int runT[2] = {0, 0};
     unsigned int st = 0;
+    const int nb = (colLen + 31) >> 5;
     for (int k0 = 0; k0 < colLen; k0 += 32) {
+        if (lane < 2) a.ws.coarse[lane][(size_t)d * nb + (k0 >> 5)] = lane ? runT[1] : runT[0];
         const int k = k0 + lane;
         unsigned long long src = 0, dst = 0;
         long long bytes = 0;

@@ -38,17 +38,18 @@ struct FusedArgs {
     int kmax[2];
     int kmaxLong;
     int minTileShift[2];
+    int bulkEngines;                       // as CopyArgs::bulkEngines
     ClassParams cls;                       // tileShift[] = upper bounds; the kernel picks the actual shifts
 };
 
 __host__ __device__ inline size_t fused_desc_offset(int R) {     // from the end of the ring; keeps SegDesc 32 B-aligned
-    return (COPY_SLOTS * 8 + 2 * (size_t)(R + 1) * 4 + 31) & ~(size_t)31;
+    return (COPY_MBAR_BYTES + 2 * (size_t)(R + 1) * 4 + 31) & ~(size_t)31;
 }
 __host__ __device__ inline size_t fused_aux_bytes(int R) { return fused_desc_offset(R) + (size_t)R * R * sizeof(SegDesc); }
 
 __device__ __forceinline__ int floor_log2_ll(long long v) { return v <= 0 ? 0 : 63 - __clzll(v); }
 
-// dynamic smem: [ring: ringBytes][mbar: COPY_SLOTS x u64][colBase bulk: R+1][colBase vec: R+1][pad][SegDesc R*R]
+// dynamic smem: [ring: ringBytes][mbar: COPY_MAX_ENGINES x COPY_SLOTS x u64][colBase bulk: R+1][colBase vec: R+1][pad][SegDesc R*R]
 __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const FusedArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = lane_id();
@@ -57,7 +58,7 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
     const int R = a.R, RR = R * R;
     unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + a.ringBytes);
     int* colBase[2];
-    colBase[0] = reinterpret_cast<int*>(mbar + COPY_SLOTS);
+    colBase[0] = reinterpret_cast<int*>(mbar + COPY_MAX_ENGINES * COPY_SLOTS);
     colBase[1] = colBase[0] + (R + 1);
     SegDesc* sdesc = reinterpret_cast<SegDesc*>(smem + a.ringBytes + fused_desc_offset(R));
     // prologue scratch, dead before the first TMA load lands in the ring (<= 17.3 KB at R = 32)
@@ -72,8 +73,9 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
     const bool writer = blockIdx.x == 0;
 
     griddep_launch_dependents();           // a following call of this library may start its prologue
-    if (warp == 2 && lane == 0) {
-        for (int i = 0; i < COPY_SLOTS; ++i) mbar_init(smem_u32(&mbar[i]), 1);
+    const int E = a.bulkEngines;
+    if (threadIdx.x >= 64 && threadIdx.x < 64 + E * COPY_SLOTS) {
+        mbar_init(smem_u32(&mbar[threadIdx.x - 64]), 1);
         fence_mbar_init();
     }
     griddep_wait();                        // everything below reads what the stream's previous kernel wrote
@@ -106,8 +108,9 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
     long long totalElems = 0;
     for (int s = 0; s < R; ++s) totalElems += rowTot[s];
     const long long totalBytes = totalElems * a.elemSize;
-    constexpr int NV = NW - 1;
-    const int nB = (int)gridDim.x, nV = (int)gridDim.x * NV;
+    const int NV = NW - E;
+    const int nB = (int)gridDim.x * E, nV = (int)gridDim.x * NV;
+    const unsigned int subRing = (a.ringBytes / (unsigned int)E) & ~127u;
     ClassParams cls = a.cls;
     cls.tileShift[LIST_BULK] = max(a.minTileShift[LIST_BULK], min(a.cls.tileShift[LIST_BULK], floor_log2_ll(totalBytes / (2 * nB))));
     cls.tileShift[LIST_VEC] = max(a.minTileShift[LIST_VEC], min(a.cls.tileShift[LIST_VEC], floor_log2_ll(totalBytes / (2 * nV))));
@@ -141,23 +144,25 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
     }
     __syncthreads();
     if (warp < 2) {                        // cross-column tile bases (R <= 32: one warp scan per list)
-        const int v = lane < R ? colT[warp][lane] : 0;
+        const int* ct = warp ? colT[1] : colT[0];
+        int* cb = warp ? colBase[1] : colBase[0];
+        const int v = lane < R ? ct[lane] : 0;
         const int incl = warp_incl_scan(v);
-        if (lane == 0) colBase[warp][0] = 0;
-        if (lane < R) colBase[warp][lane + 1] = incl;
+        if (lane == 0) cb[0] = 0;
+        if (lane < R) cb[lane + 1] = incl;
     }
     fence_proxy_async_smem();              // scratch reads/writes (generic proxy) before TMA writes to the same bytes
     __syncthreads();                       // the scratch is dead from here on; the ring may be filled
 
     // ---- a4: the copy engines of the big path, fed from shared memory --------------------------------
-    if (warp == 0) {
+    if (warp < E) {
         Cursor<LIST_BULK, true> cur;
-        cur.init(sdesc, colBase[LIST_BULK], &a.ctl->next[LIST_BULK], cls, R, R, nB, (int)blockIdx.x,
+        cur.init(sdesc, colBase[LIST_BULK], nullptr, &a.ctl->next[LIST_BULK], cls, R, R, nB, (int)blockIdx.x * E + warp,
                  a.kmax[LIST_BULK], a.kmaxLong, 1);
-        bulk_engine<true>(cur, smem, mbar, a.ringBytes);
+        bulk_engine<true>(cur, smem + (size_t)warp * subRing, mbar + warp * COPY_SLOTS, subRing, 1);
     } else {
         Cursor<LIST_VEC, true> cur;
-        cur.init(sdesc, colBase[LIST_VEC], &a.ctl->next[LIST_VEC], cls, R, R, nV, (int)blockIdx.x * NV + warp - 1,
+        cur.init(sdesc, colBase[LIST_VEC], nullptr, &a.ctl->next[LIST_VEC], cls, R, R, nV, (int)blockIdx.x * NV + warp - E,
                  a.kmax[LIST_VEC], a.kmaxLong, 1);
         vector_engine<true>(cur);
     }

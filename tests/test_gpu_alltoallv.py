@@ -32,6 +32,11 @@ def default_params():
     nx.ncclx_set_param(nx.PARAM_BULK_TILE_SHIFT, 15)
     nx.ncclx_set_param(nx.PARAM_VEC_TILE_SHIFT, 14)
     nx.ncclx_set_param(nx.PARAM_SCAN_CTAS, 16)
+    nx.ncclx_set_param(nx.PARAM_COPY_BULK_ENGINES, 1)
+    nx.ncclx_set_param(nx.PARAM_COPY_PENDING_STORES, 1)
+    nx.ncclx_set_param(nx.PARAM_COPY_KMAX, 6)
+    nx.ncclx_set_param(nx.PARAM_COPY_STATIC_EIGHTHS, 0)
+    nx.ncclx_set_param(nx.PARAM_PDL, 1)
 
 
 def make_send(C, dtype, seed=0):
@@ -122,13 +127,27 @@ def test_ragged_bulk_tail_and_tiny_segments():
 @pytest.mark.parametrize("param,value", [("FORCE_VECTOR", 1), ("COPY_CTAS_PER_SM", 2), ("COPY_CTAS_PER_SM", 4),
                                          ("BULK_TILE_SHIFT", 12), ("BULK_TILE_SHIFT", 16), ("VEC_TILE_SHIFT", 10),
                                          ("BULK_MIN_BYTES", 16), ("BULK_MIN_BYTES", 1 << 20), ("SCAN_CTAS", 1),
-                                         ("SCAN_CTAS", 64)])
+                                         ("SCAN_CTAS", 64), ("COPY_BULK_ENGINES", 2), ("COPY_BULK_ENGINES", 4),
+                                         ("COPY_PENDING_STORES", 4), ("COPY_PENDING_STORES", 8), ("COPY_KMAX", 1),
+                                         ("COPY_KMAX", 17), ("COPY_STATIC_EIGHTHS", 4), ("COPY_STATIC_EIGHTHS", 8),
+                                         ("PDL", 0)])
 def test_launch_configurations_agree(param, value):
     nx.ncclx_set_param(getattr(nx, "PARAM_" + param), value)
     cfg = W.scaled_a2a(W.a2a_config(3), 64)
     C = cfg.counts
     send = make_send(C, "bf16", 4)
     assert_a2a_matches(send, C, "bf16")
+
+
+@pytest.mark.parametrize("engines", [2, 4])
+def test_small_R_and_cfg5_shapes_with_several_bulk_engines(engines):
+    """E bulk engine warps per CTA (ring split E ways) on the single-launch path and on short-segment traffic."""
+    nx.ncclx_set_param(nx.PARAM_COPY_BULK_ENGINES, engines)
+    rng = np.random.default_rng(engines)
+    C = rng.integers(0, 60_000, (8, 8)) * 8
+    assert_a2a_matches(make_send(C, "bf16", 21), C, "bf16")
+    cfg = W.scaled_a2a(W.a2a_config(5), 2)
+    assert_a2a_matches(make_send(cfg.counts, "bf16", 22), cfg.counts, "bf16")
 
 
 def test_cfg5_small_messages_full_compare():
