@@ -255,8 +255,9 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the per-config table (cfg1/cfg5 latency, cfg2 warm/cold)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--latency-replays", type=int, default=10000)
-    ap.add_argument("--probe", type=int, default=0, choices=[0, 1, 2, 3, 4, 5, 6],
-                    help="run ONLY BASELINE.json config N eagerly for --steps iterations (for ncu captures of one config)")
+    ap.add_argument("--probe", type=int, default=0, choices=[0, 1, 2, 3, 4, 5, 6, 7, 8],
+                    help="run ONLY BASELINE.json config N (1-5) eagerly for --steps iterations, or one of the widenings "
+                         "(6 = NEXT-4 latency, 7 = NEXT-1 dynamic, 8 = NEXT-3 top-k): the commands ncu captures are taken from")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -524,6 +525,9 @@ def latency_extra(torch, nx, peak, reps):
     (b) dispatch + combine back to back (the MoE layer's two consecutive AllToAlls): plain stream order vs the
     split-phase form with two plan slots, where the combine's metadata phase runs beside the dispatch's payload."""
     res = {}
+    x = torch.zeros(32, device="cuda")
+    # context: what ANY one-kernel graph replay costs between two CUDA events on this box (a 32-element torch add)
+    res["floor_one_tiny_kernel_graph"] = graph_p50(torch, lambda: x.add_(1), reps)
     a1 = A2A(W.a2a_config(1), torch, nx, with_back=True)
 
     def pair1():
@@ -563,8 +567,10 @@ def latency_extra(torch, nx, peak, reps):
 def probe(args, torch, nx, peak):
     """One config, eager launches, CUDA-event time per call (the command ncu captures are taken from)."""
     n = args.probe
-    if n == 6:
-        print(json.dumps({"probe": "next4_latency", **latency_extra(torch, nx, peak, args.steps)}))
+    if n in (6, 7, 8):
+        res = (latency_extra(torch, nx, peak, args.steps) if n == 6 else
+               dynamic_extra(torch, nx, peak, args.steps) if n == 7 else topk_extra(torch, nx, peak))
+        print(json.dumps({"probe": {6: "next4_latency", 7: "next1_dynamic", 8: "next3_topk"}[n], **res}))
         nx.ncclx_finalize()
         return 0
     if n in (1, 3, 5):

@@ -579,7 +579,7 @@ int ncclx_alltoallv_dynamic_dev(const void* const* send, const int64_t* sendSpli
         LaunchScope ls(NCCLX_KERNEL_DYN, s);
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3((unsigned)R);
-        cfg.blockDim = dim3(32);
+        cfg.blockDim = dim3(DYN_DESC_WARPS * 32);
         cfg.stream = s;
         cudaLaunchAttribute attr[1];
         setPdl(cfg, attr);

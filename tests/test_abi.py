@@ -48,6 +48,8 @@ def test_calls_fail_loudly_without_init(L):
     assert L.ncclx_allreduce_sum(1, 1, 8, 2, 0, None) == 3
     assert L.ncclx_reducescatter_sum(1, 1, 8, 2, 0, None) == 3
     assert L.ncclx_alltoallv_host(1, 1, 1, 2, 4, 0, None) == 3
+    assert L.ncclx_alltoallv_prepare_dev(0, 1, 1, 1, 2, 4, 0, None) == 3
+    assert L.ncclx_alltoallv_execute_dev(0, None) == 3
     with pytest.raises(binding.NcclxError):
         binding.ncclx_finalize()
 
