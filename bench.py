@@ -642,9 +642,21 @@ def run_e2e(torch, nx, a3, r2, r4, step_bytes, world, dist, steps):
         estep()
     torch.cuda.synchronize()
     dt = max_over_ranks(time.perf_counter() - t0, dist, "cuda")
+    # A/B: the same step with the kernels' direct access to pinned host memory switched off (device staging)
+    staged_ms = None
+    if world == 1:
+        nx.ncclx_set_param(nx.PARAM_HOST_ZERO_COPY, 0)
+        estep()
+        t1 = time.perf_counter()
+        estep()
+        staged_ms = (time.perf_counter() - t1) * 1e3
+        nx.ncclx_set_param(nx.PARAM_HOST_ZERO_COPY, 1)
     return {"value": round(whole_job_value(world, step_bytes, dt / steps * 1e3), 2), "unit": "GB/s", "steps": steps,
             "ms_per_step": round(dt / steps * 1e3, 2), "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-            "roundtrip_identity": bool(ok), "api": "ncclx_alltoallv_host x2 + ncclx_allreduce_sum_host + ncclx_reducescatter_sum_host"}
+            "roundtrip_identity": bool(ok), "api": "ncclx_alltoallv_host x2 + ncclx_allreduce_sum_host + ncclx_reducescatter_sum_host",
+            "transport": "pinned host buffers: AllToAllv and AllReduce kernels read/write host memory directly over PCIe "
+                         "(both directions at once); ReduceScatter staged through device memory",
+            "ms_per_step_all_staged": None if staged_ms is None else round(staged_ms, 2)}
 
 
 if __name__ == "__main__":

@@ -225,11 +225,14 @@ int ncclx_moe_combine_topk_sum_dev(const void* const* expert_out, const int32_t*
 
 /* ---- host-buffer forms (the end-to-end path: H2D + kernels + D2H inside the call) ------ *
  *
- * Same semantics, but every pointer is a HOST pointer (pinned memory gives full PCIe
- * speed; pageable works).  `send`/`recv` are HOST arrays of R HOST pointers and the counts
- * are HOST arrays.  The library stages through its own device buffers (grown on demand with
- * cudaMalloc and kept until ncclx_finalize), runs the device path on `stream`, copies the
- * results back and synchronises `stream` before returning.  Not capturable.
+ * Same semantics, but every pointer is a HOST pointer.  `send`/`recv` are HOST arrays of R HOST
+ * pointers and the counts are HOST arrays.  When EVERY data buffer in use is pinned (cudaHostAlloc /
+ * cudaHostRegister, e.g. torch's pin_memory()), the same kernels read and write the host buffers
+ * directly over PCIe (zero-copy: the inbound and outbound halves of the call share the full-duplex
+ * link instead of running one after the other; NCCLX_PARAM_HOST_ZERO_COPY = 0 turns it off).
+ * Otherwise (pageable memory) the library stages through its own device buffers (grown on demand with
+ * cudaMalloc and kept until ncclx_finalize): H2D copies, the device path on `stream`, D2H copies.
+ * Either way `stream` is synchronised before returning.  Not capturable.
  * AllToAllv: recv[d] receives exactly sum_s C[s][d] elements; recvcounts_host is filled. */
 int ncclx_alltoallv_host(const void* const* send, const int64_t* sendcounts_host, void* const* recv,
                          int64_t* recvcounts_host, int R, ncclx_dtype_t dtype, ncclx_stream_t stream);
@@ -259,6 +262,7 @@ typedef enum {
     NCCLX_PARAM_FUSED_MIN_TILE_SHIFT = 13, /* smallest bulk tile the single-launch path may choose (log2 bytes, 10..16), default 12 */
     NCCLX_PARAM_COPY_PENDING_STORES = 14, /* bulk engine: stores left unreclaimed in the ring after each store (1..8), default 1 */
     NCCLX_PARAM_COPY_BULK_ENGINES = 15,   /* bulk (TMA) engine warps per copy CTA, each with 1/E of the ring: 1 (default), 2 or 4 */
+    NCCLX_PARAM_HOST_ZERO_COPY = 16,      /* 1 (default): the *_host calls let the kernels access PINNED host buffers directly */
     NCCLX_PARAM_COUNT_
 } ncclx_param_t;
 

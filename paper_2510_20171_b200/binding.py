@@ -32,6 +32,7 @@ PARAM_FUSED_MAX_RANKS = 12
 PARAM_FUSED_MIN_TILE_SHIFT = 13
 PARAM_COPY_PENDING_STORES = 14
 PARAM_COPY_BULK_ENGINES = 15
+PARAM_HOST_ZERO_COPY = 16
 NUM_PLANS = 4
 
 KERNEL_COUNTS, KERNEL_COPY, KERNEL_REDUCE, KERNEL_DYN, KERNEL_TOPK, KERNEL_FUSED = 0, 1, 2, 3, 4, 5

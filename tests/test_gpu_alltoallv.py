@@ -250,16 +250,28 @@ def test_graph_capture_counts_by_reference():
             assert back(recv[d], "bf16").tobytes() == exp[d].tobytes()
 
 
-def test_host_buffer_form():
-    cfg = W.scaled_a2a(W.a2a_config(3), 128)
-    C = cfg.counts
-    R = cfg.R
-    send_np = make_send(C, "bf16", 70)
-    pinned = [torch.from_numpy(a.view(np.int16)).pin_memory() for a in send_np]
-    out = [torch.empty(int(C[:, d].sum()), dtype=torch.int16).pin_memory() for d in range(R)]
-    RCh = np.zeros((R, R), np.int64)
-    nx.ncclx_alltoallv_host(pinned, np.ascontiguousarray(C), out, RCh, R, "bf16")
-    exp, eRC, *_ = oracle_a2a(send_np, C, "bf16", slack_elems=0)
-    assert (RCh == eRC).all()
-    for d in range(R):
-        assert out[d].numpy().view(np.uint16).tobytes() == exp[d].tobytes()
+@pytest.mark.parametrize("mode", ["pinned_zero_copy", "pinned_staged", "pageable"])
+def test_host_buffer_form(mode):
+    """Host-buffer entry point: pinned buffers are accessed by the kernels directly (zero-copy), pageable ones
+    (or NCCLX_PARAM_HOST_ZERO_COPY = 0) are staged through device memory; same result either way."""
+    nx.ncclx_set_param(nx.PARAM_HOST_ZERO_COPY, 0 if mode == "pinned_staged" else 1)
+    try:
+        cfg = W.scaled_a2a(W.a2a_config(3), 128)
+        C = cfg.counts
+        R = cfg.R
+        send_np = make_send(C, "bf16", 70)
+        if mode == "pageable":
+            src = [a.copy() for a in send_np]
+            out = [np.full(int(C[:, d].sum()) + 8, 0xA5A5, np.uint16) for d in range(R)]
+        else:
+            src = [torch.from_numpy(a.view(np.int16)).pin_memory() for a in send_np]
+            out = [torch.full((int(C[:, d].sum()) + 8,), -23131, dtype=torch.int16).pin_memory() for d in range(R)]
+        RCh = np.zeros((R, R), np.int64)
+        nx.ncclx_alltoallv_host(src, np.ascontiguousarray(C), out, RCh, R, "bf16")
+        exp, eRC, *_ = oracle_a2a(send_np, C, "bf16", slack_elems=8)
+        assert (RCh == eRC).all()
+        for d in range(R):
+            got = out[d] if mode == "pageable" else out[d].numpy().view(np.uint16)
+            assert got.tobytes() == exp[d].tobytes()          # incl. the untouched 0xA5 tail
+    finally:
+        nx.ncclx_set_param(nx.PARAM_HOST_ZERO_COPY, 1)

@@ -150,18 +150,30 @@ def test_errors_and_noop():
     assert e.value.code == 1
 
 
-def test_host_buffer_forms():
-    R, n = 4, 8 * 5000
-    xs = [W.np_values(R * n, "bf16", 600 + k) for k in range(R)]
-    pin = [torch.from_numpy(a.view(np.int16)).pin_memory() for a in xs]
-    out_ar = [torch.empty(R * n, dtype=torch.int16).pin_memory() for _ in range(R)]
-    out_rs = [torch.empty(n, dtype=torch.int16).pin_memory() for _ in range(R)]
-    nx.ncclx_allreduce_sum_host(pin, out_ar, R * n, R, "bf16")
-    nx.ncclx_reducescatter_sum_host(pin, out_rs, n, R, "bf16")
-    exp = oracle.allreduce_sum(xs, "bf16", nthreads=4)
-    for r in range(R):
-        assert out_ar[r].numpy().view(np.uint16).tobytes() == exp[r].tobytes()
-        assert out_rs[r].numpy().view(np.uint16).tobytes() == exp[0][r * n:(r + 1) * n].tobytes()
+@pytest.mark.parametrize("mode", ["pinned_zero_copy", "pinned_staged", "pageable"])
+def test_host_buffer_forms(mode):
+    nx.ncclx_set_param(nx.PARAM_HOST_ZERO_COPY, 0 if mode == "pinned_staged" else 1)
+    try:
+        R, n = 4, 8 * 5000
+        xs = [W.np_values(R * n, "bf16", 600 + k) for k in range(R)]
+        if mode == "pageable":
+            src = [a.copy() for a in xs]
+            out_ar = [np.zeros(R * n, np.uint16) for _ in range(R)]
+            out_rs = [np.zeros(n, np.uint16) for _ in range(R)]
+            view = lambda t: t
+        else:
+            src = [torch.from_numpy(a.view(np.int16)).pin_memory() for a in xs]
+            out_ar = [torch.empty(R * n, dtype=torch.int16).pin_memory() for _ in range(R)]
+            out_rs = [torch.empty(n, dtype=torch.int16).pin_memory() for _ in range(R)]
+            view = lambda t: t.numpy().view(np.uint16)
+        nx.ncclx_allreduce_sum_host(src, out_ar, R * n, R, "bf16")
+        nx.ncclx_reducescatter_sum_host(src, out_rs, n, R, "bf16")
+        exp = oracle.allreduce_sum(xs, "bf16", nthreads=4)
+        for r in range(R):
+            assert view(out_ar[r]).tobytes() == exp[r].tobytes()
+            assert view(out_rs[r]).tobytes() == exp[0][r * n:(r + 1) * n].tobytes()
+    finally:
+        nx.ncclx_set_param(nx.PARAM_HOST_ZERO_COPY, 1)
 
 
 # ---- NEXT-2: FTAR-style ReduceCopy step -------------------------------------------------
