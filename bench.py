@@ -255,9 +255,9 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the per-config table (cfg1/cfg5 latency, cfg2 warm/cold)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--latency-replays", type=int, default=10000)
-    ap.add_argument("--probe", type=int, default=0, choices=[0, 1, 2, 3, 4, 5, 6, 7, 8],
+    ap.add_argument("--probe", type=int, default=0, choices=[0, 1, 2, 3, 4, 5, 6, 7, 8, 9],
                     help="run ONLY BASELINE.json config N (1-5) eagerly for --steps iterations, or one of the widenings "
-                         "(6 = NEXT-4 latency, 7 = NEXT-1 dynamic, 8 = NEXT-3 top-k): the commands ncu captures are taken from")
+                         "(6 = NEXT-4 latency, 7 = NEXT-1 dynamic, 8 = NEXT-3 top-k, 9 = HBM streaming ceilings): the commands ncu captures are taken from")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -416,6 +416,8 @@ def main():
         per["next2_reducecopy_cta_sweep"] = reducecopy_extra(torch, nx, peak)
         per["next3_topk_R64_T4096_k4"] = topk_extra(torch, nx, peak)
         per["next4_latency"] = latency_extra(torch, nx, peak, min(args.latency_replays, 2000))
+        per["hbm_ceiling_probe"] = ceiling_extra(torch, nx, peak)
+        roofline["practical_ceiling_GBps"] = {k: per["hbm_ceiling_probe"][k]["GBps"] for k in ("read_only", "write_only", "copy")}
         line["per_config"] = per
 
     # ---- e2e: same step through the host-buffer C ABI (H2D + kernels + D2H inside the timed region) --------
@@ -505,6 +507,19 @@ def reducecopy_extra(torch, nx, peak):
     return res
 
 
+def ceiling_extra(torch, nx, peak, nbytes=4 << 30):
+    """read-only / write-only / copy streaming micro-probe (256-bit accesses, one pass over 4 GiB,
+    far beyond L2): the practical HBM ceilings the kernels' roofline fractions are read against."""
+    src = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    dst = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    src.fill_(7)
+    res = {"bytes": nbytes}
+    for mode, name, moved in ((0, "read_only", nbytes), (1, "write_only", nbytes), (2, "copy", 2 * nbytes)):
+        t = event_times_ms(torch, lambda: nx.ncclx_stream_probe(mode, src, dst, nbytes), 10)
+        res[name] = {"ms_median": round(float(np.median(t)), 4), **frac(moved / (np.median(t) * 1e-3) / 1e9, peak)}
+    return res
+
+
 def graph_p50(torch, enqueue, reps, warm=20):
     """Capture `enqueue` once (after one eager run on a side stream), time `reps` replays with CUDA events."""
     side = torch.cuda.Stream()
@@ -567,10 +582,11 @@ def latency_extra(torch, nx, peak, reps):
 def probe(args, torch, nx, peak):
     """One config, eager launches, CUDA-event time per call (the command ncu captures are taken from)."""
     n = args.probe
-    if n in (6, 7, 8):
+    if n in (6, 7, 8, 9):
         res = (latency_extra(torch, nx, peak, args.steps) if n == 6 else
-               dynamic_extra(torch, nx, peak, args.steps) if n == 7 else topk_extra(torch, nx, peak))
-        print(json.dumps({"probe": {6: "next4_latency", 7: "next1_dynamic", 8: "next3_topk"}[n], **res}))
+               dynamic_extra(torch, nx, peak, args.steps) if n == 7 else
+               topk_extra(torch, nx, peak) if n == 8 else ceiling_extra(torch, nx, peak))
+        print(json.dumps({"probe": {6: "next4_latency", 7: "next1_dynamic", 8: "next3_topk", 9: "hbm_ceiling"}[n], **res}))
         nx.ncclx_finalize()
         return 0
     if n in (1, 3, 5):

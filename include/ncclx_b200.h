@@ -287,6 +287,12 @@ int ncclx_profile_read(int kernel, double* total_ms, int64_t* launches);
 int ncclx_profile_reset(void);
 int64_t ncclx_launch_count(void);
 
+/* HBM streaming micro-probe (measurement aid): one pass of 256-bit accesses over `bytes`
+ * (multiple of 32; 32-byte aligned DEVICE pointers).  mode 0 = read-only over src (dst may be NULL),
+ * 1 = write-only over dst (src may be NULL; contents become a fixed pattern), 2 = copy src -> dst.  Enqueue
+ * only; time it with events.  Gives the practical read / write / copy ceilings of the part. */
+int ncclx_stream_probe(int mode, const void* src, void* dst, size_t bytes, ncclx_stream_t stream);
+
 /* Number of SMs of the device the library was initialised on (0 before init). */
 int ncclx_sm_count(void);
 

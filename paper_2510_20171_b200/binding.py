@@ -45,7 +45,7 @@ SYMBOLS = [
     "ncclx_reducescatter_sum_host", "ncclx_set_param", "ncclx_get_param", "ncclx_profile_read",
     "ncclx_profile_reset", "ncclx_launch_count", "ncclx_sm_count", "ncclx_init_dynamic", "ncclx_alltoallv_dynamic_dev",
     "ncclx_reducecopy_sum", "ncclx_moe_dispatch_topk_dev", "ncclx_moe_combine_topk_sum_dev",
-    "ncclx_alltoallv_prepare_dev", "ncclx_alltoallv_execute_dev",
+    "ncclx_alltoallv_prepare_dev", "ncclx_alltoallv_execute_dev", "ncclx_stream_probe",
 ]
 
 
@@ -90,6 +90,7 @@ def lib() -> ctypes.CDLL:
         L.ncclx_reducecopy_sum.argtypes = [vp, vp, vp, vp, ctypes.c_size_t, ctypes.c_int, ctypes.c_size_t, ctypes.c_int, vp]
         L.ncclx_moe_dispatch_topk_dev.argtypes = [vp, vp, vp, vp, vp] + [ctypes.c_int] * 5 + [vp]
         L.ncclx_moe_combine_topk_sum_dev.argtypes = [vp, vp, vp, vp] + [ctypes.c_int] * 5 + [vp]
+        L.ncclx_stream_probe.argtypes = [ctypes.c_int, vp, vp, ctypes.c_size_t, vp]
         L.ncclx_set_param.argtypes = [ctypes.c_int, i64]
         L.ncclx_get_param.argtypes = [ctypes.c_int, i64p]
         L.ncclx_profile_read.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double), i64p]
@@ -253,6 +254,10 @@ def ncclx_reducescatter_sum_host(send: Sequence, recv: Sequence, recvcount: int,
 
 
 # ---- tuning / measurement -------------------------------------------------------------------------
+
+def ncclx_stream_probe(mode: int, src, dst, nbytes: int, stream=None) -> None:
+    _ck(lib().ncclx_stream_probe(mode, _ptr(src), _ptr(dst), nbytes, _stream(stream)), "ncclx_stream_probe")
+
 
 def ncclx_set_param(param: int, value: int) -> None:
     _ck(lib().ncclx_set_param(param, value), "ncclx_set_param")

@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libncclx_b200.so")
 SOURCES = [os.path.join(CSRC, "ncclx_b200.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("common.cuh", "counts_kernel.cuh", "copy_kernel.cuh", "reduce_kernel.cuh", "dynamic_kernel.cuh", "topk_kernel.cuh", "fused_kernel.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("common.cuh", "counts_kernel.cuh", "copy_kernel.cuh", "reduce_kernel.cuh", "dynamic_kernel.cuh", "topk_kernel.cuh", "fused_kernel.cuh", "probe_kernel.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "ncclx_b200.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "--ftz=false", "--prec-div=true",

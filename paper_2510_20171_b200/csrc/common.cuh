@@ -28,6 +28,7 @@ struct WorkCtl {
     unsigned int next[2];     // dynamic tile-claim counters, one per work list
     unsigned int status;      // sticky: bit 0 = negative count seen
     unsigned int done;        // CTAs of the running copy kernel that have drained their engines
+    unsigned int pad_probe;   // sink of the streaming micro-probe (never read)
 };
 
 struct Workspace {

@@ -16,6 +16,7 @@
 #include "counts_kernel.cuh"
 #include "dynamic_kernel.cuh"
 #include "fused_kernel.cuh"
+#include "probe_kernel.cuh"
 #include "reduce_kernel.cuh"
 #include "topk_kernel.cuh"
 
@@ -177,6 +178,9 @@ int launchCopy(const Workspace& ws, const SegDesc* desc, const int* const coarse
     cp.ctl = ws.ctl; cp.ncols = ncols; cp.colLen = colLen;
     cp.cls = cls;
     cp.ringBytes = chooseRingBytes(cps, ncols, colLen);
+    // the work list's bulk tile (fixed when it was built) must fit ~2.5 times into one engine's share of the
+    // ring; a larger tile could never be staged (parameters changed between prepare and execute)
+    if (((size_t)5 << cls.tileShift[0]) / 2 > cp.ringBytes / (size_t)g.params[NCCLX_PARAM_COPY_BULK_ENGINES]) return NCCLX_ERR_ARG;
     cp.staticEighths = (int)g.params[NCCLX_PARAM_COPY_STATIC_EIGHTHS];
     cp.kmax[0] = (int)g.params[NCCLX_PARAM_COPY_KMAX];
     cp.kmax[1] = 8;
@@ -820,6 +824,17 @@ int ncclx_reducescatter_sum_host(const void* const* send, void* const* recv, siz
 }
 
 // ---- tuning / measurement --------------------------------------------------------------------
+
+int ncclx_stream_probe(int mode, const void* src, void* dst, size_t bytes, ncclx_stream_t stream) {
+    if (!g.ready) return NCCLX_ERR_NOT_INITIALIZED;
+    if (mode < 0 || mode > 2 || (mode != 1 && !src) || (mode != 0 && !dst) || bytes % 32) return NCCLX_ERR_ARG;
+    if ((((uintptr_t)src | (uintptr_t)dst) & 31u) != 0) return NCCLX_ERR_ARG;
+    if (bytes == 0) return NCCLX_OK;
+    stream_probe_kernel<<<g.smCount * 8, PROBE_THREADS, 0, static_cast<cudaStream_t>(stream)>>>(
+        mode, static_cast<const unsigned char*>(src), static_cast<unsigned char*>(dst), bytes / 32, &g.ws.ctl->pad_probe);
+    CK(cudaGetLastError());
+    return NCCLX_OK;
+}
 
 int ncclx_set_param(int param, int64_t value) {
     if (param < 0 || param >= NCCLX_PARAM_COUNT_) return NCCLX_ERR_ARG;

@@ -213,3 +213,24 @@ def test_reducecopy_misaligned_and_errors():
     with pytest.raises(nx.binding.NcclxError) as e:
         nx.ncclx_reducecopy_sum(da, db, out, None, n, "u8")
     assert e.value.code == 2
+
+
+def test_stream_probe_modes():
+    """Measurement aid: copy mode copies, read-only leaves both buffers alone, write-only fills."""
+    n = 32 * 100_003
+    src = torch.randint(0, 255, (n,), dtype=torch.uint8, device="cuda")
+    dst = torch.full((n + 32,), 0xA5, dtype=torch.uint8, device="cuda")
+    ref = src.clone()
+    nx.ncclx_stream_probe(0, src, None, n)
+    torch.cuda.synchronize()
+    assert torch.equal(src, ref) and bool((dst == 0xA5).all())
+    nx.ncclx_stream_probe(2, src, dst, n)
+    torch.cuda.synchronize()
+    assert torch.equal(dst[:n], ref) and bool((dst[n:] == 0xA5).all())
+    nx.ncclx_stream_probe(1, None, dst, n)
+    torch.cuda.synchronize()
+    w = dst[:n].view(torch.int32).view(-1, 8).cpu()
+    assert bool((w[:, 0] == torch.arange(n // 32, dtype=torch.int32)).all()) and bool((w[:, 1:] == torch.arange(1, 8, dtype=torch.int32)).all())
+    assert bool((dst[n:] == 0xA5).all())
+    with pytest.raises(nx.binding.NcclxError):
+        nx.ncclx_stream_probe(2, src, dst, n + 1)
