@@ -267,3 +267,50 @@ def test_double_buffered_dispatch_and_combine(use_graph):
             n = int(C[s].sum())
             got = back(bk[s], "bf16")
             assert got[:n].tobytes() == send_np[s][:n].tobytes() and (got[n:] == 0xA5A5).all()
+
+
+@pytest.mark.parametrize("R", [8, 48])
+def test_graph_with_memcpy_and_memset_nodes_before_the_call(R):
+    """The metadata kernels are launched with programmatic stream serialisation; inside a captured graph their
+    predecessor may be a memcpy or memset node instead of a kernel (the router's output copied into the count
+    matrix).  One-kernel (R = 8) and two-kernel (R = 48) paths; counts by reference through the captured copy."""
+    rng = np.random.default_rng(R)
+    cap_rows, width = 64, 128
+    rowsA = rng.integers(0, cap_rows // 2, (R, R))
+    rowsB = rng.integers(0, cap_rows // 2, (R, R)) * (rng.random((R, R)) < 0.5)
+    cap = cap_rows * R * width
+    send_np = [W.np_values(cap, "bf16", 90 + s) for s in range(R)]
+    send = [to_dev(a) for a in send_np]
+    recv = [sentinel(cap * 2) for _ in range(R)]
+    staging = torch.from_numpy((rowsA * width).astype(np.int64)).cuda()      # "router output"
+    Cd = torch.zeros_like(staging)
+    RCd = torch.zeros_like(staging)
+    st, rt = nx.device_ptr_table(send), nx.device_ptr_table(recv)
+
+    def enqueue():
+        for r in recv:
+            r.fill_(SENT8)                                                    # fill kernels / memset nodes
+        RCd.zero_()
+        Cd.copy_(staging)                                                     # D2D memcpy node right before the call
+        nx.ncclx_alltoallv_dev(st, Cd, rt, RCd, R, "bf16")
+
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        enqueue()
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        enqueue()
+    import oracle
+    for rows in (rowsA, rowsB):
+        C = (rows * width).astype(np.int64)
+        staging.copy_(torch.from_numpy(C))
+        graph.replay()
+        torch.cuda.synchronize()
+        exp = [np.full(cap, 0xA5A5, np.uint16) for _ in range(R)]
+        RC, *_ = oracle.alltoallv(send_np, C, exp, "bf16", nthreads=4)
+        assert (RCd.cpu().numpy() == RC).all()
+        for d in range(R):
+            assert back(recv[d], "bf16").tobytes() == exp[d].tobytes()
