@@ -62,7 +62,7 @@ typedef enum {
 /* ---- lifetime ------------------------------------------------------------------------- */
 
 /* Allocates the workspace (offset matrices, segment descriptors, work counters, status word:
- * about 64 * max_ranks^2 bytes) on `device`, sets kernel attributes and queries the SM count.
+ * NCCLX_NUM_PLANS slots of about 60 * max_ranks^2 bytes each) on `device`, sets kernel attributes and queries the SM count.
  * Call OUTSIDE stream capture.  Calling it again re-initialises (after an implicit finalize).
  * 1 <= max_ranks <= NCCLX_MAX_RANKS. */
 int ncclx_init(int max_ranks, int device);
