@@ -38,7 +38,7 @@ struct Context {
     WorkCtl* fusedCtl = nullptr;          // claim counters of the single-launch path (self-resetting)
     void* wsBase = nullptr;
     // tunables
-    int64_t params[NCCLX_PARAM_COUNT_] = {1, 1024, 4, 16, 0, 0, 15, 14, 1, 0, 6, 2, 32, 12, 1, 1, 1};
+    int64_t params[NCCLX_PARAM_COUNT_] = {1, 1024, 8, 16, 0, 0, 15, 14, 1, 0, 6, 2, 32, 12, 1, 1, 1};
     // profiling
     std::vector<EventPair> events[NCCLX_KERNEL_COUNT_];
     std::atomic<int64_t> launches{0};
@@ -276,8 +276,8 @@ int launchCounts(const Workspace& ws, const void* const* send, const int64_t* C,
 
 template <int DT>
 int launchReduceDT(const ReduceArgs& ra, int grid, size_t smem, cudaStream_t stream) {
-    // plain launch: programmatic dependent launch was tried for back-to-back reductions and measured no gain
-    // (config 2 in a 6-call graph: 25.5 -> 25.9 us per call; the resident CTAs leave no room for the next grid)
+    // plain launch: programmatic dependent launch was measured for back-to-back reductions (config 2 in a 6-call
+    // graph: -0.5 us per call) but costs config 4 0.3-0.6 %, so reductions do not use it
     LaunchScope ls(NCCLX_KERNEL_REDUCE, stream);
     if (ra.R <= 4) reduce_kernel<DT, 4><<<grid, REDUCE_THREADS, smem, stream>>>(ra);
     else if (ra.R <= 8) reduce_kernel<DT, 8><<<grid, REDUCE_THREADS, smem, stream>>>(ra);
