@@ -514,7 +514,8 @@ def ceiling_extra(torch, nx, peak, nbytes=4 << 30):
     dst = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
     src.fill_(7)
     res = {"bytes": nbytes}
-    for mode, name, moved in ((0, "read_only", nbytes), (1, "write_only", nbytes), (2, "copy", 2 * nbytes)):
+    for mode, name, moved in ((0, "read_only", nbytes), (1, "write_only", nbytes), (2, "copy", 2 * nbytes),
+                              (3, "write_only_tma", nbytes)):
         t = event_times_ms(torch, lambda: nx.ncclx_stream_probe(mode, src, dst, nbytes), 10)
         res[name] = {"ms_median": round(float(np.median(t)), 4), **frac(moved / (np.median(t) * 1e-3) / 1e9, peak)}
     return res

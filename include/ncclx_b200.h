@@ -290,7 +290,8 @@ int64_t ncclx_launch_count(void);
 
 /* HBM streaming micro-probe (measurement aid): one pass of 256-bit accesses over `bytes`
  * (multiple of 32; 32-byte aligned DEVICE pointers).  mode 0 = read-only over src (dst may be NULL),
- * 1 = write-only over dst (src may be NULL; contents become a fixed pattern), 2 = copy src -> dst.  Enqueue
+ * 1 = write-only over dst (src may be NULL; contents become a fixed pattern), 2 = copy src -> dst,
+ * 3 = write-only through TMA bulk stores of 32 KiB (bytes a multiple of 32 KiB).  Enqueue
  * only; time it with events.  Gives the practical read / write / copy ceilings of the part. */
 int ncclx_stream_probe(int mode, const void* src, void* dst, size_t bytes, ncclx_stream_t stream);
 

@@ -827,9 +827,16 @@ int ncclx_reducescatter_sum_host(const void* const* send, void* const* recv, siz
 
 int ncclx_stream_probe(int mode, const void* src, void* dst, size_t bytes, ncclx_stream_t stream) {
     if (!g.ready) return NCCLX_ERR_NOT_INITIALIZED;
-    if (mode < 0 || mode > 2 || (mode != 1 && !src) || (mode != 0 && !dst) || bytes % 32) return NCCLX_ERR_ARG;
+    if (mode < 0 || mode > 3 || ((mode == 0 || mode == 2) && !src) || (mode != 0 && !dst) || bytes % 32) return NCCLX_ERR_ARG;
     if ((((uintptr_t)src | (uintptr_t)dst) & 31u) != 0) return NCCLX_ERR_ARG;
     if (bytes == 0) return NCCLX_OK;
+    if (mode == 3) {
+        if (bytes % PROBE_BULK_BYTES) return NCCLX_ERR_ARG;
+        stream_probe_bulk_store_kernel<<<g.smCount * 4, 128, 0, static_cast<cudaStream_t>(stream)>>>(
+            static_cast<unsigned char*>(dst), bytes / PROBE_BULK_BYTES);
+        CK(cudaGetLastError());
+        return NCCLX_OK;
+    }
     stream_probe_kernel<<<g.smCount * 8, PROBE_THREADS, 0, static_cast<cudaStream_t>(stream)>>>(
         mode, static_cast<const unsigned char*>(src), static_cast<unsigned char*>(dst), bytes / 32, &g.ws.ctl->pad_probe);
     CK(cudaGetLastError());

@@ -5,6 +5,7 @@
 //                       checksum that is written only if it hits an impossible value (keeps the loads alive)
 //   mode 1  write-only: every 32-byte vector of dst is stored once (256-bit, L1 no-allocate)
 //   mode 2  copy      : dst = src with the same loads and stores
+//   mode 3  write-only through the TMA: dst is filled with cp.async.bulk shared->global stores of 32 KiB
 #pragma once
 #include "common.cuh"
 
@@ -39,6 +40,23 @@ __global__ void __launch_bounds__(PROBE_THREADS) stream_probe_kernel(int mode, c
         }
     }
     if (mode == 0 && acc == 0x9e3779b9u) *sink = acc;      // practically never true: only keeps the loads observable
+}
+
+constexpr int PROBE_BULK_BYTES = 32 * 1024;
+
+__global__ void __launch_bounds__(128) stream_probe_bulk_store_kernel(unsigned char* dst, unsigned long long nchunks) {
+    __shared__ __align__(128) unsigned char buf[PROBE_BULK_BYTES];
+    for (int i = threadIdx.x; i < PROBE_BULK_BYTES / 4; i += 128) reinterpret_cast<unsigned int*>(buf)[i] = (unsigned int)i;
+    fence_proxy_async_smem();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (unsigned long long c = blockIdx.x; c < nchunks; c += gridDim.x) {
+            bulk_s2g(dst + c * PROBE_BULK_BYTES, smem_u32(buf), PROBE_BULK_BYTES);
+            bulk_commit();
+            bulk_wait_read<6>();           // the source never changes; only bound the queue depth
+        }
+        bulk_wait_all<0>();
+    }
 }
 
 }  // namespace ncclx

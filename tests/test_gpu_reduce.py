@@ -234,3 +234,9 @@ def test_stream_probe_modes():
     assert bool((dst[n:] == 0xA5).all())
     with pytest.raises(nx.binding.NcclxError):
         nx.ncclx_stream_probe(2, src, dst, n + 1)
+    chunk = 32 * 1024
+    big = torch.full((5 * chunk + 64,), 0xA5, dtype=torch.uint8, device="cuda")
+    nx.ncclx_stream_probe(3, None, big, 5 * chunk)               # TMA bulk stores of a fixed 32 KiB pattern
+    torch.cuda.synchronize()
+    w = big[:5 * chunk].view(torch.int32).view(5, chunk // 4).cpu()
+    assert bool((w == torch.arange(chunk // 4, dtype=torch.int32)).all()) and bool((big[5 * chunk:] == 0xA5).all())
