@@ -44,16 +44,6 @@ struct CopyArgs {
     ClassParams cls;
 };
 
-#ifdef NCCLX_EXPERIMENTS
-__device__ int g_exp_mode = 0;             // _work probes only: 1 = skip stores, 2 = skip loads (results invalid)
-__device__ long long g_exp_cycles[256 * 8];
-#define EXP_T0() const long long t0_ = clock64()
-#define EXP_ACC(i) do { expc[i] += clock64() - t0_; } while (0)
-#else
-#define EXP_T0() do {} while (0)
-#define EXP_ACC(i) do {} while (0)
-#endif
-
 __host__ __device__ inline int coarse_blocks(int colLen) { return (colLen + 31) >> 5; }
 
 // Warp-uniform cursor over one work list.  All lanes hold identical state except the descriptor
@@ -426,11 +416,6 @@ template <bool SM>
 __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned char* ring, unsigned long long* mbar,
                                             const unsigned int ringBytes, const int maxPending) {
     const int lane = lane_id();
-#ifdef NCCLX_EXPERIMENTS
-    const int expMode = g_exp_mode;
-    long long expc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    const long long tStart = clock64();
-#endif
     const unsigned int tileBytes = 1u << cur.tileShift;
     const uint32_t ring0 = smem_u32(ring);
     unsigned long long mDst = 0;          // slot registers (lane j <-> slot j)
@@ -457,13 +442,8 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
                 if (lane == slot) { mDst = (unsigned long long)dstp; mLen = len16; mOff = po; mV = vStart; }
                 if (lane == 0) {
                     const uint32_t bar = smem_u32(&mbar[slot]);
-#ifdef NCCLX_EXPERIMENTS
-                    if (expMode == 2) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory"); } else
-#endif
-                    {
-                        mbar_expect_tx(bar, len16);
-                        bulk_g2s(ring0 + po, srcp, len16, bar);
-                    }
+                    mbar_expect_tx(bar, len16);
+                    bulk_g2s(ring0 + po, srcp, len16, bar);
                 }
                 const unsigned int adv = (len16 + 127u) & ~127u;
                 vHead = vStart + adv;
@@ -474,7 +454,7 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
             const int tail = (int)(len & 15u);        // only the last tile of a ragged segment
             if (lane < tail) dstp[len16 + lane] = __ldg(srcp + len16 + lane);
             cur.next();
-            { EXP_T0(); more = cur.ensure(); EXP_ACC(0); }
+            more = cur.ensure();
         }
         if (iStore == iLoad) {
             if (!more) break;
@@ -486,36 +466,23 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
             continue;
         }
         const int slot = iStore % COPY_SLOTS;
-        { EXP_T0(); mbar_wait(smem_u32(&mbar[slot]), (uint32_t)((iStore / COPY_SLOTS) & 1)); EXP_ACC(1); }
-#ifdef NCCLX_EXPERIMENTS
-        expc[5] += 1;
-#endif
+        mbar_wait(smem_u32(&mbar[slot]), (uint32_t)((iStore / COPY_SLOTS) & 1));
         const unsigned int dlo = __shfl_sync(0xffffffffu, (unsigned int)mDst, slot);
         const unsigned int dhi = __shfl_sync(0xffffffffu, (unsigned int)(mDst >> 32), slot);
         const unsigned int slen = __shfl_sync(0xffffffffu, mLen, slot);
         const unsigned int soff = __shfl_sync(0xffffffffu, mOff, slot);
         if (lane == 0) {
-#ifdef NCCLX_EXPERIMENTS
-            if (expMode != 1)
-#endif
             bulk_s2g(reinterpret_cast<void*>(((unsigned long long)dhi << 32) | dlo), ring0 + soff, slen);
             bulk_commit();
         }
         ++iStore;
-        { EXP_T0();
         while (iStore - freed > maxPending) {                     // at most maxPending stores keep ring bytes
             if (lane == 0) bulk_release_oldest(iStore - freed);
             ++freed;
         }
-        __syncwarp(); EXP_ACC(2); }
+        __syncwarp();
     }
-    { EXP_T0(); if (lane == 0) bulk_wait_all<0>(); EXP_ACC(3); }
-#ifdef NCCLX_EXPERIMENTS
-    if (lane == 0) {
-        expc[4] = clock64() - tStart;
-        for (int i = 0; i < 8; ++i) g_exp_cycles[(blockIdx.x & 255) * 8 + i] = expc[i];
-    }
-#endif
+    if (lane == 0) bulk_wait_all<0>();
 }
 
 // ================= vector engine: one warp per tile ===========================================

@@ -897,9 +897,5 @@ int ncclx_profile_reset(void) {
 
 int64_t ncclx_launch_count(void) { return g.launches.load(); }
 
-#ifdef NCCLX_EXPERIMENTS
-int ncclx_exp_set_mode(int mode) { return cudaMemcpyToSymbol(g_exp_mode, &mode, sizeof(int)) == cudaSuccess ? 0 : 4; }
-int ncclx_exp_read_cycles(long long* host) { return cudaMemcpyFromSymbol(host, g_exp_cycles, sizeof(long long) * 256 * 8) == cudaSuccess ? 0 : 4; }
-#endif
 
 }  // extern "C"
