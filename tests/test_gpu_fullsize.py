@@ -119,3 +119,41 @@ def test_cfg2_full_size_all_outputs_identical_on_device():
     exp = oracle.allreduce_sum([host_bits(x) for x in xs], "bf16", nthreads=8)
     for r in range(cfg.R):
         assert host_bits(out[r]).tobytes() == exp[r].tobytes()
+
+
+@pytest.mark.parametrize("fused", [32, 0])
+def test_single_segment_larger_than_4GiB(fused):
+    """Maximum-size edge case: one (s, d) segment of 4.5 GiB + 17 bytes (u8 counts), i.e. byte offsets beyond
+    2^32 inside a segment, on the single-launch path and on the two-kernel path.  Pure data movement, so the
+    expected bytes are the source bytes: compared in full on the device, and against the CPU oracle on the small
+    neighbouring segments and on sampled windows of the big one (incl. the tiles around every 2^32 boundary)."""
+    import oracle
+    nx.ncclx_set_param(nx.PARAM_FUSED_MAX_RANKS, fused)
+    try:
+        big = (9 << 29) + 17
+        C = np.array([[1000, big], [33, 4097]], np.int64)
+        g = torch.Generator(device="cuda").manual_seed(123)
+        send0 = torch.randint(0, 256, (int(C[0].sum()),), dtype=torch.uint8, device="cuda", generator=g)
+        send1 = torch.randint(0, 256, (int(C[1].sum()),), dtype=torch.uint8, device="cuda", generator=g)
+        recv0 = torch.full((int(C[:, 0].sum()) + 64,), 0xA5, dtype=torch.uint8, device="cuda")
+        recv1 = torch.full((int(C[:, 1].sum()) + 64,), 0xA5, dtype=torch.uint8, device="cuda")
+        Cd = torch.from_numpy(C).cuda()
+        RCd = torch.zeros_like(Cd)
+        nx.ncclx_alltoallv_dev(nx.device_ptr_table([send0, send1]), Cd, nx.device_ptr_table([recv0, recv1]), RCd, 2, "u8")
+        torch.cuda.synchronize()
+        assert (RCd.cpu().numpy() == C.T).all()
+        # definition: recv[1] = send[0][1000 : 1000+big] ++ send[1][33 : 33+4097]; recv[0] = send[0][:1000] ++ send[1][:33]
+        assert torch.equal(recv1[:big], send0[1000:1000 + big])
+        assert torch.equal(recv1[big:big + 4097], send1[33:]) and bool((recv1[big + 4097:] == 0xA5).all())
+        assert torch.equal(recv0[:1000], send0[:1000]) and torch.equal(recv0[1000:1033], send1[:33])
+        assert bool((recv0[1033:] == 0xA5).all())
+        # oracle on a reduced problem carved out around each 2^32 boundary of the big segment (same bytes, same layout)
+        for centre in (1 << 32, big - 40000):
+            lo = centre - 70000
+            n = 140000 if centre == (1 << 32) else big - lo
+            sub_send = [send0[1000 + lo:1000 + lo + n].cpu().numpy(), np.zeros(0, np.uint8)]
+            exp = [np.zeros(0, np.uint8), np.full(n, 0xA5, np.uint8)]
+            oracle.alltoallv(sub_send, np.array([[0, n], [0, 0]], np.int64), exp, "u8")
+            assert recv1[lo:lo + n].cpu().numpy().tobytes() == exp[1].tobytes()
+    finally:
+        nx.ncclx_set_param(nx.PARAM_FUSED_MAX_RANKS, 32)
