@@ -23,7 +23,7 @@ static_assert(sizeof(SegDesc) == 32, "SegDesc must be 32 bytes");
 enum { LIST_BULK = 0, LIST_VEC = 1 };
 
 // Device-resident control block.  The claim counters are zero between kernels: the copy kernel's last
-// CTA resets them on its way out (workctl_checkout), and the counts kernel zeroes them as well.
+// CTA resets them on its way out (workctl_checkout); ncclx_init zeroes them once.
 struct WorkCtl {
     unsigned int next[2];     // dynamic tile-claim counters, one per work list
     unsigned int status;      // sticky: bit 0 = negative count seen

@@ -7,13 +7,14 @@
 //   * persistent grid, one CTA per SM (x ctasPerSM), work discovered on the device from the
 //     descriptor table the counts kernel wrote -- the host knows neither sizes nor tile counts,
 //     so the launch is graph-capturable with a fixed grid (L387, L401);
-//   * work unit = a tile of at most 2^tileShift bytes of ONE segment; tiles are claimed
-//     dynamically in guided chunks from a global counter => balance by BYTES (and by time), not
-//     by segment or by rank (config 3 skew is 250x across segments, 150x across ranks);
-//   * LONG / aligned segments ("bulk" list): warp 0 drives a ring of shared-memory stages with
-//     descriptor-less 1-D TMA: cp.async.bulk global->shared (mbarrier complete_tx) and
-//     cp.async.bulk shared->global (bulk async-groups).  One elected lane issues everything;
-//     S-1 tile loads (tens of KB) stay in flight per SM with no register staging;
+//   * work unit = a tile of at most 2^tileShift bytes of ONE segment; after one static first chunk per
+//     engine, tiles are claimed dynamically, in order, in guided chunks from a global counter that
+//     resets itself => balance by BYTES (and by time), not by segment or by rank (config 3 skew is
+//     250x across segments, 150x across ranks);
+//   * LONG / aligned segments ("bulk" list): warp 0 (optionally warps 0..E-1) drives a byte-granular
+//     ring in shared memory with descriptor-less 1-D TMA: cp.async.bulk global->shared (mbarrier
+//     complete_tx) and cp.async.bulk shared->global (bulk async-groups).  One elected lane issues
+//     everything; ~180 KB of loads stay in flight per SM with no register staging;
 //   * SHORT or unaligned segments ("vector" list): warps 1..N-1 copy with 16-byte vectorised,
 //     fully coalesced ld/st (falling back to 8/4/2/1-byte units when source and destination
 //     misalignment differ), head/tail bytes handled per tile.
