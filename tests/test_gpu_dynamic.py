@@ -75,7 +75,8 @@ def test_fig17_worked_example(golden_dir):
 
 
 @pytest.mark.parametrize("R,n,J,scale,seed", [(2, 4, 2, 9, 0), (4, 8, 3, 5000, 1), (8, 16, 3, 40000, 2), (16, 64, 4, 3000, 3),
-                                              (64, 128, 3, 2000, 4), (100, 40, 3, 300, 5), (40, 300, 9, 200, 6)])
+                                              (64, 128, 3, 2000, 4), (100, 40, 3, 300, 5), (40, 300, 9, 200, 6),
+                                              (64, 480, 2, 100, 7)])
 def test_random_lists_with_duplicates(R, n, J, scale, seed):
     rng = np.random.default_rng(seed)
     Ls = (rng.integers(0, scale, (R, n)) * rng.integers(0, 2, (R, n))).astype(np.int64)
