@@ -110,6 +110,36 @@ def test_cfg4_full_size_reducescatter():
     assert float((flat.float() != 0).float().mean()) > 0.99
 
 
+@pytest.mark.parametrize("dtype", ["f32", "f16"])
+def test_cfg4_shape_other_dtypes_large(dtype):
+    """Config 4's shape (R = 16 ReduceScatter, gradient-like N(0, 1e-3) values) in the other two reduction dtypes
+    at a size far beyond L2 (4 GiB of input): two whole output blocks and 200 000 sampled elements + the block
+    boundaries against the oracle."""
+    R = 16
+    es = 4 if dtype == "f32" else 2
+    N = (4 << 30) // (R * es)                       # elements per rank: 4 GiB of input in total
+    n = N // R
+    td = torch.float32 if dtype == "f32" else torch.float16
+    xs = [W.torch_values(N, dtype, 7000 + k, 1e-3) for k in range(R)]
+    out = [torch.empty(n, dtype=td, device="cuda") for _ in range(R)]
+    nx.ncclx_reducescatter_sum(nx.device_ptr_table(xs), nx.device_ptr_table(out), n, R, dtype)
+    torch.cuda.synchronize()
+    npdt = np.float32 if dtype == "f32" else np.uint16
+
+    def bits(t):
+        return t.view(torch.int32 if dtype == "f32" else torch.int16).cpu().numpy().view(npdt)
+    for r in (R - 1, 3):
+        exp = oracle.allreduce_sum([bits(x[r * n:(r + 1) * n]) for x in xs], dtype, nthreads=8)[0]
+        assert bits(out[r]).tobytes() == exp.tobytes(), f"block {r}"
+    rng = np.random.default_rng(2)
+    idx = np.concatenate([rng.integers(0, N, 200_000)] +
+                         [np.arange(max(0, b * n - 1024), min(N, b * n + 1024)) for b in range(R + 1)])
+    it = torch.from_numpy(idx).cuda()
+    vals = np.stack([bits(x[it]) for x in xs])
+    exp = oracle.reduce_samples(vals, dtype)
+    assert bits(torch.cat(out)[it]).tobytes() == exp.tobytes()
+
+
 def test_cfg2_full_size_all_outputs_identical_on_device():
     cfg = W.reduce_config(2)
     xs = [W.torch_values(cfg.count, "bf16", 1000 + k) for k in range(cfg.R)]
