@@ -416,6 +416,7 @@ def main():
         per["next2_reducecopy_cta_sweep"] = reducecopy_extra(torch, nx, peak)
         per["next3_topk_R64_T4096_k4"] = topk_extra(torch, nx, peak)
         per["next4_latency"] = latency_extra(torch, nx, peak, min(args.latency_replays, 2000))
+        per["cfg4_shape_other_dtypes"] = reduce_dtype_extra(torch, nx, peak)
         per["hbm_ceiling_probe"] = ceiling_extra(torch, nx, peak)
         roofline["practical_ceiling_GBps"] = {k: per["hbm_ceiling_probe"][k]["GBps"] for k in ("read_only", "write_only", "copy")}
         line["per_config"] = per
@@ -518,6 +519,18 @@ def ceiling_extra(torch, nx, peak, nbytes=4 << 30):
                               (3, "write_only_tma", nbytes)):
         t = event_times_ms(torch, lambda: nx.ncclx_stream_probe(mode, src, dst, nbytes), 10)
         res[name] = {"ms_median": round(float(np.median(t)), 4), **frac(moved / (np.median(t) * 1e-3) / 1e9, peak)}
+    return res
+
+
+def reduce_dtype_extra(torch, nx, peak):
+    """Config 4's shape (R = 16 ReduceScatter, N(0, 1e-3)) in the other reduction dtypes, 4 GiB of input."""
+    res = {}
+    for dtype, es in (("f32", 4), ("f16", 2)):
+        cfg = W.ReduceConfig(f"cfg4_shape_{dtype}", "reducescatter", 16, (4 << 30) // (16 * es), dtype, 3, 1e-3)
+        r = Reduce(cfg, torch, nx)
+        t = event_times_ms(torch, r.run, 10)
+        res[dtype] = {"ms_median": round(float(np.median(t)), 4), "bytes": r.bytes, **frac(r.bytes / (np.median(t) * 1e-3) / 1e9, peak)}
+        del r
     return res
 
 
