@@ -583,6 +583,16 @@ def latency_extra(torch, nx, peak, reps):
         nx.ncclx_alltoallv_execute_dev(0)
         main.wait_stream(side)
         nx.ncclx_alltoallv_execute_dev(1)
+    # the paper's inference regime (L90, L471: a few MB per operation, < 128 KB per peer): one row per pair
+    for name, rows, width in (("R64_one_10KB_row_per_pair", np.ones((64, 64), np.int64), 5120),
+                              ("R128_one_14KB_row_for_28pct_of_pairs", (a5.cfg.rows > 4).astype(np.int64), 7168)):
+        w = A2A(W.A2AConfig(name, rows.shape[0], width, "bf16", 1, rows), torch, nx, with_back=False)
+        r = {"bytes_each_way": w.bytes_one_way, "engines_chosen_on_device": graph_p50(torch, w.dispatch, reps)}
+        nx.ncclx_set_param(nx.PARAM_COPY_BULK_ENGINES, 1)
+        r["one_engine"] = graph_p50(torch, w.dispatch, reps)
+        nx.ncclx_set_param(nx.PARAM_COPY_BULK_ENGINES, 0)
+        res["small_" + name] = r
+        del w
     res["cfg5_pair_stream_order"] = graph_p50(torch, pair_plain, reps)
     res["cfg5_pair_double_buffered"] = graph_p50(torch, pair_double_buffered, reps)
     ok = all(bool((a5.back[s][:n] == a5.send[s][:n]).all()) for s, n in enumerate(a5.send_elems) if n)

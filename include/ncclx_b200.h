@@ -262,7 +262,8 @@ typedef enum {
     NCCLX_PARAM_FUSED_MAX_RANKS = 12, /* ncclx_alltoallv_dev runs as ONE kernel for R <= this (0..32; 0 = never), default 32 */
     NCCLX_PARAM_FUSED_MIN_TILE_SHIFT = 13, /* smallest bulk tile the single-launch path may choose (log2 bytes, 10..16), default 12 */
     NCCLX_PARAM_COPY_PENDING_STORES = 14, /* bulk engine: stores left unreclaimed in the ring after each store (1..8), default 1 */
-    NCCLX_PARAM_COPY_BULK_ENGINES = 15,   /* bulk (TMA) engine warps per copy CTA, each with 1/E of the ring: 1 (default), 2 or 4 */
+    NCCLX_PARAM_COPY_BULK_ENGINES = 15,   /* bulk (TMA) engine warps per copy CTA, each with 1/E of the ring: 1, 2, 4, or 0 (default): chosen on */
+                                          /* the device -- 4 for calls of few tiles per SM (latency-bound), 1 for long ones (HBM-bound)         */
     NCCLX_PARAM_HOST_ZERO_COPY = 16,      /* 1 (default): the *_host calls let the kernels access PINNED host buffers directly */
     NCCLX_PARAM_COUNT_
 } ncclx_param_t;

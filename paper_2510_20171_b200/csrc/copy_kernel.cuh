@@ -41,7 +41,8 @@ struct CopyArgs {
     int kmax[2];                           // max tiles per dynamic claim, per list (short-segment regime)
     int kmaxLong;                          // same, when segments average >= 8 tiles
     int maxPendingStores;                  // 1..8: stores whose shared-memory read may be outstanding before the engine waits
-    int bulkEngines;                       // E = 1, 2 or 4 bulk engine warps per CTA (ring split E ways); warps E..15 are vector engines
+    int bulkEngines;                       // E = 1, 2 or 4 bulk engine warps per CTA (ring split E ways); warps E..15 are vector
+                                           // engines; 0 = chosen on the device from the tile count (choose_bulk_engines)
     ClassParams cls;
 };
 
@@ -515,6 +516,17 @@ __device__ __forceinline__ void workctl_checkout(WorkCtl* ctl, bool used) {
     }
 }
 
+// Number of bulk engine warps when the host leaves the choice to the device (grid-uniform: depends only on the
+// work list's totals).  A short call (few tiles per SM) is bound by the per-tile latency of one elected lane --
+// measured: R = 64 with one 10 KB row per pair takes 40 us with one engine and 27 us with four -- while a long
+// one is HBM-bound and slightly better off with one deep ring (config 3: -0.7 % with two engines).
+__device__ __forceinline__ int choose_bulk_engines(int requested, int totalTiles, int grid, unsigned int ringBytes, int tileShift) {
+    int E = requested;
+    if (E == 0) E = totalTiles <= 48 * grid ? 4 : (totalTiles <= 96 * grid ? 2 : 1);
+    while (E > 1 && (1u << tileShift) > ((ringBytes / (unsigned int)E) & ~127u)) E >>= 1;    // a tile must fit in one share
+    return E;
+}
+
 // First chunk of every engine is static (chunk e to engine e; see Cursor::init); a positive staticEighths
 // instead assigns that share of ALL tiles as contiguous static ranges (kept for A/B runs).
 __device__ __forceinline__ int static_first_chunk(int total, int nEngines, int kmax, int kmaxLong, int RR, int eighths) {
@@ -534,7 +546,6 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
     int* colBase[2];
     colBase[0] = reinterpret_cast<int*>(mbar + COPY_MAX_ENGINES * COPY_SLOTS);
     colBase[1] = colBase[0] + (R + 1);
-    const int E = a.bulkEngines;
     const int nbR = R * coarse_blocks(a.colLen);
     int* coarse[2] = {nullptr, nullptr};
     if (a.useCoarse) { coarse[0] = colBase[1] + (R + 1); coarse[1] = coarse[0] + nbR; }
@@ -542,7 +553,7 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
     // ---- prologue: mbarrier init (overlaps the counts kernel under PDL), then cross-column tile
     //      bases = scan of the R per-column totals the counts kernel wrote, and the coarse indexes ----
     griddep_launch_dependents();           // the next call's metadata kernel may become resident (it waits for us)
-    if (threadIdx.x >= 64 && threadIdx.x < 64 + E * COPY_SLOTS) {
+    if (threadIdx.x >= 64 && threadIdx.x < 64 + COPY_MAX_ENGINES * COPY_SLOTS) {
         mbar_init(smem_u32(&mbar[threadIdx.x - 64]), 1);
         fence_mbar_init();
     }
@@ -565,6 +576,7 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
     }
     __syncthreads();
 
+    const int E = choose_bulk_engines(a.bulkEngines, colBase[LIST_BULK][R], (int)gridDim.x, a.ringBytes, a.cls.tileShift[LIST_BULK]);
     const int NV = COPY_THREADS / 32 - E;              // vector engines per CTA
     const int nB = (int)gridDim.x * E, nV = (int)gridDim.x * NV;
     const unsigned int subRing = (a.ringBytes / (unsigned int)E) & ~127u;

@@ -73,8 +73,7 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
     const bool writer = blockIdx.x == 0;
 
     griddep_launch_dependents();           // a following call of this library may start its prologue
-    const int E = a.bulkEngines;
-    if (threadIdx.x >= 64 && threadIdx.x < 64 + E * COPY_SLOTS) {
+    if (threadIdx.x >= 64 && threadIdx.x < 64 + COPY_MAX_ENGINES * COPY_SLOTS) {
         mbar_init(smem_u32(&mbar[threadIdx.x - 64]), 1);
         fence_mbar_init();
     }
@@ -108,6 +107,13 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
     long long totalElems = 0;
     for (int s = 0; s < R; ++s) totalElems += rowTot[s];
     const long long totalBytes = totalElems * a.elemSize;
+    // engines from the byte total (same regimes as choose_bulk_engines: up to 48 / 96 maximum-size tiles per CTA)
+    int E = a.bulkEngines;
+    if (E == 0) {
+        const long long maxTiles = totalBytes >> a.cls.tileShift[LIST_BULK];
+        E = maxTiles <= 48ll * gridDim.x ? 4 : (maxTiles <= 96ll * gridDim.x ? 2 : 1);
+    }
+    while (E > 1 && (1u << a.cls.tileShift[LIST_BULK]) > ((a.ringBytes / (unsigned int)E) & ~127u)) E >>= 1;
     const int NV = NW - E;
     const int nB = (int)gridDim.x * E, nV = (int)gridDim.x * NV;
     const unsigned int subRing = (a.ringBytes / (unsigned int)E) & ~127u;

@@ -38,7 +38,7 @@ struct Context {
     WorkCtl* fusedCtl = nullptr;          // claim counters of the single-launch path (self-resetting)
     void* wsBase = nullptr;
     // tunables
-    int64_t params[NCCLX_PARAM_COUNT_] = {1, 1024, 8, 16, 0, 0, 15, 14, 1, 0, 6, 2, 32, 12, 1, 1, 1};
+    int64_t params[NCCLX_PARAM_COUNT_] = {1, 1024, 8, 16, 0, 0, 15, 14, 1, 0, 6, 2, 32, 12, 1, 0, 1};
     // profiling
     std::vector<EventPair> events[NCCLX_KERNEL_COUNT_];
     std::atomic<int64_t> launches{0};
@@ -152,7 +152,8 @@ ClassParams classParams() {
     const int cps = (int)g.params[NCCLX_PARAM_COPY_CTAS_PER_SM];
     const size_t worstAux = COPY_MBAR_BYTES + 2 * (size_t)(g.maxRanks + 1) * 4 + kMaxCoarseBytes + 16 + 128;
     const size_t budget = copyBudget(cps);
-    const size_t ring = (budget > worstAux ? budget - worstAux : 0) / (size_t)g.params[NCCLX_PARAM_COPY_BULK_ENGINES];   // per engine
+    const size_t engines = g.params[NCCLX_PARAM_COPY_BULK_ENGINES] > 0 ? (size_t)g.params[NCCLX_PARAM_COPY_BULK_ENGINES] : 1;
+    const size_t ring = (budget > worstAux ? budget - worstAux : 0) / engines;   // per engine (0 = device's choice: falls back to fewer engines if a tile would not fit)
     c.tileShift[0] = (int)g.params[NCCLX_PARAM_BULK_TILE_SHIFT];
     while (c.tileShift[0] > 10 && ((size_t)5 << c.tileShift[0]) / 2 > ring) --c.tileShift[0];   // >= 2.5 tiles fit per engine
     c.tileShift[1] = (int)g.params[NCCLX_PARAM_VEC_TILE_SHIFT];
@@ -177,10 +178,11 @@ int launchCopy(const Workspace& ws, const SegDesc* desc, const int* const coarse
     cp.useCoarse = coarseBytes(ncols, colLen) > 0 ? 1 : 0;
     cp.ctl = ws.ctl; cp.ncols = ncols; cp.colLen = colLen;
     cp.cls = cls;
+    cp.bulkEngines = (int)g.params[NCCLX_PARAM_COPY_BULK_ENGINES];
     cp.ringBytes = chooseRingBytes(cps, ncols, colLen);
     // the work list's bulk tile (fixed when it was built) must fit ~2.5 times into one engine's share of the
     // ring; a larger tile could never be staged (parameters changed between prepare and execute)
-    if (((size_t)5 << cls.tileShift[0]) / 2 > cp.ringBytes / (size_t)g.params[NCCLX_PARAM_COPY_BULK_ENGINES]) return NCCLX_ERR_ARG;
+    if (((size_t)5 << cls.tileShift[0]) / 2 > cp.ringBytes / (size_t)(cp.bulkEngines > 0 ? cp.bulkEngines : 1)) return NCCLX_ERR_ARG;
     cp.staticEighths = (int)g.params[NCCLX_PARAM_COPY_STATIC_EIGHTHS];
     cp.kmax[0] = (int)g.params[NCCLX_PARAM_COPY_KMAX];
     cp.kmax[1] = 8;
@@ -217,7 +219,7 @@ int launchFused(const void* const* send, const int64_t* C, void* const* recv, in
     const size_t aux = fused_aux_bytes(R);
     fa.ringBytes = (unsigned int)((budget - aux) & ~(size_t)127);
     fa.bulkEngines = (int)g.params[NCCLX_PARAM_COPY_BULK_ENGINES];
-    while (fa.cls.tileShift[0] > 10 && ((size_t)5 << fa.cls.tileShift[0]) / 2 > fa.ringBytes / fa.bulkEngines) --fa.cls.tileShift[0];
+    while (fa.cls.tileShift[0] > 10 && ((size_t)5 << fa.cls.tileShift[0]) / 2 > fa.ringBytes / (fa.bulkEngines > 0 ? fa.bulkEngines : 1)) --fa.cls.tileShift[0];
     fa.send = send; fa.recv = recv;
     fa.C = reinterpret_cast<const long long*>(C);
     fa.RC = reinterpret_cast<long long*>(RC);
@@ -858,7 +860,7 @@ int ncclx_set_param(int param, int64_t value) {
     case NCCLX_PARAM_FUSED_MAX_RANKS: if (value < 0 || value > FUSED_MAX_R) return NCCLX_ERR_ARG; break;
     case NCCLX_PARAM_FUSED_MIN_TILE_SHIFT: if (value < 10 || value > 16) return NCCLX_ERR_ARG; break;
     case NCCLX_PARAM_COPY_PENDING_STORES: if (value < 1 || value > 8) return NCCLX_ERR_ARG; break;
-    case NCCLX_PARAM_COPY_BULK_ENGINES: if (value != 1 && value != 2 && value != 4) return NCCLX_ERR_ARG; break;
+    case NCCLX_PARAM_COPY_BULK_ENGINES: if (value != 0 && value != 1 && value != 2 && value != 4) return NCCLX_ERR_ARG; break;
     default: if (value < 0) return NCCLX_ERR_ARG; break;
     }
     g.params[param] = value;

@@ -32,7 +32,7 @@ def default_params():
     nx.ncclx_set_param(nx.PARAM_BULK_TILE_SHIFT, 15)
     nx.ncclx_set_param(nx.PARAM_VEC_TILE_SHIFT, 14)
     nx.ncclx_set_param(nx.PARAM_SCAN_CTAS, 16)
-    nx.ncclx_set_param(nx.PARAM_COPY_BULK_ENGINES, 1)
+    nx.ncclx_set_param(nx.PARAM_COPY_BULK_ENGINES, 0)
     nx.ncclx_set_param(nx.PARAM_COPY_PENDING_STORES, 1)
     nx.ncclx_set_param(nx.PARAM_COPY_KMAX, 6)
     nx.ncclx_set_param(nx.PARAM_COPY_STATIC_EIGHTHS, 0)
@@ -127,7 +127,7 @@ def test_ragged_bulk_tail_and_tiny_segments():
 @pytest.mark.parametrize("param,value", [("FORCE_VECTOR", 1), ("COPY_CTAS_PER_SM", 2), ("COPY_CTAS_PER_SM", 4),
                                          ("BULK_TILE_SHIFT", 12), ("BULK_TILE_SHIFT", 16), ("VEC_TILE_SHIFT", 10),
                                          ("BULK_MIN_BYTES", 16), ("BULK_MIN_BYTES", 1 << 20), ("SCAN_CTAS", 1),
-                                         ("SCAN_CTAS", 64), ("COPY_BULK_ENGINES", 2), ("COPY_BULK_ENGINES", 4),
+                                         ("SCAN_CTAS", 64), ("COPY_BULK_ENGINES", 1), ("COPY_BULK_ENGINES", 2), ("COPY_BULK_ENGINES", 4),
                                          ("COPY_PENDING_STORES", 4), ("COPY_PENDING_STORES", 8), ("COPY_KMAX", 1),
                                          ("COPY_KMAX", 17), ("COPY_STATIC_EIGHTHS", 4), ("COPY_STATIC_EIGHTHS", 8),
                                          ("PDL", 0)])
