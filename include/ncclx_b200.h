@@ -249,7 +249,7 @@ typedef enum {
                                       /* smaller or unaligned ones take the vector path. default 1024  */
     NCCLX_PARAM_REDUCE_CTAS_PER_SM = 2, /* reduce grid = this * SM count, default 8 (more CTAs than   */
                                       /* fit at once: the hardware scheduler evens out short calls)   */
-    NCCLX_PARAM_SCAN_CTAS = 3,        /* upper bound on CTAs of the counts kernel, default 16          */
+    NCCLX_PARAM_SCAN_CTAS = 3,        /* upper bound on CTAs of the counts kernel, default 32          */
     NCCLX_PARAM_PROFILE = 4,          /* 1: bracket each kernel with CUDA events (never while capturing) */
     NCCLX_PARAM_FORCE_VECTOR = 5,     /* 1: send every segment down the vector path (for A/B runs)     */
     NCCLX_PARAM_BULK_TILE_SHIFT = 6,  /* log2 bytes of a bulk tile = one smem ring stage (12..16), default 15 */

@@ -38,7 +38,7 @@ struct Context {
     WorkCtl* fusedCtl = nullptr;          // claim counters of the single-launch path (self-resetting)
     void* wsBase = nullptr;
     // tunables
-    int64_t params[NCCLX_PARAM_COUNT_] = {1, 1024, 8, 16, 0, 0, 15, 14, 1, 0, 6, 2, 32, 12, 1, 0, 1};
+    int64_t params[NCCLX_PARAM_COUNT_] = {1, 1024, 8, 32, 0, 0, 15, 14, 1, 0, 6, 2, 32, 12, 1, 0, 1};
     // profiling
     std::vector<EventPair> events[NCCLX_KERNEL_COUNT_];
     std::atomic<int64_t> launches{0};

@@ -31,7 +31,7 @@ def default_params():
     nx.ncclx_set_param(nx.PARAM_FORCE_VECTOR, 0)
     nx.ncclx_set_param(nx.PARAM_BULK_TILE_SHIFT, 15)
     nx.ncclx_set_param(nx.PARAM_VEC_TILE_SHIFT, 14)
-    nx.ncclx_set_param(nx.PARAM_SCAN_CTAS, 16)
+    nx.ncclx_set_param(nx.PARAM_SCAN_CTAS, 32)
     nx.ncclx_set_param(nx.PARAM_COPY_BULK_ENGINES, 0)
     nx.ncclx_set_param(nx.PARAM_COPY_PENDING_STORES, 1)
     nx.ncclx_set_param(nx.PARAM_COPY_KMAX, 6)
