@@ -520,9 +520,11 @@ __device__ __forceinline__ void workctl_checkout(WorkCtl* ctl, bool used) {
 // work list's totals).  A short call (few tiles per SM) is bound by the per-tile latency of one elected lane --
 // measured: R = 64 with one 10 KB row per pair takes 40 us with one engine and 27 us with four -- while a long
 // one is HBM-bound and slightly better off with one deep ring (config 3: -0.7 % with two engines).
-__device__ __forceinline__ int choose_bulk_engines(int requested, int totalTiles, int grid, unsigned int ringBytes, int tileShift) {
+// When most of the work is on the vector list (unaligned traffic) the warps stay vector engines.
+__device__ __forceinline__ int choose_bulk_engines(int requested, int totalTiles, int vecTiles, int grid, unsigned int ringBytes,
+                                                   int tileShift) {
     int E = requested;
-    if (E == 0) E = totalTiles <= 48 * grid ? 4 : (totalTiles <= 96 * grid ? 2 : 1);
+    if (E == 0) E = vecTiles > totalTiles ? 1 : (totalTiles <= 48 * grid ? 4 : (totalTiles <= 96 * grid ? 2 : 1));
     while (E > 1 && (1u << tileShift) > ((ringBytes / (unsigned int)E) & ~127u)) E >>= 1;    // a tile must fit in one share
     return E;
 }
@@ -576,7 +578,8 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
     }
     __syncthreads();
 
-    const int E = choose_bulk_engines(a.bulkEngines, colBase[LIST_BULK][R], (int)gridDim.x, a.ringBytes, a.cls.tileShift[LIST_BULK]);
+    const int E = choose_bulk_engines(a.bulkEngines, colBase[LIST_BULK][R], colBase[LIST_VEC][R], (int)gridDim.x, a.ringBytes,
+                                      a.cls.tileShift[LIST_BULK]);
     const int NV = COPY_THREADS / 32 - E;              // vector engines per CTA
     const int nB = (int)gridDim.x * E, nV = (int)gridDim.x * NV;
     const unsigned int subRing = (a.ringBytes / (unsigned int)E) & ~127u;

@@ -114,9 +114,8 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
         E = maxTiles <= 48ll * gridDim.x ? 4 : (maxTiles <= 96ll * gridDim.x ? 2 : 1);
     }
     while (E > 1 && (1u << a.cls.tileShift[LIST_BULK]) > ((a.ringBytes / (unsigned int)E) & ~127u)) E >>= 1;
-    const int NV = NW - E;
-    const int nB = (int)gridDim.x * E, nV = (int)gridDim.x * NV;
-    const unsigned int subRing = (a.ringBytes / (unsigned int)E) & ~127u;
+    int NV = NW - E;
+    int nB = (int)gridDim.x * E, nV = (int)gridDim.x * NV;
     ClassParams cls = a.cls;
     cls.tileShift[LIST_BULK] = max(a.minTileShift[LIST_BULK], min(a.cls.tileShift[LIST_BULK], floor_log2_ll(totalBytes / (2 * nB))));
     cls.tileShift[LIST_VEC] = max(a.minTileShift[LIST_VEC], min(a.cls.tileShift[LIST_VEC], floor_log2_ll(totalBytes / (2 * nV))));
@@ -160,6 +159,10 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
     fence_proxy_async_smem();              // scratch reads/writes (generic proxy) before TMA writes to the same bytes
     __syncthreads();                       // the scratch is dead from here on; the ring may be filled
 
+    if (a.bulkEngines == 0 && colBase[LIST_VEC][R] > colBase[LIST_BULK][R]) {     // mostly unaligned traffic: keep the
+        E = 1; NV = NW - 1; nB = (int)gridDim.x; nV = (int)gridDim.x * NV;          // warps as vector engines
+    }
+    const unsigned int subRing = (a.ringBytes / (unsigned int)E) & ~127u;
     // ---- a4: the copy engines of the big path, fed from shared memory --------------------------------
     if (warp < E) {
         Cursor<LIST_BULK, true> cur;
