@@ -275,3 +275,24 @@ def test_host_buffer_form(mode):
             assert got.tobytes() == exp[d].tobytes()          # incl. the untouched 0xA5 tail
     finally:
         nx.ncclx_set_param(nx.PARAM_HOST_ZERO_COPY, 1)
+
+
+@pytest.mark.parametrize("fused", [32, 0])
+def test_every_source_destination_misalignment_pair(fused):
+    """All 16 x 16 combinations of source / destination base misalignment modulo 16 with odd byte counts: co-aligned
+    pairs take the 16-byte vector path, the others the funnel-shift path (aligned vectors on both sides), each
+    with its own head and tail bytes; small enough for the whole receive capacity to be compared every time."""
+    nx.ncclx_set_param(nx.PARAM_FUSED_MAX_RANKS, fused)
+    try:
+        rng = np.random.default_rng(77)
+        C = np.array([[4099, 63, 1], [777, 20001, 64], [65, 0, 129]], np.int64)
+        send = make_send(C, "u8", 12)
+        exp, eRC, *_ = oracle_a2a(send, C, "u8")
+        for ms in range(16):
+            for md in range(16):
+                got, RC, _, _ = run_a2a(send, C, "u8", mis_send=ms, mis_recv=md)
+                assert (RC == eRC).all()
+                for d in range(3):
+                    assert got[d].tobytes() == exp[d].tobytes(), f"mis_send={ms} mis_recv={md} recv[{d}]"
+    finally:
+        nx.ncclx_set_param(nx.PARAM_FUSED_MAX_RANKS, 32)
