@@ -200,7 +200,9 @@ def oracle_sample_state(div=4):
     return {"a2a": a, "ar": ar, "rs": rs}, nbytes, sample
 
 
-def run_oracle_leg(steps, warmup, div=4):
+def run_oracle_leg(steps, warmup, div=4, single_thread=True):
+    """The oracle as it stands on the box's host cores: (a) single-threaded, (b) on all cores
+    (OpenMP over destination ranks / element ranges), on the same bounded sample."""
     cores = os.cpu_count() or 1
     state, nbytes, sample = oracle_sample_state(div)
     for _ in range(max(0, warmup)):
@@ -209,8 +211,15 @@ def run_oracle_leg(steps, warmup, div=4):
     for _ in range(steps):
         oracle_sample_step(state, cores)
     dt = (time.perf_counter() - t0) / steps
-    return {"value": round(nbytes / dt / 1e9, 3), "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": sample,
-            "s_per_sample_step": round(dt, 3)}, dt
+    out = {"value": round(nbytes / dt / 1e9, 3), "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": sample,
+           "s_per_sample_step": round(dt, 3), "all_cores": round(nbytes / dt / 1e9, 3), "single_thread": None}
+    if single_thread:
+        t0 = time.perf_counter()
+        oracle_sample_step(state, 1)
+        d1 = time.perf_counter() - t0
+        out["single_thread"] = round(nbytes / d1 / 1e9, 3)
+        out["s_per_sample_step_single_thread"] = round(d1, 3)
+    return out, dt
 
 
 # ------------------------------------------------------------------------------------ multi-rank host logic
@@ -255,9 +264,11 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the per-config table (cfg1/cfg5 latency, cfg2 warm/cold)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--latency-replays", type=int, default=10000)
-    ap.add_argument("--probe", type=int, default=0, choices=[0, 1, 2, 3, 4, 5, 6, 7, 8, 9],
+    ap.add_argument("--probe", type=int, default=0, choices=list(range(0, 15)),
                     help="run ONLY BASELINE.json config N (1-5) eagerly for --steps iterations, or one of the widenings "
-                         "(6 = NEXT-4 latency, 7 = NEXT-1 dynamic, 8 = NEXT-3 top-k, 9 = HBM streaming ceilings): the commands ncu captures are taken from")
+                         "(6 = NEXT-4 latency, 7 = NEXT-1 dynamic, 8 = NEXT-3 top-k, 9 = HBM streaming ceilings, 10 = per-SM timeline of a "
+                         "config-5 copy [instrumented build], 11 = misaligned segments, 12 = NEXT-2 ReduceCopy variants + per-CTA ceiling, "
+                         "13 = top-k at PAPER.md Table 3's decode shapes, 14 = R > 256 small messages): the commands ncu captures are taken from")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -266,7 +277,7 @@ def main():
 
     config = {"workload": "cfg3 MoE dispatch+combine AllToAllv (R=64, 16384 tok x 5120 bf16, Zipf 1.1) + cfg2 AllReduce "
                           "(R=8, 4Mi bf16) + cfg4 ReduceScatter (R=16, 256Mi bf16/rank); BASELINE.json configs[2],[1],[3]",
-              "bytes_per_step_GiB": None, "l2": "inputs larger than L2 (48.6 GiB touched per step vs 126 MB)",
+              "bytes_per_step_GiB": 48.625, "l2": "inputs larger than L2 (48.6 GiB touched per step vs 126 MB)",
               "parallelism": f"replicas x{world} (path does not shard across GPUs)"}
 
     if args.impl == "reference":
@@ -299,7 +310,7 @@ def main():
     r2 = Reduce(W.reduce_config(2), torch, nx)
     r4 = Reduce(W.reduce_config(4), torch, nx)
     step_bytes = 2 * 2 * a3.bytes_one_way + r2.bytes + r4.bytes
-    config["bytes_per_step_GiB"] = round(step_bytes / GiB, 3)
+    assert config["bytes_per_step_GiB"] == round(step_bytes / GiB, 3)
 
     def step():
         a3.dispatch(); a3.combine(); r2.run(); r4.run()
@@ -354,13 +365,16 @@ def main():
                                                     "share_of_step": round(red_ms / ms_total, 4)},
                                   "counts_kernel": {"avg_ms": round(cnt_ms / max(cnt_n, 1), 5), "launches": cnt_n,
                                                     "share_of_step": round(cnt_ms / ms_total, 5)}}}
-    tr = os.path.join(ROOT, "profiles", "traffic.csv")        # dram bytes per launch from the committed ncu capture
+    # dram bytes per launch from the committed ncu capture: profiles/traffic.csv is (re)written from the capture's raw
+    # page by `python -m paper_2510_20171_b200.ncu_traffic` (ncu cannot run inside this timed process)
+    tr = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tr):
         try:
             import csv
             for row in csv.DictReader(open(tr)):
                 if row["kernel"] == "segment_copy_kernel" and row["workload"] == "cfg3_dispatch":
                     roofline["traffic"] = int(row["bytes_per_launch"])
+                    roofline["traffic_source"] = row["source"]
         except Exception:
             pass
 
@@ -408,18 +422,55 @@ def main():
                 a.dispatch()
             t = event_times_ms(torch, g.replay, reps, warm=20)
             p50 = float(np.percentile(t, 50))
+            # cross-check: the same number of replays back to back under ONE event pair, total / replays
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(reps):
+                g.replay()
+            e1.record()
+            torch.cuda.synchronize()
             per[f"cfg{idx}_graph_replay"] = {"replays": reps, "p50_us": round(p50 * 1e3, 2), "p99_us": round(float(np.percentile(t, 99)) * 1e3, 2),
-                                             "mean_us": round(float(t.mean()) * 1e3, 2), "bytes_each_way": a.bytes_one_way,
+                                             "mean_us": round(float(t.mean()) * 1e3, 2),
+                                             "total_over_replays_us": round(e0.elapsed_time(e1) / reps * 1e3, 2),
+                                             "bytes_each_way": a.bytes_one_way,
                                              **frac(2 * a.bytes_one_way / (p50 * 1e-3) / 1e9, peak)}
             del a, g
-        per["next1_alltoallv_dynamic_R64_tok256"] = dynamic_extra(torch, nx, peak, min(args.latency_replays, 2000))
+        lr = min(args.latency_replays, 2000)
+        per["next1_alltoallv_dynamic_R64_tok256"] = dynamic_extra(torch, nx, peak, lr)
         per["next2_reducecopy_cta_sweep"] = reducecopy_extra(torch, nx, peak)
         per["next3_topk_R64_T4096_k4"] = topk_extra(torch, nx, peak)
-        per["next4_latency"] = latency_extra(torch, nx, peak, min(args.latency_replays, 2000))
+        per["next3_topk_table3_shapes"] = topk_table3_extra(torch, nx, peak, min(lr, 500))
+        per["next4_latency"] = latency_extra(torch, nx, peak, lr)
+        per["large_R_small_messages"] = large_r_extra(torch, nx, peak, min(lr, 500))
+        per["misaligned_segments"] = misaligned_extra(torch, nx, peak)
         per["cfg4_shape_other_dtypes"] = reduce_dtype_extra(torch, nx, peak)
         per["hbm_ceiling_probe"] = ceiling_extra(torch, nx, peak)
         roofline["practical_ceiling_GBps"] = {k: per["hbm_ceiling_probe"][k]["GBps"] for k in ("read_only", "write_only", "copy")}
         line["per_config"] = per
+        # the five BASELINE.json configs in compact form, also inside `roofline` (a key the driver's record keeps whole):
+        # us p50/p99 for the latency configs, GB/s + both roofline fractions for the bandwidth configs
+        c1, c5 = per["cfg1_graph_replay"], per["cfg5_graph_replay"]
+        c2 = per["cfg2_allreduce_cold"]
+        summary = {
+            "cfg1_us_p50": c1["p50_us"], "cfg1_us_p99": c1["p99_us"],
+            "cfg2_us_per_call_p50": c2["us_per_call_p50"], "cfg2_us_per_call_p99": c2["us_per_call_p99"],
+            "cfg2_GBps": c2["GBps"], "cfg2_frac_nominal": c2["frac_of_nominal_8TBps"],
+            "cfg3_dispatch_GBps": per["cfg3_dispatch"]["GBps"], "cfg3_dispatch_frac_nominal": per["cfg3_dispatch"]["frac_of_nominal_8TBps"],
+            "cfg3_dispatch_frac_measured": per["cfg3_dispatch"]["frac_of_measured"],
+            "cfg3_combine_GBps": per["cfg3_combine"]["GBps"],
+            "cfg4_GBps": per["cfg4_reducescatter"]["GBps"], "cfg4_frac_nominal": per["cfg4_reducescatter"]["frac_of_nominal_8TBps"],
+            "cfg4_frac_measured": per["cfg4_reducescatter"]["frac_of_measured"],
+            "cfg5_us_p50": c5["p50_us"], "cfg5_us_p99": c5["p99_us"], "cfg5_us_total_over_replays": c5["total_over_replays_us"],
+            "cfg5_GBps": c5["GBps"], "cfg5_frac_nominal": c5["frac_of_nominal_8TBps"],
+            "next1_dynamic_us_p50": per["next1_alltoallv_dynamic_R64_tok256"]["p50_us"],
+            "next1_dynamic_frac_nominal": per["next1_alltoallv_dynamic_R64_tok256"]["frac_of_nominal_8TBps"],
+            "misaligned_odd_bf16_GBps": per["misaligned_segments"]["R16_bf16_odd_counts"]["GBps"],
+            "misaligned_odd_u8_GBps": per["misaligned_segments"]["R16_u8_odd_counts"]["GBps"],
+            "topk_dispatch_ms": per["next3_topk_R64_T4096_k4"]["dispatch"]["ms"],
+            "topk_combine_ms": per["next3_topk_R64_T4096_k4"]["combine"]["ms"],
+        }
+        roofline["configs"] = summary
 
     # ---- e2e: same step through the host-buffer C ABI (H2D + kernels + D2H inside the timed region) --------
     if not args.no_e2e:
@@ -431,6 +482,8 @@ def main():
         line["cpu_baseline"] = cb
 
     if rank == 0:
+        if "configs" in roofline:
+            line["configs_summary"] = roofline["configs"]       # last key: survives a truncated stdout tail
         print(json.dumps(line))
     nx.ncclx_finalize()
     if dist is not None:
@@ -440,33 +493,53 @@ def main():
 
 def dynamic_extra(torch, nx, peak, reps):
     """the paper's full AllToAllvDynamic interface on an inference-shaped MoE dispatch
-    (R=64, 256 tokens x 5120 bf16 per rank, 128 experts + one redundant hot expert), CUDA-graph replays."""
+    (R=64, 256 tokens x 5120 bf16 per rank, 128 experts + one redundant hot expert), CUDA-graph replays; and two such
+    calls (two layers) back to back: stream order vs double-buffered in two plan slots (L483)."""
     Ls, idx, bl, J = W.dynamic_moe_metadata()
     R, n = Ls.shape
     nx.ncclx_init_dynamic(n, R * R * J)
     tot = Ls.sum(axis=1)
-    send = [W.torch_values(int(t), "bf16", 5000 + s) for s, t in enumerate(tot)]
-    recv = [torch.empty(int(tot[s]), dtype=torch.bfloat16, device="cuda") for d in range(R) for s in range(R)]
-    st, rt = nx.device_ptr_table(send), nx.device_ptr_table(recv)
-    Ld, Id, Bd = (torch.from_numpy(np.ascontiguousarray(x)).cuda() for x in (Ls, idx, bl))
-    allL = torch.empty((R, R, n), dtype=torch.int64, device="cuda")
 
-    def call():
-        nx.ncclx_alltoallv_dynamic_dev(st, Ld, n, Id, idx.shape[1], Bd, J, rt, allL, R, "bf16")
-    call(); torch.cuda.synchronize()
-    g = torch.cuda.CUDAGraph()
-    with torch.cuda.graph(g):
-        call()
-    t = event_times_ms(torch, g.replay, reps, warm=20)
+    def problem(seed):
+        send = [W.torch_values(int(t), "bf16", seed + s) for s, t in enumerate(tot)]
+        recv = [torch.empty(int(tot[s]), dtype=torch.bfloat16, device="cuda") for d in range(R) for s in range(R)]
+        return {"send": send, "recv": recv, "st": nx.device_ptr_table(send), "rt": nx.device_ptr_table(recv),
+                "all": torch.empty((R, R, n), dtype=torch.int64, device="cuda")}
+    A, B = problem(5000), problem(5100)
+    Ld, Id, Bd = (torch.from_numpy(np.ascontiguousarray(x)).cuda() for x in (Ls, idx, bl))
+    side = torch.cuda.Stream()
+
+    def call(p=A):
+        nx.ncclx_alltoallv_dynamic_dev(p["st"], Ld, n, Id, idx.shape[1], Bd, J, p["rt"], p["all"], R, "bf16")
+
+    def prep(slot, p):
+        nx.ncclx_alltoallv_dynamic_prepare_dev(slot, p["st"], Ld, n, Id, idx.shape[1], Bd, J, p["rt"], p["all"], R, "bf16")
+
+    def pair_plain():
+        call(A); call(B)
+
+    def pair_double_buffered():
+        main = torch.cuda.current_stream()
+        prep(0, A)
+        side.wait_stream(main)
+        with torch.cuda.stream(side):
+            prep(1, B)
+        nx.ncclx_alltoallv_execute_dev(0)
+        main.wait_stream(side)
+        nx.ncclx_alltoallv_execute_dev(1)
+    one = graph_p50(torch, call, reps)
     moved = 0
     for s_ in range(R):
         pos = 0
         for d in range(R):
             moved += int(Ls[s_, idx[s_, pos:pos + bl[s_, d]]].sum()) * 2
             pos += int(bl[s_, d])
-    p50 = float(np.percentile(t, 50))
-    return {"replays": reps, "p50_us": round(p50 * 1e3, 2), "p99_us": round(float(np.percentile(t, 99)) * 1e3, 2),
-            "bytes_each_way": moved, "segments": int(bl.sum()), **frac(2 * moved / (p50 * 1e-3) / 1e9, peak)}
+    res = {"replays": reps, **one, "bytes_each_way": moved, "segments": int(bl.sum()),
+           **frac(2 * moved / (one["p50_us"] * 1e-6) / 1e9, peak)}
+    for name, fn in (("pair_stream_order", pair_plain), ("pair_double_buffered", pair_double_buffered)):
+        r = graph_p50(torch, fn, reps)
+        res[name] = {**r, **frac(4 * moved / (r["p50_us"] * 1e-6) / 1e9, peak)}
+    return res
 
 
 def topk_extra(torch, nx, peak, R=64, T=4096, k=4, width=5120):
@@ -492,19 +565,33 @@ def topk_extra(torch, nx, peak, R=64, T=4096, k=4, width=5120):
             "note": "unfused path would move 2*k*rows per direction plus the shuffle / the separate k-way sum"}
 
 
-def reducecopy_extra(torch, nx, peak):
-    """FTAR-style ReduceCopy step: 512 MiB bf16 message, 8 MiB chunks,
-    out + fwd written (4 x message bytes of traffic), GB/s as a function of the number of 512-thread CTAs."""
-    n = 256 << 20
+def reducecopy_extra(torch, nx, peak, few=(1, 2, 4), many=(8, 16, 32, 64, 148)):
+    """FTAR-style ReduceCopy step: bf16 message, 8 MiB chunks, out + fwd
+    written (4 x message bytes of traffic), as a function of the number of CTAs, for both inner loops
+    (pipelined register loads / TMA-fed shared-memory ring); and, at 1 / 2 / 4 CTAs, the per-SM ceiling beside it:
+    the streaming copy probe on the same fixed grid (1:1 read:write like the 2-read / 2-write step)."""
+    n = 64 << 20                                   # 128 MiB message: a 1-CTA pass stays well under a second
     a = W.torch_values(n, "bf16", 6001)
     b = W.torch_values(n, "bf16", 6002, 1e-3)
     out, fwd = torch.empty_like(a), torch.empty_like(a)
-    res = {"message_MiB": n * 2 >> 20, "chunk_MiB": 8, "threads_per_cta": 512, "by_ctas": {}}
-    for ctas in (1, 2, 4, 8, 16, 32, 64, 148):
-        t = event_times_ms(torch, lambda: nx.ncclx_reducecopy_sum(a, b, out, fwd, n, "bf16", 8 << 20, ctas), 5, warm=2)
-        m = float(np.median(t))
-        res["by_ctas"][str(ctas)] = {"ms": round(m, 3), "traffic_GBps": round(4 * n * 2 / (m * 1e-3) / 1e9, 1),
-                                     "message_GBps": round(n * 2 / (m * 1e-3) / 1e9, 1)}
+    res = {"message_MiB": n * 2 >> 20, "chunk_MiB": 8, "by_ctas": {}}
+    src8, dst8 = a.view(torch.uint8), out.view(torch.uint8)
+    for ctas in few + many:
+        row = {}
+        for tma, name in ((0, "pipelined"), (1, "tma_ring")):
+            nx.ncclx_set_param(nx.PARAM_REDUCECOPY_TMA, tma)
+            t = event_times_ms(torch, lambda: nx.ncclx_reducecopy_sum(a, b, out, fwd, n, "bf16", 8 << 20, ctas), 5, warm=2)
+            m = float(np.median(t))
+            row[name] = {"ms": round(m, 3), "traffic_GBps": round(4 * n * 2 / (m * 1e-3) / 1e9, 1),
+                         "message_GBps": round(n * 2 / (m * 1e-3) / 1e9, 1)}
+        nx.ncclx_set_param(nx.PARAM_REDUCECOPY_TMA, 0)
+        if ctas in few:
+            t = event_times_ms(torch, lambda: nx.ncclx_stream_probe_ctas(2, src8, dst8, n * 2, ctas), 5, warm=2)
+            m = float(np.median(t))
+            row["copy_probe_ceiling_GBps"] = round(2 * n * 2 / (m * 1e-3) / 1e9, 1)
+            best = max(row["pipelined"]["traffic_GBps"], row["tma_ring"]["traffic_GBps"])
+            row["best_frac_of_ceiling"] = round(best / row["copy_probe_ceiling_GBps"], 3)
+        res["by_ctas"][str(ctas)] = row
     return res
 
 
@@ -532,6 +619,109 @@ def reduce_dtype_extra(torch, nx, peak):
         res[dtype] = {"ms_median": round(float(np.median(t)), 4), "bytes": r.bytes, **frac(r.bytes / (np.median(t) * 1e-3) / 1e9, peak)}
         del r
     return res
+
+
+def misaligned_extra(torch, nx, peak):
+    """Element-granular counts ('s_i number of tokens'): segments whose source and destination are
+    misaligned differently modulo 16 -- odd bf16 counts, odd byte counts -- against the same bytes 16B-aligned.
+    R = 16, ~360 MB each way; every byte goes through the TMA ring either way."""
+    rng = np.random.default_rng(0)
+    res = {}
+    for key, rows, width, dtype in (("R16_bf16_odd_counts", rng.integers(300000, 400000, (16, 16)) * 2 + 1, 1, "bf16"),
+                                    ("R16_bf16_aligned_counts", rng.integers(75000, 100000, (16, 16)) * 8, 1, "bf16"),
+                                    ("R16_bf16_aligned_counts_4x_bytes", rng.integers(300000, 400000, (16, 16)) * 8, 1, "bf16"),
+                                    ("R16_u8_odd_counts", rng.integers(600000, 800000, (16, 16)) * 2 + 1, 1, "u8"),
+                                    ("R64_bf16_odd_rows_of_5121", np.ones((64, 64), np.int64) * 41, 5121, "bf16")):
+        a = A2A(W.A2AConfig(key, rows.shape[0], width, dtype, 1, rows.astype(np.int64)), torch, nx, with_back=False)
+        t = event_times_ms(torch, a.dispatch, 10)
+        m = float(np.median(t))
+        res[key] = {"MB_each_way": round(a.bytes_one_way / 1e6, 1), "ms": round(m, 4), **frac(2 * a.bytes_one_way / (m * 1e-3) / 1e9, peak)}
+        del a
+    res["odd_bf16_over_aligned"] = round(res["R16_bf16_odd_counts"]["GBps"] / res["R16_bf16_aligned_counts"]["GBps"], 3)
+    return res
+
+
+def topk_table3_extra(torch, nx, peak, reps, shapes=None):
+    """PAPER.md Table 3 (L493-516): decode-shaped MoE layer, k in {1, 4}, 128 / 256 tokens per rank, hidden 5120 bf16,
+    R in {32, 64, 128}: dispatch -> combine replayed in ONE CUDA graph.  (a) top-k calls, one-call form (each runs its own
+    metadata kernel); (b) plan-slot form (one metadata kernel per layer, the combine reuses the dispatch's offsets);
+    (c) the plain AllToAllv pair on the same bytes with the k*T copies materialised by the caller."""
+    width = 5120
+    res = {}
+    for R, T, k in (shapes or [(R, T, k) for R in (32, 64, 128) for T in (128, 256) for k in (1, 4)]):
+        pos, C = W.topk_routing(R, T, k, 2 * R, seed=R + T + k)
+        X = [W.torch_values(T * width, "bf16", 9000 + s) for s in range(R)]
+        recv = [torch.empty(max(int(C[:, d].sum()), 1) * width, dtype=torch.bfloat16, device="cuda") for d in range(R)]
+        Z = [torch.empty(T * width, dtype=torch.bfloat16, device="cuda") for _ in range(R)]
+        dpos, dC = torch.from_numpy(pos).cuda(), torch.from_numpy(C).cuda()
+        dRC = torch.empty_like(dC)
+        xt, rt, zt = nx.device_ptr_table(X), nx.device_ptr_table(recv), nx.device_ptr_table(Z)
+
+        def one_call():
+            nx.ncclx_moe_dispatch_topk_dev(xt, dpos, dC, rt, dRC, R, T, k, width, "bf16")
+            nx.ncclx_moe_combine_topk_sum_dev(rt, dpos, dC, zt, R, T, k, width, "bf16")
+
+        def planned():
+            nx.ncclx_moe_topk_prepare_dev(1, dC, dRC, R)
+            nx.ncclx_moe_dispatch_topk_execute_dev(1, xt, dpos, rt, T, k, width, "bf16")
+            nx.ncclx_moe_combine_topk_sum_execute_dev(1, rt, dpos, zt, T, k, width, "bf16")
+        # plain AllToAllv on the materialised k*T rows (what a caller without the top-k calls would move)
+        Cel = C * width
+        mat = A2A(W.A2AConfig("mat", R, width, "bf16", 1, C), torch, nx, with_back=True)
+
+        def plain_pair():
+            mat.dispatch(); mat.combine()
+        row = {"one_call": graph_p50(torch, one_call, reps), "plan_slot": graph_p50(torch, planned, reps),
+               "plain_alltoallv_pair_materialised": graph_p50(torch, plain_pair, reps),
+               "bytes_topk_pair": 2 * (1 + k) * R * T * width * 2, "bytes_plain_pair": 4 * int(Cel.sum()) * 2}
+        ok = all(torch.equal(z.float(), k * x.float()) for z, x in zip(Z[:2], X[:2]))
+        row["combine_of_dispatch_equals_k_times_x"] = bool(ok)
+        res[f"R{R}_T{T}_k{k}"] = row
+        del mat, X, recv, Z
+    return res
+
+
+def large_r_extra(torch, nx, peak, reps):
+    """R > 256 (the coarse index of the descriptor table no longer fits the copy kernel's 16 KB of shared memory:
+    claims locate their segment with the 128-ary search in L2): small-message shapes, one 14 KB row for ~30 % of the
+    pairs, against R = 128 (the T_c*(N-1) term grows with the rank count)."""
+    res = {}
+    nx.ncclx_finalize()
+    nx.ncclx_init(1024, torch.cuda.current_device())
+    for R in (128, 256, 512, 1024):
+        rng = np.random.default_rng(R)
+        rows = (rng.random((R, R)) < 0.3).astype(np.int64)
+        w = A2A(W.A2AConfig(f"R{R}", R, 7168, "bf16", 1, rows), torch, nx, with_back=False)
+        r = graph_p50(torch, w.dispatch, reps)
+        res[f"R{R}"] = {"pairs": int(rows.sum()), "bytes_each_way": w.bytes_one_way, **r,
+                        **frac(2 * w.bytes_one_way / (r["p50_us"] * 1e-6) / 1e9, peak)}
+        del w
+    nx.ncclx_finalize()
+    nx.ncclx_init(128, torch.cuda.current_device())
+    return res
+
+
+def timeline_probe(torch, nx, peak, cfg_index=5):
+    """Instrumented build only (python -m paper_2510_20171_b200.build --timeline; NCCLX_B200_LIB=<that .so>): per-CTA
+    %globaltimer stamps of ONE config-5 copy kernel -> where the time beyond bytes / bandwidth goes (start-up, ramp, tail)."""
+    a = A2A(W.a2a_config(cfg_index), torch, nx, with_back=False)
+    for _ in range(5):
+        a.dispatch()
+    torch.cuda.synchronize()
+    tl = nx.ncclx_debug_timeline().astype(np.int64)
+    names = ["enter", "metadata_ready", "first_load", "first_store", "last_store", "drained", "exit"]
+    t0 = int(tl[:, 0].min())
+    cols = {nm: (tl[:, i] - t0) / 1e3 for i, nm in enumerate(names)}           # us since the first CTA entered
+    out = {"ctas": int(tl.shape[0]), "bulk_tiles": int(tl[0, 7]), "bytes_moved": 2 * a.bytes_one_way, "us": {}}
+    for nm, v in cols.items():
+        out["us"][nm] = {"min": round(float(v.min()), 2), "median": round(float(np.median(v)), 2), "max": round(float(v.max()), 2)}
+    span = float(cols["exit"].max())
+    busy = float(np.median(cols["last_store"] - cols["first_load"]))
+    out["kernel_span_us"] = round(span, 2)
+    out["median_cta_streaming_window_us"] = round(busy, 2)
+    out["at_6.9TBps_us"] = round(2 * a.bytes_one_way / 6.9e12 * 1e6, 2)
+    out["per_cta"] = [[round(float(cols[nm][i]), 2) for nm in names] for i in range(tl.shape[0])]
+    return out
 
 
 def graph_p50(torch, enqueue, reps, warm=20):
@@ -606,11 +796,19 @@ def latency_extra(torch, nx, peak, reps):
 def probe(args, torch, nx, peak):
     """One config, eager launches, CUDA-event time per call (the command ncu captures are taken from)."""
     n = args.probe
-    if n in (6, 7, 8, 9):
+    if n >= 6:
         res = (latency_extra(torch, nx, peak, args.steps) if n == 6 else
                dynamic_extra(torch, nx, peak, args.steps) if n == 7 else
-               topk_extra(torch, nx, peak) if n == 8 else ceiling_extra(torch, nx, peak))
-        print(json.dumps({"probe": {6: "next4_latency", 7: "next1_dynamic", 8: "next3_topk", 9: "hbm_ceiling"}[n], **res}))
+               topk_extra(torch, nx, peak) if n == 8 else
+               ceiling_extra(torch, nx, peak) if n == 9 else
+               timeline_probe(torch, nx, peak) if n == 10 else
+               misaligned_extra(torch, nx, peak) if n == 11 else
+               reducecopy_extra(torch, nx, peak) if n == 12 else
+               topk_table3_extra(torch, nx, peak, args.steps) if n == 13 else
+               large_r_extra(torch, nx, peak, args.steps))
+        names = {6: "next4_latency", 7: "next1_dynamic", 8: "next3_topk", 9: "hbm_ceiling", 10: "cfg5_timeline", 11: "misaligned",
+                 12: "next2_reducecopy", 13: "next3_topk_table3", 14: "large_R"}
+        print(json.dumps({"probe": names[n], **res}))
         nx.ncclx_finalize()
         return 0
     if n in (1, 3, 5):

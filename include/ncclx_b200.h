@@ -23,8 +23,13 @@
  *     synchronisation, no allocation, no host<->device copy.  They may be captured into a
  *     CUDA graph; a replay re-reads the device-resident metadata.  One workspace exists per
  *     process: calls must be ordered on ONE stream at a time (or by events).
- *   - Return value: 0 = NCCLX_OK, otherwise an ncclx_result_t; nothing is enqueued on error.
- *     No exceptions, no abort, nothing printed.  ncclx_strerror() names a code.
+ *   - Return value: 0 = NCCLX_OK, otherwise an ncclx_result_t.  Every argument and configuration check is made
+ *     BEFORE the call's first kernel launch, so an NCCLX_ERR_ARG / _DTYPE / _NOT_INITIALIZED / _CAPTURE return
+ *     means nothing was enqueued and no buffer or workspace was touched (ncclx_launch_count() does not move).
+ *     Only NCCLX_ERR_CUDA (a launch the CUDA runtime itself refused) can follow an earlier successful launch of
+ *     the same call.  No exceptions, no abort, nothing printed.  ncclx_strerror() names a code.
+ *   - Entry points may be called from several host threads (one internal mutex); the workspace rule above
+ *     still applies to what they enqueue.
  *   - There is no CPU fallback: without a CUDA device ncclx_init fails with
  *     NCCLX_ERR_CUDA and every other call fails with NCCLX_ERR_NOT_INITIALIZED.
  */
@@ -38,7 +43,7 @@
 extern "C" {
 #endif
 
-#define NCCLX_B200_VERSION 100 /* 0.1.0 */
+#define NCCLX_B200_VERSION 200 /* 0.2.0 */
 #define NCCLX_MAX_RANKS 1024   /* hard upper bound on R (ncclx_init max_ranks) */
 
 typedef void* ncclx_stream_t; /* a cudaStream_t */
@@ -98,7 +103,7 @@ int ncclx_version(void);
  * sum_s C[s][d] elements; overflow is undefined (as in NCCL).  send and recv buffers must not
  * overlap.  Segment addresses may have any element alignment; full speed is only promised
  * when every segment's source address, destination address and byte length are multiples of
- * 16 (the cp.async.bulk path); everything else takes the vector path.
+ * 16 (TMA in and out); everything else is loaded by the TMA as aligned spans and stored by warps (vector list).
  * The inverse ("combine") is the same call with send := recv, sendcounts := recvcounts.
  * For R <= 32 (NCCLX_PARAM_FUSED_MAX_RANKS) the call is ONE kernel launch (the small-message fast path,
  * PAPER.md L483): every CTA rebuilds offsets and work list from the <= 8 KB count matrix in shared memory
@@ -121,9 +126,12 @@ int ncclx_alltoallv_dev(const void* const* send, const int64_t* sendcounts_dev, 
  * prepare(p) must be ordered before execute(p), and execute(p) before the next prepare(p), by stream order
  * or events; different slots are independent, so the combine's prepare (whose counts are the dispatch's
  * recvcounts, complete as soon as the dispatch's prepare is) can run on a second stream WHILE the dispatch's
- * payload moves.  ncclx_alltoallv_dev == prepare(0) + execute(0) for R > 32, one fused kernel otherwise;
- * the dynamic and top-k calls also use slot 0.  Arguments as for ncclx_alltoallv_dev; 0 <= plan <
- * NCCLX_NUM_PLANS; execute returns NCCLX_ERR_ARG for a slot that was never prepared.  Both capturable. */
+ * payload moves.  ncclx_alltoallv_dev == prepare(0) + execute(0) for R > 32, one fused kernel otherwise (slot 0
+ * is then left as it was).  The one-call dynamic and top-k entry points also (re)build slot 0: after them slot 0
+ * holds THEIR plan (a dynamic plan can be executed again with ncclx_alltoallv_execute_dev(0); a top-k plan makes
+ * it return NCCLX_ERR_ARG).  Tunables (ncclx_set_param) are snapshotted into the slot by prepare: execute uses
+ * the values the work list was built with.  Arguments as for ncclx_alltoallv_dev; 0 <= plan < NCCLX_NUM_PLANS;
+ * execute returns NCCLX_ERR_ARG for a slot that holds no AllToAllv / AllToAllvDynamic plan.  Both capturable. */
 #define NCCLX_NUM_PLANS 4
 int ncclx_alltoallv_prepare_dev(int plan, const void* const* send, const int64_t* sendcounts_dev, void* const* recv,
                                 int64_t* recvcounts_dev, int R, ncclx_dtype_t dtype, ncclx_stream_t stream);
@@ -156,8 +164,16 @@ int ncclx_device_status(uint32_t* status_host, ncclx_stream_t stream);
  * Device status bits (ncclx_device_status): 0 negative split length (treated as 0), 1 split index outside
  * [0,nsplits) (skipped), 2 block length < 0 or > maxBlockLen or list overrun (clamped).
  * Each recvbuffs[d][s] must hold sum_i L_s[i] elements and must not overlap any send buffer.
- * Call ncclx_init_dynamic(max_splits, max_segments) once after ncclx_init, outside capture. */
+ * Call ncclx_init_dynamic(max_splits, max_segments) once after ncclx_init, outside capture (allocates one
+ * descriptor table of max_segments entries per plan slot).
+ * Split-phase form (double buffering, L483): ncclx_alltoallv_dynamic_prepare_dev(plan, ...) enqueues only the
+ * metadata kernel into plan slot `plan`; ncclx_alltoallv_execute_dev(plan) then moves the payload AND writes
+ * recvAllSplitLengths (it rides along with the payload).  ncclx_alltoallv_dynamic_dev == prepare(0) + execute(0). */
 int ncclx_init_dynamic(int max_splits, int64_t max_segments);
+int ncclx_alltoallv_dynamic_prepare_dev(int plan, const void* const* send, const int64_t* sendSplitLengths_dev, int nsplits,
+                                        const int64_t* sendIndices_dev, int maxIndices,
+                                        const int64_t* sendIndicesBlockLens_dev, int maxBlockLen, void* const* recvbuffs,
+                                        int64_t* recvAllSplitLengths_dev, int R, ncclx_dtype_t dtype, ncclx_stream_t stream);
 int ncclx_alltoallv_dynamic_dev(const void* const* send, const int64_t* sendSplitLengths_dev, int nsplits,
                                 const int64_t* sendIndices_dev, int maxIndices,
                                 const int64_t* sendIndicesBlockLens_dev, int maxBlockLen, void* const* recvbuffs,
@@ -192,7 +208,9 @@ int ncclx_reducescatter_sum(const void* const* send, void* const* recv, size_t r
  * to both; either may be NULL but not both ("avoid unnecessary HBM stores in the intermediate forwarding
  * steps").  The message is walked in fixed chunks of `chunk_bytes` (paper: S = 8 MB; 0 selects 8 MiB) by a
  * FIXED grid of `num_ctas` CTAs x 512 threads (paper: 2 CTAs suffice to stay hidden under the network;
- * 0 selects 2) -- the SM-frugal regime, as opposed to the full-chip ncclx_allreduce_sum.
+ * 0 selects 2) -- the SM-frugal regime, as opposed to the full-chip ncclx_allreduce_sum.  Two inner loops with
+ * identical results (NCCLX_PARAM_REDUCECOPY_TMA): software-pipelined 256-bit register loads, or a producer warp
+ * feeding a 6-stage shared-memory ring with cp.async.bulk.
  * a, b, out, fwd: DEVICE pointers to `count` elements; out/fwd may alias a or b exactly (in place), other
  * overlap is undefined.  dtype in {BF16, F32, F16}.  32-byte aligned pointers and chunk size take the
  * 256-bit vector path, anything else a scalar path with the same arithmetic.  Capturable. */
@@ -222,6 +240,17 @@ int ncclx_moe_dispatch_topk_dev(const void* const* tokens, const int32_t* pos_de
 int ncclx_moe_combine_topk_sum_dev(const void* const* expert_out, const int32_t* pos_dev,
                                    const int64_t* sendcounts_rows_dev, void* const* out, int R, int T, int k,
                                    int width, ncclx_dtype_t dtype, ncclx_stream_t stream);
+/* Plan-slot form (PAPER.md L483 double buffering, for the k > 1 flow of Table 3): the metadata phase (a1, a2: row
+ * offsets + recvcounts) goes into plan slot `plan` ONCE per MoE layer, and both the dispatch and the combine of that
+ * layer execute against it -- the combine needs the DISPATCH's offsets, so it launches no metadata kernel at all --
+ * while the next layer prepares another slot.  prepare(p) must be ordered before the executes that use p, and those
+ * before the next prepare(p).  execute returns NCCLX_ERR_ARG for a slot that holds no top-k plan.  R is the plan's. */
+int ncclx_moe_topk_prepare_dev(int plan, const int64_t* sendcounts_rows_dev, int64_t* recvcounts_rows_dev, int R,
+                               ncclx_stream_t stream);
+int ncclx_moe_dispatch_topk_execute_dev(int plan, const void* const* tokens, const int32_t* pos_dev, void* const* recv,
+                                        int T, int k, int width, ncclx_dtype_t dtype, ncclx_stream_t stream);
+int ncclx_moe_combine_topk_sum_execute_dev(int plan, const void* const* expert_out, const int32_t* pos_dev, void* const* out,
+                                           int T, int k, int width, ncclx_dtype_t dtype, ncclx_stream_t stream);
 
 /* ---- host-buffer forms (the end-to-end path: H2D + kernels + D2H inside the call) ------ *
  *
@@ -244,30 +273,24 @@ int ncclx_reducescatter_sum_host(const void* const* send, void* const* recv, siz
 /* ---- tuning and measurement (not part of the paper's contract) -------------------------- */
 
 typedef enum {
-    NCCLX_PARAM_COPY_CTAS_PER_SM = 0, /* persistent segment-copy CTAs per SM (1..4), default 1        */
-    NCCLX_PARAM_BULK_MIN_BYTES = 1,   /* 16B-aligned segments >= this many bytes take cp.async.bulk;   */
-                                      /* smaller or unaligned ones take the vector path. default 1024  */
-    NCCLX_PARAM_REDUCE_CTAS_PER_SM = 2, /* reduce grid = this * SM count, default 8 (more CTAs than   */
-                                      /* fit at once: the hardware scheduler evens out short calls)   */
-    NCCLX_PARAM_SCAN_CTAS = 3,        /* upper bound on CTAs of the counts kernel, default 32          */
-    NCCLX_PARAM_PROFILE = 4,          /* 1: bracket each kernel with CUDA events (never while capturing) */
-    NCCLX_PARAM_FORCE_VECTOR = 5,     /* 1: send every segment down the vector path (for A/B runs)     */
-    NCCLX_PARAM_BULK_TILE_SHIFT = 6,  /* log2 bytes of a bulk tile = one smem ring stage (12..16), default 15 */
-    NCCLX_PARAM_VEC_TILE_SHIFT = 7,   /* log2 bytes of a vector-path tile (10..20), default 14          */
-    NCCLX_PARAM_PDL = 8,              /* 1 (default): launch the copy kernel with programmatic dependent   */
-                                      /* launch so its prologue overlaps the counts kernel; 0: plain order */
-    NCCLX_PARAM_COPY_STATIC_EIGHTHS = 9, /* 0..8: share of copy tiles assigned statically per engine, default 0 */
-    NCCLX_PARAM_COPY_KMAX = 10,       /* max tiles per dynamic claim when segments are short (1..64), default 6 */
-    NCCLX_PARAM_COPY_KMAX_LONG = 11,  /* same when segments average >= 8 tiles (1..64), default 2          */
-    NCCLX_PARAM_FUSED_MAX_RANKS = 12, /* ncclx_alltoallv_dev runs as ONE kernel for R <= this (0..32; 0 = never), default 32 */
-    NCCLX_PARAM_FUSED_MIN_TILE_SHIFT = 13, /* smallest bulk tile the single-launch path may choose (log2 bytes, 10..16), default 12 */
-    NCCLX_PARAM_COPY_PENDING_STORES = 14, /* bulk engine: stores left unreclaimed in the ring after each store (1..8), default 1 */
-    NCCLX_PARAM_COPY_BULK_ENGINES = 15,   /* bulk (TMA) engine warps per copy CTA, each with 1/E of the ring: 1, 2, 4, or 0 (default): chosen on */
-                                          /* the device -- 4 for calls of few tiles per SM (latency-bound), 1 for long ones (HBM-bound)         */
-    NCCLX_PARAM_HOST_ZERO_COPY = 16,      /* 1 (default): the *_host calls let the kernels access PINNED host buffers directly */
+    NCCLX_PARAM_BULK_MIN_BYTES = 0,     /* 16B-aligned segments >= this many bytes go on the bulk list (32 KiB tiles, TMA in and out);  */
+                                        /* smaller or unaligned ones on the vector list (TMA in, warp stores out). default 1024         */
+    NCCLX_PARAM_REDUCE_CTAS_PER_SM = 1, /* reduce grid = this * SM count (1..64), default 8 (more CTAs than fit at once: the hardware  */
+                                        /* scheduler evens out short calls)                                                            */
+    NCCLX_PARAM_PROFILE = 2,            /* 1: bracket each kernel with CUDA events (never while capturing)                              */
+    NCCLX_PARAM_BULK_TILE_SHIFT = 3,    /* log2 bytes of a bulk tile (12..16), default 15                                               */
+    NCCLX_PARAM_PDL = 4,                /* 1 (default): programmatic dependent launch -- a kernel's prologue overlaps the tail of the   */
+                                        /* kernel before it (reductions: only below 1 GiB of input); 0: plain stream order              */
+    NCCLX_PARAM_COPY_KMAX = 5,          /* max bulk tiles per dynamic claim when segments are short (1..64), default 6                  */
+    NCCLX_PARAM_FUSED_MAX_RANKS = 6,    /* ncclx_alltoallv_dev runs as ONE kernel for R <= this (0..32; 0 = never), default 32          */
+    NCCLX_PARAM_COPY_BULK_ENGINES = 7,  /* bulk (TMA) engine warps per copy CTA: 1, 2, 4, or 0 (default): chosen on the device -- 4 for */
+                                        /* calls of few tiles per SM (latency-bound), 1 for long ones (HBM-bound)                       */
+    NCCLX_PARAM_HOST_ZERO_COPY = 8,     /* 1 (default): the *_host calls let the kernels access PINNED host buffers directly           */
+    NCCLX_PARAM_REDUCECOPY_TMA = 9,     /* ncclx_reducecopy_sum inner loop: 0 (default) pipelined register loads, 1 TMA-fed smem ring   */
     NCCLX_PARAM_COUNT_
 } ncclx_param_t;
 
+/* Process-global; take effect for work lists built AFTER the call (a prepared plan slot keeps its snapshot). */
 int ncclx_set_param(int param, int64_t value);
 int ncclx_get_param(int param, int64_t* value);
 
@@ -295,6 +318,15 @@ int64_t ncclx_launch_count(void);
  * 3 = write-only through TMA bulk stores of 32 KiB (bytes a multiple of 32 KiB).  Enqueue
  * only; time it with events.  Gives the practical read / write / copy ceilings of the part. */
 int ncclx_stream_probe(int mode, const void* src, void* dst, size_t bytes, ncclx_stream_t stream);
+/* Same probe on a FIXED grid of num_ctas >= 1 CTAs x 1024 threads (128 KB of loads in flight per CTA): the per-SM
+ * ceiling the SM-frugal ncclx_reducecopy_sum (2 CTAs) is read against. */
+int ncclx_stream_probe_ctas(int mode, const void* src, void* dst, size_t bytes, int num_ctas, ncclx_stream_t stream);
+
+/* Instrumented builds only (python -m paper_2510_20171_b200.build --timeline; -DXDEV_TIMELINE): copies the per-CTA
+ * globaltimer stamps of the LAST segment_copy_kernel launch to stamps_host[ctas][*fields] (ns; fields: kernel entry,
+ * metadata ready, first load issued, first store issued, last store issued, engine drained, exit, bulk tiles of the
+ * call).  max_ctas >= ncclx_sm_count().  Synchronises the device.  NCCLX_ERR_ARG in a normal build. */
+int ncclx_debug_timeline(uint64_t* stamps_host, int max_ctas, int* fields);
 
 /* Number of SMs of the device the library was initialised on (0 before init). */
 int ncclx_sm_count(void);

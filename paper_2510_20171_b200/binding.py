@@ -11,28 +11,23 @@ import os
 from typing import Sequence
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libncclx_b200.so")
+# NCCLX_B200_LIB selects another build of the same library (the instrumented -DXDEV_TIMELINE one); never a fallback
+LIB_PATH = os.environ.get("NCCLX_B200_LIB") or os.path.join(HERE, "libncclx_b200.so")
 
 BF16, F32, F16, U8 = 0, 1, 2, 3
 DTYPE_ID = {"bf16": BF16, "f32": F32, "f16": F16, "u8": U8}
 
-PARAM_COPY_CTAS_PER_SM = 0
-PARAM_BULK_MIN_BYTES = 1
-PARAM_REDUCE_CTAS_PER_SM = 2
-PARAM_SCAN_CTAS = 3
-PARAM_PROFILE = 4
-PARAM_FORCE_VECTOR = 5
-PARAM_BULK_TILE_SHIFT = 6
-PARAM_VEC_TILE_SHIFT = 7
-PARAM_PDL = 8
-PARAM_COPY_STATIC_EIGHTHS = 9
-PARAM_COPY_KMAX = 10
-PARAM_COPY_KMAX_LONG = 11
-PARAM_FUSED_MAX_RANKS = 12
-PARAM_FUSED_MIN_TILE_SHIFT = 13
-PARAM_COPY_PENDING_STORES = 14
-PARAM_COPY_BULK_ENGINES = 15
-PARAM_HOST_ZERO_COPY = 16
+PARAM_BULK_MIN_BYTES = 0
+PARAM_REDUCE_CTAS_PER_SM = 1
+PARAM_PROFILE = 2
+PARAM_BULK_TILE_SHIFT = 3
+PARAM_PDL = 4
+PARAM_COPY_KMAX = 5
+PARAM_FUSED_MAX_RANKS = 6
+PARAM_COPY_BULK_ENGINES = 7
+PARAM_HOST_ZERO_COPY = 8
+PARAM_REDUCECOPY_TMA = 9
+PARAM_COUNT = 10
 NUM_PLANS = 4
 
 KERNEL_COUNTS, KERNEL_COPY, KERNEL_REDUCE, KERNEL_DYN, KERNEL_TOPK, KERNEL_FUSED = 0, 1, 2, 3, 4, 5
@@ -45,7 +40,9 @@ SYMBOLS = [
     "ncclx_reducescatter_sum_host", "ncclx_set_param", "ncclx_get_param", "ncclx_profile_read",
     "ncclx_profile_reset", "ncclx_launch_count", "ncclx_sm_count", "ncclx_init_dynamic", "ncclx_alltoallv_dynamic_dev",
     "ncclx_reducecopy_sum", "ncclx_moe_dispatch_topk_dev", "ncclx_moe_combine_topk_sum_dev",
-    "ncclx_alltoallv_prepare_dev", "ncclx_alltoallv_execute_dev", "ncclx_stream_probe",
+    "ncclx_alltoallv_prepare_dev", "ncclx_alltoallv_execute_dev", "ncclx_stream_probe", "ncclx_stream_probe_ctas",
+    "ncclx_alltoallv_dynamic_prepare_dev", "ncclx_moe_topk_prepare_dev", "ncclx_moe_dispatch_topk_execute_dev",
+    "ncclx_moe_combine_topk_sum_execute_dev", "ncclx_debug_timeline",
 ]
 
 
@@ -91,6 +88,13 @@ def lib() -> ctypes.CDLL:
         L.ncclx_moe_dispatch_topk_dev.argtypes = [vp, vp, vp, vp, vp] + [ctypes.c_int] * 5 + [vp]
         L.ncclx_moe_combine_topk_sum_dev.argtypes = [vp, vp, vp, vp] + [ctypes.c_int] * 5 + [vp]
         L.ncclx_stream_probe.argtypes = [ctypes.c_int, vp, vp, ctypes.c_size_t, vp]
+        L.ncclx_stream_probe_ctas.argtypes = [ctypes.c_int, vp, vp, ctypes.c_size_t, ctypes.c_int, vp]
+        L.ncclx_alltoallv_dynamic_prepare_dev.argtypes = [ctypes.c_int, vp, vp, ctypes.c_int, vp, ctypes.c_int, vp, ctypes.c_int, vp, vp,
+                                                          ctypes.c_int, ctypes.c_int, vp]
+        L.ncclx_moe_topk_prepare_dev.argtypes = [ctypes.c_int, vp, vp, ctypes.c_int, vp]
+        L.ncclx_moe_dispatch_topk_execute_dev.argtypes = [ctypes.c_int, vp, vp, vp] + [ctypes.c_int] * 4 + [vp]
+        L.ncclx_moe_combine_topk_sum_execute_dev.argtypes = [ctypes.c_int, vp, vp, vp] + [ctypes.c_int] * 4 + [vp]
+        L.ncclx_debug_timeline.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
         L.ncclx_set_param.argtypes = [ctypes.c_int, i64]
         L.ncclx_get_param.argtypes = [ctypes.c_int, i64p]
         L.ncclx_profile_read.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double), i64p]
@@ -196,6 +200,32 @@ def ncclx_alltoallv_dynamic_dev(send_table, split_lengths_dev, nsplits: int, ind
         "ncclx_alltoallv_dynamic_dev")
 
 
+def ncclx_alltoallv_dynamic_prepare_dev(plan: int, send_table, split_lengths_dev, nsplits: int, indices_dev, max_indices: int,
+                                        block_lens_dev, max_block_len: int, recvbuffs_table, recv_all_split_lengths_dev,
+                                        R: int, dtype, stream=None) -> None:
+    _ck(lib().ncclx_alltoallv_dynamic_prepare_dev(plan, _ptr(send_table), _ptr(split_lengths_dev), nsplits, _ptr(indices_dev),
+                                                  max_indices, _ptr(block_lens_dev), max_block_len, _ptr(recvbuffs_table),
+                                                  _ptr(recv_all_split_lengths_dev), R, _dt(dtype), _stream(stream)),
+        "ncclx_alltoallv_dynamic_prepare_dev")
+
+
+def ncclx_moe_topk_prepare_dev(plan: int, sendcounts_rows_dev, recvcounts_rows_dev, R: int, stream=None) -> None:
+    _ck(lib().ncclx_moe_topk_prepare_dev(plan, _ptr(sendcounts_rows_dev), _ptr(recvcounts_rows_dev), R, _stream(stream)),
+        "ncclx_moe_topk_prepare_dev")
+
+
+def ncclx_moe_dispatch_topk_execute_dev(plan: int, tokens_table, pos_dev, recv_table, T: int, k: int, width: int, dtype,
+                                        stream=None) -> None:
+    _ck(lib().ncclx_moe_dispatch_topk_execute_dev(plan, _ptr(tokens_table), _ptr(pos_dev), _ptr(recv_table), T, k, width,
+                                                  _dt(dtype), _stream(stream)), "ncclx_moe_dispatch_topk_execute_dev")
+
+
+def ncclx_moe_combine_topk_sum_execute_dev(plan: int, expert_out_table, pos_dev, out_table, T: int, k: int, width: int, dtype,
+                                           stream=None) -> None:
+    _ck(lib().ncclx_moe_combine_topk_sum_execute_dev(plan, _ptr(expert_out_table), _ptr(pos_dev), _ptr(out_table), T, k, width,
+                                                     _dt(dtype), _stream(stream)), "ncclx_moe_combine_topk_sum_execute_dev")
+
+
 def ncclx_allreduce_sum(send_table, recv_table, count: int, R: int, dtype, stream=None) -> None:
     _ck(lib().ncclx_allreduce_sum(_ptr(send_table), _ptr(recv_table), count, R, _dt(dtype), _stream(stream)),
         "ncclx_allreduce_sum")
@@ -257,6 +287,20 @@ def ncclx_reducescatter_sum_host(send: Sequence, recv: Sequence, recvcount: int,
 
 def ncclx_stream_probe(mode: int, src, dst, nbytes: int, stream=None) -> None:
     _ck(lib().ncclx_stream_probe(mode, _ptr(src), _ptr(dst), nbytes, _stream(stream)), "ncclx_stream_probe")
+
+
+def ncclx_stream_probe_ctas(mode: int, src, dst, nbytes: int, num_ctas: int, stream=None) -> None:
+    _ck(lib().ncclx_stream_probe_ctas(mode, _ptr(src), _ptr(dst), nbytes, num_ctas, _stream(stream)), "ncclx_stream_probe_ctas")
+
+
+def ncclx_debug_timeline():
+    """Instrumented builds only: (ctas x fields) uint64 array of globaltimer stamps of the last copy-kernel launch."""
+    import numpy as np
+    n = ncclx_sm_count()
+    buf = np.zeros((n, 16), np.uint64)
+    fields = ctypes.c_int(0)
+    _ck(lib().ncclx_debug_timeline(buf.ctypes.data, n, ctypes.byref(fields)), "ncclx_debug_timeline")
+    return buf.reshape(-1)[:n * fields.value].reshape(n, fields.value)
 
 
 def ncclx_set_param(param: int, value: int) -> None:

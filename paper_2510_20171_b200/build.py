@@ -29,6 +29,9 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in DEPS)
 
 
+LIB_TIMELINE = os.path.join(HERE, "libncclx_b200_timeline.so")
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         tmp = LIB + f".tmp{os.getpid()}"
@@ -38,6 +41,18 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_timeline() -> str:
+    """Instrumented build (-DXDEV_TIMELINE): segment_copy_kernel stamps %globaltimer per CTA.  A measurement aid kept out of
+    the default library; select it with NCCLX_B200_LIB=<path> (bench.py --probe 10 reads the stamps)."""
+    tmp = LIB_TIMELINE + f".tmp{os.getpid()}"
+    subprocess.check_call([nvcc(), *NVCC_FLAGS, "-DXDEV_TIMELINE", "-o", tmp, *SOURCES])
+    os.replace(tmp, LIB_TIMELINE)
+    return LIB_TIMELINE
+
+
 if __name__ == "__main__":
     import sys
-    print(build(force=True, verbose="-v" in sys.argv))
+    if "--timeline" in sys.argv:
+        print(build_timeline())
+    else:
+        print(build(force=True, verbose="-v" in sys.argv))

@@ -7,7 +7,7 @@
 #error "libncclx_b200 is written for sm_100a (B200) only"
 #endif
 
-namespace ncclx {
+namespace xdev {
 
 // One (source s, destination d) segment of the AllToAllv, in destination-major order
 // q = d*R + s -- the order in which the packed receive buffers are laid out,
@@ -45,16 +45,15 @@ __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
 // Classification shared by the counts kernel (which builds the per-list tile prefixes) and the copy
 // kernel (which re-derives a segment's tile count from its descriptor): number of tiles the segment
 // contributes to work list L.  A segment is on exactly one list: BULK iff source and destination are
-// 16-byte aligned and it has at least bulkMinBytes bytes (and the vector path is not forced).
+// 16-byte aligned and it has at least bulkMinBytes bytes.
 struct ClassParams {
     long long bulkMinBytes;
-    int forceVector;
     int tileShift[2];
 };
 __device__ __forceinline__ int seg_tiles(int L, unsigned long long src, unsigned long long dst, long long bytes,
                                          const ClassParams& cp) {
     if (bytes <= 0) return 0;
-    const bool bulk = !cp.forceVector && (((src | dst) & 15ull) == 0) && bytes >= cp.bulkMinBytes;
+    const bool bulk = (((src | dst) & 15ull) == 0) && bytes >= cp.bulkMinBytes;
     if (bulk != (L == 0)) return 0;
     return (int)((bytes + (1ll << cp.tileShift[L]) - 1) >> cp.tileShift[L]);
 }
@@ -89,13 +88,10 @@ __device__ __forceinline__ void griddep_launch_dependents() { asm volatile("grid
 __device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 // ---- streaming global accesses --------------------------------------------------------------
-__device__ __forceinline__ uint4 ld_stream_nc(const uint4* p) {   // read-only for the whole kernel
-    uint4 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
-                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
-    return r;
-}
-__device__ __forceinline__ uint4 ld_stream(const uint4* p) {      // may alias an output (in-place)
+// (No ld.global.nc anywhere: with programmatic dependent launch a kernel's CTAs are resident while the kernel before
+// it in the stream still writes the very bytes they will read after griddepcontrol.wait, and the non-coherent path
+// formally needs data that is read-only for the kernel's whole lifetime.)
+__device__ __forceinline__ uint4 ld_stream(const uint4* p) {      // coherent; may alias an output (in-place)
     uint4 r;
     asm volatile("ld.global.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
                  : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p) : "memory");
@@ -136,6 +132,9 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
+}
 __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
     uint32_t ok;
     asm volatile("{\n\t.reg .pred p;\n\t"
@@ -165,4 +164,4 @@ template <int N> __device__ __forceinline__ void bulk_wait_all() {
     asm volatile("cp.async.bulk.wait_group %0;" :: "n"(N) : "memory");
 }
 
-}  // namespace ncclx
+}  // namespace xdev

@@ -4,46 +4,68 @@
 // S/BW of L447.
 //
 // B200 design (not the paper's H100 kernel):
-//   * persistent grid, one CTA per SM (x ctasPerSM), work discovered on the device from the
-//     descriptor table the counts kernel wrote -- the host knows neither sizes nor tile counts,
-//     so the launch is graph-capturable with a fixed grid (L387, L401);
+//   * persistent grid, one CTA per SM, work discovered on the device from the descriptor table the
+//     metadata kernel wrote -- the host knows neither sizes nor tile counts, so the launch is
+//     graph-capturable with a fixed grid (L387, L401);
 //   * work unit = a tile of at most 2^tileShift bytes of ONE segment; after one static first chunk per
 //     engine, tiles are claimed dynamically, in order, in guided chunks from a global counter that
 //     resets itself => balance by BYTES (and by time), not by segment or by rank (config 3 skew is
 //     250x across segments, 150x across ranks);
-//   * LONG / aligned segments ("bulk" list): warp 0 (optionally warps 0..E-1) drives a byte-granular
-//     ring in shared memory with descriptor-less 1-D TMA: cp.async.bulk global->shared (mbarrier
-//     complete_tx) and cp.async.bulk shared->global (bulk async-groups).  One elected lane issues
-//     everything; ~180 KB of loads stay in flight per SM with no register staging;
-//   * SHORT or unaligned segments ("vector" list): warps 1..N-1 copy with 16-byte vectorised,
-//     fully coalesced ld/st (falling back to 8/4/2/1-byte units when source and destination
-//     misalignment differ), head/tail bytes handled per tile.
+//   * EVERY payload byte is loaded by the TMA (descriptor-less 1-D cp.async.bulk global->shared, completion on
+//     an mbarrier) into a byte-granular ring in shared memory, so ~200 KB of loads are in flight per SM without
+//     register staging, whatever the alignment:
+//       - "bulk" list (source, destination 16-byte aligned, >= bulkMinBytes): tiles of 32 KiB, stored with
+//         cp.async.bulk shared->global; one elected lane of warp 0 (or of warps 0..E-1) issues everything;
+//       - "vector" list (short segments and ANY other alignment -- counts are element-granular):
+//         each engine warp owns a share of the ring, loads the 16-byte-aligned SPAN that covers a 2 KiB piece
+//         of its tile, and the warp then moves it from shared memory to the destination with aligned 16-byte
+//         stores, funnel-shifting when source and destination are misaligned differently (head / tail bytes by
+//         lanes).  (Round 1 copied these global->registers->global with ~61 KB in flight per SM: 3.7 TB/s.)
+//   * the ring is split between the two lists on the device, grid-uniformly, from their tile totals.
 #pragma once
 #include "common.cuh"
 
-namespace ncclx {
+namespace xdev {
 
-constexpr int COPY_THREADS = 512;          // warp 0: bulk engine; warps 1..15: vector engines
+constexpr int COPY_THREADS = 512;          // 16 warps: bulk engines first, then vector engines (split chosen on the device)
+constexpr int COPY_WARPS = COPY_THREADS / 32;
 constexpr int COPY_SLOTS = 32;             // outstanding bulk tiles per engine (mbarriers; slot j lives in lane j): <= 32
 constexpr int COPY_MAX_ENGINES = 4;        // bulk engines (warps 0..E-1) per CTA, each with its own share of the ring
-constexpr int COPY_MBAR_BYTES = COPY_MAX_ENGINES * COPY_SLOTS * 8;
+constexpr int VEC_SLOTS = 16;              // outstanding staged pieces per vector engine
+constexpr int VEC_SUB_BYTES = 2048;        // bytes of a vector tile staged per TMA load (multiple of 16)
+constexpr int VEC_DIRECT_MAX = 48;         // pieces shorter than this are copied by lanes, global -> global
+constexpr int VEC_MAX_IN_BULK_MIX = 9;     // vector engines when both lists have work: the bulk engines keep >= 7/16 of the ring
+constexpr int COPY_MBAR_COUNT = COPY_MAX_ENGINES * COPY_SLOTS + COPY_WARPS * VEC_SLOTS;
+constexpr int COPY_MBAR_BYTES = COPY_MBAR_COUNT * 8;
+constexpr int COPY_KMAX_LONG = 2;          // max tiles per dynamic claim when segments average >= 8 tiles (measured: config 3)
+constexpr int COPY_KMAX_VEC = 8;           // max tiles per dynamic claim on the vector list
+
+// Optional side job for the warps that are not engines at the start of the kernel: `copies` copies of the int64
+// array src[0..n) (negative values written as 0) to dst + c*n.  AllToAllvDynamic's recvAllSplitLengths (PAPER.md
+// L439: every rank receives all split lengths) rides along with the payload instead of sitting in front of it.
+struct SideJob {
+    const long long* src;
+    long long* dst;                        // null: no side job
+    long long n;
+    int copies;
+};
 
 struct CopyArgs {
     const SegDesc* desc;
     const int* colTiles[2];
-    const int* coarse[2];                  // per list: tiles of column d before its descriptor 32*j, [d*nb + j] (counts kernel)
+    const int* coarse[2];                  // per list: tiles of column d before its descriptor 32*j, [d*nb + j] (metadata kernel)
     WorkCtl* ctl;
     int ncols;                             // destination columns of the descriptor table (= R)
     int colLen;                            // descriptor slots per column (R for the plain call, R*maxBlockLen for the dynamic one)
     int useCoarse;                         // 1: stage both coarse indexes in shared memory (2*ncols*nb ints)
-    unsigned int ringBytes;                // shared-memory ring size, multiple of 128, >= 3 tiles
-    int staticEighths;                     // 0..8: share of the tiles assigned statically (contiguous per engine)
-    int kmax[2];                           // max tiles per dynamic claim, per list (short-segment regime)
-    int kmaxLong;                          // same, when segments average >= 8 tiles
-    int maxPendingStores;                  // 1..8: stores whose shared-memory read may be outstanding before the engine waits
-    int bulkEngines;                       // E = 1, 2 or 4 bulk engine warps per CTA (ring split E ways); warps E..15 are vector
-                                           // engines; 0 = chosen on the device from the tile count (choose_bulk_engines)
+    unsigned int ringBytes;                // shared-memory ring size, multiple of 128
+    int kmax;                              // max tiles per dynamic claim on the bulk list (short-segment regime)
+    int bulkEngines;                       // E = 1, 2 or 4 bulk engine warps per CTA; 0 = chosen on the device from the tile count
     ClassParams cls;
+    SideJob side;
+#ifdef XDEV_TIMELINE
+    unsigned long long* timeline;          // [grid][TL_COUNT] globaltimer stamps (instrumented build only)
+#endif
 };
 
 __host__ __device__ inline int coarse_blocks(int colLen) { return (colLen + 31) >> 5; }
@@ -86,7 +108,7 @@ struct Cursor {
     __device__ __forceinline__ void load_desc(int qq, uint4& a, uint4& b) const {
         if (qq < RR) {
             const uint4* p = reinterpret_cast<const uint4*>(desc + qq);
-            if constexpr (SM) { a = p[0]; b = p[1]; } else { a = __ldg(p); b = __ldg(p + 1); }
+            if constexpr (SM) { a = p[0]; b = p[1]; } else { a = ld_stream(p); b = ld_stream(p + 1); }   // coherent: the kernel before us wrote them (PDL)
         } else {
             a = make_uint4(0, 0, 0, 0); b = make_uint4(0, 0, 0, 0);
         }
@@ -212,14 +234,15 @@ struct Cursor {
         const int tl = tt - colBase[d];
         const SegDesc* col = desc + (size_t)d * colLen;
         int s0 = 0, n = colLen;                 // smallest s with col[s].pfx[L] > tl lies in [s0, s0+n)
-        while (n > 32) {                   // 128-ary rounds: every lane probes 4 block ends per L2 round trip
+        while (n >= 32) {                  // 128-ary rounds: every lane probes 4 block ends per L2 round trip; ends with at most
+                                           // 31 candidates, so that they AND the predecessor slot fit in one 32-descriptor window
             const int step = (n + 127) >> 7;
             int cnt = 0;
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const int b = lane * 4 + u;
                 const int idx = s0 + min((b + 1) * step, n) - 1;
-                const int pv = SM ? col[idx].pfx[L] : __ldg(&col[idx].pfx[L]);
+                const int pv = col[idx].pfx[L];
                 cnt += (pv <= tl) ? 1 : 0;
             }
             int m = cnt;                   // blocks entirely <= tl (monotone, so a plain count)
@@ -352,33 +375,9 @@ struct Cursor {
     __device__ __forceinline__ void next() { ++t; ++kInSeg; }
 };
 
-// ---- vector path -------------------------------------------------------------------------------
-template <typename T> __device__ __forceinline__ T ld_unit(const T* p) { return __ldg(p); }
-template <> __device__ __forceinline__ uint4 ld_unit<uint4>(const uint4* p) { return ld_stream_nc(p); }
-template <typename T> __device__ __forceinline__ void st_unit(T* p, const T& v) { *p = v; }
-template <> __device__ __forceinline__ void st_unit<uint4>(uint4* p, const uint4& v) { st_stream(p, v); }
-
-template <typename T, int U>
-__device__ __forceinline__ void warp_copy_units(const unsigned char* src, unsigned char* dst, long long n) {
-    const T* s = reinterpret_cast<const T*>(src);
-    T* d = reinterpret_cast<T*>(dst);
-    long long i = lane_id();
-    for (; i + (U - 1) * 32 < n; i += U * 32) {
-        T v[U];
-#pragma unroll
-        for (int j = 0; j < U; ++j) v[j] = ld_unit(s + i + j * 32);
-#pragma unroll
-        for (int j = 0; j < U; ++j) st_unit(d + i + j * 32, v[j]);
-    }
-    for (; i < n; i += 32) st_unit(d + i, ld_unit(s + i));
-}
-
-// Source and destination misaligned DIFFERENTLY modulo 16 (element-granular counts, e.g. odd bf16 counts): copy
-// with aligned 16-byte accesses on both sides anyway -- every destination vector is assembled from the two aligned
-// source vectors that straddle it with a funnel shift.  dst must be 16-byte aligned here and m = src % 16 in 1..15.
-// The second source vector of the last destination vector always holds at least one needed byte (m >= 1), so no
-// load touches a 16-byte chunk without valid data.  (Measured, R = 16, 360 MB each way: odd bf16 counts 3.31 ->
-// 3.74 TB/s, odd byte counts 2.11 -> 3.67 TB/s against 1/2/4/8-byte units.)
+// ---- vector list: shared memory -> global with any alignment --------------------------------------------------
+// Destination vector j (16-byte aligned) = bytes [sh + 16 j, sh + 16 j + 16) of the aligned shared-memory image:
+// the two aligned 16-byte words that straddle it, joined with a funnel shift (sh = 4*wsel + bsh/8, warp-uniform).
 __device__ __forceinline__ uint4 shift_join(const uint4& a, const uint4& b, const int wsel, const int bsh) {
     const unsigned int w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
     uint4 o;
@@ -391,78 +390,67 @@ __device__ __forceinline__ uint4 shift_join(const uint4& a, const uint4& b, cons
     return o;
 }
 
-__device__ __forceinline__ void warp_copy_shifted(const unsigned char* src, unsigned char* dst, const long long nvec) {
-    constexpr int U = 4;
-    const int m = (int)((unsigned long long)src & 15ull);
-    const int wsel = m >> 2, bsh = (m & 3) * 8;
-    const uint4* sa = reinterpret_cast<const uint4*>(src - m);             // aligned down
-    uint4* d = reinterpret_cast<uint4*>(dst);
-    long long i = lane_id();
-    for (; i + (U - 1) * 32 < nvec; i += U * 32) {
-        uint4 a[U], b[U];
+// One warp: write `len` bytes to global `dst` (any alignment) from the shared-memory image `sm` (16-byte aligned) of
+// the aligned source span that holds them from byte offset ms (0..15) on.  Head and tail (< 16 bytes each) go byte
+// by byte, the body as aligned 16-byte stores; every shared-memory word read lies inside the loaded span
+// [0, align16(ms + len)) (the second word of a join is only read when it holds a needed byte: sh >= 1).
+__device__ __forceinline__ void warp_drain_shifted(unsigned char* dst, const unsigned char* sm, const unsigned int ms, const unsigned int len) {
+    const unsigned int lane = (unsigned int)lane_id();
+    unsigned int hb = (16u - (unsigned int)((unsigned long long)dst & 15ull)) & 15u;
+    if (hb > len) hb = len;
+    if (lane < hb) dst[lane] = sm[ms + lane];
+    const unsigned int pos = ms + hb;                  // shared-memory offset of the first body byte
+    const unsigned int nvec = (len - hb) >> 4;
+    const unsigned int sh = pos & 15u;
+    const uint4* sv = reinterpret_cast<const uint4*>(sm) + (pos >> 4);
+    uint4* dv = reinterpret_cast<uint4*>(dst + hb);
+    constexpr unsigned int U = 4;
+    if (sh == 0) {
+        for (unsigned int i = lane; i < nvec; i += 32 * U) {
+            uint4 v[U];
 #pragma unroll
-        for (int j = 0; j < U; ++j) { a[j] = ld_stream_nc(sa + i + j * 32); b[j] = ld_stream_nc(sa + i + j * 32 + 1); }
+            for (unsigned int u = 0; u < U; ++u) if (i + 32 * u < nvec) v[u] = sv[i + 32 * u];
 #pragma unroll
-        for (int j = 0; j < U; ++j) st_stream(d + i + j * 32, shift_join(a[j], b[j], wsel, bsh));
+            for (unsigned int u = 0; u < U; ++u) if (i + 32 * u < nvec) st_stream(dv + i + 32 * u, v[u]);
+        }
+    } else {
+        const int wsel = (int)(sh >> 2), bsh = (int)(sh & 3u) * 8;
+        for (unsigned int i = lane; i < nvec; i += 32 * U) {
+            uint4 a[U], b[U];
+#pragma unroll
+            for (unsigned int u = 0; u < U; ++u) if (i + 32 * u < nvec) { a[u] = sv[i + 32 * u]; b[u] = sv[i + 32 * u + 1]; }
+#pragma unroll
+            for (unsigned int u = 0; u < U; ++u) if (i + 32 * u < nvec) st_stream(dv + i + 32 * u, shift_join(a[u], b[u], wsel, bsh));
+        }
     }
-    for (; i < nvec; i += 32) st_stream(d + i, shift_join(ld_stream_nc(sa + i), ld_stream_nc(sa + i + 1), wsel, bsh));
+    const unsigned int done = hb + (nvec << 4);
+    if (lane < len - done) dst[done + lane] = sm[ms + done + lane];          // tail < 16
 }
 
-// Copy len bytes src -> dst with one warp; any alignment.
-__device__ __forceinline__ void warp_copy_bytes(const unsigned char* src, unsigned char* dst, long long len) {
-    const unsigned int diff = (unsigned int)(((unsigned long long)src ^ (unsigned long long)dst) & 15ull);
-    if (diff != 0 && len >= 64) {          // differing misalignment: aligned vectors + funnel shift
-        long long head = (long long)((16 - (int)((unsigned long long)dst & 15ull)) & 15);
-        if (lane_id() < head) dst[lane_id()] = __ldg(src + lane_id());
-        src += head; dst += head; len -= head;
-        const long long nvec = len >> 4;
-        warp_copy_shifted(src, dst, nvec);
-        const long long done = nvec << 4;
-        const int tail = (int)(len - done);                                // < 16
-        if (lane_id() < tail) dst[done + lane_id()] = __ldg(src + done + lane_id());
-        return;
-    }
-    const int g = diff == 0 ? 16 : (int)(diff & (0u - diff));          // common alignment granule
-    long long head = (long long)((g - (int)((unsigned long long)dst & (unsigned long long)(g - 1))) & (g - 1));
-    if (head > len) head = len;
-    if (lane_id() < head) dst[lane_id()] = __ldg(src + lane_id());    // head < 16 <= 32 lanes
-    src += head; dst += head; len -= head;
-    const long long units = len / g;
-    switch (g) {
-    case 16: warp_copy_units<uint4, 8>(src, dst, units); break;
-    case 8:  warp_copy_units<uint2, 8>(src, dst, units); break;
-    case 4:  warp_copy_units<unsigned int, 8>(src, dst, units); break;
-    case 2:  warp_copy_units<unsigned short, 8>(src, dst, units); break;
-    default: warp_copy_units<unsigned char, 8>(src, dst, units); break;
-    }
-    const long long done = units * g;
-    const int tail = (int)(len - done);                                // < 16
-    if (lane_id() < tail) dst[done + lane_id()] = __ldg(src + done + lane_id());
+#ifdef XDEV_TIMELINE
+enum { TL_ENTER = 0, TL_READY, TL_FIRST_LOAD, TL_FIRST_STORE, TL_LAST_STORE, TL_DRAINED, TL_EXIT, TL_TILES, TL_COUNT };
+__device__ __forceinline__ unsigned long long tl_now() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
 }
+#define TL_STAMP(tl, k) do { if (tl) (tl)[k] = tl_now(); } while (0)
+#define TL_STAMP_ONCE(tl, k) do { if ((tl) && (tl)[k] == 0ull) (tl)[k] = tl_now(); } while (0)
+#else
+#define TL_STAMP(tl, k) do { } while (0)
+#define TL_STAMP_ONCE(tl, k) do { } while (0)
+#endif
 
 // ================= bulk engine: byte-granular TMA ring driven by one elected lane (one warp) ========
 // The ring is a circular BYTE buffer (not fixed-size stages): every tile takes exactly
 // align128(len) bytes, so short tiles (config 5: 10-28 KiB) keep as many bytes in flight as
 // long ones.  Up to COPY_SLOTS tiles are outstanding; slot j's bookkeeping (destination,
 // length, smem offset, virtual start) lives in the registers of lane j.
-// A store's ring bytes are reclaimed with cp.async.bulk.wait_group.read: after a store is issued the engine
-// waits until at most maxPending (1..8) stores still read shared memory.
-__device__ __forceinline__ void bulk_release_oldest(int pending) {   // lane 0; pending = stores not yet known to be read (1..8)
-    switch (pending) {
-    case 1: bulk_wait_read<0>(); break;
-    case 2: bulk_wait_read<1>(); break;
-    case 3: bulk_wait_read<2>(); break;
-    case 4: bulk_wait_read<3>(); break;
-    case 5: bulk_wait_read<4>(); break;
-    case 6: bulk_wait_read<5>(); break;
-    case 7: bulk_wait_read<6>(); break;
-    default: bulk_wait_read<7>(); break;
-    }
-}
-
+// A store's ring bytes are reclaimed with cp.async.bulk.wait_group.read as soon as the NEXT store has been issued
+// (keeping up to 8 stores unreclaimed was measured 10 % slower on config 5: the ring is for LOADS in flight).
 template <bool SM>
 __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned char* ring, unsigned long long* mbar,
-                                            const unsigned int ringBytes, const int maxPending) {
+                                            const unsigned int ringBytes, unsigned long long* tl) {
     const int lane = lane_id();
     const unsigned int tileBytes = 1u << cur.tileShift;
     const uint32_t ring0 = smem_u32(ring);
@@ -492,6 +480,7 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
                     const uint32_t bar = smem_u32(&mbar[slot]);
                     mbar_expect_tx(bar, len16);
                     bulk_g2s(ring0 + po, srcp, len16, bar);
+                    TL_STAMP_ONCE(tl, TL_FIRST_LOAD);
                 }
                 const unsigned int adv = (len16 + 127u) & ~127u;
                 vHead = vStart + adv;
@@ -500,7 +489,7 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
                 ++iLoad;
             }
             const int tail = (int)(len & 15u);        // only the last tile of a ragged segment
-            if (lane < tail) dstp[len16 + lane] = __ldg(srcp + len16 + lane);
+            if (lane < tail) dstp[len16 + lane] = srcp[len16 + lane];
             cur.next();
             more = cur.ensure();
         }
@@ -522,28 +511,97 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
         if (lane == 0) {
             bulk_s2g(reinterpret_cast<void*>(((unsigned long long)dhi << 32) | dlo), ring0 + soff, slen);
             bulk_commit();
+            TL_STAMP_ONCE(tl, TL_FIRST_STORE);
+            TL_STAMP(tl, TL_LAST_STORE);
         }
         ++iStore;
-        while (iStore - freed > maxPending) {                     // at most maxPending stores keep ring bytes
-            if (lane == 0) bulk_release_oldest(iStore - freed);
+        if (iStore - freed > 1) {                                 // at most ONE store keeps its ring bytes: reclaim the older one
+            if (lane == 0) bulk_wait_read<1>();
             ++freed;
         }
         __syncwarp();
     }
-    if (lane == 0) bulk_wait_all<0>();
+    if (lane == 0) { bulk_wait_all<0>(); TL_STAMP(tl, TL_DRAINED); }
 }
 
-// ================= vector engine: one warp per tile ===========================================
+// ================= vector engine: one warp, its own share of the ring, TMA loads + warp stores ================
+// The engine walks its tiles in pieces of at most VEC_SUB_BYTES; the first piece of a tile ends where the
+// DESTINATION reaches a 16-byte boundary, so every later piece of the tile starts destination-aligned and only the
+// tile's ends need byte stores.  For a piece [s, s+len) of the source, the TMA loads the aligned span
+// [s & ~15, align16(s + len)) -- cp.async.bulk needs 16-byte aligned addresses and sizes, not aligned SEGMENTS;
+// the up-to-15 bytes read on either side share a 16-byte word with valid data, so they lie inside the caller's
+// allocation.  Up to VEC_SLOTS pieces are in flight per engine (bookkeeping in lanes 0..15, as in the bulk engine),
+// also across tile and segment boundaries.  A landed piece is moved to the destination by the whole warp
+// (warp_drain_shifted); its ring bytes are free as soon as the warp has read them.
 template <bool SM>
-__device__ __forceinline__ void vector_engine(Cursor<LIST_VEC, SM>& cur) {
-    const long long tileBytes = 1ll << cur.tileShift;
-    while (cur.ensure()) {
-        const long long off = cur.tile_off();
-        const long long rest = cur.bytes - off;
-        const long long len = rest < tileBytes ? rest : tileBytes;
-        warp_copy_bytes(reinterpret_cast<const unsigned char*>(cur.src + off),
-                        reinterpret_cast<unsigned char*>(cur.dst + off), len);
-        cur.next();
+__device__ __forceinline__ void vector_engine(Cursor<LIST_VEC, SM>& cur, unsigned char* ring, unsigned long long* mbar,
+                                              const unsigned int ringBytes) {
+    const int lane = lane_id();
+    const unsigned int tileBytes = 1u << cur.tileShift;
+    const uint32_t ring0 = smem_u32(ring);
+    unsigned long long mDst = 0;          // slot registers (lane j <-> slot j, j < VEC_SLOTS)
+    unsigned int mLen = 0, mOff = 0, mMs = 0, mV = 0;
+    unsigned int vHead = 0, phys = 0;
+    int iLoad = 0, iStore = 0;
+    unsigned int sub = 0;                 // bytes of the current tile already issued
+    bool more = cur.ensure();
+    while (true) {
+        while (more) {
+            const long long toff = cur.tile_off();
+            const long long rest = cur.bytes - toff;
+            const unsigned int tlen = rest < (long long)tileBytes ? (unsigned int)rest : tileBytes;
+            const unsigned long long s = cur.src + (unsigned long long)toff + sub;
+            const unsigned long long d = cur.dst + (unsigned long long)toff + sub;
+            unsigned int len = VEC_SUB_BYTES - (unsigned int)(d & 15ull);
+            if (len > tlen - sub) len = tlen - sub;
+            if (len < VEC_DIRECT_MAX) {                            // tiny piece: lanes copy it directly
+                const unsigned char* sp = reinterpret_cast<const unsigned char*>(s);
+                unsigned char* dp = reinterpret_cast<unsigned char*>(d);
+                for (unsigned int b = lane; b < len; b += 32) dp[b] = sp[b];
+            } else {
+                const unsigned int ms = (unsigned int)(s & 15ull);
+                const unsigned int ld = (ms + len + 15u) & ~15u;
+                const unsigned int pad = phys + ld > ringBytes ? ringBytes - phys : 0u;   // wrap
+                const unsigned int vTail = iStore < iLoad ? __shfl_sync(0xffffffffu, mV, iStore % VEC_SLOTS) : vHead;
+                if (iLoad - iStore >= VEC_SLOTS || vHead + pad + ld - vTail > ringBytes) break;   // drain a landed piece first
+                const unsigned int vStart = vHead + pad;
+                const unsigned int po = pad ? 0u : phys;
+                const int slot = iLoad % VEC_SLOTS;
+                if (lane == slot) { mDst = d; mLen = len; mOff = po; mMs = ms; mV = vStart; }
+                if (lane == 0) {
+                    const uint32_t bar = smem_u32(&mbar[slot]);
+                    mbar_expect_tx(bar, ld);
+                    bulk_g2s(ring0 + po, reinterpret_cast<const void*>(s - ms), ld, bar);
+                }
+                const unsigned int adv = (ld + 127u) & ~127u;
+                vHead = vStart + adv;
+                phys = po + adv;
+                if (phys >= ringBytes) phys = 0;
+                ++iLoad;
+            }
+            sub += len;
+            if (sub >= tlen) {
+                sub = 0;
+                cur.next();
+                more = cur.ensure();
+            }
+        }
+        if (iStore == iLoad) {
+            if (!more) break;
+            phys = 0;                      // nothing in flight: restart the ring at offset 0 (the piece did not fit behind phys)
+            continue;
+        }
+        const int slot = iStore % VEC_SLOTS;
+        mbar_wait(smem_u32(&mbar[slot]), (uint32_t)((iStore / VEC_SLOTS) & 1));
+        const unsigned int dlo = __shfl_sync(0xffffffffu, (unsigned int)mDst, slot);
+        const unsigned int dhi = __shfl_sync(0xffffffffu, (unsigned int)(mDst >> 32), slot);
+        const unsigned int slen = __shfl_sync(0xffffffffu, mLen, slot);
+        const unsigned int soff = __shfl_sync(0xffffffffu, mOff, slot);
+        const unsigned int sms = __shfl_sync(0xffffffffu, mMs, slot);
+        warp_drain_shifted(reinterpret_cast<unsigned char*>(((unsigned long long)dhi << 32) | dlo), ring + soff, sms, slen);
+        ++iStore;
+        __syncwarp();                      // every lane has read its words before the TMA may overwrite them
+        if (lane == 0) fence_proxy_async_smem();
     }
 }
 
@@ -562,28 +620,71 @@ __device__ __forceinline__ void workctl_checkout(WorkCtl* ctl, bool used) {
     }
 }
 
-// Number of bulk engine warps when the host leaves the choice to the device (grid-uniform: depends only on the
-// work list's totals).  A short call (few tiles per SM) is bound by the per-tile latency of one elected lane --
-// measured: R = 64 with one 10 KB row per pair takes 40 us with one engine and 27 us with four -- while a long
-// one is HBM-bound and slightly better off with one deep ring (config 3: -0.7 % with two engines).
-// When most of the work is on the vector list (unaligned traffic) the warps stay vector engines.
-__device__ __forceinline__ int choose_bulk_engines(int requested, int totalTiles, int vecTiles, int grid, unsigned int ringBytes,
-                                                   int tileShift) {
-    int E = requested;
-    if (E == 0) E = vecTiles > totalTiles ? 1 : (totalTiles <= 48 * grid ? 4 : (totalTiles <= 96 * grid ? 2 : 1));
-    while (E > 1 && (1u << tileShift) > ((ringBytes / (unsigned int)E) & ~127u)) E >>= 1;    // a tile must fit in one share
-    return E;
+// How a CTA's 16 warps and its ring are divided between the two work lists -- grid-uniform: depends only on the
+// lists' tile totals.
+//   * no vector tiles: E bulk engines share the whole ring.  E = 4 for a call of few tiles per SM (bound by the
+//     per-tile latency of one elected lane -- measured: R = 64 with one 10 KB row per pair takes 40 us with one
+//     engine and 27 us with four), 2 up to 96 tiles per SM, else 1 (HBM-bound: one deep ring is slightly better,
+//     config 3: -0.7 % with two engines);
+//   * no bulk tiles: all 16 warps are vector engines with 1/16 of the ring each;
+//   * both: the vector engines get one 1/16 unit each, as many as their share of the bytes (1..9), the bulk engines
+//     the rest (>= 7/16 of the ring, which the host sized the bulk tile for).
+struct RingPlan {
+    int E, NV;                             // bulk engines = warps [0, E), vector engines = warps [E, E + NV)
+    unsigned int bulkShare, vecShare;      // ring bytes per bulk / per vector engine (multiples of 128)
+    unsigned int vecBase;                  // ring offset of vector engine 0's share
+};
+__device__ __forceinline__ RingPlan plan_ring(int requestedE, int bulkTiles, int vecTiles, int grid, unsigned int ringBytes,
+                                              int bulkShift, int vecShift) {
+    RingPlan p;
+    const unsigned int unit = (ringBytes / COPY_WARPS) & ~127u;
+    unsigned int bulkBytes = ringBytes;
+    p.NV = 0;
+    if (vecTiles > 0) {
+        if (bulkTiles == 0) { p.NV = COPY_WARPS; bulkBytes = 0; }
+        else {
+            const long long wb = (long long)bulkTiles << bulkShift, wv = (long long)vecTiles << vecShift;
+            p.NV = (int)((wv * COPY_WARPS + (wb + wv) / 2) / (wb + wv));
+            p.NV = max(1, min(VEC_MAX_IN_BULK_MIX, p.NV));
+            bulkBytes = ringBytes - (unsigned int)p.NV * unit;
+        }
+    }
+    int E = 0;
+    if (bulkTiles > 0) {
+        E = requestedE;
+        if (E == 0) E = bulkTiles <= 48 * grid ? 4 : (bulkTiles <= 96 * grid ? 2 : 1);
+        while (E > 1 && (1u << bulkShift) > ((bulkBytes / (unsigned int)E) & ~127u)) E >>= 1;    // a tile must fit in one share
+        if (E + p.NV > COPY_WARPS) E = COPY_WARPS - p.NV;
+    }
+    p.E = E;
+    p.bulkShare = E ? (bulkBytes / (unsigned int)E) & ~127u : 0u;
+    p.vecShare = unit;
+    p.vecBase = bulkBytes & ~127u;
+    return p;
 }
 
-// First chunk of every engine is static (chunk e to engine e; see Cursor::init); a positive staticEighths
-// instead assigns that share of ALL tiles as contiguous static ranges (kept for A/B runs).
-__device__ __forceinline__ int static_first_chunk(int total, int nEngines, int kmax, int kmaxLong, int RR, int eighths) {
-    if (eighths > 0) return (int)(((long long)total * eighths / 8) / nEngines);
+// First chunk of every engine is static (chunk e to engine e; see Cursor::init).
+__device__ __forceinline__ int static_first_chunk(int total, int nEngines, int kmax, int kmaxLong, int RR) {
+    if (nEngines <= 0) return 0;
     const int km = total >= 8 * RR ? kmaxLong : kmax;
     return max(1, min(km, total / (4 * nEngines)));
 }
 
-// dynamic smem layout: [ring: ringBytes][mbar: COPY_MAX_ENGINES x COPY_SLOTS x u64][colBase bulk: R+1 ints][colBase vec: R+1 ints]
+// Side job (see SideJob): warps [firstWarp, 16) of every CTA, before their engine role.
+__device__ __forceinline__ void run_side_job(const SideJob& j, int firstWarp) {
+    const int warp = threadIdx.x >> 5;
+    if (!j.dst || warp < firstWarp) return;
+    const long long nthreads = (long long)gridDim.x * (COPY_WARPS - firstWarp) * 32;
+    const long long tid = ((long long)blockIdx.x * (COPY_WARPS - firstWarp) + (warp - firstWarp)) * 32 + lane_id();
+    for (long long i = tid; i < j.n; i += nthreads) {
+        long long v = j.src[i];
+        v = v > 0 ? v : 0;
+        long long* out = j.dst + i;
+        for (int c = 0; c < j.copies; ++c) out[(long long)c * j.n] = v;
+    }
+}
+
+// dynamic smem layout: [ring: ringBytes][mbar: COPY_MBAR_COUNT x u64][colBase bulk: R+1 ints][colBase vec: R+1 ints]
 //                      [coarse bulk: R*nb ints][coarse vec: R*nb ints]   (the last two only if useCoarse)
 __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const CopyArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -592,23 +693,28 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
     const int R = a.ncols;
     unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + a.ringBytes);
     int* colBase[2];
-    colBase[0] = reinterpret_cast<int*>(mbar + COPY_MAX_ENGINES * COPY_SLOTS);
+    colBase[0] = reinterpret_cast<int*>(mbar + COPY_MBAR_COUNT);
     colBase[1] = colBase[0] + (R + 1);
     const int nbR = R * coarse_blocks(a.colLen);
     int* coarse[2] = {nullptr, nullptr};
     if (a.useCoarse) { coarse[0] = colBase[1] + (R + 1); coarse[1] = coarse[0] + nbR; }
+#ifdef XDEV_TIMELINE
+    unsigned long long* tl = (a.timeline && threadIdx.x == 0) ? a.timeline + (size_t)blockIdx.x * TL_COUNT : nullptr;
+    if (tl) { for (int i = 0; i < TL_COUNT; ++i) tl[i] = 0ull; }
+#else
+    unsigned long long* tl = nullptr;
+#endif
+    TL_STAMP(tl, TL_ENTER);
 
-    // ---- prologue: mbarrier init (overlaps the counts kernel under PDL), then cross-column tile
-    //      bases = scan of the R per-column totals the counts kernel wrote, and the coarse indexes ----
+    // ---- prologue: mbarrier init (overlaps the metadata kernel under PDL), then cross-column tile
+    //      bases = scan of the R per-column totals the metadata kernel wrote, and the coarse indexes ----
     griddep_launch_dependents();           // the next call's metadata kernel may become resident (it waits for us)
-    if (threadIdx.x >= 64 && threadIdx.x < 64 + COPY_MAX_ENGINES * COPY_SLOTS) {
-        mbar_init(smem_u32(&mbar[threadIdx.x - 64]), 1);
-        fence_mbar_init();
-    }
+    for (int i = threadIdx.x; i < COPY_MBAR_COUNT; i += COPY_THREADS) mbar_init(smem_u32(&mbar[i]), 1);
+    fence_mbar_init();
     griddep_wait();
     if (a.useCoarse && warp >= 2) {
         for (int i = threadIdx.x - 64; i < 2 * nbR; i += COPY_THREADS - 64)
-            coarse[0][i] = i < nbR ? __ldg(a.coarse[0] + i) : __ldg(a.coarse[1] + (i - nbR));
+            coarse[0][i] = i < nbR ? a.coarse[0][i] : a.coarse[1][i - nbR];
     }
     if (warp < 2) {
         const int* ct = warp ? a.colTiles[1] : a.colTiles[0];
@@ -623,27 +729,33 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
         }
     }
     __syncthreads();
+    TL_STAMP(tl, TL_READY);
 
-    const int E = choose_bulk_engines(a.bulkEngines, colBase[LIST_BULK][R], colBase[LIST_VEC][R], (int)gridDim.x, a.ringBytes,
-                                      a.cls.tileShift[LIST_BULK]);
-    const int NV = COPY_THREADS / 32 - E;              // vector engines per CTA
-    const int nB = (int)gridDim.x * E, nV = (int)gridDim.x * NV;
-    const unsigned int subRing = (a.ringBytes / (unsigned int)E) & ~127u;
+    const int totB = colBase[LIST_BULK][R], totV = colBase[LIST_VEC][R];
+    const RingPlan rp = plan_ring(a.bulkEngines, totB, totV, (int)gridDim.x, a.ringBytes, a.cls.tileShift[LIST_BULK],
+                                  a.cls.tileShift[LIST_VEC]);
+    const int nB = (int)gridDim.x * rp.E, nV = (int)gridDim.x * rp.NV;
     const int RR = a.ncols * a.colLen;
-    const int stB = static_first_chunk(colBase[LIST_BULK][R], nB, a.kmax[LIST_BULK], a.kmaxLong, RR, a.staticEighths);
-    const int stV = static_first_chunk(colBase[LIST_VEC][R], nV, a.kmax[LIST_VEC], a.kmaxLong, RR, a.staticEighths);
-    if (warp < E) {
+    const int stB = static_first_chunk(totB, nB, a.kmax, COPY_KMAX_LONG, RR);
+    const int stV = static_first_chunk(totV, nV, COPY_KMAX_VEC, COPY_KMAX_LONG, RR);
+#ifdef XDEV_TIMELINE
+    if (tl) tl[TL_TILES] = (unsigned long long)totB;
+#endif
+    run_side_job(a.side, COPY_WARPS / 2);
+    if (warp < rp.E) {
         Cursor<LIST_BULK> cur;
         cur.init(a.desc, colBase[LIST_BULK], coarse[LIST_BULK], &a.ctl->next[LIST_BULK], a.cls, a.ncols, a.colLen, nB,
-                 (int)blockIdx.x * E + warp, a.kmax[LIST_BULK], a.kmaxLong, stB);
-        bulk_engine<false>(cur, smem + (size_t)warp * subRing, mbar + warp * COPY_SLOTS, subRing, a.maxPendingStores);
-    } else {
+                 (int)blockIdx.x * rp.E + warp, a.kmax, COPY_KMAX_LONG, stB);
+        bulk_engine<false>(cur, smem + (size_t)warp * rp.bulkShare, mbar + warp * COPY_SLOTS, rp.bulkShare, warp == 0 ? tl : nullptr);
+    } else if (warp < rp.E + rp.NV) {
+        const int v = warp - rp.E;
         Cursor<LIST_VEC> cur;
         cur.init(a.desc, colBase[LIST_VEC], coarse[LIST_VEC], &a.ctl->next[LIST_VEC], a.cls, a.ncols, a.colLen, nV,
-                 (int)blockIdx.x * NV + warp - E, a.kmax[LIST_VEC], a.kmaxLong, stV);
-        vector_engine<false>(cur);
+                 (int)blockIdx.x * rp.NV + v, COPY_KMAX_VEC, COPY_KMAX_LONG, stV);
+        vector_engine<false>(cur, smem + rp.vecBase + (size_t)v * rp.vecShare, mbar + COPY_MAX_ENGINES * COPY_SLOTS + v * VEC_SLOTS, rp.vecShare);
     }
-    workctl_checkout(a.ctl, colBase[LIST_BULK][R] > stB * nB || colBase[LIST_VEC][R] > stV * nV);
+    workctl_checkout(a.ctl, totB > stB * nB || totV > stV * nV);
+    TL_STAMP(tl, TL_EXIT);
 }
 
-}  // namespace ncclx
+}  // namespace xdev

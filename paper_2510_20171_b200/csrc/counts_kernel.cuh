@@ -20,15 +20,15 @@
 #pragma once
 #include "common.cuh"
 
-namespace ncclx {
+namespace xdev {
 
 constexpr int COUNTS_THREADS = 512;
 constexpr int COUNTS_ROWS_PER_PASS = 8;
 constexpr int COUNTS_COLS_UNROLL = 4;     // x32 lanes = 128 prefix columns per pass
 
 struct CountsArgs {
-    const void* const* send;      // device table
-    void* const* recv;            // device table
+    const void* const* send;      // device table (null: no descriptors wanted, offsets and RC only)
+    void* const* recv;            // device table (null likewise)
     const long long* C;           // R*R, by reference
     long long* RC;                // R*R out
     Workspace ws;
@@ -64,9 +64,9 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
 #pragma unroll
     for (int i = 0; i < PT; ++i) {
         const int s = threadIdx.x + i * COUNTS_THREADS;
-        sp[i] = s < R ? (unsigned long long)a.send[s] : 0ull;
+        sp[i] = (s < R && a.send) ? (unsigned long long)a.send[s] : 0ull;        // null tables: offsets only (top-k calls)
     }
-    const unsigned long long rp = threadIdx.x < Wc ? (unsigned long long)a.recv[d0 + threadIdx.x] : 0ull;
+    const unsigned long long rp = (threadIdx.x < Wc && a.recv) ? (unsigned long long)a.recv[d0 + threadIdx.x] : 0ull;
     bool parked = false;
 
     // ---- phase 1: warp per group of RB source rows: soff for the owned columns ---------------
@@ -177,4 +177,4 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
     }
 }
 
-}  // namespace ncclx
+}  // namespace xdev

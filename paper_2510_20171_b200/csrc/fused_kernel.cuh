@@ -19,7 +19,7 @@
 #pragma once
 #include "copy_kernel.cuh"
 
-namespace ncclx {
+namespace xdev {
 
 constexpr int FUSED_MAX_R = 32;            // R*R <= 1024 descriptors = 32 KB of shared memory
 
@@ -35,8 +35,7 @@ struct FusedArgs {
     int R;
     long long elemSize;
     unsigned int ringBytes;                // multiple of 128, >= 32 KB (the prologue's scratch aliases the ring)
-    int kmax[2];
-    int kmaxLong;
+    int kmax;                              // as CopyArgs::kmax
     int minTileShift[2];
     int bulkEngines;                       // as CopyArgs::bulkEngines
     ClassParams cls;                       // tileShift[] = upper bounds; the kernel picks the actual shifts
@@ -49,7 +48,7 @@ __host__ __device__ inline size_t fused_aux_bytes(int R) { return fused_desc_off
 
 __device__ __forceinline__ int floor_log2_ll(long long v) { return v <= 0 ? 0 : 63 - __clzll(v); }
 
-// dynamic smem: [ring: ringBytes][mbar: COPY_MAX_ENGINES x COPY_SLOTS x u64][colBase bulk: R+1][colBase vec: R+1][pad][SegDesc R*R]
+// dynamic smem: [ring: ringBytes][mbar: COPY_MBAR_COUNT x u64][colBase bulk: R+1][colBase vec: R+1][pad][SegDesc R*R]
 __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const FusedArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = lane_id();
@@ -58,7 +57,7 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
     const int R = a.R, RR = R * R;
     unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + a.ringBytes);
     int* colBase[2];
-    colBase[0] = reinterpret_cast<int*>(mbar + COPY_MAX_ENGINES * COPY_SLOTS);
+    colBase[0] = reinterpret_cast<int*>(mbar + COPY_MBAR_COUNT);
     colBase[1] = colBase[0] + (R + 1);
     SegDesc* sdesc = reinterpret_cast<SegDesc*>(smem + a.ringBytes + fused_desc_offset(R));
     // prologue scratch, dead before the first TMA load lands in the ring (<= 17.3 KB at R = 32)
@@ -73,10 +72,8 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
     const bool writer = blockIdx.x == 0;
 
     griddep_launch_dependents();           // a following call of this library may start its prologue
-    if (threadIdx.x >= 64 && threadIdx.x < 64 + COPY_MAX_ENGINES * COPY_SLOTS) {
-        mbar_init(smem_u32(&mbar[threadIdx.x - 64]), 1);
-        fence_mbar_init();
-    }
+    for (int i = threadIdx.x; i < COPY_MBAR_COUNT; i += COPY_THREADS) mbar_init(smem_u32(&mbar[i]), 1);
+    fence_mbar_init();
     griddep_wait();                        // everything below reads what the stream's previous kernel wrote
 
     // ---- step 0: the whole count matrix and both pointer tables -> shared memory (one round trip) -----
@@ -107,18 +104,16 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
     long long totalElems = 0;
     for (int s = 0; s < R; ++s) totalElems += rowTot[s];
     const long long totalBytes = totalElems * a.elemSize;
-    // engines from the byte total (same regimes as choose_bulk_engines: up to 48 / 96 maximum-size tiles per CTA)
-    int E = a.bulkEngines;
-    if (E == 0) {
+    // about two tiles per engine, assuming the engine split of a call that is all on one list (E bulk engines by the
+    // regimes of plan_ring: up to 48 / 96 maximum-size tiles per CTA; 16 vector engines)
+    int E0 = a.bulkEngines;
+    if (E0 == 0) {
         const long long maxTiles = totalBytes >> a.cls.tileShift[LIST_BULK];
-        E = maxTiles <= 48ll * gridDim.x ? 4 : (maxTiles <= 96ll * gridDim.x ? 2 : 1);
+        E0 = maxTiles <= 48ll * gridDim.x ? 4 : (maxTiles <= 96ll * gridDim.x ? 2 : 1);
     }
-    while (E > 1 && (1u << a.cls.tileShift[LIST_BULK]) > ((a.ringBytes / (unsigned int)E) & ~127u)) E >>= 1;
-    int NV = NW - E;
-    int nB = (int)gridDim.x * E, nV = (int)gridDim.x * NV;
     ClassParams cls = a.cls;
-    cls.tileShift[LIST_BULK] = max(a.minTileShift[LIST_BULK], min(a.cls.tileShift[LIST_BULK], floor_log2_ll(totalBytes / (2 * nB))));
-    cls.tileShift[LIST_VEC] = max(a.minTileShift[LIST_VEC], min(a.cls.tileShift[LIST_VEC], floor_log2_ll(totalBytes / (2 * nV))));
+    cls.tileShift[LIST_BULK] = max(a.minTileShift[LIST_BULK], min(a.cls.tileShift[LIST_BULK], floor_log2_ll(totalBytes / (2ll * gridDim.x * E0))));
+    cls.tileShift[LIST_VEC] = max(a.minTileShift[LIST_VEC], min(a.cls.tileShift[LIST_VEC], floor_log2_ll(totalBytes / (2ll * gridDim.x * COPY_WARPS))));
 
     // ---- step 3 (a1, a2, a3): warp per destination column: RC, roff, descriptors, tile prefixes ------
     for (int d = warp; d < R; d += NW) {
@@ -159,23 +154,23 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
     fence_proxy_async_smem();              // scratch reads/writes (generic proxy) before TMA writes to the same bytes
     __syncthreads();                       // the scratch is dead from here on; the ring may be filled
 
-    if (a.bulkEngines == 0 && colBase[LIST_VEC][R] > colBase[LIST_BULK][R]) {     // mostly unaligned traffic: keep the
-        E = 1; NV = NW - 1; nB = (int)gridDim.x; nV = (int)gridDim.x * NV;          // warps as vector engines
-    }
-    const unsigned int subRing = (a.ringBytes / (unsigned int)E) & ~127u;
+    const int totB = colBase[LIST_BULK][R], totV = colBase[LIST_VEC][R];
+    const RingPlan rp = plan_ring(a.bulkEngines, totB, totV, (int)gridDim.x, a.ringBytes, cls.tileShift[LIST_BULK], cls.tileShift[LIST_VEC]);
+    const int nB = (int)gridDim.x * rp.E, nV = (int)gridDim.x * rp.NV;
     // ---- a4: the copy engines of the big path, fed from shared memory --------------------------------
-    if (warp < E) {
+    if (warp < rp.E) {
         Cursor<LIST_BULK, true> cur;
-        cur.init(sdesc, colBase[LIST_BULK], nullptr, &a.ctl->next[LIST_BULK], cls, R, R, nB, (int)blockIdx.x * E + warp,
-                 a.kmax[LIST_BULK], a.kmaxLong, 1);
-        bulk_engine<true>(cur, smem + (size_t)warp * subRing, mbar + warp * COPY_SLOTS, subRing, 1);
-    } else {
+        cur.init(sdesc, colBase[LIST_BULK], nullptr, &a.ctl->next[LIST_BULK], cls, R, R, nB, (int)blockIdx.x * rp.E + warp,
+                 a.kmax, COPY_KMAX_LONG, 1);
+        bulk_engine<true>(cur, smem + (size_t)warp * rp.bulkShare, mbar + warp * COPY_SLOTS, rp.bulkShare, nullptr);
+    } else if (warp < rp.E + rp.NV) {
+        const int v = warp - rp.E;
         Cursor<LIST_VEC, true> cur;
-        cur.init(sdesc, colBase[LIST_VEC], nullptr, &a.ctl->next[LIST_VEC], cls, R, R, nV, (int)blockIdx.x * NV + warp - E,
-                 a.kmax[LIST_VEC], a.kmaxLong, 1);
-        vector_engine<true>(cur);
+        cur.init(sdesc, colBase[LIST_VEC], nullptr, &a.ctl->next[LIST_VEC], cls, R, R, nV, (int)blockIdx.x * rp.NV + v,
+                 COPY_KMAX_VEC, COPY_KMAX_LONG, 1);
+        vector_engine<true>(cur, smem + rp.vecBase + (size_t)v * rp.vecShare, mbar + COPY_MAX_ENGINES * COPY_SLOTS + v * VEC_SLOTS, rp.vecShare);
     }
-    workctl_checkout(a.ctl, colBase[LIST_BULK][R] > nB || colBase[LIST_VEC][R] > nV);
+    workctl_checkout(a.ctl, (nB > 0 && totB > nB) || (nV > 0 && totV > nV));
 }
 
-}  // namespace ncclx
+}  // namespace xdev

@@ -9,20 +9,22 @@
 #pragma once
 #include "common.cuh"
 
-namespace ncclx {
+namespace xdev {
 
-constexpr int PROBE_THREADS = 256;
+constexpr int PROBE_THREADS = 256;         // full-chip form: 8 CTAs per SM
+constexpr int PROBE_THREADS_FEW = 1024;    // few-CTA form (per-SM ceiling): one CTA fills an SM, 128 KB of loads in flight
 constexpr int PROBE_UNROLL = 4;
 
-__global__ void __launch_bounds__(PROBE_THREADS) stream_probe_kernel(int mode, const unsigned char* src, unsigned char* dst,
+template <int NT>
+__global__ void __launch_bounds__(NT) stream_probe_kernel(int mode, const unsigned char* src, unsigned char* dst,
                                                                       unsigned long long nvec, unsigned int* sink) {
-    const unsigned long long stride = (unsigned long long)gridDim.x * PROBE_THREADS * PROBE_UNROLL;
+    const unsigned long long stride = (unsigned long long)gridDim.x * NT * PROBE_UNROLL;
     unsigned int acc = 0;
-    for (unsigned long long base = (unsigned long long)blockIdx.x * PROBE_THREADS * PROBE_UNROLL; base < nvec; base += stride) {
+    for (unsigned long long base = (unsigned long long)blockIdx.x * NT * PROBE_UNROLL; base < nvec; base += stride) {
         u32x8 v[PROBE_UNROLL];
 #pragma unroll
         for (int u = 0; u < PROBE_UNROLL; ++u) {
-            const unsigned long long i = base + (unsigned long long)u * PROBE_THREADS + threadIdx.x;
+            const unsigned long long i = base + (unsigned long long)u * NT + threadIdx.x;
             if (mode != 1) {
                 if (i < nvec) v[u] = ld_stream256(src + i * 32);
             } else {
@@ -32,7 +34,7 @@ __global__ void __launch_bounds__(PROBE_THREADS) stream_probe_kernel(int mode, c
         }
 #pragma unroll
         for (int u = 0; u < PROBE_UNROLL; ++u) {
-            const unsigned long long i = base + (unsigned long long)u * PROBE_THREADS + threadIdx.x;
+            const unsigned long long i = base + (unsigned long long)u * NT + threadIdx.x;
             if (i < nvec) {
                 if (mode == 0) acc ^= v[u].lo.x ^ v[u].lo.y ^ v[u].lo.z ^ v[u].lo.w ^ v[u].hi.x ^ v[u].hi.y ^ v[u].hi.z ^ v[u].hi.w;
                 else st_stream256(dst + i * 32, v[u]);
@@ -59,4 +61,4 @@ __global__ void __launch_bounds__(128) stream_probe_bulk_store_kernel(unsigned c
     }
 }
 
-}  // namespace ncclx
+}  // namespace xdev

@@ -19,7 +19,7 @@
 #include <cuda_fp16.h>
 #include "common.cuh"
 
-namespace ncclx {
+namespace xdev {
 
 constexpr int REDUCE_THREADS = 128;
 enum { RED_BF16 = 0, RED_F32 = 1, RED_F16 = 2 };
@@ -208,6 +208,8 @@ __global__ void __launch_bounds__(REDUCE_THREADS) reduce_kernel(const ReduceArgs
     const int R = a.R;
     constexpr int ES = DT == RED_F32 ? 4 : 2;
 
+    griddep_launch_dependents();           // no-ops unless launched with programmatic stream serialisation (short calls)
+    griddep_wait();
     if (threadIdx.x == 0) sMis = 0;
     __syncthreads();
     int mis = 0;
@@ -250,10 +252,17 @@ __global__ void __launch_bounds__(REDUCE_THREADS) reduce_kernel(const ReduceArgs
 // `fwd` that the next peer will receive (ReduceCopy: "combine the reduction and forwarding copy ... avoids
 // redundant HBM load"; `out` may be NULL in the intermediate steps: "avoid unnecessary HBM stores"), or
 // both.  The message is processed in fixed chunks of S bytes (paper: 8 MB) by a FIXED, small number of
-// CTAs x 512 threads (paper: 2 CTAs suffice against the network): throughput per CTA comes from
-// instruction-level parallelism (L335), here RC_UNROLL independent 256-bit loads per input per thread.
+// CTAs (paper: 2 CTAs x 512 threads suffice against the network): throughput per CTA comes from
+// instruction-level parallelism (L335 "enhance instruction level parallelism to saturate GPU resources").
+// Two variants (NCCLX_PARAM_REDUCECOPY_TMA):
+//   reducecopy_kernel      512 threads, software-pipelined: the 2 x RC_UNROLL 256-bit loads of tile i+1 are issued
+//                          before the adds and stores of tile i (also across chunk boundaries), so the CTA never
+//                          alternates between a load phase and a store phase (round 1 did: 96 GB/s per CTA);
+//   reducecopy_tma_kernel  a producer warp streams `a` and `b` through a 6-stage shared-memory ring with
+//                          cp.async.bulk (192 KB in flight per CTA, no registers); 512 consumer threads add from
+//                          shared memory and store.
 constexpr int RC_THREADS = 512;
-constexpr int RC_UNROLL = 4;
+constexpr int RC_UNROLL = 2;
 
 struct ReduceCopyArgs {
     const unsigned char* a;
@@ -264,50 +273,107 @@ struct ReduceCopyArgs {
     unsigned long long chunkElems;
 };
 
+// Walks the message chunk by chunk (in order), and inside a chunk in tiles of `tileVecs` 32-byte vectors, tile index
+// blockIdx.x, += gridDim.x.  Vector path only (chunk bytes % 32 == 0).
+template <int ES>
+struct RcTileIt {
+    unsigned long long count, chunkElems, c0, t, nvec, tileVecs;
+    __device__ __forceinline__ void chunk_begin() {
+        const unsigned long long cn = min(chunkElems, count - c0);
+        nvec = cn / (32 / ES);
+        t = (unsigned long long)blockIdx.x * tileVecs;
+    }
+    __device__ __forceinline__ void init(const ReduceCopyArgs& p, unsigned long long tileVecs_) {
+        count = p.count; chunkElems = p.chunkElems; tileVecs = tileVecs_; c0 = 0;
+        chunk_begin();
+        settle();
+    }
+    __device__ __forceinline__ void settle() {             // skip chunks in which this CTA has no tile (left)
+        while (t >= nvec) {
+            c0 += chunkElems;
+            if (c0 >= count) return;
+            chunk_begin();
+        }
+    }
+    __device__ __forceinline__ bool valid() const { return c0 < count; }
+    __device__ __forceinline__ void advance() { t += (unsigned long long)gridDim.x * tileVecs; settle(); }
+    __device__ __forceinline__ unsigned long long byte_off() const { return c0 * ES + t * 32; }   // of the tile's first vector
+    __device__ __forceinline__ unsigned long long vecs() const { return min(tileVecs, nvec - t); }
+};
+
+template <int DT>
+__device__ __forceinline__ u32x8 rc_add(const u32x8& xa, const u32x8& xb) {
+    Acc<DT> lo, hi;
+    lo.set(xa.lo); hi.set(xa.hi);
+    lo.add(xb.lo); hi.add(xb.hi);
+    u32x8 o;
+    o.lo = lo.pack(); o.hi = hi.pack();
+    return o;
+}
+
+// elements after the last full 32-byte vector (only the last chunk can have any), scalar
+template <int DT>
+__device__ __forceinline__ void rc_ragged_tail(const ReduceCopyArgs& p, int tid) {
+    constexpr int ES = DT == RED_F32 ? 4 : 2;
+    constexpr int EPV = 32 / ES;
+    if (blockIdx.x != 0) return;
+    const unsigned long long lastC0 = ((p.count - 1) / p.chunkElems) * p.chunkElems;
+    const unsigned long long i = lastC0 + ((p.count - lastC0) / EPV) * EPV + tid;
+    if (i < p.count) {
+        const float acc = __fadd_rn(load_elem<DT>(p.a, i), load_elem<DT>(p.b, i));
+        if (p.out) store_elem<DT>(p.out, i, acc);
+        if (p.fwd) store_elem<DT>(p.fwd, i, acc);
+    }
+}
+
 template <int DT>
 __global__ void __launch_bounds__(RC_THREADS) reducecopy_kernel(const ReduceCopyArgs p) {
     constexpr int ES = DT == RED_F32 ? 4 : 2;
-    constexpr int EPV = 32 / ES;
     const bool vec = ((((unsigned long long)p.a | (unsigned long long)p.b | (unsigned long long)p.out |
                         (unsigned long long)p.fwd) & 31ull) == 0) && ((p.chunkElems * ES) & 31ull) == 0;
-    for (unsigned long long c0 = 0; c0 < p.count; c0 += p.chunkElems) {        // chunk by chunk, in order
-        const unsigned long long cn = min(p.chunkElems, p.count - c0);
-        if (vec) {
-            const unsigned long long nvec = cn / EPV;
-            const unsigned long long base = c0 * ES;
-            // a CTA's tile = RC_UNROLL x 512 vectors, interleaved so that every load instruction is coalesced
-            for (unsigned long long t = (unsigned long long)blockIdx.x * RC_THREADS * RC_UNROLL; t < nvec;
-                 t += (unsigned long long)gridDim.x * RC_THREADS * RC_UNROLL) {
-                u32x8 xa[RC_UNROLL], xb[RC_UNROLL];
+    if (vec) {
+        // a CTA's tile = RC_UNROLL x 512 vectors, interleaved so that every load instruction is coalesced
+        RcTileIt<ES> it;
+        it.init(p, (unsigned long long)RC_THREADS * RC_UNROLL);
+        u32x8 xa[RC_UNROLL], xb[RC_UNROLL];
+        unsigned long long off = 0, nv = 0;
+        if (it.valid()) {
+            off = it.byte_off(); nv = it.vecs();
+#pragma unroll
+            for (int u = 0; u < RC_UNROLL; ++u) {
+                const unsigned long long v = (unsigned long long)u * RC_THREADS + threadIdx.x;
+                if (v < nv) { xa[u] = ld_stream256(p.a + off + v * 32); xb[u] = ld_stream256(p.b + off + v * 32); }
+            }
+        }
+        while (it.valid()) {
+            it.advance();
+            u32x8 na[RC_UNROLL], nb[RC_UNROLL];
+            unsigned long long noff = 0, nnv = 0;
+            if (it.valid()) {                              // tile i+1's loads go out before tile i's adds and stores
+                noff = it.byte_off(); nnv = it.vecs();
 #pragma unroll
                 for (int u = 0; u < RC_UNROLL; ++u) {
-                    const unsigned long long v = t + (unsigned long long)u * RC_THREADS + threadIdx.x;
-                    if (v < nvec) { xa[u] = ld_stream256(p.a + base + v * 32); xb[u] = ld_stream256(p.b + base + v * 32); }
+                    const unsigned long long v = (unsigned long long)u * RC_THREADS + threadIdx.x;
+                    if (v < nnv) { na[u] = ld_stream256(p.a + noff + v * 32); nb[u] = ld_stream256(p.b + noff + v * 32); }
                 }
+            }
 #pragma unroll
-                for (int u = 0; u < RC_UNROLL; ++u) {
-                    const unsigned long long v = t + (unsigned long long)u * RC_THREADS + threadIdx.x;
-                    if (v < nvec) {
-                        Acc<DT> lo, hi;
-                        lo.set(xa[u].lo); hi.set(xa[u].hi);
-                        lo.add(xb[u].lo); hi.add(xb[u].hi);
-                        u32x8 o;
-                        o.lo = lo.pack(); o.hi = hi.pack();
-                        if (p.out) st_stream256(p.out + base + v * 32, o);
-                        if (p.fwd) st_stream256(p.fwd + base + v * 32, o);
-                    }
+            for (int u = 0; u < RC_UNROLL; ++u) {
+                const unsigned long long v = (unsigned long long)u * RC_THREADS + threadIdx.x;
+                if (v < nv) {
+                    const u32x8 o = rc_add<DT>(xa[u], xb[u]);
+                    if (p.out) st_stream256(p.out + off + v * 32, o);
+                    if (p.fwd) st_stream256(p.fwd + off + v * 32, o);
                 }
             }
-            // ragged tail of the chunk (only the last chunk can have one)
-            if (blockIdx.x == 0) {
-                const unsigned long long i = c0 + nvec * EPV + threadIdx.x;
-                if (i < c0 + cn) {
-                    const float acc = __fadd_rn(load_elem<DT>(p.a, i), load_elem<DT>(p.b, i));
-                    if (p.out) store_elem<DT>(p.out, i, acc);
-                    if (p.fwd) store_elem<DT>(p.fwd, i, acc);
-                }
-            }
-        } else {
+#pragma unroll
+            for (int u = 0; u < RC_UNROLL; ++u) { xa[u] = na[u]; xb[u] = nb[u]; }
+            off = noff; nv = nnv;
+        }
+        rc_ragged_tail<DT>(p, threadIdx.x);
+    } else {
+        for (unsigned long long c0 = 0; c0 < p.count; c0 += p.chunkElems) {        // chunk by chunk, in order
+            const unsigned long long cn = min(p.chunkElems, p.count - c0);
             for (unsigned long long i = c0 + (unsigned long long)blockIdx.x * RC_THREADS + threadIdx.x; i < c0 + cn;
                  i += (unsigned long long)gridDim.x * RC_THREADS) {
                 const float acc = __fadd_rn(load_elem<DT>(p.a, i), load_elem<DT>(p.b, i));
@@ -318,4 +384,62 @@ __global__ void __launch_bounds__(RC_THREADS) reducecopy_kernel(const ReduceCopy
     }
 }
 
-}  // namespace ncclx
+// ---- TMA-fed variant ------------------------------------------------------------------------------------------
+constexpr int RCT_CONSUMERS = 512;
+constexpr int RCT_THREADS = RCT_CONSUMERS + 32;            // + one producer warp
+constexpr int RCT_STAGES = 6;
+constexpr int RCT_TILE_BYTES = RCT_CONSUMERS * 32;         // per input: one 32-byte vector per consumer thread
+constexpr int RCT_SMEM_BYTES = RCT_STAGES * 2 * RCT_TILE_BYTES + 2 * RCT_STAGES * 8 + 128;
+
+// dynamic smem: [stage][a tile | b tile] ... [full mbarriers][empty mbarriers]; requires the vector-path alignment
+// (checked by the host)
+template <int DT>
+__global__ void __launch_bounds__(RCT_THREADS, 1) reducecopy_tma_kernel(const ReduceCopyArgs p) {
+    constexpr int ES = DT == RED_F32 ? 4 : 2;
+    extern __shared__ __align__(128) unsigned char rct_smem[];
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(rct_smem + RCT_STAGES * 2 * RCT_TILE_BYTES);
+    unsigned long long* empty = full + RCT_STAGES;
+    const int warp = threadIdx.x >> 5, lane = lane_id();
+    if (threadIdx.x < RCT_STAGES) {
+        mbar_init(smem_u32(&full[threadIdx.x]), 1);
+        mbar_init(smem_u32(&empty[threadIdx.x]), RCT_CONSUMERS / 32);
+    }
+    fence_mbar_init();
+    __syncthreads();
+    RcTileIt<ES> it;
+    it.init(p, RCT_CONSUMERS);
+    if (warp == RCT_CONSUMERS / 32) {                      // producer warp: one elected lane issues the bulk loads
+        if (lane == 0) {
+            for (unsigned int i = 0; it.valid(); ++i, it.advance()) {
+                const unsigned int st = i % RCT_STAGES;
+                if (i >= RCT_STAGES) mbar_wait(smem_u32(&empty[st]), ((i / RCT_STAGES) - 1) & 1);
+                const unsigned int bytes = (unsigned int)it.vecs() * 32u;
+                const uint32_t bar = smem_u32(&full[st]);
+                const uint32_t dst = smem_u32(rct_smem + (size_t)st * 2 * RCT_TILE_BYTES);
+                mbar_expect_tx(bar, 2 * bytes);
+                bulk_g2s(dst, p.a + it.byte_off(), bytes, bar);
+                bulk_g2s(dst + RCT_TILE_BYTES, p.b + it.byte_off(), bytes, bar);
+            }
+        }
+    } else {
+        for (unsigned int i = 0; it.valid(); ++i, it.advance()) {
+            const unsigned int st = i % RCT_STAGES;
+            mbar_wait(smem_u32(&full[st]), (i / RCT_STAGES) & 1);
+            const unsigned long long off = it.byte_off();
+            if (threadIdx.x < it.vecs()) {
+                const unsigned char* sa = rct_smem + (size_t)st * 2 * RCT_TILE_BYTES + threadIdx.x * 32;
+                u32x8 xa, xb;
+                xa.lo = *reinterpret_cast<const uint4*>(sa); xa.hi = *reinterpret_cast<const uint4*>(sa + 16);
+                xb.lo = *reinterpret_cast<const uint4*>(sa + RCT_TILE_BYTES); xb.hi = *reinterpret_cast<const uint4*>(sa + RCT_TILE_BYTES + 16);
+                const u32x8 o = rc_add<DT>(xa, xb);
+                if (p.out) st_stream256(p.out + off + threadIdx.x * 32, o);
+                if (p.fwd) st_stream256(p.fwd + off + threadIdx.x * 32, o);
+            }
+            __syncwarp();                                  // the warp's reads of the stage are done
+            if (lane == 0) mbar_arrive(smem_u32(&empty[st]));
+        }
+        rc_ragged_tail<DT>(p, threadIdx.x);
+    }
+}
+
+}  // namespace xdev

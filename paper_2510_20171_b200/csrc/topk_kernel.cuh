@@ -16,7 +16,7 @@
 #include "common.cuh"
 #include "reduce_kernel.cuh"
 
-namespace ncclx {
+namespace xdev {
 
 constexpr int TOPK_THREADS = 256;
 constexpr int TOPK_UNROLL = 2;             // dispatch: vectors per lane in flight per copy (4 measured 8 % slower)
@@ -165,4 +165,4 @@ __global__ void __launch_bounds__(TOPK_THREADS) topk_combine_kernel(const TopkAr
     }
 }
 
-}  // namespace ncclx
+}  // namespace xdev

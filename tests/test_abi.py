@@ -33,7 +33,7 @@ def test_header_symbols_all_exported(L):
 
 
 def test_version_and_strerror(L):
-    assert L.ncclx_version() == 100
+    assert L.ncclx_version() == 200
     assert L.ncclx_strerror(0) == b"ok"
     for code in range(1, 6):
         assert len(L.ncclx_strerror(code)) > 3
@@ -50,6 +50,12 @@ def test_calls_fail_loudly_without_init(L):
     assert L.ncclx_alltoallv_host(1, 1, 1, 2, 4, 0, None) == 3
     assert L.ncclx_alltoallv_prepare_dev(0, 1, 1, 1, 2, 4, 0, None) == 3
     assert L.ncclx_alltoallv_execute_dev(0, None) == 3
+    assert L.ncclx_alltoallv_dynamic_prepare_dev(0, 1, 1, 4, 1, 4, 1, 2, 1, 1, 2, 0, None) == 3
+    assert L.ncclx_moe_topk_prepare_dev(0, 1, 2, 4, None) == 3
+    assert L.ncclx_moe_dispatch_topk_execute_dev(0, 1, 1, 1, 4, 2, 16, 0, None) == 3
+    assert L.ncclx_moe_combine_topk_sum_execute_dev(0, 1, 1, 1, 4, 2, 16, 0, None) == 3
+    assert L.ncclx_stream_probe_ctas(2, 32, 64, 32, 1, None) == 3
+    assert L.ncclx_debug_timeline(None, 0, None) == 3
     with pytest.raises(binding.NcclxError):
         binding.ncclx_finalize()
 
@@ -57,7 +63,9 @@ def test_calls_fail_loudly_without_init(L):
 def test_param_validation(L):
     from paper_2510_20171_b200 import binding as b
     assert L.ncclx_set_param(99, 1) == 1
-    assert L.ncclx_set_param(b.PARAM_COPY_CTAS_PER_SM, 9) == 1
+    assert L.ncclx_set_param(b.PARAM_COPY_BULK_ENGINES, 3) == 1
+    assert L.ncclx_set_param(b.PARAM_PDL, 2) == 1
+    assert b.PARAM_COUNT <= 10                      # the tuning surface stays small
     assert L.ncclx_set_param(b.PARAM_BULK_MIN_BYTES, 8) == 1
     assert L.ncclx_set_param(b.PARAM_BULK_TILE_SHIFT, 20) == 1
     b.ncclx_set_param(b.PARAM_BULK_MIN_BYTES, 4096)

@@ -26,16 +26,10 @@ def ctx():
 @pytest.fixture(autouse=True)
 def default_params():
     yield
-    nx.ncclx_set_param(nx.PARAM_COPY_CTAS_PER_SM, 1)
     nx.ncclx_set_param(nx.PARAM_BULK_MIN_BYTES, 1024)
-    nx.ncclx_set_param(nx.PARAM_FORCE_VECTOR, 0)
     nx.ncclx_set_param(nx.PARAM_BULK_TILE_SHIFT, 15)
-    nx.ncclx_set_param(nx.PARAM_VEC_TILE_SHIFT, 14)
-    nx.ncclx_set_param(nx.PARAM_SCAN_CTAS, 32)
     nx.ncclx_set_param(nx.PARAM_COPY_BULK_ENGINES, 0)
-    nx.ncclx_set_param(nx.PARAM_COPY_PENDING_STORES, 1)
     nx.ncclx_set_param(nx.PARAM_COPY_KMAX, 6)
-    nx.ncclx_set_param(nx.PARAM_COPY_STATIC_EIGHTHS, 0)
     nx.ncclx_set_param(nx.PARAM_PDL, 1)
 
 
@@ -124,13 +118,11 @@ def test_ragged_bulk_tail_and_tiny_segments():
     assert_a2a_matches(send, C2, "u8")
 
 
-@pytest.mark.parametrize("param,value", [("FORCE_VECTOR", 1), ("COPY_CTAS_PER_SM", 2), ("COPY_CTAS_PER_SM", 4),
-                                         ("BULK_TILE_SHIFT", 12), ("BULK_TILE_SHIFT", 16), ("VEC_TILE_SHIFT", 10),
-                                         ("BULK_MIN_BYTES", 16), ("BULK_MIN_BYTES", 1 << 20), ("SCAN_CTAS", 1),
-                                         ("SCAN_CTAS", 64), ("COPY_BULK_ENGINES", 1), ("COPY_BULK_ENGINES", 2), ("COPY_BULK_ENGINES", 4),
-                                         ("COPY_PENDING_STORES", 4), ("COPY_PENDING_STORES", 8), ("COPY_KMAX", 1),
-                                         ("COPY_KMAX", 17), ("COPY_STATIC_EIGHTHS", 4), ("COPY_STATIC_EIGHTHS", 8),
-                                         ("PDL", 0)])
+# BULK_MIN_BYTES = 2^40 sends every segment down the vector list (TMA-staged pieces + warp stores) although all are aligned
+@pytest.mark.parametrize("param,value", [("BULK_MIN_BYTES", 1 << 40), ("BULK_MIN_BYTES", 16), ("BULK_MIN_BYTES", 1 << 20),
+                                         ("BULK_TILE_SHIFT", 12), ("BULK_TILE_SHIFT", 16),
+                                         ("COPY_BULK_ENGINES", 1), ("COPY_BULK_ENGINES", 2), ("COPY_BULK_ENGINES", 4),
+                                         ("COPY_KMAX", 1), ("COPY_KMAX", 17), ("PDL", 0)])
 def test_launch_configurations_agree(param, value):
     nx.ncclx_set_param(getattr(nx, "PARAM_" + param), value)
     cfg = W.scaled_a2a(W.a2a_config(3), 64)

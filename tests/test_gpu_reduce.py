@@ -181,7 +181,17 @@ def test_host_buffer_forms(mode):
 @pytest.mark.parametrize("dtype", ["bf16", "f32", "f16"])
 @pytest.mark.parametrize("n,chunk,ctas", [(8 * 1024 * 1024 // 2 * 3 + 8 * 100 + 5, 8 << 20, 2), (100_003, 4096, 1),
                                           (16 * 512 * 4 * 3, 16 * 512 * 4 * 2, 3), (777, 0, 0)])
-def test_reducecopy_matches_two_rank_oracle(dtype, n, chunk, ctas):
+@pytest.mark.parametrize("tma", [0, 1])
+def test_reducecopy_matches_two_rank_oracle(dtype, n, chunk, ctas, tma):
+    """Both inner loops (NCCLX_PARAM_REDUCECOPY_TMA: pipelined register loads / TMA-fed shared-memory ring)."""
+    nx.ncclx_set_param(nx.PARAM_REDUCECOPY_TMA, tma)
+    try:
+        _reducecopy_case(dtype, n, chunk, ctas)
+    finally:
+        nx.ncclx_set_param(nx.PARAM_REDUCECOPY_TMA, 0)
+
+
+def _reducecopy_case(dtype, n, chunk, ctas):
     a = inject_specials(W.np_values(n, dtype, 1), dtype, 1)
     b = inject_specials(W.np_values(n, dtype, 2, 1e-3), dtype, 2)
     exp = oracle.allreduce_sum([a, b], dtype, nthreads=4)[0]
@@ -213,6 +223,22 @@ def test_reducecopy_misaligned_and_errors():
     with pytest.raises(nx.binding.NcclxError) as e:
         nx.ncclx_reducecopy_sum(da, db, out, None, n, "u8")
     assert e.value.code == 2
+
+
+def test_stream_probe_few_cta_form():
+    """Per-SM ceiling probe (fixed small grid of 1024-thread CTAs): same copy semantics."""
+    n = 32 * 70_001
+    src = torch.randint(0, 255, (n,), dtype=torch.uint8, device="cuda")
+    dst = torch.full((n + 32,), 0xA5, dtype=torch.uint8, device="cuda")
+    for ctas in (1, 2, 4):
+        dst.fill_(0xA5)
+        nx.ncclx_stream_probe_ctas(2, src, dst, n, ctas)
+        torch.cuda.synchronize()
+        assert torch.equal(dst[:n], src) and bool((dst[n:] == 0xA5).all())
+    with pytest.raises(nx.binding.NcclxError):
+        nx.ncclx_stream_probe_ctas(2, src, dst, n, 0)
+    with pytest.raises(nx.binding.NcclxError):
+        nx.ncclx_debug_timeline()                               # not an instrumented build
 
 
 def test_stream_probe_modes():

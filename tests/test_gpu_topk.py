@@ -19,7 +19,7 @@ def ctx():
     nx.ncclx_finalize()
 
 
-def run_both(R, T, k, width, dtype, seed, experts=None, mis=0, scramble_y=True):
+def run_both(R, T, k, width, dtype, seed, experts=None, mis=0, scramble_y=True, plan=None):
     pos, C = W.topk_routing(R, T, k, experts or 2 * R, seed)
     X = [W.np_values(T * width, dtype, 700 + s) for s in range(R)]
     slack = 8
@@ -32,7 +32,13 @@ def run_both(R, T, k, width, dtype, seed, experts=None, mis=0, scramble_y=True):
     dpos = torch.from_numpy(pos).cuda()
     dC = torch.from_numpy(C).cuda()
     dRC = torch.zeros_like(dC)
-    nx.ncclx_moe_dispatch_topk_dev(nx.device_ptr_table(dX), dpos, dC, nx.device_ptr_table(drecv), dRC, R, T, k, width, dtype)
+    if plan is None:
+        nx.ncclx_moe_dispatch_topk_dev(nx.device_ptr_table(dX), dpos, dC, nx.device_ptr_table(drecv), dRC, R, T, k, width, dtype)
+    else:                           # plan-slot form: ONE metadata phase serves the dispatch and (below) the combine
+        n0 = nx.ncclx_launch_count()
+        nx.ncclx_moe_topk_prepare_dev(plan, dC, dRC, R)
+        nx.ncclx_moe_dispatch_topk_execute_dev(plan, nx.device_ptr_table(dX), dpos, nx.device_ptr_table(drecv), T, k, width, dtype)
+        assert nx.ncclx_launch_count() - n0 == 2
     st = nx.ncclx_device_status()
     torch.cuda.synchronize()
     assert st == est and (dRC.cpu().numpy() == eRC).all()
@@ -48,7 +54,12 @@ def run_both(R, T, k, width, dtype, seed, experts=None, mis=0, scramble_y=True):
     dY = [to_dev(y, mis) for y in Y]
     eZ, est2 = oracle.moe_combine_topk_sum(Y, pos, C, width, dtype)
     dZ = [sentinel(T * width * ES[dtype], mis) for _ in range(R)]
-    nx.ncclx_moe_combine_topk_sum_dev(nx.device_ptr_table(dY), dpos, dC, nx.device_ptr_table(dZ), R, T, k, width, dtype)
+    if plan is None:
+        nx.ncclx_moe_combine_topk_sum_dev(nx.device_ptr_table(dY), dpos, dC, nx.device_ptr_table(dZ), R, T, k, width, dtype)
+    else:
+        n0 = nx.ncclx_launch_count()
+        nx.ncclx_moe_combine_topk_sum_execute_dev(plan, nx.device_ptr_table(dY), dpos, nx.device_ptr_table(dZ), T, k, width, dtype)
+        assert nx.ncclx_launch_count() - n0 == 1           # the combine reuses the dispatch's offsets: no metadata kernel
     st2 = nx.ncclx_device_status()
     torch.cuda.synchronize()
     assert st2 == est2
@@ -61,6 +72,38 @@ def run_both(R, T, k, width, dtype, seed, experts=None, mis=0, scramble_y=True):
 @pytest.mark.parametrize("R,T,k,width", [(2, 5, 1, 16), (4, 33, 2, 64), (8, 100, 4, 128), (16, 64, 8, 80), (64, 32, 4, 512)])
 def test_dispatch_and_combine_match_oracle(dtype, R, T, k, width):
     run_both(R, T, k, width, dtype, seed=R + k)
+
+
+@pytest.mark.parametrize("plan", [0, 2])
+@pytest.mark.parametrize("R,T,k,width,dtype", [(8, 100, 4, 128, "bf16"), (64, 128, 4, 5120, "bf16"), (32, 256, 1, 5120, "bf16"),
+                                               (16, 64, 8, 80, "f32")])
+def test_plan_slot_form_matches_oracle(plan, R, T, k, width, dtype):
+    """ncclx_moe_topk_prepare_dev + the two execute calls (PAPER.md L483 double buffering for the k > 1 flow), incl.
+    Table 3's decode shapes (k in {1, 4}, 128 / 256 tokens per rank, hidden 5120)."""
+    run_both(R, T, k, width, dtype, seed=3 * R + k, plan=plan)
+
+
+def test_plan_slot_kinds_are_checked():
+    R = 4
+    C = torch.from_numpy(np.full((R, R), 3, np.int64)).cuda()
+    RC = torch.zeros_like(C)
+    t = torch.zeros(64, dtype=torch.int64, device="cuda")
+    nx.ncclx_moe_topk_prepare_dev(1, C, RC, R)
+    n0 = nx.ncclx_launch_count()
+    with pytest.raises(nx.binding.NcclxError) as e:
+        nx.ncclx_alltoallv_execute_dev(1)                       # slot 1 holds a top-k plan, not a work list
+    assert e.value.code == 1
+    with pytest.raises(nx.binding.NcclxError) as e:
+        nx.ncclx_moe_dispatch_topk_execute_dev(3, t, t, t, 4, 2, 16, "bf16")     # slot 3 was never prepared
+    assert e.value.code == 1
+    with pytest.raises(nx.binding.NcclxError) as e:
+        nx.ncclx_moe_dispatch_topk_execute_dev(1, t, t, t, 4, 0, 16, "bf16")     # k = 0
+    assert e.value.code == 1
+    with pytest.raises(nx.binding.NcclxError) as e:
+        nx.ncclx_moe_topk_prepare_dev(1, C, C, R)                                # aliased count matrices
+    assert e.value.code == 1
+    assert nx.ncclx_launch_count() == n0, "an argument error must not enqueue anything"
+    torch.cuda.synchronize()
 
 
 @pytest.mark.parametrize("mis,width", [(2, 16), (16, 24), (0, 7), (6, 33)])
