@@ -708,13 +708,19 @@ def timeline_probe(torch, nx, peak, cfg_index=5):
     for _ in range(5):
         a.dispatch()
     torch.cuda.synchronize()
-    tl = nx.ncclx_debug_timeline().astype(np.int64)
+    tl, ct = nx.ncclx_debug_timeline()
+    tl, ct = tl.astype(np.int64), ct.astype(np.int64)
+    ct = ct[ct[:, 0] > 0]                                              # CTAs of the counts kernel that ran
     names = ["enter", "metadata_ready", "first_load", "first_store", "last_store", "drained", "exit"]
-    t0 = int(tl[:, 0].min())
-    cols = {nm: (tl[:, i] - t0) / 1e3 for i, nm in enumerate(names)}           # us since the first CTA entered
+    t0 = int(min(tl[:, 0].min(), ct[:, 0].min() if len(ct) else tl[:, 0].min()))
+    cols = {nm: (tl[:, i] - t0) / 1e3 for i, nm in enumerate(names)}           # us since the first CTA of either kernel entered
     out = {"ctas": int(tl.shape[0]), "bulk_tiles": int(tl[0, 7]), "bytes_moved": 2 * a.bytes_one_way, "us": {}}
     for nm, v in cols.items():
         out["us"][nm] = {"min": round(float(v.min()), 2), "median": round(float(np.median(v)), 2), "max": round(float(v.max()), 2)}
+    cnames = ["enter", "dependency_wait_over", "phase1_done", "barrier_passed", "tile_totals_known", "exit"]
+    out["counts_kernel_ctas"] = int(len(ct))
+    out["counts_kernel_us"] = {nm: {"min": round(float(((ct[:, i] - t0) / 1e3).min()), 2), "median": round(float(np.median((ct[:, i] - t0) / 1e3)), 2),
+                                     "max": round(float(((ct[:, i] - t0) / 1e3).max()), 2)} for i, nm in enumerate(cnames)} if len(ct) else {}
     span = float(cols["exit"].max())
     busy = float(np.median(cols["last_store"] - cols["first_load"]))
     out["kernel_span_us"] = round(span, 2)

@@ -325,7 +325,9 @@ int ncclx_stream_probe_ctas(int mode, const void* src, void* dst, size_t bytes, 
 /* Instrumented builds only (python -m paper_2510_20171_b200.build --timeline; -DXDEV_TIMELINE): copies the per-CTA
  * globaltimer stamps of the LAST segment_copy_kernel launch to stamps_host[ctas][*fields] (ns; fields: kernel entry,
  * metadata ready, first load issued, first store issued, last store issued, engine drained, exit, bulk tiles of the
- * call).  max_ctas >= ncclx_sm_count().  Synchronises the device.  NCCLX_ERR_ARG in a normal build. */
+ * call), followed by 1024 x 8 stamps of the LAST counts_kernel launch (per CTA: entry, dependency wait over, phase 1
+ * done, barrier passed, tile totals known, exit).  stamps_host holds (ncclx_sm_count() * *fields + 8192) uint64;
+ * max_ctas >= ncclx_sm_count().  Synchronises the device.  NCCLX_ERR_ARG in a normal build. */
 int ncclx_debug_timeline(uint64_t* stamps_host, int max_ctas, int* fields);
 
 /* Number of SMs of the device the library was initialised on (0 before init). */

@@ -294,13 +294,14 @@ def ncclx_stream_probe_ctas(mode: int, src, dst, nbytes: int, num_ctas: int, str
 
 
 def ncclx_debug_timeline():
-    """Instrumented builds only: (ctas x fields) uint64 array of globaltimer stamps of the last copy-kernel launch."""
+    """Instrumented builds only: (copy: ctas x fields, counts: 1024 x 8) uint64 globaltimer stamps of the last launches."""
     import numpy as np
     n = ncclx_sm_count()
-    buf = np.zeros((n, 16), np.uint64)
+    buf = np.zeros(n * 16 + 8192, np.uint64)
     fields = ctypes.c_int(0)
     _ck(lib().ncclx_debug_timeline(buf.ctypes.data, n, ctypes.byref(fields)), "ncclx_debug_timeline")
-    return buf.reshape(-1)[:n * fields.value].reshape(n, fields.value)
+    f = fields.value
+    return buf[:n * f].reshape(n, f), buf[n * f:n * f + 8192].reshape(1024, 8)
 
 
 def ncclx_set_param(param: int, value: int) -> None:

@@ -36,6 +36,7 @@ struct Workspace {
     long long* roff;          // R*R, roff[d*R+s]
     SegDesc* desc;            // R*R, desc[d*R+s]
     int* colTiles[2];         // R each: tiles of list L in column d
+    int* colKiB;              // R: KiB of column d's bulk-list segments (-> average tile size -> bulk engines per CTA)
     int* coarse[2];           // R*ceil(colLen/32) each: tiles of list L in column d before its descriptor 32*j
     WorkCtl* ctl;
 };
@@ -86,6 +87,10 @@ __device__ __forceinline__ long long warp_sum(long long v) {
 // completed and its writes are visible.  Both are no-ops when the launch carries no such attribute.
 __device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// L2 prefetch: a hint with no correctness implication (L2 is the GPU's point of coherence, so a line prefetched before
+// griddepcontrol.wait cannot go stale) -- used to pull cold metadata into L2 in ONE DRAM round trip.
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
 
 // ---- streaming global accesses --------------------------------------------------------------
 // (No ld.global.nc anywhere: with programmatic dependent launch a kernel's CTAs are resident while the kernel before

@@ -32,13 +32,15 @@ constexpr int COPY_WARPS = COPY_THREADS / 32;
 constexpr int COPY_SLOTS = 32;             // outstanding bulk tiles per engine (mbarriers; slot j lives in lane j): <= 32
 constexpr int COPY_MAX_ENGINES = 4;        // bulk engines (warps 0..E-1) per CTA, each with its own share of the ring
 constexpr int VEC_SLOTS = 16;              // outstanding staged pieces per vector engine
-constexpr int VEC_SUB_BYTES = 2048;        // bytes of a vector tile staged per TMA load (multiple of 16)
+constexpr int VEC_SUB_BYTES = 4096;        // bytes of a vector tile staged per TMA load (multiple of 16, <= 4096: slot word)
 constexpr int VEC_DIRECT_MAX = 48;         // pieces shorter than this are copied by lanes, global -> global
-constexpr int VEC_MAX_IN_BULK_MIX = 9;     // vector engines when both lists have work: the bulk engines keep >= 7/16 of the ring
+constexpr int VEC_MAX_IN_BULK_MIX = 13;    // vector engines when both lists have work: the bulk engines keep >= 3/16 of the ring (>= 1 tile)
 constexpr int COPY_MBAR_COUNT = COPY_MAX_ENGINES * COPY_SLOTS + COPY_WARPS * VEC_SLOTS;
 constexpr int COPY_MBAR_BYTES = COPY_MBAR_COUNT * 8;
 constexpr int COPY_KMAX_LONG = 2;          // max tiles per dynamic claim when segments average >= 8 tiles (measured: config 3)
 constexpr int COPY_KMAX_VEC = 8;           // max tiles per dynamic claim on the vector list
+constexpr int COPY_CLAIM_DIV = 4;          // guided claims: K = remaining / (COPY_CLAIM_DIV * engines), clamped to [1, kmax]: an engine holds up to three
+                                           // chunks (current, staged, claimed), so chunks shrink early (config 5: 2 -> 4: 163 -> 157 us with two engines)
 
 // Optional side job for the warps that are not engines at the start of the kernel: `copies` copies of the int64
 // array src[0..n) (negative values written as 0) to dst + c*n.  AllToAllvDynamic's recvAllSplitLengths (PAPER.md
@@ -53,6 +55,7 @@ struct SideJob {
 struct CopyArgs {
     const SegDesc* desc;
     const int* colTiles[2];
+    const int* colKiB;                     // per column: KiB of its bulk-list segments (metadata kernel)
     const int* coarse[2];                  // per list: tiles of column d before its descriptor 32*j, [d*nb + j] (metadata kernel)
     WorkCtl* ctl;
     int ncols;                             // destination columns of the descriptor table (= R)
@@ -84,16 +87,45 @@ __host__ __device__ inline int coarse_blocks(int colLen) { return (colLen + 31) 
 // start-up.  Long-segment regime (config 3): small in-order claims resolve inside the cached windows.
 // Without a coarse index (table too large for shared memory) the block is found by a 128-ary search in L2.
 // SM = true: the descriptor table lives in SHARED memory (single-launch path, fused_kernel.cuh).
-template <int L, bool SM = false>
-struct Cursor {
+// What all engines of one work list share, in shared memory (one copy per list and CTA): keeps ~25 registers per
+// thread out of the cursor, whose cold fields were being spilled in the engines' hot loops.
+struct CursorEnv {
     const SegDesc* desc;
     const int* colBase;                    // smem, ncols+1 entries, colBase[ncols] = total tiles
     const int* coarse;                     // smem, ncols*nb entries, or null
     unsigned int* counter;
     ClassParams cls;
-    int ncols, colLen, nb, RR, tileShift, total, nEngines, kmax, kmin;
-    int staticK, engineId;                 // first chunk is assigned statically: [engineId*staticK, +staticK)
+    int ncols, colLen, nb, RR, total, nEngines, kmax, kmin, claimDiv;
+    int staticK;                           // first chunk is assigned statically: [engineId*staticK, +staticK)
     int dynBase;                           // tiles >= dynBase are claimed dynamically
+    bool longSegs, indexed, pipelined;
+};
+__device__ __forceinline__ void cursor_env_init(CursorEnv* e, int L, const SegDesc* desc, const int* colBase, const int* coarse,
+                                                unsigned int* counter, const ClassParams& cls, int ncols, int colLen, int nEngines,
+                                                int kmax, int kmaxLong, int staticK, int claimDiv) {
+    e->desc = desc; e->colBase = colBase; e->coarse = coarse; e->counter = counter; e->cls = cls;
+    e->ncols = ncols; e->colLen = colLen; e->nb = coarse_blocks(colLen); e->RR = ncols * colLen;
+    e->total = colBase[ncols];
+    e->nEngines = nEngines > 0 ? nEngines : 1;
+    // long segments (>= 8 tiles each on average): claims resolve inside the cached window, so take
+    // small chunks and keep all SMs in a tight moving window of HBM; short segments: amortise the
+    // per-claim work over a few tiles and hide it behind the previous chunk.
+    e->longSegs = e->total >= 8 * e->RR;
+    e->indexed = coarse != nullptr || e->nb == 1;
+    e->pipelined = e->indexed && !e->longSegs;
+    e->kmax = e->longSegs ? kmaxLong : kmax;
+    e->staticK = staticK;
+    e->claimDiv = claimDiv;
+    // a short list (few tiles per engine) pays per claim, a long one for the imbalance of its last chunks
+    e->kmin = e->total >= 32 * e->nEngines ? 1 : 2;
+    e->dynBase = staticK * e->nEngines;
+    (void)L;
+}
+
+template <int L, bool SM = false>
+struct Cursor {
+    const CursorEnv* env;                  // everything that is the same for all engines of the list (shared memory)
+    int tileShift, engineId;
     int pendCur, pendK;                    // lane 0: a chunk claimed ahead of need (atomic in flight)
     int t, tEnd;                           // current tile, end of the claimed chunk
     int q, kInSeg, segTiles;               // current segment, tile within it, its tile count
@@ -103,11 +135,11 @@ struct Cursor {
     uint4 w0, w1, n0, n1;                  // this lane's descriptor in each window
     int cCur, cK, cQw, cEnd, cPrev, cTl;   // pipelined mode: the staged NEXT chunk and where it starts
     uint4 c0, c1;                          // its window (load in flight until adopt())
-    bool first, exhausted, haveWindow, longSegs, indexed, pipelined, cHave, needPrefetch;
+    bool first, exhausted, haveWindow, cHave, needPrefetch;
 
     __device__ __forceinline__ void load_desc(int qq, uint4& a, uint4& b) const {
-        if (qq < RR) {
-            const uint4* p = reinterpret_cast<const uint4*>(desc + qq);
+        if (qq < env->RR) {
+            const uint4* p = reinterpret_cast<const uint4*>(env->desc + qq);
             if constexpr (SM) { a = p[0]; b = p[1]; } else { a = ld_stream(p); b = ld_stream(p + 1); }   // coherent: the kernel before us wrote them (PDL)
         } else {
             a = make_uint4(0, 0, 0, 0); b = make_uint4(0, 0, 0, 0);
@@ -115,7 +147,7 @@ struct Cursor {
     }
     __device__ __forceinline__ int my_tiles() const {
         return seg_tiles(L, ((unsigned long long)w0.y << 32) | w0.x, ((unsigned long long)w0.w << 32) | w0.z,
-                         (long long)(((unsigned long long)w1.y << 32) | w1.x), cls);
+                         (long long)(((unsigned long long)w1.y << 32) | w1.x), env->cls);
     }
     __device__ __forceinline__ void take(int fromLane) {    // adopt the descriptor held by lane `fromLane`
         const unsigned int sx = __shfl_sync(0xffffffffu, w0.x, fromLane), sy = __shfl_sync(0xffffffffu, w0.y, fromLane);
@@ -128,73 +160,60 @@ struct Cursor {
         q = qw + fromLane;
     }
 
-    // staticK_ tiles per engine are assigned statically ([engineId*staticK, +staticK): no atomic on the
-    // start-up path); tiles >= staticK*nEngines are claimed dynamically, IN ORDER, in guided chunks.
+    // env->staticK tiles per engine are assigned statically ([engineId*env->staticK, +env->staticK): no atomic on the
+    // start-up path); tiles >= env->staticK*env->nEngines are claimed dynamically, IN ORDER, in guided chunks.
     // Measured on B200: the in-order dynamic claim keeps all SMs inside one moving window of HBM and is
     // ~7 % faster than contiguous static ranges (148 far-apart streams), so only the FIRST chunk of each
     // engine is static (chunk e to engine e, which is also what in-order claims would hand out).
-    __device__ __forceinline__ void init(const SegDesc* desc_, const int* colBase_, const int* coarse_, unsigned int* counter_,
-                                         const ClassParams& cls_, int ncols_, int colLen_, int nEngines_, int engineId_,
-                                         int kmax_, int kmaxLong_, int staticK_) {
-        desc = desc_; colBase = colBase_; coarse = coarse_; counter = counter_; cls = cls_;
-        ncols = ncols_; colLen = colLen_; nb = coarse_blocks(colLen_); RR = ncols_ * colLen_;
-        tileShift = cls_.tileShift[L]; total = colBase_[ncols_];
-        nEngines = nEngines_; engineId = engineId_;
-        // long segments (>= 8 tiles each on average): claims resolve inside the cached window, so take
-        // small chunks and keep all SMs in a tight moving window of HBM; short segments: amortise the
-        // per-claim work over a few tiles and hide it behind the previous chunk.
-        longSegs = total >= 8 * RR;
-        indexed = coarse_ != nullptr || nb == 1;
-        pipelined = indexed && !longSegs;
-        kmax = longSegs ? kmaxLong_ : kmax_;
-        staticK = staticK_;
-        kmin = total >= 8 * nEngines ? 2 : 1;
-        dynBase = staticK * nEngines;
-        pendCur = total; pendK = 0;        // reads as "drained" unless a claim is issued
+    __device__ __forceinline__ void init(const CursorEnv* env_, int engineId_) {
+        env = env_;
+        engineId = engineId_;
+        tileShift = env_->cls.tileShift[L];
+        pendCur = env->total; pendK = 0;        // reads as "drained" unless a claim is issued
         t = tEnd = 0; q = 0; kInSeg = segTiles = 0; src = dst = 0; bytes = 0;
         qw = qn = 0; w0 = w1 = n0 = n1 = c0 = c1 = make_uint4(0, 0, 0, 0);
         cCur = cK = cQw = cEnd = cPrev = cTl = 0;
         first = true;
         haveWindow = false;
         cHave = needPrefetch = false;
-        exhausted = (total == 0);
+        exhausted = (env->total == 0);
         if (exhausted) return;
-        if (!pipelined) {
-            if (total > dynBase) claim_issue(dynBase);
-        } else if (staticK > 0) {
-            const int c = engineId * staticK;
-            if (c < total) stage_next(c, staticK);             // else: nothing for this engine (then total <= dynBase)
-            if (total > dynBase) claim_issue(dynBase);
+        if (!env->pipelined) {
+            if (env->total > env->dynBase) claim_issue(env->dynBase);
+        } else if (env->staticK > 0) {
+            const int c = engineId * env->staticK;
+            if (c < env->total) stage_next(c, env->staticK);             // else: nothing for this engine (then env->total <= env->dynBase)
+            if (env->total > env->dynBase) claim_issue(env->dynBase);
         } else {
-            claim_issue(dynBase);
+            claim_issue(env->dynBase);
             prefetch_next();                                   // waits for the atomic once, at start-up
         }
     }
 
-    // Lane 0 issues the atomic for a later dynamic chunk; the result is consumed one chunk (pipelined:
+    // Lane 0 issues the atomic for a later dynamic chunk; the result is consumed one chunk (env->pipelined:
     // two chunks) later, so its L2 round trip overlaps the copying.
     __device__ __forceinline__ void claim_issue(int counterHint) {
         if (lane_id() == 0) {
-            const int rem = total - min(total, counterHint);
-            pendK = max(kmin, min(kmax, rem / (2 * nEngines)));
-            pendCur = dynBase + (int)atomicAdd(counter, (unsigned int)pendK);
+            const int rem = env->total - min(env->total, counterHint);
+            pendK = max(env->kmin, min(env->kmax, rem / (env->claimDiv * env->nEngines)));
+            pendCur = env->dynBase + (int)atomicAdd(env->counter, (unsigned int)pendK);
         }
     }
 
     // Shared-memory search: column d that owns global tile tt, tile index tl inside the column, the
     // 32-descriptor block j of the column that holds it and the tiles of the column before that block.
     __device__ __forceinline__ void find_block(int tt, int& d, int& tl, int& j, int& prev) const {
-        int lo = 0, hi = ncols;            // colBase[lo] <= tt < colBase[hi]
+        int lo = 0, hi = env->ncols;            // env->colBase[lo] <= tt < env->colBase[hi]
         while (hi - lo > 1) {
             const int mid = (lo + hi) >> 1;
-            if (colBase[mid] <= tt) lo = mid; else hi = mid;
+            if (env->colBase[mid] <= tt) lo = mid; else hi = mid;
         }
         d = lo;
-        tl = tt - colBase[d];
+        tl = tt - env->colBase[d];
         j = 0; prev = 0;
-        if (nb > 1) {
-            const int* cr = coarse + d * nb;
-            int a = 0, b = nb;             // cr[a] <= tl < cr[b]  (cr[nb] = +inf)
+        if (env->nb > 1) {
+            const int* cr = env->coarse + d * env->nb;
+            int a = 0, b = env->nb;             // cr[a] <= tl < cr[b]  (cr[env->nb] = +inf)
             while (b - a > 1) {
                 const int mid = (a + b) >> 1;
                 if (cr[mid] <= tl) a = mid; else b = mid;
@@ -212,28 +231,28 @@ struct Cursor {
         kInSeg = tl - (m > 0 ? before : prev);
     }
 
-    // Find the segment that owns global tile index tt (0 <= tt < total) and (re)load the windows there.
+    // Find the segment that owns global tile index tt (0 <= tt < env->total) and (re)load the windows there.
     __device__ __forceinline__ void locate(int tt) {
         const int lane = lane_id();
-        if (indexed) {
+        if (env->indexed) {
             int d, tl, j, prev;
             find_block(tt, d, tl, j, prev);
-            qw = d * colLen + 32 * j;
+            qw = d * env->colLen + 32 * j;
             load_desc(qw + lane, w0, w1);
             qn = qw + 32;
             load_desc(qn + lane, n0, n1);
-            position(tl, prev, (d + 1) * colLen);
+            position(tl, prev, (d + 1) * env->colLen);
             return;
         }
-        int lo = 0, hi = ncols;            // colBase[lo] <= tt < colBase[hi]
+        int lo = 0, hi = env->ncols;            // env->colBase[lo] <= tt < env->colBase[hi]
         while (hi - lo > 1) {
             const int mid = (lo + hi) >> 1;
-            if (colBase[mid] <= tt) lo = mid; else hi = mid;
+            if (env->colBase[mid] <= tt) lo = mid; else hi = mid;
         }
         const int d = lo;
-        const int tl = tt - colBase[d];
-        const SegDesc* col = desc + (size_t)d * colLen;
-        int s0 = 0, n = colLen;                 // smallest s with col[s].pfx[L] > tl lies in [s0, s0+n)
+        const int tl = tt - env->colBase[d];
+        const SegDesc* col = env->desc + (size_t)d * env->colLen;
+        int s0 = 0, n = env->colLen;                 // smallest s with col[s].pfx[L] > tl lies in [s0, s0+n)
         while (n >= 32) {                  // 128-ary rounds: every lane probes 4 block ends per L2 round trip; ends with at most
                                            // 31 candidates, so that they AND the predecessor slot fit in one 32-descriptor window
             const int step = (n + 127) >> 7;
@@ -254,20 +273,20 @@ struct Cursor {
         // last round doubles as the window load; the window starts one descriptor early so that the
         // predecessor's prefix (needed for the tile index inside the segment) comes with it
         const int sb = s0 > 0 ? s0 - 1 : 0;
-        qw = d * colLen + sb;
+        qw = d * env->colLen + sb;
         load_desc(qw + lane, w0, w1);
         qn = qw + 32;
         load_desc(qn + lane, n0, n1);
-        position(tl, 0, (d + 1) * colLen);
+        position(tl, 0, (d + 1) * env->colLen);
     }
 
-    // ---- pipelined mode ------------------------------------------------------------------------
+    // ---- env->pipelined mode ------------------------------------------------------------------------
     __device__ __forceinline__ void stage_next(int cur, int k) {   // chunk [cur, cur+k): find its block, start the window load
         int d, j;
         find_block(cur, d, cTl, j, cPrev);
         cCur = cur; cK = k;
-        cQw = d * colLen + 32 * j;
-        cEnd = (d + 1) * colLen;
+        cQw = d * env->colLen + 32 * j;
+        cEnd = (d + 1) * env->colLen;
         load_desc(cQw + lane_id(), c0, c1);
         cHave = true;
     }
@@ -275,13 +294,13 @@ struct Cursor {
         needPrefetch = false;
         const int pc = __shfl_sync(0xffffffffu, pendCur, 0);
         const int pk = __shfl_sync(0xffffffffu, pendK, 0);
-        if (pc >= total || pc < 0) { cHave = false; return; }
+        if (pc >= env->total || pc < 0) { cHave = false; return; }
         stage_next(pc, pk);
         claim_issue(pc + pk);
     }
     __device__ __forceinline__ void adopt() {              // the staged chunk becomes the current one
         t = cCur;
-        tEnd = min(cCur + cK, total);
+        tEnd = min(cCur + cK, env->total);
         qw = cQw; w0 = c0; w1 = c1;
         qn = qw + 32;
         load_desc(qn + lane_id(), n0, n1);
@@ -302,7 +321,7 @@ struct Cursor {
             qn = qw + 32;
             load_desc(qn + lane_id(), n0, n1);
             cl = -1;
-            if (qw >= RR) { exhausted = true; break; }      // cannot happen while t < total
+            if (qw >= env->RR) { exhausted = true; break; }      // cannot happen while t < env->total
         }
         kInSeg = 0;
     }
@@ -331,7 +350,7 @@ struct Cursor {
             qn = qw + 32;
             load_desc(qn + lane_id(), n0, n1);
             cl = -1;
-            if (qw >= RR) return false;
+            if (qw >= env->RR) return false;
         }
         return false;
     }
@@ -340,32 +359,32 @@ struct Cursor {
     __device__ __forceinline__ bool ensure() {
         if (exhausted) return false;
         if (t < tEnd) {
-            if (needPrefetch) prefetch_next();     // (pipelined) after the chunk's first tile is on its way
+            if (needPrefetch) prefetch_next();     // (env->pipelined) after the chunk's first tile is on its way
             if (kInSeg >= segTiles) advance_segment();
             return !exhausted;
         }
-        if (pipelined) {
+        if (env->pipelined) {
             if (needPrefetch) prefetch_next();
             if (!cHave) { exhausted = true; return false; }
             adopt();
             return true;
         }
         int cur, k;
-        if (first && staticK > 0) {        // static share: no atomic on the start-up path
+        if (first && env->staticK > 0) {        // static share: no atomic on the start-up path
             first = false;
-            cur = engineId * staticK;
-            k = staticK;
-            if (cur >= total) { exhausted = true; return false; }
+            cur = engineId * env->staticK;
+            k = env->staticK;
+            if (cur >= env->total) { exhausted = true; return false; }
         } else {
             first = false;
             cur = __shfl_sync(0xffffffffu, pendCur, 0);
             k = __shfl_sync(0xffffffffu, pendK, 0);
-            if (cur >= total || cur < 0) { exhausted = true; return false; }
+            if (cur >= env->total || cur < 0) { exhausted = true; return false; }
             claim_issue(cur + k);
         }
-        const bool near = longSegs && haveWindow && cur >= t && advance_by(cur - t);
+        const bool near = env->longSegs && haveWindow && cur >= t && advance_by(cur - t);
         t = cur;
-        tEnd = min(cur + k, total);
+        tEnd = min(cur + k, env->total);
         if (!near) locate(t);
         haveWindow = true;
         return true;
@@ -377,54 +396,61 @@ struct Cursor {
 
 // ---- vector list: shared memory -> global with any alignment --------------------------------------------------
 // Destination vector j (16-byte aligned) = bytes [sh + 16 j, sh + 16 j + 16) of the aligned shared-memory image:
-// the two aligned 16-byte words that straddle it, joined with a funnel shift (sh = 4*wsel + bsh/8, warp-uniform).
-__device__ __forceinline__ uint4 shift_join(const uint4& a, const uint4& b, const int wsel, const int bsh) {
+// the two aligned 16-byte words that straddle it, joined with funnel shifts (sh = 4*WSEL + bsh/8).  WSEL is a template
+// parameter so that the word selection is static; the (warp-uniform) dispatch happens once per piece.
+template <int WSEL>
+__device__ __forceinline__ uint4 shift_join(const uint4& a, const uint4& b, const int bsh) {
     const unsigned int w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
-    uint4 o;
-    switch (wsel) {                        // warp-uniform
-    case 0:  o = make_uint4(__funnelshift_r(w[0], w[1], bsh), __funnelshift_r(w[1], w[2], bsh), __funnelshift_r(w[2], w[3], bsh), __funnelshift_r(w[3], w[4], bsh)); break;
-    case 1:  o = make_uint4(__funnelshift_r(w[1], w[2], bsh), __funnelshift_r(w[2], w[3], bsh), __funnelshift_r(w[3], w[4], bsh), __funnelshift_r(w[4], w[5], bsh)); break;
-    case 2:  o = make_uint4(__funnelshift_r(w[2], w[3], bsh), __funnelshift_r(w[3], w[4], bsh), __funnelshift_r(w[4], w[5], bsh), __funnelshift_r(w[5], w[6], bsh)); break;
-    default: o = make_uint4(__funnelshift_r(w[3], w[4], bsh), __funnelshift_r(w[4], w[5], bsh), __funnelshift_r(w[5], w[6], bsh), __funnelshift_r(w[6], w[7], bsh)); break;
+    return make_uint4(__funnelshift_r(w[WSEL], w[WSEL + 1], bsh), __funnelshift_r(w[WSEL + 1], w[WSEL + 2], bsh),
+                      __funnelshift_r(w[WSEL + 2], w[WSEL + 3], bsh), __funnelshift_r(w[WSEL + 3], w[WSEL + 4], bsh));
+}
+template <int WSEL>
+__device__ __forceinline__ void drain_shifted_body(const uint4* sv, uint4* dv, const unsigned int nvec, const int bsh, const unsigned int lane) {
+    unsigned int i = lane;
+    for (; i + 32 < nvec; i += 64) {                       // two full warp rows per trip, loads first, no predicates
+        const uint4 a0 = sv[i], b0 = sv[i + 1], a1 = sv[i + 32], b1 = sv[i + 33];
+        st_stream(dv + i, shift_join<WSEL>(a0, b0, bsh));
+        st_stream(dv + i + 32, shift_join<WSEL>(a1, b1, bsh));
     }
-    return o;
+    for (; i < nvec; i += 32) st_stream(dv + i, shift_join<WSEL>(sv[i], sv[i + 1], bsh));
 }
 
 // One warp: write `len` bytes to global `dst` (any alignment) from the shared-memory image `sm` (16-byte aligned) of
-// the aligned source span that holds them from byte offset ms (0..15) on.  Head and tail (< 16 bytes each) go byte
-// by byte, the body as aligned 16-byte stores; every shared-memory word read lies inside the loaded span
-// [0, align16(ms + len)) (the second word of a join is only read when it holds a needed byte: sh >= 1).
+// the aligned source span that holds them from byte offset ms (0..15) on.  Head and tail (< 16 bytes each, only at the
+// ends of a tile) go byte by byte, the body as aligned 16-byte stores; every shared-memory word read lies inside the
+// loaded span [0, align16(ms + len)) (the second word of a join is only read when it holds a needed byte: sh >= 1).
 __device__ __forceinline__ void warp_drain_shifted(unsigned char* dst, const unsigned char* sm, const unsigned int ms, const unsigned int len) {
     const unsigned int lane = (unsigned int)lane_id();
     unsigned int hb = (16u - (unsigned int)((unsigned long long)dst & 15ull)) & 15u;
-    if (hb > len) hb = len;
-    if (lane < hb) dst[lane] = sm[ms + lane];
-    const unsigned int pos = ms + hb;                  // shared-memory offset of the first body byte
+    if (hb) {                                              // warp-uniform
+        if (hb > len) hb = len;
+        if (lane < hb) dst[lane] = sm[ms + lane];
+    }
+    const unsigned int pos = ms + hb;                      // shared-memory offset of the first body byte
     const unsigned int nvec = (len - hb) >> 4;
     const unsigned int sh = pos & 15u;
     const uint4* sv = reinterpret_cast<const uint4*>(sm) + (pos >> 4);
     uint4* dv = reinterpret_cast<uint4*>(dst + hb);
-    constexpr unsigned int U = 4;
     if (sh == 0) {
-        for (unsigned int i = lane; i < nvec; i += 32 * U) {
-            uint4 v[U];
-#pragma unroll
-            for (unsigned int u = 0; u < U; ++u) if (i + 32 * u < nvec) v[u] = sv[i + 32 * u];
-#pragma unroll
-            for (unsigned int u = 0; u < U; ++u) if (i + 32 * u < nvec) st_stream(dv + i + 32 * u, v[u]);
+        unsigned int i = lane;
+        for (; i + 96 < nvec; i += 128) {
+            const uint4 v0 = sv[i], v1 = sv[i + 32], v2 = sv[i + 64], v3 = sv[i + 96];
+            st_stream(dv + i, v0); st_stream(dv + i + 32, v1); st_stream(dv + i + 64, v2); st_stream(dv + i + 96, v3);
         }
+        for (; i < nvec; i += 32) st_stream(dv + i, sv[i]);
     } else {
-        const int wsel = (int)(sh >> 2), bsh = (int)(sh & 3u) * 8;
-        for (unsigned int i = lane; i < nvec; i += 32 * U) {
-            uint4 a[U], b[U];
-#pragma unroll
-            for (unsigned int u = 0; u < U; ++u) if (i + 32 * u < nvec) { a[u] = sv[i + 32 * u]; b[u] = sv[i + 32 * u + 1]; }
-#pragma unroll
-            for (unsigned int u = 0; u < U; ++u) if (i + 32 * u < nvec) st_stream(dv + i + 32 * u, shift_join(a[u], b[u], wsel, bsh));
+        const int bsh = (int)(sh & 3u) * 8;
+        switch (sh >> 2) {                                 // warp-uniform, once per piece
+        case 0:  drain_shifted_body<0>(sv, dv, nvec, bsh, lane); break;
+        case 1:  drain_shifted_body<1>(sv, dv, nvec, bsh, lane); break;
+        case 2:  drain_shifted_body<2>(sv, dv, nvec, bsh, lane); break;
+        default: drain_shifted_body<3>(sv, dv, nvec, bsh, lane); break;
         }
     }
     const unsigned int done = hb + (nvec << 4);
-    if (lane < len - done) dst[done + lane] = sm[ms + done + lane];          // tail < 16
+    if (done < len) {                                      // warp-uniform; tail < 16
+        if (lane < len - done) dst[done + lane] = sm[ms + done + lane];
+    }
 }
 
 #ifdef XDEV_TIMELINE
@@ -533,55 +559,60 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
 // allocation.  Up to VEC_SLOTS pieces are in flight per engine (bookkeeping in lanes 0..15, as in the bulk engine),
 // also across tile and segment boundaries.  A landed piece is moved to the destination by the whole warp
 // (warp_drain_shifted); its ring bytes are free as soon as the warp has read them.
-template <bool SM>
-__device__ __forceinline__ void vector_engine(Cursor<LIST_VEC, SM>& cur, unsigned char* ring, unsigned long long* mbar,
-                                              const unsigned int ringBytes) {
+// The engine runs on either work list (L): when the bulk list holds only a small part of a mostly unaligned call,
+// the vector engines sweep it up as well (plan_ring: bulkByVec) instead of idling warps as bulk engines.
+// Measured (R = 16, 360 MB each way, odd bf16 counts): the loop is instruction-issue bound, so per-piece work is kept
+// minimal -- tile state in registers, one packed slot word, word selection of the funnel shift resolved per piece.
+template <int L, bool SM>
+__device__ __forceinline__ void vector_engine(Cursor<L, SM>& cur, unsigned char* ring, unsigned long long* mbar,
+                                              const unsigned int ringBytes, int& pieceSeq) {
     const int lane = lane_id();
     const unsigned int tileBytes = 1u << cur.tileShift;
     const uint32_t ring0 = smem_u32(ring);
     unsigned long long mDst = 0;          // slot registers (lane j <-> slot j, j < VEC_SLOTS)
-    unsigned int mLen = 0, mOff = 0, mMs = 0, mV = 0;
-    unsigned int vHead = 0, phys = 0;
-    int iLoad = 0, iStore = 0;
-    unsigned int sub = 0;                 // bytes of the current tile already issued
+    unsigned int mPack = 0, mAlloc = 0;   // ring offset >> 7 | len << 11 | source misalignment << 24;  ring bytes to release
+    unsigned int used = 0, phys = 0;      // ring bytes held by pieces in flight (incl. wrap padding); allocation offset
+    int iLoad = pieceSeq, iStore = pieceSeq;   // piece numbers continue across the engine's runs: slot = number mod VEC_SLOTS, and the
+                                               // slot's mbarrier has completed number / VEC_SLOTS phases before this piece
+    unsigned long long tS = 0, tD = 0;    // the rest of the current tile
+    unsigned int tRem = 0;
     bool more = cur.ensure();
     while (true) {
         while (more) {
-            const long long toff = cur.tile_off();
-            const long long rest = cur.bytes - toff;
-            const unsigned int tlen = rest < (long long)tileBytes ? (unsigned int)rest : tileBytes;
-            const unsigned long long s = cur.src + (unsigned long long)toff + sub;
-            const unsigned long long d = cur.dst + (unsigned long long)toff + sub;
-            unsigned int len = VEC_SUB_BYTES - (unsigned int)(d & 15ull);
-            if (len > tlen - sub) len = tlen - sub;
+            if (tRem == 0) {
+                const long long toff = cur.tile_off();
+                const long long rest = cur.bytes - toff;
+                tRem = rest < (long long)tileBytes ? (unsigned int)rest : tileBytes;
+                tS = cur.src + (unsigned long long)toff;
+                tD = cur.dst + (unsigned long long)toff;
+            }
+            unsigned int len = VEC_SUB_BYTES - ((unsigned int)tD & 15u);
+            if (len > tRem) len = tRem;
             if (len < VEC_DIRECT_MAX) {                            // tiny piece: lanes copy it directly
-                const unsigned char* sp = reinterpret_cast<const unsigned char*>(s);
-                unsigned char* dp = reinterpret_cast<unsigned char*>(d);
+                const unsigned char* sp = reinterpret_cast<const unsigned char*>(tS);
+                unsigned char* dp = reinterpret_cast<unsigned char*>(tD);
                 for (unsigned int b = lane; b < len; b += 32) dp[b] = sp[b];
             } else {
-                const unsigned int ms = (unsigned int)(s & 15ull);
+                const unsigned int ms = (unsigned int)tS & 15u;
                 const unsigned int ld = (ms + len + 15u) & ~15u;
+                const unsigned int adv = (ld + 127u) & ~127u;
                 const unsigned int pad = phys + ld > ringBytes ? ringBytes - phys : 0u;   // wrap
-                const unsigned int vTail = iStore < iLoad ? __shfl_sync(0xffffffffu, mV, iStore % VEC_SLOTS) : vHead;
-                if (iLoad - iStore >= VEC_SLOTS || vHead + pad + ld - vTail > ringBytes) break;   // drain a landed piece first
-                const unsigned int vStart = vHead + pad;
+                if (iLoad - iStore >= VEC_SLOTS || used + pad + adv > ringBytes) break;   // drain a landed piece first
                 const unsigned int po = pad ? 0u : phys;
-                const int slot = iLoad % VEC_SLOTS;
-                if (lane == slot) { mDst = d; mLen = len; mOff = po; mMs = ms; mV = vStart; }
+                const int slot = iLoad & (VEC_SLOTS - 1);
+                if (lane == slot) { mDst = tD; mPack = (po >> 7) | (len << 11) | (ms << 24); mAlloc = pad + adv; }
                 if (lane == 0) {
                     const uint32_t bar = smem_u32(&mbar[slot]);
                     mbar_expect_tx(bar, ld);
-                    bulk_g2s(ring0 + po, reinterpret_cast<const void*>(s - ms), ld, bar);
+                    bulk_g2s(ring0 + po, reinterpret_cast<const void*>(tS - ms), ld, bar);
                 }
-                const unsigned int adv = (ld + 127u) & ~127u;
-                vHead = vStart + adv;
+                used += pad + adv;
                 phys = po + adv;
                 if (phys >= ringBytes) phys = 0;
                 ++iLoad;
             }
-            sub += len;
-            if (sub >= tlen) {
-                sub = 0;
+            tS += len; tD += len; tRem -= len;
+            if (tRem == 0) {
                 cur.next();
                 more = cur.ensure();
             }
@@ -591,18 +622,19 @@ __device__ __forceinline__ void vector_engine(Cursor<LIST_VEC, SM>& cur, unsigne
             phys = 0;                      // nothing in flight: restart the ring at offset 0 (the piece did not fit behind phys)
             continue;
         }
-        const int slot = iStore % VEC_SLOTS;
+        const int slot = iStore & (VEC_SLOTS - 1);
         mbar_wait(smem_u32(&mbar[slot]), (uint32_t)((iStore / VEC_SLOTS) & 1));
         const unsigned int dlo = __shfl_sync(0xffffffffu, (unsigned int)mDst, slot);
         const unsigned int dhi = __shfl_sync(0xffffffffu, (unsigned int)(mDst >> 32), slot);
-        const unsigned int slen = __shfl_sync(0xffffffffu, mLen, slot);
-        const unsigned int soff = __shfl_sync(0xffffffffu, mOff, slot);
-        const unsigned int sms = __shfl_sync(0xffffffffu, mMs, slot);
-        warp_drain_shifted(reinterpret_cast<unsigned char*>(((unsigned long long)dhi << 32) | dlo), ring + soff, sms, slen);
+        const unsigned int pk = __shfl_sync(0xffffffffu, mPack, slot);
+        used -= __shfl_sync(0xffffffffu, mAlloc, slot);
+        warp_drain_shifted(reinterpret_cast<unsigned char*>(((unsigned long long)dhi << 32) | dlo), ring + ((pk & 0x7ffu) << 7),
+                           pk >> 24, (pk >> 11) & 0x1fffu);
         ++iStore;
         __syncwarp();                      // every lane has read its words before the TMA may overwrite them
         if (lane == 0) fence_proxy_async_smem();
     }
+    pieceSeq = iLoad;
 }
 
 // The claim counters reset themselves: every CTA checks out once all its engines are drained (each
@@ -625,34 +657,46 @@ __device__ __forceinline__ void workctl_checkout(WorkCtl* ctl, bool used) {
 //   * no vector tiles: E bulk engines share the whole ring.  E = 4 for a call of few tiles per SM (bound by the
 //     per-tile latency of one elected lane -- measured: R = 64 with one 10 KB row per pair takes 40 us with one
 //     engine and 27 us with four), 2 up to 96 tiles per SM, else 1 (HBM-bound: one deep ring is slightly better,
-//     config 3: -0.7 % with two engines);
-//   * no bulk tiles: all 16 warps are vector engines with 1/16 of the ring each;
-//   * both: the vector engines get one 1/16 unit each, as many as their share of the bytes (1..9), the bulk engines
-//     the rest (>= 7/16 of the ring, which the host sized the bulk tile for).
+//     config 3: -0.7 % with two engines) -- but never fewer than the average tile size asks for (short tiles);
+//   * no bulk tiles, or the bulk list holds less than ~1/9 of the bytes: all 16 warps are vector engines with 1/16 of
+//     the ring each; they take the vector list first and then sweep up the bulk list (bulkByVec);
+//   * otherwise: the vector engines get one 1/16 unit each, as many as their share of the bytes (1..13), the bulk
+//     engines the rest (>= 3/16 of the ring; the host sized the bulk tile to fit that).
 struct RingPlan {
     int E, NV;                             // bulk engines = warps [0, E), vector engines = warps [E, E + NV)
+    bool bulkByVec;                        // the vector engines also process the bulk list (E == 0 although it has tiles)
     unsigned int bulkShare, vecShare;      // ring bytes per bulk / per vector engine (multiples of 128)
     unsigned int vecBase;                  // ring offset of vector engine 0's share
 };
 __device__ __forceinline__ RingPlan plan_ring(int requestedE, int bulkTiles, int vecTiles, int grid, unsigned int ringBytes,
-                                              int bulkShift, int vecShift) {
+                                              int bulkShift, int vecShift, long long bulkKiB) {
     RingPlan p;
     const unsigned int unit = (ringBytes / COPY_WARPS) & ~127u;
     unsigned int bulkBytes = ringBytes;
     p.NV = 0;
+    p.bulkByVec = false;
     if (vecTiles > 0) {
-        if (bulkTiles == 0) { p.NV = COPY_WARPS; bulkBytes = 0; }
+        const long long wb = (long long)bulkTiles << bulkShift, wv = (long long)vecTiles << vecShift;
+        if (wb * 8 <= wv) { p.NV = COPY_WARPS; bulkBytes = 0; p.bulkByVec = bulkTiles > 0; }
         else {
-            const long long wb = (long long)bulkTiles << bulkShift, wv = (long long)vecTiles << vecShift;
             p.NV = (int)((wv * COPY_WARPS + (wb + wv) / 2) / (wb + wv));
             p.NV = max(1, min(VEC_MAX_IN_BULK_MIX, p.NV));
             bulkBytes = ringBytes - (unsigned int)p.NV * unit;
         }
     }
     int E = 0;
-    if (bulkTiles > 0) {
+    if (bulkTiles > 0 && !p.bulkByVec) {
         E = requestedE;
-        if (E == 0) E = bulkTiles <= 48 * grid ? 4 : (bulkTiles <= 96 * grid ? 2 : 1);
+        if (E == 0) {
+            E = bulkTiles <= 48 * grid ? 4 : (bulkTiles <= 96 * grid ? 2 : 1);
+            // one engine turns a tile around in ~1.2 us (measured: R = 256 / 512 with one 14 KB row per pair, 1 vs 4
+            // engines: 173 -> 114 us, 587 -> 393 us), an SM's share of HBM is ~23 GB/s each way: E x average tile >= ~30 KB
+            if (bulkKiB >= 0) {
+                const long long avg = (bulkKiB << 10) / bulkTiles;
+                const int need = avg >= 30 * 1024 ? 1 : (avg >= 15 * 1024 ? 2 : 4);
+                E = max(E, need);
+            }
+        }
         while (E > 1 && (1u << bulkShift) > ((bulkBytes / (unsigned int)E) & ~127u)) E >>= 1;    // a tile must fit in one share
         if (E + p.NV > COPY_WARPS) E = COPY_WARPS - p.NV;
     }
@@ -670,6 +714,55 @@ __device__ __forceinline__ int static_first_chunk(int total, int nEngines, int k
     return max(1, min(km, total / (4 * nEngines)));
 }
 
+// Step a4 for one CTA: split warps and ring (plan_ring), run the engines.  Returns whether any dynamic claim counter
+// may have been used (grid-uniform; for workctl_checkout).  fusedStatic > 0: the single-launch path's static share.
+template <bool SM>
+__device__ __forceinline__ bool run_copy_engines(const SegDesc* desc, int* const colBase[2], int* const coarse[2], WorkCtl* ctl,
+                                                 const ClassParams& cls, int ncols, int colLen, int requestedE, int kmax,
+                                                 int fusedStatic, long long bulkKiB, int claimDiv, unsigned char* smem, unsigned long long* mbar,
+                                                 unsigned int ringBytes, unsigned long long* tl) {
+    __shared__ CursorEnv envs[2];
+    const int warp = threadIdx.x >> 5;
+    const int totB = colBase[LIST_BULK][ncols], totV = colBase[LIST_VEC][ncols];
+    const RingPlan rp = plan_ring(requestedE, totB, totV, (int)gridDim.x, ringBytes, cls.tileShift[LIST_BULK], cls.tileShift[LIST_VEC], bulkKiB);
+    const int nV = (int)gridDim.x * rp.NV;
+    const int nB = rp.bulkByVec ? nV : (int)gridDim.x * rp.E;
+    const int RR = ncols * colLen;
+    const int stB = fusedStatic > 0 ? fusedStatic : static_first_chunk(totB, nB, kmax, COPY_KMAX_LONG, RR);
+    const int stV = fusedStatic > 0 ? fusedStatic : static_first_chunk(totV, nV, COPY_KMAX_VEC, COPY_KMAX_LONG, RR);
+#ifdef XDEV_TIMELINE
+    if (tl) tl[TL_TILES] = (unsigned long long)totB;
+#endif
+    if (threadIdx.x == 0)
+        cursor_env_init(&envs[LIST_BULK], LIST_BULK, desc, colBase[LIST_BULK], coarse[LIST_BULK], &ctl->next[LIST_BULK], cls, ncols, colLen,
+                        nB, kmax, COPY_KMAX_LONG, stB, claimDiv);
+    if (threadIdx.x == 32)
+        cursor_env_init(&envs[LIST_VEC], LIST_VEC, desc, colBase[LIST_VEC], coarse[LIST_VEC], &ctl->next[LIST_VEC], cls, ncols, colLen,
+                        nV, COPY_KMAX_VEC, COPY_KMAX_LONG, stV, claimDiv);
+    __syncthreads();
+    if (warp < rp.E) {
+        Cursor<LIST_BULK, SM> cur;
+        cur.init(&envs[LIST_BULK], (int)blockIdx.x * rp.E + warp);
+        bulk_engine<SM>(cur, smem + (size_t)warp * rp.bulkShare, mbar + warp * COPY_SLOTS, rp.bulkShare, warp == 0 ? tl : nullptr);
+    } else if (warp < rp.E + rp.NV) {
+        const int v = warp - rp.E;
+        unsigned char* myRing = smem + rp.vecBase + (size_t)v * rp.vecShare;
+        unsigned long long* myBar = mbar + COPY_MAX_ENGINES * COPY_SLOTS + v * VEC_SLOTS;
+        int pieceSeq = 0;
+        {
+            Cursor<LIST_VEC, SM> cur;
+            cur.init(&envs[LIST_VEC], (int)blockIdx.x * rp.NV + v);
+            vector_engine<LIST_VEC, SM>(cur, myRing, myBar, rp.vecShare, pieceSeq);
+        }
+        if (rp.bulkByVec) {
+            Cursor<LIST_BULK, SM> cur;
+            cur.init(&envs[LIST_BULK], (int)blockIdx.x * rp.NV + v);
+            vector_engine<LIST_BULK, SM>(cur, myRing, myBar, rp.vecShare, pieceSeq);
+        }
+    }
+    return (nB > 0 && totB > stB * nB) || (nV > 0 && totV > stV * nV);
+}
+
 // Side job (see SideJob): warps [firstWarp, 16) of every CTA, before their engine role.
 __device__ __forceinline__ void run_side_job(const SideJob& j, int firstWarp) {
     const int warp = threadIdx.x >> 5;
@@ -684,7 +777,7 @@ __device__ __forceinline__ void run_side_job(const SideJob& j, int firstWarp) {
     }
 }
 
-// dynamic smem layout: [ring: ringBytes][mbar: COPY_MBAR_COUNT x u64][colBase bulk: R+1 ints][colBase vec: R+1 ints]
+// dynamic smem layout: [ring: ringBytes][mbar: COPY_MBAR_COUNT x u64][bulk KiB: i64][colBase bulk: R+1 ints][colBase vec: R+1 ints]
 //                      [coarse bulk: R*nb ints][coarse vec: R*nb ints]   (the last two only if useCoarse)
 __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const CopyArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -693,7 +786,8 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
     const int R = a.ncols;
     unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + a.ringBytes);
     int* colBase[2];
-    colBase[0] = reinterpret_cast<int*>(mbar + COPY_MBAR_COUNT);
+    long long* totKiB = reinterpret_cast<long long*>(mbar + COPY_MBAR_COUNT);
+    colBase[0] = reinterpret_cast<int*>(totKiB + 1);
     colBase[1] = colBase[0] + (R + 1);
     const int nbR = R * coarse_blocks(a.colLen);
     int* coarse[2] = {nullptr, nullptr};
@@ -727,34 +821,20 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
             if (c0 + lane < R) cb[c0 + lane + 1] = run + incl;
             run += __shfl_sync(0xffffffffu, incl, 31);
         }
+        if (warp == 1) {                   // bytes of the bulk list (-> average tile size, plan_ring)
+            long long k = 0;
+            for (int c = lane; c < R; c += 32) k += a.colKiB[c];
+            k = warp_sum(k);
+            if (lane == 0) *totKiB = k;
+        }
     }
     __syncthreads();
     TL_STAMP(tl, TL_READY);
 
-    const int totB = colBase[LIST_BULK][R], totV = colBase[LIST_VEC][R];
-    const RingPlan rp = plan_ring(a.bulkEngines, totB, totV, (int)gridDim.x, a.ringBytes, a.cls.tileShift[LIST_BULK],
-                                  a.cls.tileShift[LIST_VEC]);
-    const int nB = (int)gridDim.x * rp.E, nV = (int)gridDim.x * rp.NV;
-    const int RR = a.ncols * a.colLen;
-    const int stB = static_first_chunk(totB, nB, a.kmax, COPY_KMAX_LONG, RR);
-    const int stV = static_first_chunk(totV, nV, COPY_KMAX_VEC, COPY_KMAX_LONG, RR);
-#ifdef XDEV_TIMELINE
-    if (tl) tl[TL_TILES] = (unsigned long long)totB;
-#endif
     run_side_job(a.side, COPY_WARPS / 2);
-    if (warp < rp.E) {
-        Cursor<LIST_BULK> cur;
-        cur.init(a.desc, colBase[LIST_BULK], coarse[LIST_BULK], &a.ctl->next[LIST_BULK], a.cls, a.ncols, a.colLen, nB,
-                 (int)blockIdx.x * rp.E + warp, a.kmax, COPY_KMAX_LONG, stB);
-        bulk_engine<false>(cur, smem + (size_t)warp * rp.bulkShare, mbar + warp * COPY_SLOTS, rp.bulkShare, warp == 0 ? tl : nullptr);
-    } else if (warp < rp.E + rp.NV) {
-        const int v = warp - rp.E;
-        Cursor<LIST_VEC> cur;
-        cur.init(a.desc, colBase[LIST_VEC], coarse[LIST_VEC], &a.ctl->next[LIST_VEC], a.cls, a.ncols, a.colLen, nV,
-                 (int)blockIdx.x * rp.NV + v, COPY_KMAX_VEC, COPY_KMAX_LONG, stV);
-        vector_engine<false>(cur, smem + rp.vecBase + (size_t)v * rp.vecShare, mbar + COPY_MAX_ENGINES * COPY_SLOTS + v * VEC_SLOTS, rp.vecShare);
-    }
-    workctl_checkout(a.ctl, totB > stB * nB || totV > stV * nV);
+    const bool usedCounters = run_copy_engines<false>(a.desc, colBase, coarse, a.ctl, a.cls, a.ncols, a.colLen, a.bulkEngines, a.kmax, 0,
+                                                      *totKiB, COPY_CLAIM_DIV, smem, mbar, a.ringBytes, tl);
+    workctl_checkout(a.ctl, usedCounters);
     TL_STAMP(tl, TL_EXIT);
 }
 

@@ -12,19 +12,16 @@
 // L2-resident re-read of at most R*R*8 bytes per CTA).  The cross-column tile base is left to
 // the copy kernel, which scans the R per-column totals itself.
 //
-// This kernel sits on the small-message latency path (config 5: ~5 % of the call), so all global
-// loads are issued up front with high memory-level parallelism: each warp sums ROWS_PER_PASS rows
-// at once (ROWS_PER_PASS independent loads per lane per step) and the pointer tables are staged
-// in shared memory while those loads fly; phase 2 then only reads shared memory and streams out
-// its results.
+// This kernel sits on the small-message latency path (config 5: ~5 % of the call; a per-CTA %globaltimer timeline
+// of it is in profiles/r2_cfg5_timeline.md), so both phases are laid out for latency: phase 1 issues all global
+// loads up front (a few lanes per row, no warp scans), the pointer tables are staged in shared memory while
+// those loads fly, and phase 2 spreads the (column, row block) items over all warps and only reads shared memory.
 #pragma once
 #include "common.cuh"
 
 namespace xdev {
 
 constexpr int COUNTS_THREADS = 512;
-constexpr int COUNTS_ROWS_PER_PASS = 8;
-constexpr int COUNTS_COLS_UNROLL = 4;     // x32 lanes = 128 prefix columns per pass
 
 struct CountsArgs {
     const void* const* send;      // device table (null: no descriptors wanted, offsets and RC only)
@@ -36,9 +33,19 @@ struct CountsArgs {
     int W;                        // columns per CTA (<= 32)
     long long elemSize;               // bytes per count unit (an element, or a whole row for the top-k calls)
     ClassParams cls;
+#ifdef XDEV_TIMELINE
+    unsigned long long* timeline;     // [CTAs][8] globaltimer stamps (instrumented build only)
+#endif
 };
 
-// dynamic smem: long long cval[R][W+1], sofs[R][W+1] (+1: conflict-free column reads), u64 sendPtr[R], recvPtr[W]
+#ifdef XDEV_TIMELINE
+#define CT_STAMP(k) do { if (threadIdx.x == 0 && a.timeline) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); a.timeline[(size_t)blockIdx.x * 8 + (k)] = t_; } } while (0)
+#else
+#define CT_STAMP(k) do { } while (0)
+#endif
+
+// dynamic smem: long long cval[R][W+1], sofs[R][W+1] (+1: conflict-free column reads), u64 sendPtr[R], recvPtr[W],
+//               long long tileTot[W*nb], rowsBefore[W*nb], byteTot[W*nb]   (nb = ceil(R/32))
 __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int R = a.R, W = a.W, P = W + 1;
@@ -50,15 +57,22 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
     const int lane = lane_id();
     const int warp = threadIdx.x >> 5;
     constexpr int nwarps = COUNTS_THREADS / 32;
-    constexpr int RB = COUNTS_ROWS_PER_PASS;
-    constexpr int DU = COUNTS_COLS_UNROLL;
     const int d0 = blockIdx.x * W;
     const int Wc = min(W, R - d0);
 
+    CT_STAMP(0);
     griddep_launch_dependents();                 // let the copy kernel's CTAs start their prologue
+    // the count matrix is usually cold (the previous call streamed far more than L2 holds): the grid prefetches all of
+    // it into L2 with one DRAM round trip, before and after the dependency wait (before: while the stream's previous
+    // kernel drains; after: in case that took long enough for the lines to be evicted again)
+    const size_t cLines = ((size_t)R * R * 8 + 127) >> 7;
+    const size_t gtid = (size_t)blockIdx.x * COUNTS_THREADS + threadIdx.x, gthreads = (size_t)gridDim.x * COUNTS_THREADS;
+    for (size_t i = gtid; i < cLines; i += gthreads) prefetch_l2(reinterpret_cast<const char*>(a.C) + (i << 7));
     griddep_wait();                              // (launched with PDL itself: the stream's previous kernel must be complete)
-    // pointer tables: issue the loads now, park them in shared memory only after phase 1's loads are
-    // in flight too (one DRAM round trip instead of two on a cold start)
+    for (size_t i = gtid; i < cLines; i += gthreads) prefetch_l2(reinterpret_cast<const char*>(a.C) + (i << 7));
+    CT_STAMP(1);
+    // pointer tables: issue the loads now, park them in shared memory after phase 1's loads are in flight too (one
+    // DRAM round trip instead of two on a cold start)
     constexpr int PT = 2;                        // covers R <= 1024 with 512 threads
     unsigned long long sp[PT];
 #pragma unroll
@@ -67,80 +81,96 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
         sp[i] = (s < R && a.send) ? (unsigned long long)a.send[s] : 0ull;        // null tables: offsets only (top-k calls)
     }
     const unsigned long long rp = (threadIdx.x < Wc && a.recv) ? (unsigned long long)a.recv[d0 + threadIdx.x] : 0ull;
-    bool parked = false;
 
-    // ---- phase 1: warp per group of RB source rows: soff for the owned columns ---------------
+    // ---- phase 1: soff for the owned columns = row prefix C[s][0..d0) + running sum over the owned columns ------
+    // LPR lanes share a row (LPR = 512 / R rounded down to a power of two, 8..32): lane q sums the prefix columns
+    // q, q + LPR, ..., all loads independent (a handful per lane at R <= 128), then log2(LPR) shuffle steps combine
+    // the row.  (Round 1 gave a warp 8 rows and ran a 64-bit warp reduction AND a warp scan per row: ~5 us of
+    // dependent shuffles at R = 128; this is one round trip plus a few adds.)
+    int LPR = 32;
+    while (LPR > 8 && LPR * R > COUNTS_THREADS) LPR >>= 1;    // >= 8 lanes (64 contiguous bytes) per row: coalescing at large R
+    const int rowsPerPass = COUNTS_THREADS / LPR;
+    const int q = threadIdx.x & (LPR - 1);
     bool sawNeg = false;
-    for (int sb = warp * RB; sb < R; sb += nwarps * RB) {
-        long long part[RB], c[RB];
+    for (int row0 = 0; row0 < R; row0 += rowsPerPass) {
+        const int s = row0 + threadIdx.x / LPR;
+        const bool valid = s < R;
+        const long long* row = a.C + (size_t)(valid ? s : 0) * R;
+        constexpr int OW = 4;                                          // owned columns kept in registers (W <= 4: R <= 128)
+        long long own[OW];
 #pragma unroll
-        for (int r = 0; r < RB; ++r) {
-            part[r] = 0;
-            c[r] = (sb + r < R && lane < Wc) ? a.C[(size_t)(sb + r) * R + d0 + lane] : 0;
+        for (int j = 0; j < OW; ++j) own[j] = (valid && q == 0 && j < Wc) ? row[d0 + j] : 0;
+        long long part = 0;
+        constexpr int LU = 16;                                         // independent loads per trip
+        for (int dd = q; dd < d0; dd += LPR * LU) {
+            long long v[LU];
+#pragma unroll
+            for (int u = 0; u < LU; ++u) { const int x = dd + u * LPR; v[u] = (valid && x < d0) ? row[x] : 0; }
+#pragma unroll
+            for (int u = 0; u < LU; ++u) part += v[u] > 0 ? v[u] : 0;
         }
-        // prefix columns [0, d0): RB x DU independent loads are issued before any of them is consumed
-        for (int db = 0; db < d0; db += 32 * DU) {
-            long long v[RB][DU];
-#pragma unroll
-            for (int r = 0; r < RB; ++r) {
-#pragma unroll
-                for (int u = 0; u < DU; ++u) {
-                    const int d = db + u * 32 + lane;
-                    v[r][u] = (sb + r < R && d < d0) ? a.C[(size_t)(sb + r) * R + d] : 0;
-                }
-            }
-#pragma unroll
-            for (int r = 0; r < RB; ++r) {
-#pragma unroll
-                for (int u = 0; u < DU; ++u) part[r] += v[r][u] > 0 ? v[r][u] : 0;
-            }
-        }
-        if (!parked) {                                            // every thread passes here at most once
-            parked = true;
+        if (row0 == 0) {                                               // every thread passes here exactly once
 #pragma unroll
             for (int i = 0; i < PT; ++i) {
-                const int s = threadIdx.x + i * COUNTS_THREADS;
-                if (s < R) sendPtr[s] = sp[i];
+                const int t = threadIdx.x + i * COUNTS_THREADS;
+                if (t < R) sendPtr[t] = sp[i];
             }
             if (threadIdx.x < Wc) recvPtr[threadIdx.x] = rp;
         }
+        for (int o = LPR >> 1; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+        if (valid && q == 0) {
+            long long run = part;
 #pragma unroll
-        for (int r = 0; r < RB; ++r) {
-            const int s = sb + r;
-            if (s >= R) break;                                    // warp-uniform
-            const long long base = warp_sum(part[r]);
-            long long cc = c[r];
-            if (cc < 0) { sawNeg = true; cc = 0; }
-            const long long incl = warp_incl_scan(cc);
-            if (lane < Wc) {
-                const long long so = base + incl - cc;
-                cval[(size_t)s * P + lane] = cc;
-                sofs[(size_t)s * P + lane] = so;
-                a.ws.soff[(size_t)s * R + d0 + lane] = so;
+            for (int j = 0; j < OW; ++j) {
+                if (j < Wc) {
+                    long long cc = own[j];
+                    if (cc < 0) { sawNeg = true; cc = 0; }
+                    cval[(size_t)s * P + j] = cc;
+                    sofs[(size_t)s * P + j] = run;
+                    a.ws.soff[(size_t)s * R + d0 + j] = run;
+                    run += cc;
+                }
+            }
+            for (int j = OW; j < Wc; ++j) {
+                long long cc = row[d0 + j];
+                if (cc < 0) { sawNeg = true; cc = 0; }
+                cval[(size_t)s * P + j] = cc;
+                sofs[(size_t)s * P + j] = run;
+                a.ws.soff[(size_t)s * R + d0 + j] = run;
+                run += cc;
             }
         }
     }
-    if (!parked) {                                                // warps that owned no row group
-#pragma unroll
-        for (int i = 0; i < PT; ++i) {
-            const int s = threadIdx.x + i * COUNTS_THREADS;
-            if (s < R) sendPtr[s] = sp[i];
-        }
-        if (threadIdx.x < Wc) recvPtr[threadIdx.x] = rp;
-    }
     if (sawNeg) atomicOr(&a.ws.ctl->status, 1u);
+    CT_STAMP(2);
     __syncthreads();
+    CT_STAMP(3);
 
-    // ---- phase 2: warp per owned destination column d: RC, roff, descriptors, tile prefixes --
-    for (int j = warp; j < Wc; j += nwarps) {
-        const int d = d0 + j;
-        const unsigned long long dstBase = recvPtr[j];
-        long long run = 0;
-        int runT[2] = {0, 0};
-        const int nb = (R + 31) >> 5;
-        for (int s0 = 0; s0 < R; s0 += 32) {
-            if (lane < 2) a.ws.coarse[lane][(size_t)d * nb + (s0 >> 5)] = lane ? runT[1] : runT[0];     // coarse index for the copy kernel's search
-            const int s = s0 + lane;
+    // ---- phase 2: one work item per (owned column j, block b of 32 source rows), items round-robin over the warps ----
+    // (round 1 ran one warp per COLUMN, serially over the row blocks: with few columns per CTA most warps idled through
+    //  the longest dependent chain of the kernel.)  An item needs two column-wise prefixes: the elements before the block
+    //  (-> roff, destination addresses) and the tiles before it (-> work-list prefixes).  The first is a masked sum over
+    //  shared memory; the second depends on the first (tile counts depend on the addresses), so: pass 1 computes every
+    //  item's tile totals, pass 2 (after one barrier) recomputes the item with its tile base and writes everything out.
+    const int nb = (R + 31) >> 5;
+    const int nItems = Wc * nb;
+    long long* tileTot = reinterpret_cast<long long*>(recvPtr + W);      // [W*nb] tiles of the item: bulk << 32 | vector
+    long long* rowsBefore = tileTot + (size_t)W * nb;                    // [W*nb] elements of the column before the block
+    long long* byteTot = rowsBefore + (size_t)W * nb;                    // [W*nb] bytes of the item's bulk-list segments
+    for (int pass = 0; pass < 2; ++pass) {
+        for (int item = warp; item < nItems; item += nwarps) {
+            const int j = item / nb, b = item - j * nb;
+            const int d = d0 + j;
+            long long run;
+            if (pass == 0) {
+                long long part = 0;
+                for (int sp2 = lane; sp2 < b * 32; sp2 += 32) part += cval[(size_t)sp2 * P + j];
+                run = warp_sum(part);
+                if (lane == 0) rowsBefore[item] = run;
+            } else {
+                run = rowsBefore[item];
+            }
+            const int s = b * 32 + lane;
             const bool valid = s < R;
             const long long c = valid ? cval[(size_t)s * P + j] : 0;
             const long long incl = warp_incl_scan(c);
@@ -150,31 +180,49 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
             int tb = 0, tv = 0;
             if (valid) {
                 src = sendPtr[s] + (unsigned long long)(sofs[(size_t)s * P + j] * a.elemSize);
-                dst = dstBase + (unsigned long long)(ro * a.elemSize);
+                dst = recvPtr[j] + (unsigned long long)(ro * a.elemSize);
                 tb = seg_tiles(LIST_BULK, src, dst, bytes, a.cls);
                 tv = seg_tiles(LIST_VEC, src, dst, bytes, a.cls);
             }
             const long long it = warp_incl_scan(((long long)tb << 32) | (long long)(unsigned int)tv);   // both lists at once
-            const int ib = (int)(it >> 32);
-            const int iv = (int)(unsigned int)it;
+            if (pass == 0) {
+                const long long bb = warp_sum(tb > 0 ? bytes : 0);
+                if (lane == 31) tileTot[item] = it;
+                if (lane == 0) byteTot[item] = bb;
+                continue;
+            }
+            long long base = 0, allT = 0, allB = 0;                        // tiles of the column before this block / in total
+            for (int bp = lane; bp < nb; bp += 32) {
+                const long long t = tileTot[(size_t)j * nb + bp];
+                if (bp < b) base += t;
+                allT += t;
+                allB += byteTot[(size_t)j * nb + bp];
+            }
+            base = warp_sum(base);
+            if (lane < 2) a.ws.coarse[lane][(size_t)d * nb + b] = lane ? (int)(unsigned int)base : (int)(base >> 32);   // coarse index for the copy kernel's search
             if (valid) {
                 const size_t q = (size_t)d * R + s;
+                const long long pf = base + it;
                 a.RC[q] = c;
                 a.ws.roff[q] = ro;
                 uint4* out = reinterpret_cast<uint4*>(a.ws.desc + q);
                 out[0] = make_uint4((unsigned int)src, (unsigned int)(src >> 32), (unsigned int)dst, (unsigned int)(dst >> 32));
                 out[1] = make_uint4((unsigned int)bytes, (unsigned int)((unsigned long long)bytes >> 32),
-                                    (unsigned int)(runT[0] + ib), (unsigned int)(runT[1] + iv));
+                                    (unsigned int)(pf >> 32), (unsigned int)pf);
             }
-            run += __shfl_sync(0xffffffffu, incl, 31);
-            runT[0] += __shfl_sync(0xffffffffu, ib, 31);
-            runT[1] += __shfl_sync(0xffffffffu, iv, 31);
+            if (b == 0) {                                                  // column totals, once per column
+                allT = warp_sum(allT);
+                allB = warp_sum(allB);
+                if (lane == 0) {
+                    a.ws.colTiles[LIST_BULK][d] = (int)(allT >> 32);
+                    a.ws.colTiles[LIST_VEC][d] = (int)(unsigned int)allT;
+                    a.ws.colKiB[d] = (int)(allB >> 10);
+                }
+            }
         }
-        if (lane == 0) {
-            a.ws.colTiles[LIST_BULK][d] = runT[0];
-            a.ws.colTiles[LIST_VEC][d] = runT[1];
-        }
+        if (pass == 0) { __syncthreads(); CT_STAMP(4); }
     }
+    CT_STAMP(5);
 }
 
 }  // namespace xdev

@@ -7,7 +7,7 @@
 // reserved", Fig. 17).
 //
 // ONE metadata kernel (round 1 had two, 12 us in front of a 70 us copy):
-//   dyn_build_kernel  grid R x 1024 threads: CTA d builds column d of the table, slots k = s*J + j, j < J =
+//   dyn_build_kernel  grid R x 512 threads: CTA d builds column d of the table, slots k = s*J + j, j < J =
 //                     maxBlockLen, in s-major order.
 //     phase A  warp per source s (32 sources in flight per CTA): the warp re-derives what it needs of rank s's
 //              metadata instead of reading it from a preceding kernel -- list offset ioff[s][d] = sum of row s of
@@ -27,9 +27,11 @@
 
 namespace xdev {
 
-constexpr int DYN_THREADS = 1024;
+constexpr int DYN_THREADS = 512;
 constexpr int DYN_WARPS = DYN_THREADS / 32;
 constexpr int DYN_SMEM_SLOTS = 4096;      // columns up to this many slots are staged in shared memory (32 B per slot)
+constexpr int DYN_SU = 4;                 // sources a warp works on at once (their dependent loads overlap)
+constexpr int DYN_CHUNK = 128;            // split lengths scanned per step: 4 per lane
 
 struct DynArgs {
     const void* const* send;          // R
@@ -48,7 +50,11 @@ struct __align__(32) DynSlot {        // same 32-byte stride as SegDesc, so the 
     long long pad;
 };
 
-// dynamic smem: DynSlot[min(colLen, DYN_SMEM_SLOTS)] (none when the column is longer)
+__host__ __device__ inline size_t dyn_smem_bytes(int colLen) {
+    return (size_t)DYN_WARPS * DYN_SU * (DYN_CHUNK + 1) * 8 + (colLen <= DYN_SMEM_SLOTS ? (size_t)colLen * sizeof(DynSlot) : 0);
+}
+
+// dynamic smem: long long pref[DYN_WARPS][DYN_SU][DYN_CHUNK + 1], then DynSlot[colLen] if colLen <= DYN_SMEM_SLOTS
 __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs a) {
     extern __shared__ __align__(32) unsigned char dyn_smem[];
     __shared__ long long sWarpTot[DYN_WARPS];
@@ -57,80 +63,137 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
     const int R = a.R, n = a.n, J = a.maxBlockLen;
     const int colLen = R * J;
     const int nb = (colLen + 31) >> 5;
-    DynSlot* slots = colLen <= DYN_SMEM_SLOTS ? reinterpret_cast<DynSlot*>(dyn_smem)
+    long long* prefAll = reinterpret_cast<long long*>(dyn_smem);
+    DynSlot* slots = colLen <= DYN_SMEM_SLOTS ? reinterpret_cast<DynSlot*>(dyn_smem + (size_t)DYN_WARPS * DYN_SU * (DYN_CHUNK + 1) * 8)
                                               : reinterpret_cast<DynSlot*>(a.ws.desc + (size_t)d * colLen);
     griddep_launch_dependents();
     if (threadIdx.x == 0) sStatus = 0u;
     griddep_wait();                                        // the metadata may have been written by the stream's previous kernel
+    // pull the (cold) metadata into L2 with ONE DRAM round trip: the R CTAs prefetch disjoint slices of the three arrays,
+    // so the dependent loads below (block lengths -> list offset -> split index -> split offset) are L2 hits for all
+    {
+        const size_t gtid = (size_t)blockIdx.x * DYN_THREADS + threadIdx.x, gn = (size_t)gridDim.x * DYN_THREADS;
+        const size_t lL = ((size_t)R * n * 8 + 127) >> 7, lB = ((size_t)R * R * 8 + 127) >> 7, lI = ((size_t)R * a.maxIndices * 8 + 127) >> 7;
+        for (size_t i = gtid; i < lL + lB + lI; i += gn) {
+            const char* p = i < lL ? reinterpret_cast<const char*>(a.L) + (i << 7)
+                          : i < lL + lB ? reinterpret_cast<const char*>(a.blockLens) + ((i - lL) << 7)
+                                        : reinterpret_cast<const char*>(a.indices) + ((i - lL - lB) << 7);
+            prefetch_l2(p);
+        }
+    }
     unsigned int st = 0;
 
-    // ---- phase A: warp per source ----------------------------------------------------------------------------
-    for (int s = warp; s < R; s += DYN_WARPS) {
-        const long long* Ls = a.L + (size_t)s * n;
-        const long long* bls = a.blockLens + (size_t)s * R;
-        // round trip 1: row s of the block lengths, the first 128 split lengths, both base pointers
-        constexpr int PRE = 4;
-        long long lpre[PRE];
+    // ---- phase A: DYN_SU sources per warp at a time ------------------------------------------------------------
+    for (int sBase = warp; sBase < R; sBase += DYN_WARPS * DYN_SU) {
+        int src[DYN_SU];
+        long long lv[DYN_SU][4];                           // the first DYN_CHUNK split lengths: lane l holds 4l .. 4l+3
+        long long bv[DYN_SU][4];                           // the first 128 block lengths of row s: lane l holds l, l+32, ..
+        unsigned long long sp[DYN_SU], rp[DYN_SU];
+        // round trip 1: everything that does not depend on anything
 #pragma unroll
-        for (int u = 0; u < PRE; ++u) { const int i = u * 32 + lane; lpre[u] = i < n ? Ls[i] : 0; }
-        const unsigned long long sp = (unsigned long long)a.send[s];
-        const unsigned long long rp = (unsigned long long)a.recvbuffs[(size_t)d * R + s];
-        long long before = 0, mine = 0;
-        for (int d0 = 0; d0 < R; d0 += 32 * 4) {
-            long long v[4];
+        for (int u = 0; u < DYN_SU; ++u) {
+            const int s = sBase + u * DYN_WARPS;
+            src[u] = s;
+            const bool on = s < R;
+            const long long* Ls = a.L + (size_t)(on ? s : 0) * n;
+            const long long* bls = a.blockLens + (size_t)(on ? s : 0) * R;
 #pragma unroll
-            for (int u = 0; u < 4; ++u) { const int dd = d0 + u * 32 + lane; v[u] = dd < R ? bls[dd] : 0; }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int dd = d0 + u * 32 + lane;
-                if (v[u] < 0) { st |= 4u; v[u] = 0; }
-                if (v[u] > J) { st |= 4u; v[u] = J; }
-                if (dd < d) before += v[u];
-                if (dd == d) mine = v[u];
+            for (int q = 0; q < 4; ++q) {
+                const int i = 4 * lane + q;
+                lv[u][q] = (on && i < n) ? Ls[i] : 0;
+                const int dd = q * 32 + lane;
+                bv[u][q] = (on && dd < R) ? bls[dd] : 0;
             }
+            sp[u] = on ? (unsigned long long)a.send[s] : 0ull;
+            rp[u] = on ? (unsigned long long)a.recvbuffs[(size_t)d * R + s] : 0ull;
         }
-        const long long ioff = warp_sum(before);
-        const int bl = (int)warp_sum(mine);
+        long long ioff[DYN_SU];
+        int bl[DYN_SU];
+#pragma unroll
+        for (int u = 0; u < DYN_SU; ++u) {
+            long long before = 0, mine = 0;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int dd = q * 32 + lane;
+                long long v = bv[u][q];
+                if (v < 0) { st |= 4u; v = 0; }
+                if (v > J) { st |= 4u; v = J; }
+                if (dd < d) before += v;
+                if (dd == d) mine = v;
+            }
+            if (src[u] < R) {
+                const long long* bls = a.blockLens + (size_t)src[u] * R;
+                for (int dd = 128 + lane; dd < R; dd += 32) {      // R > 128: the rest of the row
+                    long long v = bls[dd];
+                    if (v < 0) { st |= 4u; v = 0; }
+                    if (v > J) { st |= 4u; v = J; }
+                    if (dd < d) before += v;
+                    if (dd == d) mine = v;
+                }
+            }
+            ioff[u] = warp_sum(before);
+            bl[u] = (int)warp_sum(mine);
+        }
         for (int j0 = 0; j0 < J; j0 += 32) {               // one pass per 32 list entries (J <= 32: one pass)
             const int j = j0 + lane;
-            // round trip 2: this lane's split index
-            long long idx = -1;
-            bool live = false;
-            if (j < bl) {
-                const long long pos = ioff + j;
-                if (pos >= a.maxIndices) st |= 4u;
-                else {
-                    idx = a.indices[(size_t)s * a.maxIndices + pos];
-                    if (idx < 0 || idx >= n) { st |= 2u; idx = -1; }
-                    else live = true;
-                }
-            }
-            // one scan per 32 split lengths; every lane picks offset and length of ITS split from the lane that holds it
-            long long base = 0, off = 0, len = 0;
-            for (int i0 = 0; i0 < n; i0 += 32) {
-                long long v;
-                if (i0 < PRE * 32) {
-                    v = lpre[0];
+            // round trip 2: this lane's split index, for all DYN_SU sources at once
+            long long idx[DYN_SU];
+            bool live[DYN_SU];
 #pragma unroll
-                    for (int u = 1; u < PRE; ++u) if ((i0 >> 5) == u) v = lpre[u];
-                } else {
-                    v = i0 + lane < n ? Ls[i0 + lane] : 0;
+            for (int u = 0; u < DYN_SU; ++u) {
+                idx[u] = -1; live[u] = false;
+                if (src[u] < R && j < bl[u]) {
+                    const long long pos = ioff[u] + j;
+                    if (pos >= a.maxIndices) st |= 4u;
+                    else idx[u] = a.indices[(size_t)src[u] * a.maxIndices + pos];
                 }
-                if (v < 0) { if (j0 == 0) st |= 1u; v = 0; }
-                const long long incl = warp_incl_scan(v);
-                const int from = (int)(idx - i0) & 31;
-                const long long po = __shfl_sync(0xffffffffu, base + incl - v, from);
-                const long long pl = __shfl_sync(0xffffffffu, v, from);
-                if (live && idx >= i0 && idx < i0 + 32) { off = po; len = pl; }
-                base += __shfl_sync(0xffffffffu, incl, 31);
             }
-            if (j < J) {
-                DynSlot o;
-                o.bytes = live ? len * a.elemSize : 0;
-                o.src = live ? sp + (unsigned long long)(off * a.elemSize) : 0ull;
-                o.dst = live ? rp + (unsigned long long)(off * a.elemSize) : 0ull;
-                o.pad = 0;
-                slots[(size_t)s * J + j] = o;
+#pragma unroll
+            for (int u = 0; u < DYN_SU; ++u) {
+                if (src[u] < R && j < bl[u] && ioff[u] + j < a.maxIndices) {
+                    if (idx[u] < 0 || idx[u] >= n) { st |= 2u; idx[u] = -1; }
+                    else live[u] = true;
+                }
+            }
+            // offsets: exclusive prefix sums of the split lengths, DYN_CHUNK at a time (lane-local 4 + one warp scan of the
+            // lane totals) into this warp's shared-memory strip; a lane then reads offset and length of ITS split
+#pragma unroll
+            for (int u = 0; u < DYN_SU; ++u) {
+                long long* pref = prefAll + ((size_t)warp * DYN_SU + u) * (DYN_CHUNK + 1);
+                long long base = 0, off = 0, len = 0;
+                if (src[u] < R) {
+                    const long long* Ls = a.L + (size_t)src[u] * n;
+                    for (int c0 = 0; c0 < n; c0 += DYN_CHUNK) {
+                        long long x[4];
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            const int i = c0 + 4 * lane + q;
+                            x[q] = c0 == 0 ? lv[u][q] : (i < n ? Ls[i] : 0);
+                            if (x[q] < 0) { if (j0 == 0) st |= 1u; x[q] = 0; }
+                        }
+                        const long long tot = x[0] + x[1] + x[2] + x[3];
+                        const long long incl = warp_incl_scan(tot);
+                        long long p = base + incl - tot;
+                        __syncwarp();                              // the previous chunk's readers are done
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) { pref[4 * lane + q] = p; p += x[q]; }
+                        if (lane == 31) pref[DYN_CHUNK] = p;
+                        __syncwarp();
+                        if (live[u] && idx[u] >= c0 && idx[u] < c0 + DYN_CHUNK) {
+                            off = pref[idx[u] - c0];
+                            len = pref[idx[u] - c0 + 1] - off;
+                        }
+                        base += __shfl_sync(0xffffffffu, incl, 31);
+                    }
+                    if (j < J) {
+                        DynSlot o;
+                        o.bytes = live[u] ? len * a.elemSize : 0;
+                        o.src = live[u] ? sp[u] + (unsigned long long)(off * a.elemSize) : 0ull;
+                        o.dst = live[u] ? rp[u] + (unsigned long long)(off * a.elemSize) : 0ull;
+                        o.pad = 0;
+                        slots[(size_t)src[u] * J + j] = o;
+                    }
+                }
             }
         }
     }
@@ -140,6 +203,7 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
 
     // ---- phase B: tile prefixes in slot order, descriptors, coarse index ------------------------------------------
     long long run = 0;                                     // tiles of the column before this round: bulk << 32 | vector
+    long long myBulkBytes = 0;
     for (int k0 = 0; k0 < colLen; k0 += DYN_THREADS) {
         const int k = k0 + threadIdx.x;
         DynSlot sl;
@@ -147,6 +211,7 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
         if (k < colLen) sl = slots[k];
         const int tb = seg_tiles(LIST_BULK, sl.src, sl.dst, sl.bytes, a.cls);
         const int tv = seg_tiles(LIST_VEC, sl.src, sl.dst, sl.bytes, a.cls);
+        if (tb > 0) myBulkBytes += sl.bytes;
         const long long it = warp_incl_scan(((long long)tb << 32) | (long long)(unsigned int)tv);
         if (lane == 31) sWarpTot[warp] = it;
         __syncthreads();
@@ -169,9 +234,15 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
         run += all;
         __syncthreads();                                   // sWarpTot is rewritten in the next round
     }
+    myBulkBytes = warp_sum(myBulkBytes);
+    if (lane == 0) sWarpTot[warp] = myBulkBytes;           // (the last round's barrier has passed: sWarpTot is free)
+    __syncthreads();
     if (threadIdx.x == 0) {
+        long long bb = 0;
+        for (int w = 0; w < DYN_WARPS; ++w) bb += sWarpTot[w];
         a.ws.colTiles[LIST_BULK][d] = (int)(run >> 32);
         a.ws.colTiles[LIST_VEC][d] = (int)(unsigned int)run;
+        a.ws.colKiB[d] = (int)(bb >> 10);
         if (sStatus) atomicOr(&a.ws.ctl->status, sStatus);
     }
 }

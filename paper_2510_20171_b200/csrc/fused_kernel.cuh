@@ -70,6 +70,7 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
     colT[0] = reinterpret_cast<int*>(rowTot + R);
     colT[1] = colT[0] + R;
     const bool writer = blockIdx.x == 0;
+    int* const nullptrs[2] = {nullptr, nullptr};
 
     griddep_launch_dependents();           // a following call of this library may start its prologue
     for (int i = threadIdx.x; i < COPY_MBAR_COUNT; i += COPY_THREADS) mbar_init(smem_u32(&mbar[i]), 1);
@@ -154,23 +155,10 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
     fence_proxy_async_smem();              // scratch reads/writes (generic proxy) before TMA writes to the same bytes
     __syncthreads();                       // the scratch is dead from here on; the ring may be filled
 
-    const int totB = colBase[LIST_BULK][R], totV = colBase[LIST_VEC][R];
-    const RingPlan rp = plan_ring(a.bulkEngines, totB, totV, (int)gridDim.x, a.ringBytes, cls.tileShift[LIST_BULK], cls.tileShift[LIST_VEC]);
-    const int nB = (int)gridDim.x * rp.E, nV = (int)gridDim.x * rp.NV;
-    // ---- a4: the copy engines of the big path, fed from shared memory --------------------------------
-    if (warp < rp.E) {
-        Cursor<LIST_BULK, true> cur;
-        cur.init(sdesc, colBase[LIST_BULK], nullptr, &a.ctl->next[LIST_BULK], cls, R, R, nB, (int)blockIdx.x * rp.E + warp,
-                 a.kmax, COPY_KMAX_LONG, 1);
-        bulk_engine<true>(cur, smem + (size_t)warp * rp.bulkShare, mbar + warp * COPY_SLOTS, rp.bulkShare, nullptr);
-    } else if (warp < rp.E + rp.NV) {
-        const int v = warp - rp.E;
-        Cursor<LIST_VEC, true> cur;
-        cur.init(sdesc, colBase[LIST_VEC], nullptr, &a.ctl->next[LIST_VEC], cls, R, R, nV, (int)blockIdx.x * rp.NV + v,
-                 COPY_KMAX_VEC, COPY_KMAX_LONG, 1);
-        vector_engine<true>(cur, smem + rp.vecBase + (size_t)v * rp.vecShare, mbar + COPY_MAX_ENGINES * COPY_SLOTS + v * VEC_SLOTS, rp.vecShare);
-    }
-    workctl_checkout(a.ctl, (nB > 0 && totB > nB) || (nV > 0 && totV > nV));
+    // ---- a4: the copy engines of the big path, fed from shared memory; the first tile of every engine is static ----
+    const bool usedCounters = run_copy_engines<true>(sdesc, colBase, nullptrs, a.ctl, cls, R, R, a.bulkEngines, a.kmax, 1, -1, 2, smem, mbar,
+                                                     a.ringBytes, nullptr);
+    workctl_checkout(a.ctl, usedCounters);
 }
 
 }  // namespace xdev

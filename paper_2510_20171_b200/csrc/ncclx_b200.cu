@@ -145,17 +145,22 @@ unsigned int chooseRingBytes(int ncols, int colLen) {
     return (unsigned int)(budget > aux ? (budget - aux) & ~(size_t)127 : 0);
 }
 
-// Smallest share of a ring the bulk engines of ONE engine warp can be left with (plan_ring in copy_kernel.cuh):
-// the vector engines take at most VEC_MAX_IN_BULK_MIX sixteenths, and `engines` bulk engines split the rest.
-size_t minBulkShare(size_t ring, int engines) {
+// What a bulk tile has to fit into (plan_ring in copy_kernel.cuh): ONCE into the smallest share the bulk engines can
+// be left with when the vector list has most of the bytes (the vector engines take at most VEC_MAX_IN_BULK_MIX
+// sixteenths of the ring; the device then runs one bulk engine), and ~2.5 times into an engine's share of the whole
+// ring when the call is all bulk.
+bool bulkTileFits(int tileShift, size_t ring, int engines) {
     const size_t unit = (ring / COPY_WARPS) & ~(size_t)127;
-    return (ring - VEC_MAX_IN_BULK_MIX * unit) / (size_t)(engines > 0 ? engines : 1);
+    const size_t tile = (size_t)1 << tileShift;
+    return tile <= ring - VEC_MAX_IN_BULK_MIX * unit && 5 * tile / 2 <= ring / (size_t)(engines > 0 ? engines : 1);
 }
 
-size_t countsSmemBytes(int R, int W) { return 2 * (size_t)R * (W + 1) * 8 + (size_t)(R + W) * 8; }
+size_t countsSmemBytes(int R, int W) { return 2 * (size_t)R * (W + 1) * 8 + (size_t)(R + W) * 8 + 3 * (size_t)W * ((R + 31) / 32) * 8; }
 
 int countsW(int R) {
-    // columns per CTA: spread over at most kScanCtas CTAs, at most 32 columns, and 2*R*(W+1)*8 <= smem
+    // columns per CTA: spread over at most kScanCtas CTAs (CTA j re-reads the row prefixes C[s][0..d0) from L2: more CTAs
+    // = more redundant reads -- one column per CTA at R = 128 was measured 2 us slower), at most 32 columns, and
+    // 2*R*(W+1)*8 <= smem
     int W = (R + kScanCtas - 1) / kScanCtas;
     if (W < 1) W = 1;
     if (W > 32) W = 32;
@@ -164,16 +169,15 @@ int countsW(int R) {
     return W;
 }
 
-// Tile sizes shared by the metadata kernel (tile prefixes) and the copy kernel: the bulk tile must fit 2.5 times into
-// the SMALLEST share any launch can give a bulk engine (max_ranks columns, a full coarse index, 9 vector engines).
+// Tile sizes shared by the metadata kernel (tile prefixes) and the copy kernel: the bulk tile must fit the SMALLEST
+// ring any launch can get (max_ranks columns, a full coarse index); see bulkTileFits.
 ClassParams classParams() {
     ClassParams c{};
     const size_t worstAux = COPY_MBAR_BYTES + 2 * (size_t)(g.maxRanks + 1) * 4 + kMaxCoarseBytes + 16 + 128;
     const size_t budget = copyBudget();
     const size_t ring = budget > worstAux ? budget - worstAux : 0;
-    const size_t share = minBulkShare(ring, (int)g.params[NCCLX_PARAM_COPY_BULK_ENGINES]);
     c.tileShift[0] = (int)g.params[NCCLX_PARAM_BULK_TILE_SHIFT];
-    while (c.tileShift[0] > 10 && ((size_t)5 << c.tileShift[0]) / 2 > share) --c.tileShift[0];
+    while (c.tileShift[0] > 10 && !bulkTileFits(c.tileShift[0], ring, (int)g.params[NCCLX_PARAM_COPY_BULK_ENGINES])) --c.tileShift[0];
     c.tileShift[1] = kVecTileShift;
     c.bulkMinBytes = g.params[NCCLX_PARAM_BULK_MIN_BYTES] < 16 ? 16 : g.params[NCCLX_PARAM_BULK_MIN_BYTES];
     return c;
@@ -199,8 +203,8 @@ int planCopy(CopyLaunch& cl, const Workspace& ws, const SegDesc* desc, const int
     cl.kmax = (int)g.params[NCCLX_PARAM_COPY_KMAX];
     cl.pdl = g.params[NCCLX_PARAM_PDL] ? 1 : 0;
     cl.ringBytes = chooseRingBytes(ncols, colLen);
-    // ~2.5 bulk tiles must fit into the smallest share a bulk engine can get; a larger tile could never be staged
-    if (((size_t)5 << cls.tileShift[0]) / 2 > minBulkShare(cl.ringBytes, cl.bulkEngines)) return NCCLX_ERR_ARG;
+    // the work list's bulk tile must fit this launch's ring (a larger tile could never be staged)
+    if (!bulkTileFits(cls.tileShift[0], cl.ringBytes, cl.bulkEngines)) return NCCLX_ERR_ARG;
     if ((size_t)VEC_SUB_BYTES + 256 > ((cl.ringBytes / COPY_WARPS) & ~127u)) return NCCLX_ERR_ARG;
     cl.smem = (size_t)cl.ringBytes + copyAuxBytes(ncols, colLen);
     return NCCLX_OK;
@@ -208,7 +212,7 @@ int planCopy(CopyLaunch& cl, const Workspace& ws, const SegDesc* desc, const int
 
 int launchCopy(const Workspace& ws, const CopyLaunch& cl, cudaStream_t stream) {
     CopyArgs cp{};
-    cp.desc = cl.desc; cp.colTiles[0] = ws.colTiles[0]; cp.colTiles[1] = ws.colTiles[1];
+    cp.desc = cl.desc; cp.colTiles[0] = ws.colTiles[0]; cp.colTiles[1] = ws.colTiles[1]; cp.colKiB = ws.colKiB;
     cp.coarse[0] = cl.coarse[0]; cp.coarse[1] = cl.coarse[1];
     cp.useCoarse = cl.useCoarse;
     cp.ctl = ws.ctl; cp.ncols = cl.ncols; cp.colLen = cl.colLen;
@@ -241,6 +245,9 @@ int launchCounts(const Workspace& ws, const void* const* send, const int64_t* C,
     ca.RC = reinterpret_cast<long long*>(RC);
     ca.ws = ws; ca.R = R; ca.W = countsW(R); ca.elemSize = es;
     ca.cls = cls;
+#ifdef XDEV_TIMELINE
+    ca.timeline = g.timeline + (size_t)g.smCount * TL_COUNT;      // counts-kernel stamps follow the copy kernel's
+#endif
     const int G = (R + ca.W - 1) / ca.W;
     const size_t csm = countsSmemBytes(R, ca.W);
     LaunchScope ls(NCCLX_KERNEL_COUNTS, stream);
@@ -266,7 +273,7 @@ int planFused(FusedArgs& fa, int R) {
     if (budget < aux + 64 * 1024) return NCCLX_ERR_ARG;
     fa.ringBytes = (unsigned int)((budget - aux) & ~(size_t)127);
     fa.bulkEngines = (int)g.params[NCCLX_PARAM_COPY_BULK_ENGINES];
-    while (fa.cls.tileShift[0] > 10 && ((size_t)5 << fa.cls.tileShift[0]) / 2 > minBulkShare(fa.ringBytes, fa.bulkEngines)) --fa.cls.tileShift[0];
+    while (fa.cls.tileShift[0] > 10 && !bulkTileFits(fa.cls.tileShift[0], fa.ringBytes, fa.bulkEngines)) --fa.cls.tileShift[0];
     fa.kmax = (int)g.params[NCCLX_PARAM_COPY_KMAX];
     fa.minTileShift[0] = kFusedMinTileShift < fa.cls.tileShift[0] ? kFusedMinTileShift : fa.cls.tileShift[0];
     fa.minTileShift[1] = 10 < fa.cls.tileShift[1] ? 10 : fa.cls.tileShift[1];
@@ -410,7 +417,10 @@ void freeAll() {
 
 template <typename K>
 int optInSmem(K kernel, int bytes) {
-    CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    cudaFuncAttributes fa{};
+    CK(cudaFuncGetAttributes(&fa, kernel));
+    const int room = g.maxSmemOptin - (int)fa.sharedSizeBytes;    // static + dynamic shared memory share the opt-in limit
+    CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes < room ? bytes : room));
     return NCCLX_OK;
 }
 
@@ -511,7 +521,7 @@ int prepareDynamic(int p, const void* const* send, const int64_t* L, int nsplits
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3((unsigned)R);
         cfg.blockDim = dim3(DYN_THREADS);
-        cfg.dynamicSmemBytes = colLen <= DYN_SMEM_SLOTS ? (size_t)colLen * sizeof(DynSlot) : 0;
+        cfg.dynamicSmemBytes = dyn_smem_bytes(colLen);
         cfg.stream = s;
         cudaLaunchAttribute attr[1];
         setPdl(cfg, attr, g.params[NCCLX_PARAM_PDL] != 0);
@@ -568,7 +578,7 @@ static int initLocked(int max_ranks, int device) {
     const size_t rr = (size_t)max_ranks * max_ranks;
     size_t off = 0;
     size_t oSoff[NCCLX_NUM_PLANS], oRoff[NCCLX_NUM_PLANS], oDesc[NCCLX_NUM_PLANS], oCt0[NCCLX_NUM_PLANS],
-        oCt1[NCCLX_NUM_PLANS], oCtl[NCCLX_NUM_PLANS], oCo0[NCCLX_NUM_PLANS], oCo1[NCCLX_NUM_PLANS];
+        oCt1[NCCLX_NUM_PLANS], oCtl[NCCLX_NUM_PLANS], oCo0[NCCLX_NUM_PLANS], oCo1[NCCLX_NUM_PLANS], oKib[NCCLX_NUM_PLANS];
     const size_t coarseInts = (size_t)max_ranks * coarse_blocks(max_ranks);
     for (int p = 0; p < NCCLX_NUM_PLANS; ++p) {
         oSoff[p] = off; off = alignUp(off + rr * 8, 256);
@@ -576,6 +586,7 @@ static int initLocked(int max_ranks, int device) {
         oDesc[p] = off; off = alignUp(off + rr * sizeof(SegDesc), 256);
         oCt0[p] = off; off = alignUp(off + (size_t)max_ranks * 4, 256);
         oCt1[p] = off; off = alignUp(off + (size_t)max_ranks * 4, 256);
+        oKib[p] = off; off = alignUp(off + (size_t)max_ranks * 4, 256);
         oCtl[p] = off; off = alignUp(off + sizeof(WorkCtl), 256);
         oCo0[p] = off; off = alignUp(off + coarseInts * 4, 256);
         oCo1[p] = off; off = alignUp(off + coarseInts * 4, 256);
@@ -592,6 +603,7 @@ static int initLocked(int max_ranks, int device) {
         w.desc = reinterpret_cast<SegDesc*>(b + oDesc[p]);
         w.colTiles[0] = reinterpret_cast<int*>(b + oCt0[p]);
         w.colTiles[1] = reinterpret_cast<int*>(b + oCt1[p]);
+        w.colKiB = reinterpret_cast<int*>(b + oKib[p]);
         w.ctl = reinterpret_cast<WorkCtl*>(b + oCtl[p]);
         w.coarse[0] = reinterpret_cast<int*>(b + oCo0[p]);
         w.coarse[1] = reinterpret_cast<int*>(b + oCo1[p]);
@@ -600,15 +612,15 @@ static int initLocked(int max_ranks, int device) {
     g.fusedCtl = reinterpret_cast<WorkCtl*>(b + oFctl);
     g.rcScratch = reinterpret_cast<long long*>(b + oRcs);
 #ifdef XDEV_TIMELINE
-    CK(cudaMalloc(&g.timeline, (size_t)g.smCount * TL_COUNT * 8));
-    CK(cudaMemset(g.timeline, 0, (size_t)g.smCount * TL_COUNT * 8));
+    CK(cudaMalloc(&g.timeline, ((size_t)g.smCount * TL_COUNT + 1024 * 8) * 8));
+    CK(cudaMemset(g.timeline, 0, ((size_t)g.smCount * TL_COUNT + 1024 * 8) * 8));
 #endif
 
     int rc;
     if ((rc = optInSmem(segment_copy_kernel, g.maxSmemOptin))) return rc;
     if ((rc = optInSmem(counts_kernel, g.maxSmemOptin))) return rc;
     if ((rc = optInSmem(alltoallv_fused_kernel, g.maxSmemOptin))) return rc;
-    if ((rc = optInSmem(dyn_build_kernel, DYN_SMEM_SLOTS * (int)sizeof(DynSlot)))) return rc;
+    if ((rc = optInSmem(dyn_build_kernel, (int)dyn_smem_bytes(DYN_SMEM_SLOTS)))) return rc;
     if ((rc = optInSmem(reducecopy_tma_kernel<RED_BF16>, RCT_SMEM_BYTES))) return rc;
     if ((rc = optInSmem(reducecopy_tma_kernel<RED_F32>, RCT_SMEM_BYTES))) return rc;
     if ((rc = optInSmem(reducecopy_tma_kernel<RED_F16>, RCT_SMEM_BYTES))) return rc;
@@ -1106,7 +1118,7 @@ int ncclx_debug_timeline(uint64_t* stamps_host, int max_ctas, int* fields) {
 #ifdef XDEV_TIMELINE
     if (!stamps_host || !fields || max_ctas < g.smCount) return NCCLX_ERR_ARG;
     CK(cudaDeviceSynchronize());
-    CK(cudaMemcpy(stamps_host, g.timeline, (size_t)g.smCount * TL_COUNT * 8, cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(stamps_host, g.timeline, ((size_t)g.smCount * TL_COUNT + 1024 * 8) * 8, cudaMemcpyDeviceToHost));
     *fields = TL_COUNT;
     return NCCLX_OK;
 #else
