@@ -701,10 +701,39 @@ def large_r_extra(torch, nx, peak, reps):
     return res
 
 
-def timeline_probe(torch, nx, peak, cfg_index=5):
+def timeline_probe(torch, nx, peak, cfg_index=5, workload=None):
     """Instrumented build only (python -m paper_2510_20171_b200.build --timeline; NCCLX_B200_LIB=<that .so>): per-CTA
-    %globaltimer stamps of ONE config-5 copy kernel -> where the time beyond bytes / bandwidth goes (start-up, ramp, tail)."""
-    a = A2A(W.a2a_config(cfg_index), torch, nx, with_back=False)
+    %globaltimer stamps of ONE copy kernel and the metadata kernel before it -> where the time beyond bytes / bandwidth
+    goes (start-up, ramp, tail).  workload: cfg5 (default), dynamic (NEXT-1's inference shape) or small64 (one 10 KB row per pair)."""
+    workload = workload or os.environ.get("NCCLX_TIMELINE_WORKLOAD", "cfg5")
+    if workload == "dynamic":
+        Ls, idx, bl, J = W.dynamic_moe_metadata()
+        R, n = Ls.shape
+        nx.ncclx_init_dynamic(n, R * R * J)
+        tot = Ls.sum(axis=1)
+        send = [W.torch_values(int(t), "bf16", 5000 + s) for s, t in enumerate(tot)]
+        recv = [torch.empty(int(tot[s]), dtype=torch.bfloat16, device="cuda") for d in range(R) for s in range(R)]
+        st, rt = nx.device_ptr_table(send), nx.device_ptr_table(recv)
+        allL = torch.empty((R, R, n), dtype=torch.int64, device="cuda")
+        Ld, Id, Bd = (torch.from_numpy(np.ascontiguousarray(x)).cuda() for x in (Ls, idx, bl))
+        moved = 0
+        for s_ in range(R):
+            pos = 0
+            for d in range(R):
+                moved += int(Ls[s_, idx[s_, pos:pos + bl[s_, d]]].sum()) * 2
+                pos += int(bl[s_, d])
+
+        class _Dyn:
+            bytes_one_way = moved
+
+            @staticmethod
+            def dispatch():
+                nx.ncclx_alltoallv_dynamic_dev(st, Ld, n, Id, idx.shape[1], Bd, J, rt, allL, R, "bf16")
+        a = _Dyn
+    elif workload == "small64":
+        a = A2A(W.A2AConfig("small64", 64, 5120, "bf16", 1, np.ones((64, 64), np.int64)), torch, nx, with_back=False)
+    else:
+        a = A2A(W.a2a_config(cfg_index), torch, nx, with_back=False)
     for _ in range(5):
         a.dispatch()
     torch.cuda.synchronize()
@@ -715,6 +744,9 @@ def timeline_probe(torch, nx, peak, cfg_index=5):
     t0 = int(min(tl[:, 0].min(), ct[:, 0].min() if len(ct) else tl[:, 0].min()))
     cols = {nm: (tl[:, i] - t0) / 1e3 for i, nm in enumerate(names)}           # us since the first CTA of either kernel entered
     out = {"ctas": int(tl.shape[0]), "bulk_tiles": int(tl[0, 7]), "bytes_moved": 2 * a.bytes_one_way, "us": {}}
+    if tl.shape[1] > 10:                                                  # finer start-up stamps of CTA thread 0 (bulk engine 0)
+        for i, nm in ((8, "env_ready"), (9, "cursor_init_done"), (10, "first_ensure_done")):
+            cols[nm] = (tl[:, i] - t0) / 1e3
     for nm, v in cols.items():
         out["us"][nm] = {"min": round(float(v.min()), 2), "median": round(float(np.median(v)), 2), "max": round(float(v.max()), 2)}
     cnames = ["enter", "dependency_wait_over", "phase1_done", "barrier_passed", "tile_totals_known", "exit"]

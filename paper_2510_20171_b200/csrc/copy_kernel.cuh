@@ -454,7 +454,7 @@ __device__ __forceinline__ void warp_drain_shifted(unsigned char* dst, const uns
 }
 
 #ifdef XDEV_TIMELINE
-enum { TL_ENTER = 0, TL_READY, TL_FIRST_LOAD, TL_FIRST_STORE, TL_LAST_STORE, TL_DRAINED, TL_EXIT, TL_TILES, TL_COUNT };
+enum { TL_ENTER = 0, TL_READY, TL_FIRST_LOAD, TL_FIRST_STORE, TL_LAST_STORE, TL_DRAINED, TL_EXIT, TL_TILES, TL_ENV, TL_CURSOR, TL_ENSURED, TL_COUNT };
 __device__ __forceinline__ unsigned long long tl_now() {
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
@@ -485,6 +485,7 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
     unsigned int vHead = 0, phys = 0;     // virtual (mod 2^32) and physical allocation offsets
     int iLoad = 0, iStore = 0, freed = 0;  // stores [0, freed) have finished reading their smem; freed <= iStore <= iLoad
     bool more = cur.ensure();
+    TL_STAMP(tl, TL_ENSURED);
     while (true) {
         // fill: issue loads while a slot and enough ring bytes are free
         while (more) {
@@ -740,9 +741,11 @@ __device__ __forceinline__ bool run_copy_engines(const SegDesc* desc, int* const
         cursor_env_init(&envs[LIST_VEC], LIST_VEC, desc, colBase[LIST_VEC], coarse[LIST_VEC], &ctl->next[LIST_VEC], cls, ncols, colLen,
                         nV, COPY_KMAX_VEC, COPY_KMAX_LONG, stV, claimDiv);
     __syncthreads();
+    TL_STAMP(tl, TL_ENV);
     if (warp < rp.E) {
         Cursor<LIST_BULK, SM> cur;
         cur.init(&envs[LIST_BULK], (int)blockIdx.x * rp.E + warp);
+        if (warp == 0) TL_STAMP(tl, TL_CURSOR);
         bulk_engine<SM>(cur, smem + (size_t)warp * rp.bulkShare, mbar + warp * COPY_SLOTS, rp.bulkShare, warp == 0 ? tl : nullptr);
     } else if (warp < rp.E + rp.NV) {
         const int v = warp - rp.E;

@@ -42,7 +42,16 @@ struct DynArgs {
     Workspace ws;                     // desc / coarse / colTiles / ctl of the plan slot
     int R, n, maxIndices, maxBlockLen, elemSize;
     ClassParams cls;
+#ifdef XDEV_TIMELINE
+    unsigned long long* timeline;     // [CTAs][8] globaltimer stamps (instrumented build only; same layout as counts_kernel's)
+#endif
 };
+
+#ifdef XDEV_TIMELINE
+#define DY_STAMP(k) do { if (threadIdx.x == 0 && a.timeline) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); a.timeline[(size_t)blockIdx.x * 8 + (k)] = t_; } } while (0)
+#else
+#define DY_STAMP(k) do { } while (0)
+#endif
 
 struct __align__(32) DynSlot {        // same 32-byte stride as SegDesc, so the table itself can serve as the slot array
     unsigned long long src, dst;
@@ -66,9 +75,11 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
     long long* prefAll = reinterpret_cast<long long*>(dyn_smem);
     DynSlot* slots = colLen <= DYN_SMEM_SLOTS ? reinterpret_cast<DynSlot*>(dyn_smem + (size_t)DYN_WARPS * DYN_SU * (DYN_CHUNK + 1) * 8)
                                               : reinterpret_cast<DynSlot*>(a.ws.desc + (size_t)d * colLen);
+    DY_STAMP(0);
     griddep_launch_dependents();
     if (threadIdx.x == 0) sStatus = 0u;
     griddep_wait();                                        // the metadata may have been written by the stream's previous kernel
+    DY_STAMP(1);
     // pull the (cold) metadata into L2 with ONE DRAM round trip: the R CTAs prefetch disjoint slices of the three arrays,
     // so the dependent loads below (block lengths -> list offset -> split index -> split offset) are L2 hits for all
     {
@@ -199,7 +210,9 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
     }
     st = __reduce_or_sync(0xffffffffu, st);
     if (lane == 0 && st) atomicOr(&sStatus, st);
+    DY_STAMP(2);
     __syncthreads();
+    DY_STAMP(3);
 
     // ---- phase B: tile prefixes in slot order, descriptors, coarse index ------------------------------------------
     long long run = 0;                                     // tiles of the column before this round: bulk << 32 | vector
@@ -234,6 +247,7 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
         run += all;
         __syncthreads();                                   // sWarpTot is rewritten in the next round
     }
+    DY_STAMP(4);
     myBulkBytes = warp_sum(myBulkBytes);
     if (lane == 0) sWarpTot[warp] = myBulkBytes;           // (the last round's barrier has passed: sWarpTot is free)
     __syncthreads();
@@ -245,6 +259,7 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
         a.ws.colKiB[d] = (int)(bb >> 10);
         if (sStatus) atomicOr(&a.ws.ctl->status, sStatus);
     }
+    DY_STAMP(5);
 }
 
 }  // namespace xdev

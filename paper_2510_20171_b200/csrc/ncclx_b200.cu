@@ -515,6 +515,9 @@ int prepareDynamic(int p, const void* const* send, const int64_t* L, int nsplits
     da.ws = ws;
     da.R = R; da.n = nsplits; da.maxIndices = maxIndices; da.maxBlockLen = maxBlockLen; da.elemSize = es;
     da.cls = cl.cls;
+#ifdef XDEV_TIMELINE
+    da.timeline = g.timeline + (size_t)g.smCount * TL_COUNT;
+#endif
     ps.kind = PLAN_NONE;
     {
         LaunchScope ls(NCCLX_KERNEL_DYN, s);
