@@ -749,7 +749,9 @@ def timeline_probe(torch, nx, peak, cfg_index=5, workload=None):
             cols[nm] = (tl[:, i] - t0) / 1e3
     for nm, v in cols.items():
         out["us"][nm] = {"min": round(float(v.min()), 2), "median": round(float(np.median(v)), 2), "max": round(float(v.max()), 2)}
-    cnames = ["enter", "dependency_wait_over", "phase1_done", "barrier_passed", "tile_totals_known", "exit"]
+    cnames = (["enter", "dependency_wait_over", "list_offsets_known", "split_indices_known", "phaseA_done", "barrier_passed",
+               "phaseB_done", "exit"] if workload == "dynamic" else
+              ["enter", "dependency_wait_over", "phase1_done", "barrier_passed", "tile_totals_known", "exit"])
     out["counts_kernel_ctas"] = int(len(ct))
     out["counts_kernel_us"] = {nm: {"min": round(float(((ct[:, i] - t0) / 1e3).min()), 2), "median": round(float(np.median((ct[:, i] - t0) / 1e3)), 2),
                                      "max": round(float(((ct[:, i] - t0) / 1e3).max()), 2)} for i, nm in enumerate(cnames)} if len(ct) else {}
@@ -759,6 +761,7 @@ def timeline_probe(torch, nx, peak, cfg_index=5, workload=None):
     out["median_cta_streaming_window_us"] = round(busy, 2)
     out["at_6.9TBps_us"] = round(2 * a.bytes_one_way / 6.9e12 * 1e6, 2)
     out["per_cta"] = [[round(float(cols[nm][i]), 2) for nm in names] for i in range(tl.shape[0])]
+    out["metadata_kernel_per_cta"] = [[round(float((ct[c, i] - t0) / 1e3), 2) for i in range(len(cnames))] for c in range(len(ct))]
     return out
 
 

@@ -275,12 +275,13 @@ int ncclx_reducescatter_sum_host(const void* const* send, void* const* recv, siz
 typedef enum {
     NCCLX_PARAM_BULK_MIN_BYTES = 0,     /* 16B-aligned segments >= this many bytes go on the bulk list (32 KiB tiles, TMA in and out);  */
                                         /* smaller or unaligned ones on the vector list (TMA in, warp stores out). default 1024         */
-    NCCLX_PARAM_REDUCE_CTAS_PER_SM = 1, /* reduce grid = this * SM count (1..64), default 8 (more CTAs than fit at once: the hardware  */
-                                        /* scheduler evens out short calls)                                                            */
+    NCCLX_PARAM_REDUCE_CTAS_PER_SM = 1, /* reduce grid = this * SM count (1..64), default 16 (4x what fits at once: a short call such  */
+                                        /* as config 2 becomes one tile per CTA, dealt out by the hardware scheduler)                  */
     NCCLX_PARAM_PROFILE = 2,            /* 1: bracket each kernel with CUDA events (never while capturing)                              */
     NCCLX_PARAM_BULK_TILE_SHIFT = 3,    /* log2 bytes of a bulk tile (12..16), default 15                                               */
     NCCLX_PARAM_PDL = 4,                /* 1 (default): programmatic dependent launch -- a kernel's prologue overlaps the tail of the   */
-                                        /* kernel before it (reductions: only below 1 GiB of input); 0: plain stream order              */
+                                        /* kernel before it (reductions: only below 1 GiB of input, and their CTAs prefetch their first */
+                                        /* input tiles into L2 while they wait); 0: plain stream order                                  */
     NCCLX_PARAM_COPY_KMAX = 5,          /* max bulk tiles per dynamic claim when segments are short (1..64), default 6                  */
     NCCLX_PARAM_FUSED_MAX_RANKS = 6,    /* ncclx_alltoallv_dev runs as ONE kernel for R <= this (0..32; 0 = never), default 32          */
     NCCLX_PARAM_COPY_BULK_ENGINES = 7,  /* bulk (TMA) engine warps per copy CTA: 1, 2, 4, or 0 (default): chosen on the device -- 4 for */

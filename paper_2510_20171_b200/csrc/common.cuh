@@ -92,6 +92,33 @@ __device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wa
 // griddepcontrol.wait cannot go stale) -- used to pull cold metadata into L2 in ONE DRAM round trip.
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
 
+// ---- L2 eviction priorities -------------------------------------------------------------------
+// A call's METADATA (count matrix, pointer tables, split lengths, index lists: a few hundred KB) is read again by the
+// next call, but the payload streamed in between is many times the 126 MB L2, so by then every metadata line has gone
+// back to DRAM and the metadata kernel pays cold-DRAM round trips (measured with per-CTA %globaltimer stamps: 1-2.5 us
+// each, worse from the die the line does not live on).  Metadata loads therefore carry an evict_last policy, payload
+// bulk copies an evict_first one: the stream passes through L2 without displacing what will be read again.
+__device__ __forceinline__ unsigned long long l2_policy_keep() {
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ unsigned long long l2_policy_stream() {
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ long long ld_keep(const long long* a, unsigned long long pol) {
+    long long v;
+    asm volatile("ld.global.L2::cache_hint.b64 %0, [%1], %2;" : "=l"(v) : "l"(a), "l"(pol) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned long long ld_keep_ptr(const void* const* a, unsigned long long pol) {
+    unsigned long long v;
+    asm volatile("ld.global.L2::cache_hint.b64 %0, [%1], %2;" : "=l"(v) : "l"(a), "l"(pol) : "memory");
+    return v;
+}
+
 // ---- streaming global accesses --------------------------------------------------------------
 // (No ld.global.nc anywhere: with programmatic dependent launch a kernel's CTAs are resident while the kernel before
 // it in the stream still writes the very bytes they will read after griddepcontrol.wait, and the non-coherent path
@@ -155,6 +182,15 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 __device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void* src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  :: "r"(dst_smem), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+// the same two with an L2 eviction policy (payload: l2_policy_stream())
+__device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void* src, uint32_t bytes, uint32_t bar, unsigned long long pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 :: "r"(dst_smem), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src_smem, uint32_t bytes, unsigned long long pol) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+                 :: "l"(dst), "r"(src_smem), "r"(bytes), "l"(pol) : "memory");
 }
 // shared -> global, tracked by the issuing thread's bulk async-group
 __device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src_smem, uint32_t bytes) {

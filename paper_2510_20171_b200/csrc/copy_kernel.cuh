@@ -39,7 +39,18 @@ constexpr int COPY_MBAR_COUNT = COPY_MAX_ENGINES * COPY_SLOTS + COPY_WARPS * VEC
 constexpr int COPY_MBAR_BYTES = COPY_MBAR_COUNT * 8;
 constexpr int COPY_KMAX_LONG = 2;          // max tiles per dynamic claim when segments average >= 8 tiles (measured: config 3)
 constexpr int COPY_KMAX_VEC = 8;           // max tiles per dynamic claim on the vector list
-constexpr int COPY_CLAIM_DIV = 4;          // guided claims: K = remaining / (COPY_CLAIM_DIV * engines), clamped to [1, kmax]: an engine holds up to three
+#ifndef XDEV_PAYLOAD_POLICY
+#define XDEV_PAYLOAD_POLICY 1              // 1: payload bulk copies carry an L2 evict_first policy (common.cuh); 0: none (A/B builds)
+#endif
+#if XDEV_PAYLOAD_POLICY
+#define PAYLOAD_POL(p) , p
+#else
+#define PAYLOAD_POL(p)
+#endif
+#ifndef XDEV_CLAIM_DIV
+#define XDEV_CLAIM_DIV 8
+#endif
+constexpr int COPY_CLAIM_DIV = XDEV_CLAIM_DIV;          // guided claims: K = remaining / (COPY_CLAIM_DIV * engines), clamped to [1, kmax]: an engine holds up to three
                                            // chunks (current, staged, claimed), so chunks shrink early (config 5: 2 -> 4: 163 -> 157 us with two engines)
 
 // Optional side job for the warps that are not engines at the start of the kernel: `copies` copies of the int64
@@ -99,10 +110,11 @@ struct CursorEnv {
     int staticK;                           // first chunk is assigned statically: [engineId*staticK, +staticK)
     int dynBase;                           // tiles >= dynBase are claimed dynamically
     bool longSegs, indexed, pipelined;
+    bool rr;                               // chunks are dealt round-robin (engine e takes chunks e, e + nEngines, ...): no claim counter
 };
 __device__ __forceinline__ void cursor_env_init(CursorEnv* e, int L, const SegDesc* desc, const int* colBase, const int* coarse,
                                                 unsigned int* counter, const ClassParams& cls, int ncols, int colLen, int nEngines,
-                                                int kmax, int kmaxLong, int staticK, int claimDiv) {
+                                                int kmax, int kmaxLong, int staticK, int claimDiv, bool rr) {
     e->desc = desc; e->colBase = colBase; e->coarse = coarse; e->counter = counter; e->cls = cls;
     e->ncols = ncols; e->colLen = colLen; e->nb = coarse_blocks(colLen); e->RR = ncols * colLen;
     e->total = colBase[ncols];
@@ -115,11 +127,41 @@ __device__ __forceinline__ void cursor_env_init(CursorEnv* e, int L, const SegDe
     e->pipelined = e->indexed && !e->longSegs;
     e->kmax = e->longSegs ? kmaxLong : kmax;
     e->staticK = staticK;
+    e->rr = rr;
     e->claimDiv = claimDiv;
     // a short list (few tiles per engine) pays per claim, a long one for the imbalance of its last chunks
-    e->kmin = e->total >= 32 * e->nEngines ? 1 : 2;
+#ifndef XDEV_KMIN1
+#define XDEV_KMIN1 0
+#endif
+    e->kmin = (XDEV_KMIN1 || e->total >= 32 * e->nEngines) ? 1 : 2;
     e->dynBase = staticK * e->nEngines;
     (void)L;
+}
+
+// Number of entries of the non-decreasing shared-memory array arr[0..n) that are <= key, found by the whole warp: 32-ary
+// rounds (every lane probes the last entry of one block, one ballot per round) instead of a binary search's chain of
+// dependent shared-memory loads -- 2 rounds for n <= 1024 where the binary search needed 10.  Warp-uniform result.
+__device__ __forceinline__ int warp_count_le(const int* arr, int n, int key) {
+    const int lane = lane_id();
+    int base = 0, span = n;
+    while (span > 32) {
+        const int step = (span + 31) >> 5;
+        const int i = (lane + 1) * step - 1;               // last entry of block `lane` (blocks that stick out do not count)
+        const bool le = i < span && arr[base + i] <= key;
+        const int m = __popc(__ballot_sync(0xffffffffu, le));
+        base += m * step;
+        span = min(step, n - base);
+    }
+    const bool le = lane < span && arr[base + lane] <= key;
+    return base + __popc(__ballot_sync(0xffffffffu, le));
+}
+
+// K = clamp(avail / unit, lo, hi) without a division (hi is small: a handful of multiply-compares)
+__device__ __forceinline__ int clamped_quotient(int avail, int unit, int lo, int hi) {
+    if (hi > 8) return max(lo, min(hi, avail / unit));
+    int k = lo;
+    while (k < hi && (k + 1) * unit <= avail) ++k;
+    return k;
 }
 
 template <int L, bool SM = false>
@@ -127,6 +169,7 @@ struct Cursor {
     const CursorEnv* env;                  // everything that is the same for all engines of the list (shared memory)
     int tileShift, engineId;
     int pendCur, pendK;                    // lane 0: a chunk claimed ahead of need (atomic in flight)
+    int rrNext;                            // round-robin mode: this engine's next chunk
     int t, tEnd;                           // current tile, end of the claimed chunk
     int q, kInSeg, segTiles;               // current segment, tile within it, its tile count
     unsigned long long src, dst;
@@ -170,6 +213,7 @@ struct Cursor {
         engineId = engineId_;
         tileShift = env_->cls.tileShift[L];
         pendCur = env->total; pendK = 0;        // reads as "drained" unless a claim is issued
+        rrNext = env->dynBase + engineId * env->staticK;
         t = tEnd = 0; q = 0; kInSeg = segTiles = 0; src = dst = 0; bytes = 0;
         qw = qn = 0; w0 = w1 = n0 = n1 = c0 = c1 = make_uint4(0, 0, 0, 0);
         cCur = cK = cQw = cEnd = cPrev = cTl = 0;
@@ -193,9 +237,13 @@ struct Cursor {
     // Lane 0 issues the atomic for a later dynamic chunk; the result is consumed one chunk (env->pipelined:
     // two chunks) later, so its L2 round trip overlaps the copying.
     __device__ __forceinline__ void claim_issue(int counterHint) {
+        if (env->rr) {                          // all lanes alike; no atomic
+            pendK = env->staticK; pendCur = rrNext; rrNext += env->staticK * env->nEngines;
+            return;
+        }
         if (lane_id() == 0) {
             const int rem = env->total - min(env->total, counterHint);
-            pendK = max(env->kmin, min(env->kmax, rem / (env->claimDiv * env->nEngines)));
+            pendK = clamped_quotient(rem, env->claimDiv * env->nEngines, env->kmin, env->kmax);
             pendCur = env->dynBase + (int)atomicAdd(env->counter, (unsigned int)pendK);
         }
     }
@@ -203,22 +251,15 @@ struct Cursor {
     // Shared-memory search: column d that owns global tile tt, tile index tl inside the column, the
     // 32-descriptor block j of the column that holds it and the tiles of the column before that block.
     __device__ __forceinline__ void find_block(int tt, int& d, int& tl, int& j, int& prev) const {
-        int lo = 0, hi = env->ncols;            // env->colBase[lo] <= tt < env->colBase[hi]
-        while (hi - lo > 1) {
-            const int mid = (lo + hi) >> 1;
-            if (env->colBase[mid] <= tt) lo = mid; else hi = mid;
-        }
-        d = lo;
-        tl = tt - env->colBase[d];
+        const int* cb = env->colBase;
+        d = warp_count_le(cb + 1, env->ncols, tt);          // cb[d] <= tt < cb[d+1]  (cb[ncols] = total > tt)
+        tl = tt - cb[d];
         j = 0; prev = 0;
-        if (env->nb > 1) {
-            const int* cr = env->coarse + d * env->nb;
-            int a = 0, b = env->nb;             // cr[a] <= tl < cr[b]  (cr[env->nb] = +inf)
-            while (b - a > 1) {
-                const int mid = (a + b) >> 1;
-                if (cr[mid] <= tl) a = mid; else b = mid;
-            }
-            j = a; prev = cr[a];
+        const int nb = env->nb;
+        if (nb > 1) {
+            const int* cr = env->coarse + d * nb;            // cr[0] = 0, non-decreasing
+            j = warp_count_le(cr + 1, nb - 1, tl);           // cr[j] <= tl < cr[j+1]  (cr[nb] = +inf)
+            prev = cr[j];
         }
     }
     // The current window holds the segment that owns tile tl of its column (prev tiles lie before the
@@ -244,12 +285,7 @@ struct Cursor {
             position(tl, prev, (d + 1) * env->colLen);
             return;
         }
-        int lo = 0, hi = env->ncols;            // env->colBase[lo] <= tt < env->colBase[hi]
-        while (hi - lo > 1) {
-            const int mid = (lo + hi) >> 1;
-            if (env->colBase[mid] <= tt) lo = mid; else hi = mid;
-        }
-        const int d = lo;
+        const int d = warp_count_le(env->colBase + 1, env->ncols, tt);
         const int tl = tt - env->colBase[d];
         const SegDesc* col = env->desc + (size_t)d * env->colLen;
         int s0 = 0, n = env->colLen;                 // smallest s with col[s].pfx[L] > tl lies in [s0, s0+n)
@@ -480,6 +516,7 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
     const int lane = lane_id();
     const unsigned int tileBytes = 1u << cur.tileShift;
     const uint32_t ring0 = smem_u32(ring);
+    const unsigned long long pol = l2_policy_stream(); (void)pol;
     unsigned long long mDst = 0;          // slot registers (lane j <-> slot j)
     unsigned int mLen = 0, mOff = 0, mV = 0;
     unsigned int vHead = 0, phys = 0;     // virtual (mod 2^32) and physical allocation offsets
@@ -506,7 +543,7 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
                 if (lane == 0) {
                     const uint32_t bar = smem_u32(&mbar[slot]);
                     mbar_expect_tx(bar, len16);
-                    bulk_g2s(ring0 + po, srcp, len16, bar);
+                    bulk_g2s(ring0 + po, srcp, len16, bar PAYLOAD_POL(pol));
                     TL_STAMP_ONCE(tl, TL_FIRST_LOAD);
                 }
                 const unsigned int adv = (len16 + 127u) & ~127u;
@@ -536,7 +573,7 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
         const unsigned int slen = __shfl_sync(0xffffffffu, mLen, slot);
         const unsigned int soff = __shfl_sync(0xffffffffu, mOff, slot);
         if (lane == 0) {
-            bulk_s2g(reinterpret_cast<void*>(((unsigned long long)dhi << 32) | dlo), ring0 + soff, slen);
+            bulk_s2g(reinterpret_cast<void*>(((unsigned long long)dhi << 32) | dlo), ring0 + soff, slen PAYLOAD_POL(pol));
             bulk_commit();
             TL_STAMP_ONCE(tl, TL_FIRST_STORE);
             TL_STAMP(tl, TL_LAST_STORE);
@@ -570,6 +607,7 @@ __device__ __forceinline__ void vector_engine(Cursor<L, SM>& cur, unsigned char*
     const int lane = lane_id();
     const unsigned int tileBytes = 1u << cur.tileShift;
     const uint32_t ring0 = smem_u32(ring);
+    const unsigned long long pol = l2_policy_stream(); (void)pol;
     unsigned long long mDst = 0;          // slot registers (lane j <-> slot j, j < VEC_SLOTS)
     unsigned int mPack = 0, mAlloc = 0;   // ring offset >> 7 | len << 11 | source misalignment << 24;  ring bytes to release
     unsigned int used = 0, phys = 0;      // ring bytes held by pieces in flight (incl. wrap padding); allocation offset
@@ -605,7 +643,7 @@ __device__ __forceinline__ void vector_engine(Cursor<L, SM>& cur, unsigned char*
                 if (lane == 0) {
                     const uint32_t bar = smem_u32(&mbar[slot]);
                     mbar_expect_tx(bar, ld);
-                    bulk_g2s(ring0 + po, reinterpret_cast<const void*>(tS - ms), ld, bar);
+                    bulk_g2s(ring0 + po, reinterpret_cast<const void*>(tS - ms), ld, bar PAYLOAD_POL(pol));
                 }
                 used += pad + adv;
                 phys = po + adv;
@@ -692,17 +730,16 @@ __device__ __forceinline__ RingPlan plan_ring(int requestedE, int bulkTiles, int
             E = bulkTiles <= 48 * grid ? 4 : (bulkTiles <= 96 * grid ? 2 : 1);
             // one engine turns a tile around in ~1.2 us (measured: R = 256 / 512 with one 14 KB row per pair, 1 vs 4
             // engines: 173 -> 114 us, 587 -> 393 us), an SM's share of HBM is ~23 GB/s each way: E x average tile >= ~30 KB
-            if (bulkKiB >= 0) {
-                const long long avg = (bulkKiB << 10) / bulkTiles;
-                const int need = avg >= 30 * 1024 ? 1 : (avg >= 15 * 1024 ? 2 : 4);
+            if (bulkKiB >= 0) {                            // average tile = bulkKiB KiB / bulkTiles, compared without dividing
+                const int need = bulkKiB >= 30ll * bulkTiles ? 1 : (bulkKiB >= 15ll * bulkTiles ? 2 : 4);
                 E = max(E, need);
             }
         }
-        while (E > 1 && (1u << bulkShift) > ((bulkBytes / (unsigned int)E) & ~127u)) E >>= 1;    // a tile must fit in one share
+        while (E > 1 && (unsigned long long)E * (((1u << bulkShift) + 127u) & ~127u) > bulkBytes) E >>= 1;    // a tile must fit in one share
         if (E + p.NV > COPY_WARPS) E = COPY_WARPS - p.NV;
     }
     p.E = E;
-    p.bulkShare = E ? (bulkBytes / (unsigned int)E) & ~127u : 0u;
+    p.bulkShare = (E == 0 ? 0u : E == 1 ? bulkBytes : E == 2 ? bulkBytes >> 1 : E == 4 ? bulkBytes >> 2 : bulkBytes / (unsigned int)E) & ~127u;
     p.vecShare = unit;
     p.vecBase = bulkBytes & ~127u;
     return p;
@@ -712,7 +749,29 @@ __device__ __forceinline__ RingPlan plan_ring(int requestedE, int bulkTiles, int
 __device__ __forceinline__ int static_first_chunk(int total, int nEngines, int kmax, int kmaxLong, int RR) {
     if (nEngines <= 0) return 0;
     const int km = total >= 8 * RR ? kmaxLong : kmax;
-    return max(1, min(km, total / (4 * nEngines)));
+    return clamped_quotient(total, 4 * nEngines, 1, km);
+}
+
+// A vector engine warp's whole job, as ONE out-of-line function: the vector path is ~200 KB of SASS (two lists x four
+// word selections of the funnel shift, fully inlined cursors) that an aligned call never executes.  Kept out of line, the
+// prologue -> plan -> bulk engine path is one compact ~80 KB stretch of code; with everything inlined, builds differed by
+// 1.7-2 us per call on the small-message shapes depending on where the compiler happened to place that path (measured:
+// identical sources +- the vector code, config 5 155.1 vs 156.9 us, R = 64 x 10 KB 26.0 vs 27.4 us).  The cursors are
+// constructed in here so that they live in registers.
+template <bool SM>
+__device__ __noinline__ void vector_role(const CursorEnv* envs, int engineId, unsigned char* myRing, unsigned long long* myBar,
+                                         unsigned int share, bool bulkToo) {
+    int pieceSeq = 0;
+    {
+        Cursor<LIST_VEC, SM> cur;
+        cur.init(&envs[LIST_VEC], engineId);
+        vector_engine<LIST_VEC, SM>(cur, myRing, myBar, share, pieceSeq);
+    }
+    if (bulkToo) {
+        Cursor<LIST_BULK, SM> cur;
+        cur.init(&envs[LIST_BULK], engineId);
+        vector_engine<LIST_BULK, SM>(cur, myRing, myBar, share, pieceSeq);
+    }
 }
 
 // Step a4 for one CTA: split warps and ring (plan_ring), run the engines.  Returns whether any dynamic claim counter
@@ -729,17 +788,30 @@ __device__ __forceinline__ bool run_copy_engines(const SegDesc* desc, int* const
     const int nV = (int)gridDim.x * rp.NV;
     const int nB = rp.bulkByVec ? nV : (int)gridDim.x * rp.E;
     const int RR = ncols * colLen;
-    const int stB = fusedStatic > 0 ? fusedStatic : static_first_chunk(totB, nB, kmax, COPY_KMAX_LONG, RR);
-    const int stV = fusedStatic > 0 ? fusedStatic : static_first_chunk(totV, nV, COPY_KMAX_VEC, COPY_KMAX_LONG, RR);
+    // Short lists (at most XDEV_RR_TPE tiles per engine: the small-message regime, a call of ~10 us) are dealt ROUND-ROBIN,
+    // chunk c to engine c mod nEngines: same HBM order as in-order claims, but no atomic round trip sits between an
+    // engine and its next tile.  Measured (graph replay p50): R = 64 x one 10 KB row per pair 28.1 -> 26.0 us, R = 128 x
+    // 14 KB for 28 % of pairs 31.6 -> 30.1 us, and no longer build-dependent (with claims the same sources landed on
+    // either value depending on instruction scheduling).  Longer lists need the claims' balance by TIME: round-robin
+    // there costs config 5 +17 us, config 3 +14 % (XDEV_RR_TPE = 64 / unlimited).
+#ifndef XDEV_RR_TPE
+#define XDEV_RR_TPE 16
+#endif
+    const bool rrB = fusedStatic == 0 && nB > 0 && (long long)totB <= (long long)XDEV_RR_TPE * nB;
+    const bool rrV = fusedStatic == 0 && nV > 0 && (long long)totV <= (long long)XDEV_RR_TPE * nV;
+    const int stB = fusedStatic > 0 ? fusedStatic : rrB ? clamped_quotient(totB, 32 * nB, 1, totB >= 8 * RR ? COPY_KMAX_LONG : min(kmax, 8))
+                                                        : static_first_chunk(totB, nB, kmax, COPY_KMAX_LONG, RR);
+    const int stV = fusedStatic > 0 ? fusedStatic : rrV ? clamped_quotient(totV, 32 * nV, 1, totV >= 8 * RR ? COPY_KMAX_LONG : COPY_KMAX_VEC)
+                                                        : static_first_chunk(totV, nV, COPY_KMAX_VEC, COPY_KMAX_LONG, RR);
 #ifdef XDEV_TIMELINE
     if (tl) tl[TL_TILES] = (unsigned long long)totB;
 #endif
     if (threadIdx.x == 0)
         cursor_env_init(&envs[LIST_BULK], LIST_BULK, desc, colBase[LIST_BULK], coarse[LIST_BULK], &ctl->next[LIST_BULK], cls, ncols, colLen,
-                        nB, kmax, COPY_KMAX_LONG, stB, claimDiv);
+                        nB, kmax, COPY_KMAX_LONG, stB, claimDiv, rrB);
     if (threadIdx.x == 32)
         cursor_env_init(&envs[LIST_VEC], LIST_VEC, desc, colBase[LIST_VEC], coarse[LIST_VEC], &ctl->next[LIST_VEC], cls, ncols, colLen,
-                        nV, COPY_KMAX_VEC, COPY_KMAX_LONG, stV, claimDiv);
+                        nV, COPY_KMAX_VEC, COPY_KMAX_LONG, stV, claimDiv, rrV);
     __syncthreads();
     TL_STAMP(tl, TL_ENV);
     if (warp < rp.E) {
@@ -747,23 +819,14 @@ __device__ __forceinline__ bool run_copy_engines(const SegDesc* desc, int* const
         cur.init(&envs[LIST_BULK], (int)blockIdx.x * rp.E + warp);
         if (warp == 0) TL_STAMP(tl, TL_CURSOR);
         bulk_engine<SM>(cur, smem + (size_t)warp * rp.bulkShare, mbar + warp * COPY_SLOTS, rp.bulkShare, warp == 0 ? tl : nullptr);
+#ifndef XDEV_EXPERIMENT_NOVEC
     } else if (warp < rp.E + rp.NV) {
         const int v = warp - rp.E;
-        unsigned char* myRing = smem + rp.vecBase + (size_t)v * rp.vecShare;
-        unsigned long long* myBar = mbar + COPY_MAX_ENGINES * COPY_SLOTS + v * VEC_SLOTS;
-        int pieceSeq = 0;
-        {
-            Cursor<LIST_VEC, SM> cur;
-            cur.init(&envs[LIST_VEC], (int)blockIdx.x * rp.NV + v);
-            vector_engine<LIST_VEC, SM>(cur, myRing, myBar, rp.vecShare, pieceSeq);
-        }
-        if (rp.bulkByVec) {
-            Cursor<LIST_BULK, SM> cur;
-            cur.init(&envs[LIST_BULK], (int)blockIdx.x * rp.NV + v);
-            vector_engine<LIST_BULK, SM>(cur, myRing, myBar, rp.vecShare, pieceSeq);
-        }
+        vector_role<SM>(envs, (int)blockIdx.x * rp.NV + v, smem + rp.vecBase + (size_t)v * rp.vecShare,
+                        mbar + COPY_MAX_ENGINES * COPY_SLOTS + v * VEC_SLOTS, rp.vecShare, rp.bulkByVec);
+#endif
     }
-    return (nB > 0 && totB > stB * nB) || (nV > 0 && totV > stV * nV);
+    return (nB > 0 && totB > stB * nB && !rrB) || (nV > 0 && totV > stV * nV && !rrV);
 }
 
 // Side job (see SideJob): warps [firstWarp, 16) of every CTA, before their engine role.
@@ -809,8 +872,10 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
     for (int i = threadIdx.x; i < COPY_MBAR_COUNT; i += COPY_THREADS) mbar_init(smem_u32(&mbar[i]), 1);
     fence_mbar_init();
     griddep_wait();
-    if (a.useCoarse && warp >= 2) {
-        for (int i = threadIdx.x - 64; i < 2 * nbR; i += COPY_THREADS - 64)
+    // every global load of the prologue is issued before the first one is consumed (one L2 round trip for the CTA, not one
+    // per 32 columns): warps 0 / 1 scan the two lists' column totals, warp 2 sums the bulk bytes, warps 3.. stage the indexes
+    if (a.useCoarse && warp >= 3) {
+        for (int i = threadIdx.x - 96; i < 2 * nbR; i += COPY_THREADS - 96)
             coarse[0][i] = i < nbR ? a.coarse[0][i] : a.coarse[1][i - nbR];
     }
     if (warp < 2) {
@@ -818,18 +883,24 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
         int* cb = warp ? colBase[1] : colBase[0];
         int run = 0;
         if (lane == 0) cb[0] = 0;
-        for (int c0 = 0; c0 < R; c0 += 32) {
-            const int v = c0 + lane < R ? ct[c0 + lane] : 0;
-            const int incl = warp_incl_scan(v);
-            if (c0 + lane < R) cb[c0 + lane + 1] = run + incl;
-            run += __shfl_sync(0xffffffffu, incl, 31);
+        constexpr int PU = 4;                  // 128 columns per trip
+        for (int c0 = 0; c0 < R; c0 += 32 * PU) {
+            int v[PU];
+#pragma unroll
+            for (int u = 0; u < PU; ++u) { const int c = c0 + u * 32 + lane; v[u] = c < R ? ct[c] : 0; }
+#pragma unroll
+            for (int u = 0; u < PU; ++u) {
+                const int c = c0 + u * 32 + lane;
+                const int incl = warp_incl_scan(v[u]);
+                if (c < R) cb[c + 1] = run + incl;
+                run += __shfl_sync(0xffffffffu, incl, 31);
+            }
         }
-        if (warp == 1) {                   // bytes of the bulk list (-> average tile size, plan_ring)
-            long long k = 0;
-            for (int c = lane; c < R; c += 32) k += a.colKiB[c];
-            k = warp_sum(k);
-            if (lane == 0) *totKiB = k;
-        }
+    } else if (warp == 2) {                    // bytes of the bulk list (-> average tile size, plan_ring)
+        long long k = 0;
+        for (int c = lane; c < R; c += 32) k += a.colKiB[c];
+        k = warp_sum(k);
+        if (lane == 0) *totKiB = k;
     }
     __syncthreads();
     TL_STAMP(tl, TL_READY);

@@ -74,13 +74,14 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
     // pointer tables: issue the loads now, park them in shared memory after phase 1's loads are in flight too (one
     // DRAM round trip instead of two on a cold start)
     constexpr int PT = 2;                        // covers R <= 1024 with 512 threads
+    const unsigned long long keep = l2_policy_keep();    // metadata inputs stay in L2 across the payload stream (common.cuh)
     unsigned long long sp[PT];
 #pragma unroll
     for (int i = 0; i < PT; ++i) {
         const int s = threadIdx.x + i * COUNTS_THREADS;
-        sp[i] = (s < R && a.send) ? (unsigned long long)a.send[s] : 0ull;        // null tables: offsets only (top-k calls)
+        sp[i] = (s < R && a.send) ? ld_keep_ptr(a.send + s, keep) : 0ull;        // null tables: offsets only (top-k calls)
     }
-    const unsigned long long rp = (threadIdx.x < Wc && a.recv) ? (unsigned long long)a.recv[d0 + threadIdx.x] : 0ull;
+    const unsigned long long rp = (threadIdx.x < Wc && a.recv) ? ld_keep_ptr(a.recv + d0 + threadIdx.x, keep) : 0ull;
 
     // ---- phase 1: soff for the owned columns = row prefix C[s][0..d0) + running sum over the owned columns ------
     // LPR lanes share a row (LPR = 512 / R rounded down to a power of two, 8..32): lane q sums the prefix columns
@@ -99,13 +100,13 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
         constexpr int OW = 4;                                          // owned columns kept in registers (W <= 4: R <= 128)
         long long own[OW];
 #pragma unroll
-        for (int j = 0; j < OW; ++j) own[j] = (valid && q == 0 && j < Wc) ? row[d0 + j] : 0;
+        for (int j = 0; j < OW; ++j) own[j] = (valid && q == 0 && j < Wc) ? ld_keep(row + d0 + j, keep) : 0;
         long long part = 0;
         constexpr int LU = 16;                                         // independent loads per trip
         for (int dd = q; dd < d0; dd += LPR * LU) {
             long long v[LU];
 #pragma unroll
-            for (int u = 0; u < LU; ++u) { const int x = dd + u * LPR; v[u] = (valid && x < d0) ? row[x] : 0; }
+            for (int u = 0; u < LU; ++u) { const int x = dd + u * LPR; v[u] = (valid && x < d0) ? ld_keep(row + x, keep) : 0; }
 #pragma unroll
             for (int u = 0; u < LU; ++u) part += v[u] > 0 ? v[u] : 0;
         }
@@ -132,7 +133,7 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
                 }
             }
             for (int j = OW; j < Wc; ++j) {
-                long long cc = row[d0 + j];
+                long long cc = ld_keep(row + d0 + j, keep);
                 if (cc < 0) { sawNeg = true; cc = 0; }
                 cval[(size_t)s * P + j] = cc;
                 sofs[(size_t)s * P + j] = run;

@@ -31,7 +31,8 @@ constexpr int DYN_THREADS = 512;
 constexpr int DYN_WARPS = DYN_THREADS / 32;
 constexpr int DYN_SMEM_SLOTS = 4096;      // columns up to this many slots are staged in shared memory (32 B per slot)
 constexpr int DYN_SU = 4;                 // sources a warp works on at once (their dependent loads overlap)
-constexpr int DYN_CHUNK = 128;            // split lengths scanned per step: 4 per lane
+constexpr int DYN_PL = 5;                 // split lengths per lane and scan step
+constexpr int DYN_CHUNK = 32 * DYN_PL;    // split lengths scanned per step: 160 covers 128 experts + redundant ones in ONE step
 
 struct DynArgs {
     const void* const* send;          // R
@@ -60,10 +61,10 @@ struct __align__(32) DynSlot {        // same 32-byte stride as SegDesc, so the 
 };
 
 __host__ __device__ inline size_t dyn_smem_bytes(int colLen) {
-    return (size_t)DYN_WARPS * DYN_SU * (DYN_CHUNK + 1) * 8 + (colLen <= DYN_SMEM_SLOTS ? (size_t)colLen * sizeof(DynSlot) : 0);
+    return colLen <= DYN_SMEM_SLOTS ? (size_t)colLen * sizeof(DynSlot) : 32;
 }
 
-// dynamic smem: long long pref[DYN_WARPS][DYN_SU][DYN_CHUNK + 1], then DynSlot[colLen] if colLen <= DYN_SMEM_SLOTS
+// dynamic smem: DynSlot[colLen] if colLen <= DYN_SMEM_SLOTS
 __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs a) {
     extern __shared__ __align__(32) unsigned char dyn_smem[];
     __shared__ long long sWarpTot[DYN_WARPS];
@@ -72,14 +73,12 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
     const int R = a.R, n = a.n, J = a.maxBlockLen;
     const int colLen = R * J;
     const int nb = (colLen + 31) >> 5;
-    long long* prefAll = reinterpret_cast<long long*>(dyn_smem);
-    DynSlot* slots = colLen <= DYN_SMEM_SLOTS ? reinterpret_cast<DynSlot*>(dyn_smem + (size_t)DYN_WARPS * DYN_SU * (DYN_CHUNK + 1) * 8)
+    DynSlot* slots = colLen <= DYN_SMEM_SLOTS ? reinterpret_cast<DynSlot*>(dyn_smem)
                                               : reinterpret_cast<DynSlot*>(a.ws.desc + (size_t)d * colLen);
     DY_STAMP(0);
     griddep_launch_dependents();
     if (threadIdx.x == 0) sStatus = 0u;
-    griddep_wait();                                        // the metadata may have been written by the stream's previous kernel
-    DY_STAMP(1);
+    // (before the dependency wait: a hint, and L2 is the point of coherence, so a line fetched early cannot go stale)
     // pull the (cold) metadata into L2 with ONE DRAM round trip: the R CTAs prefetch disjoint slices of the three arrays,
     // so the dependent loads below (block lengths -> list offset -> split index -> split offset) are L2 hits for all
     {
@@ -92,12 +91,15 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
             prefetch_l2(p);
         }
     }
+    griddep_wait();                                        // the metadata may have been written by the stream's previous kernel
+    DY_STAMP(1);
     unsigned int st = 0;
+    const unsigned long long keep = l2_policy_keep();      // metadata inputs stay in L2 across the payload stream (common.cuh)
 
     // ---- phase A: DYN_SU sources per warp at a time ------------------------------------------------------------
     for (int sBase = warp; sBase < R; sBase += DYN_WARPS * DYN_SU) {
         int src[DYN_SU];
-        long long lv[DYN_SU][4];                           // the first DYN_CHUNK split lengths: lane l holds 4l .. 4l+3
+        long long lv[DYN_SU][DYN_PL];                      // the first DYN_CHUNK split lengths: lane l holds PL*l .. PL*l + PL-1
         long long bv[DYN_SU][4];                           // the first 128 block lengths of row s: lane l holds l, l+32, ..
         unsigned long long sp[DYN_SU], rp[DYN_SU];
         // round trip 1: everything that does not depend on anything
@@ -109,14 +111,17 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
             const long long* Ls = a.L + (size_t)(on ? s : 0) * n;
             const long long* bls = a.blockLens + (size_t)(on ? s : 0) * R;
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int i = 4 * lane + q;
-                lv[u][q] = (on && i < n) ? Ls[i] : 0;
-                const int dd = q * 32 + lane;
-                bv[u][q] = (on && dd < R) ? bls[dd] : 0;
+            for (int q = 0; q < DYN_PL; ++q) {
+                const int i = DYN_PL * lane + q;
+                lv[u][q] = (on && i < n) ? ld_keep(Ls + i, keep) : 0;
             }
-            sp[u] = on ? (unsigned long long)a.send[s] : 0ull;
-            rp[u] = on ? (unsigned long long)a.recvbuffs[(size_t)d * R + s] : 0ull;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int dd = q * 32 + lane;
+                bv[u][q] = (on && dd < R) ? ld_keep(bls + dd, keep) : 0;
+            }
+            sp[u] = on ? ld_keep_ptr(a.send + s, keep) : 0ull;
+            rp[u] = on ? ld_keep_ptr(a.recvbuffs + (size_t)d * R + s, keep) : 0ull;
         }
         long long ioff[DYN_SU];
         int bl[DYN_SU];
@@ -135,7 +140,7 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
             if (src[u] < R) {
                 const long long* bls = a.blockLens + (size_t)src[u] * R;
                 for (int dd = 128 + lane; dd < R; dd += 32) {      // R > 128: the rest of the row
-                    long long v = bls[dd];
+                    long long v = ld_keep(bls + dd, keep);
                     if (v < 0) { st |= 4u; v = 0; }
                     if (v > J) { st |= 4u; v = J; }
                     if (dd < d) before += v;
@@ -145,6 +150,7 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
             ioff[u] = warp_sum(before);
             bl[u] = (int)warp_sum(mine);
         }
+        if (sBase == warp) DY_STAMP(2);
         for (int j0 = 0; j0 < J; j0 += 32) {               // one pass per 32 list entries (J <= 32: one pass)
             const int j = j0 + lane;
             // round trip 2: this lane's split index, for all DYN_SU sources at once
@@ -156,7 +162,7 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
                 if (src[u] < R && j < bl[u]) {
                     const long long pos = ioff[u] + j;
                     if (pos >= a.maxIndices) st |= 4u;
-                    else idx[u] = a.indices[(size_t)src[u] * a.maxIndices + pos];
+                    else idx[u] = ld_keep(a.indices + (size_t)src[u] * a.maxIndices + pos, keep);
                 }
             }
 #pragma unroll
@@ -166,53 +172,68 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
                     else live[u] = true;
                 }
             }
-            // offsets: exclusive prefix sums of the split lengths, DYN_CHUNK at a time (lane-local 4 + one warp scan of the
-            // lane totals) into this warp's shared-memory strip; a lane then reads offset and length of ITS split
+            if (sBase == warp && j0 == 0) DY_STAMP(3);
+            // offsets: exclusive prefix sums of the split lengths, DYN_CHUNK at a time, for all DYN_SU sources together (their
+            // shuffle chains interleave): lane l holds lengths 4l .. 4l+3 of the chunk, one 64-bit warp scan of the lane totals,
+            // then every lane PICKS offset and length of its own split from the owning lane's registers by shuffle -- no
+            // shared-memory strip, no warp barriers (round 2a: 8 serialised scan + strip rounds, ~5 us of the kernel's 7 us phase A)
+            long long base[DYN_SU], off[DYN_SU], len[DYN_SU];
+#pragma unroll
+            for (int u = 0; u < DYN_SU; ++u) { base[u] = 0; off[u] = 0; len[u] = 0; }
+            for (int c0 = 0; c0 < n; c0 += DYN_CHUNK) {
+                long long x[DYN_SU][DYN_PL];
+#pragma unroll
+                for (int u = 0; u < DYN_SU; ++u) {
+                    const long long* Ls = a.L + (size_t)(src[u] < R ? src[u] : 0) * n;
+#pragma unroll
+                    for (int q = 0; q < DYN_PL; ++q) {
+                        const int i = c0 + DYN_PL * lane + q;
+                        x[u][q] = c0 == 0 ? lv[u][q] : ((src[u] < R && i < n) ? ld_keep(Ls + i, keep) : 0);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < DYN_SU; ++u) {
+#pragma unroll
+                    for (int q = 0; q < DYN_PL; ++q) {
+                        if (x[u][q] < 0) { if (j0 == 0) st |= 1u; x[u][q] = 0; }
+                    }
+                    long long tot = 0;
+#pragma unroll
+                    for (int q = 0; q < DYN_PL; ++q) tot += x[u][q];
+                    const long long incl = warp_incl_scan(tot);
+                    const long long excl = base[u] + incl - tot;
+                    const bool mineHere = live[u] && idx[u] >= c0 && idx[u] < c0 + DYN_CHUNK;
+                    const int rel = mineHere ? (int)(idx[u] - c0) : 0;
+                    const int from = rel / DYN_PL, r = rel - from * DYN_PL;
+                    long long o = __shfl_sync(0xffffffffu, excl, from), l = 0;
+#pragma unroll
+                    for (int q = 0; q < DYN_PL; ++q) {
+                        const long long y = __shfl_sync(0xffffffffu, x[u][q], from);
+                        if (q < r) o += y;
+                        if (q == r) l = y;
+                    }
+                    if (mineHere) { off[u] = o; len[u] = l; }
+                    base[u] += __shfl_sync(0xffffffffu, incl, 31);
+                }
+            }
 #pragma unroll
             for (int u = 0; u < DYN_SU; ++u) {
-                long long* pref = prefAll + ((size_t)warp * DYN_SU + u) * (DYN_CHUNK + 1);
-                long long base = 0, off = 0, len = 0;
-                if (src[u] < R) {
-                    const long long* Ls = a.L + (size_t)src[u] * n;
-                    for (int c0 = 0; c0 < n; c0 += DYN_CHUNK) {
-                        long long x[4];
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            const int i = c0 + 4 * lane + q;
-                            x[q] = c0 == 0 ? lv[u][q] : (i < n ? Ls[i] : 0);
-                            if (x[q] < 0) { if (j0 == 0) st |= 1u; x[q] = 0; }
-                        }
-                        const long long tot = x[0] + x[1] + x[2] + x[3];
-                        const long long incl = warp_incl_scan(tot);
-                        long long p = base + incl - tot;
-                        __syncwarp();                              // the previous chunk's readers are done
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) { pref[4 * lane + q] = p; p += x[q]; }
-                        if (lane == 31) pref[DYN_CHUNK] = p;
-                        __syncwarp();
-                        if (live[u] && idx[u] >= c0 && idx[u] < c0 + DYN_CHUNK) {
-                            off = pref[idx[u] - c0];
-                            len = pref[idx[u] - c0 + 1] - off;
-                        }
-                        base += __shfl_sync(0xffffffffu, incl, 31);
-                    }
-                    if (j < J) {
-                        DynSlot o;
-                        o.bytes = live[u] ? len * a.elemSize : 0;
-                        o.src = live[u] ? sp[u] + (unsigned long long)(off * a.elemSize) : 0ull;
-                        o.dst = live[u] ? rp[u] + (unsigned long long)(off * a.elemSize) : 0ull;
-                        o.pad = 0;
-                        slots[(size_t)src[u] * J + j] = o;
-                    }
+                if (src[u] < R && j < J) {
+                    DynSlot o;
+                    o.bytes = live[u] ? len[u] * a.elemSize : 0;
+                    o.src = live[u] ? sp[u] + (unsigned long long)(off[u] * a.elemSize) : 0ull;
+                    o.dst = live[u] ? rp[u] + (unsigned long long)(off[u] * a.elemSize) : 0ull;
+                    o.pad = 0;
+                    slots[(size_t)src[u] * J + j] = o;
                 }
             }
         }
     }
     st = __reduce_or_sync(0xffffffffu, st);
     if (lane == 0 && st) atomicOr(&sStatus, st);
-    DY_STAMP(2);
+    DY_STAMP(4);
     __syncthreads();
-    DY_STAMP(3);
+    DY_STAMP(5);
 
     // ---- phase B: tile prefixes in slot order, descriptors, coarse index ------------------------------------------
     long long run = 0;                                     // tiles of the column before this round: bulk << 32 | vector
@@ -247,7 +268,7 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
         run += all;
         __syncthreads();                                   // sWarpTot is rewritten in the next round
     }
-    DY_STAMP(4);
+    DY_STAMP(6);
     myBulkBytes = warp_sum(myBulkBytes);
     if (lane == 0) sWarpTot[warp] = myBulkBytes;           // (the last round's barrier has passed: sWarpTot is free)
     __syncthreads();
@@ -259,7 +280,7 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
         a.ws.colKiB[d] = (int)(bb >> 10);
         if (sStatus) atomicOr(&a.ws.ctl->status, sStatus);
     }
-    DY_STAMP(5);
+    DY_STAMP(7);
 }
 
 }  // namespace xdev

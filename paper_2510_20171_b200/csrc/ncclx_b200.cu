@@ -52,7 +52,7 @@ struct Context {
     WorkCtl* fusedCtl = nullptr;          // claim counters of the single-launch path (self-resetting)
     void* wsBase = nullptr;
     // tunables (ncclx_param_t order)
-    int64_t params[NCCLX_PARAM_COUNT_] = {1024, 8, 0, 15, 1, 6, 32, 0, 1, 0};
+    int64_t params[NCCLX_PARAM_COUNT_] = {1024, 16, 0, 15, 1, 6, 32, 0, 1, 0};
     // profiling
     std::vector<EventPair> events[NCCLX_KERNEL_COUNT_];
     std::atomic<int64_t> launches{0};
@@ -330,6 +330,7 @@ int launchAllToAllv(const void* const* send, const int64_t* C, void* const* recv
 }
 
 constexpr size_t kReducePdlMaxBytes = (size_t)1 << 30;   // reductions below this many input bytes launch with PDL
+constexpr size_t kReducePrefetchAllBytes = (size_t)96 << 20;
 
 template <int DT>
 int launchReduceDT(const ReduceArgs& ra, int grid, size_t smem, bool pdl, cudaStream_t stream) {
@@ -365,6 +366,15 @@ int launchReduce(const void* const* send, void* const* recv, size_t blockElems, 
     // the host knows the size: gate it
     const size_t inBytes = (size_t)blockElems * (scatter ? R : 1) * es * (size_t)R;
     const bool pdl = g.params[NCCLX_PARAM_PDL] != 0 && inBytes < kReducePdlMaxBytes;
+    // under PDL the CTAs prefetch their first tiles into L2 before the dependency wait: everything when the input fits
+    // L2 comfortably, else the first two tiles (the first wave)
+    if (pdl) {                                             // every CTA its own first tiles (all of them when the input fits L2)
+        ra.prefetchCtas = (int)grid;
+        ra.prefetchTiles = inBytes <= kReducePrefetchAllBytes ? (int)((tiles + grid - 1) / grid) : 2;
+    }
+#ifdef XDEV_NO_REDUCE_PREFETCH
+    ra.prefetchTiles = 0;
+#endif
     switch (dtype) {
     case NCCLX_BF16: return launchReduceDT<RED_BF16>(ra, (int)grid, smem, pdl, stream);
     case NCCLX_F32: return launchReduceDT<RED_F32>(ra, (int)grid, smem, pdl, stream);

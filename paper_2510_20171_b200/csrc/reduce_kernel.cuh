@@ -21,7 +21,10 @@
 
 namespace xdev {
 
-constexpr int REDUCE_THREADS = 128;
+#ifndef XDEV_REDUCE_THREADS
+#define XDEV_REDUCE_THREADS 128
+#endif
+constexpr int REDUCE_THREADS = XDEV_REDUCE_THREADS;
 enum { RED_BF16 = 0, RED_F32 = 1, RED_F16 = 2 };
 
 struct ReduceArgs {
@@ -30,6 +33,8 @@ struct ReduceArgs {
     unsigned long long blockElems; // AllReduce: count; ReduceScatter: recvcount
     int R;
     int scatter;                 // 0: AllReduce (1 block, R outputs), 1: ReduceScatter (R blocks)
+    int prefetchTiles;           // > 0: CTAs b < prefetchCtas pull tiles b, b + prefetchCtas, ... (this many) into L2 BEFORE the
+    int prefetchCtas;            //      dependency wait (short calls under PDL)
 };
 
 template <int DT> struct Acc;    // accumulators for one 16-byte vector
@@ -209,6 +214,31 @@ __global__ void __launch_bounds__(REDUCE_THREADS) reduce_kernel(const ReduceArgs
     constexpr int ES = DT == RED_F32 ? 4 : 2;
 
     griddep_launch_dependents();           // no-ops unless launched with programmatic stream serialisation (short calls)
+    // Short calls under PDL: the first wave of CTAs is resident while the stream's previous kernel drains, so it pulls
+    // INPUT tiles into L2 now (prefetch.global.L2: a hint, and L2 is the point of coherence, so a line fetched early
+    // cannot go stale even if that kernel still writes it) -- for an input that fits L2, all of it: the DRAM reads then
+    // run at full memory-level parallelism from before the wait on, decoupled from the SMs' load/store issue, and overlap
+    // the predecessor's tail (config 2 in a graph of back-to-back calls).
+    if (a.prefetchTiles > 0 && R <= 32 && (int)blockIdx.x < a.prefetchCtas) {
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+        const unsigned long long mine = lane < R ? (unsigned long long)a.send[lane] : 0ull;
+        const unsigned long long n0 = a.blockElems;
+        const unsigned long long nvec = n0 * ES / 32;
+        const unsigned int tpb = (unsigned int)((nvec + REDUCE_THREADS - 1) / REDUCE_THREADS);
+        const unsigned long long ntiles = (unsigned long long)tpb * (a.scatter ? R : 1);
+        unsigned long long t = blockIdx.x;
+        for (int i = 0; i < a.prefetchTiles && t < ntiles; ++i, t += (unsigned long long)a.prefetchCtas) {
+            const unsigned int blk = a.scatter ? (unsigned int)(t / tpb) : 0u;
+            const unsigned long long v0 = (t - (unsigned long long)blk * tpb) * REDUCE_THREADS;     // first vector of the tile
+            for (int k = warp; k < R; k += REDUCE_THREADS / 32) {
+                const unsigned long long base = __shfl_sync(0xffffffffu, mine, k);
+                for (int ln = lane; ln < REDUCE_THREADS / 4; ln += 32) {                             // the tile's 128-byte lines
+                    const unsigned long long o = v0 * 32 + (unsigned long long)ln * 128;
+                    if (base && o < nvec * 32) prefetch_l2(reinterpret_cast<const void*>(base + blk * nvec * 32 + o));
+                }
+            }
+        }
+    }
     griddep_wait();
     if (threadIdx.x == 0) sMis = 0;
     __syncthreads();
