@@ -630,6 +630,7 @@ def misaligned_extra(torch, nx, peak):
     for key, rows, width, dtype in (("R16_bf16_odd_counts", rng.integers(300000, 400000, (16, 16)) * 2 + 1, 1, "bf16"),
                                     ("R16_bf16_aligned_counts", rng.integers(75000, 100000, (16, 16)) * 8, 1, "bf16"),
                                     ("R16_bf16_aligned_counts_4x_bytes", rng.integers(300000, 400000, (16, 16)) * 8, 1, "bf16"),
+                                    ("R16_bf16_odd_counts_4x_bytes", rng.integers(1200000, 1600000, (16, 16)) * 2 + 1, 1, "bf16"),
                                     ("R16_u8_odd_counts", rng.integers(600000, 800000, (16, 16)) * 2 + 1, 1, "u8"),
                                     ("R64_bf16_odd_rows_of_5121", np.ones((64, 64), np.int64) * 41, 5121, "bf16")):
         a = A2A(W.A2AConfig(key, rows.shape[0], width, dtype, 1, rows.astype(np.int64)), torch, nx, with_back=False)

@@ -17,10 +17,12 @@
 //       - "bulk" list (source, destination 16-byte aligned, >= bulkMinBytes): tiles of 32 KiB, stored with
 //         cp.async.bulk shared->global; one elected lane of warp 0 (or of warps 0..E-1) issues everything;
 //       - "vector" list (short segments and ANY other alignment -- counts are element-granular):
-//         each engine warp owns a share of the ring, loads the 16-byte-aligned SPAN that covers a 2 KiB piece
-//         of its tile, and the warp then moves it from shared memory to the destination with aligned 16-byte
-//         stores, funnel-shifting when source and destination are misaligned differently (head / tail bytes by
-//         lanes).  (Round 1 copied these global->registers->global with ~61 KB in flight per SM: 3.7 TB/s.)
+//         each engine warp owns a share of the ring and loads the 16-byte-aligned SPAN that covers a 4 KiB piece
+//         of its tile; when source and destination are misaligned differently the warp realigns the piece IN PLACE
+//         in shared memory (funnel shifts), and the body goes out as one cp.async.bulk shared->global as well
+//         (head / tail bytes, < 16 at the ends of a tile, by lanes).  (Round 1 copied these global->registers->
+//         global with ~61 KB in flight per SM: 3.7 TB/s; warp stores from shared memory: 6.09-6.14 TB/s on 1.4-1.7 GB
+//         calls; TMA stores: 6.21-6.23 TB/s; the aligned bulk list on the same bytes: 6.72 TB/s.)
 //   * the ring is split between the two lists on the device, grid-uniformly, from their tile totals.
 #pragma once
 #include "common.cuh"
@@ -32,13 +34,23 @@ constexpr int COPY_WARPS = COPY_THREADS / 32;
 constexpr int COPY_SLOTS = 32;             // outstanding bulk tiles per engine (mbarriers; slot j lives in lane j): <= 32
 constexpr int COPY_MAX_ENGINES = 4;        // bulk engines (warps 0..E-1) per CTA, each with its own share of the ring
 constexpr int VEC_SLOTS = 16;              // outstanding staged pieces per vector engine
-constexpr int VEC_SUB_BYTES = 4096;        // bytes of a vector tile staged per TMA load (multiple of 16, <= 4096: slot word)
+#ifndef XDEV_VEC_SUB_BYTES
+#define XDEV_VEC_SUB_BYTES 4096
+#endif
+constexpr int VEC_SUB_BYTES = XDEV_VEC_SUB_BYTES;        // bytes of a vector tile staged per TMA load (multiple of 16, <= 4096: slot word)
 constexpr int VEC_DIRECT_MAX = 48;         // pieces shorter than this are copied by lanes, global -> global
 constexpr int VEC_MAX_IN_BULK_MIX = 13;    // vector engines when both lists have work: the bulk engines keep >= 3/16 of the ring (>= 1 tile)
 constexpr int COPY_MBAR_COUNT = COPY_MAX_ENGINES * COPY_SLOTS + COPY_WARPS * VEC_SLOTS;
 constexpr int COPY_MBAR_BYTES = COPY_MBAR_COUNT * 8;
 constexpr int COPY_KMAX_LONG = 2;          // max tiles per dynamic claim when segments average >= 8 tiles (measured: config 3)
+#ifndef XDEV_KMAX_LONG_VEC
+#define XDEV_KMAX_LONG_VEC 2
+#endif
+constexpr int COPY_KMAX_LONG_VEC = XDEV_KMAX_LONG_VEC;   // the same for the vector list (16 engines per CTA, 16 KiB tiles)
 constexpr int COPY_KMAX_VEC = 8;           // max tiles per dynamic claim on the vector list
+#ifndef XDEV_VEC_TMA_STORE
+#define XDEV_VEC_TMA_STORE 1              // vector list: body of a piece realigned in shared memory and stored by the TMA (0: warp stores)
+#endif
 #ifndef XDEV_PAYLOAD_POLICY
 #define XDEV_PAYLOAD_POLICY 1              // 1: payload bulk copies carry an L2 evict_first policy (common.cuh); 0: none (A/B builds)
 #endif
@@ -489,6 +501,60 @@ __device__ __forceinline__ void warp_drain_shifted(unsigned char* dst, const uns
     }
 }
 
+// TMA-store variant of the drain: the body is realigned IN PLACE in shared memory (vector i of the destination-aligned
+// image overwrites slot i of the source-aligned one: every batch reads its 32 or 64 slots + the one after them into
+// registers before any lane writes), so that one cp.async.bulk shared -> global can store it; returns the shared-memory
+// address and the byte count of the body for the elected lane to issue.  Head / tail bytes (< 16 each, only at the ends
+// of a tile) are stored by lanes first: the head shares a 16-byte word with body slot 0.
+template <int WSEL>
+__device__ __forceinline__ void realign_body(uint4* sv, const unsigned int nvec, const int bsh, const unsigned int lane) {
+    unsigned int i0 = 0;
+    for (; i0 + 64 <= nvec; i0 += 64) {
+        const unsigned int i = i0 + lane;
+        const uint4 a0 = sv[i], b0 = sv[i + 1], a1 = sv[i + 32], b1 = sv[i + 33];
+        __syncwarp();
+        sv[i] = shift_join<WSEL>(a0, b0, bsh);
+        sv[i + 32] = shift_join<WSEL>(a1, b1, bsh);
+        __syncwarp();
+    }
+    for (; i0 < nvec; i0 += 32) {
+        const unsigned int i = i0 + lane;
+        uint4 a = make_uint4(0, 0, 0, 0), b = a;
+        if (i < nvec) { a = sv[i]; b = sv[i + 1]; }
+        __syncwarp();
+        if (i < nvec) sv[i] = shift_join<WSEL>(a, b, bsh);
+        __syncwarp();
+    }
+}
+__device__ __forceinline__ void warp_drain_realign(unsigned char* dst, unsigned char* sm, const unsigned int ms, const unsigned int len,
+                                                   unsigned char*& bodyDst, uint32_t& bodySmem, unsigned int& bodyBytes) {
+    const unsigned int lane = (unsigned int)lane_id();
+    unsigned int hb = (16u - (unsigned int)((unsigned long long)dst & 15ull)) & 15u;
+    if (hb > len) hb = len;
+    const unsigned int pos = ms + hb;                      // shared-memory offset of the first body byte
+    const unsigned int nvec = (len - hb) >> 4;
+    const unsigned int done = hb + (nvec << 4);
+    if (lane < hb) dst[lane] = sm[ms + lane];
+    if (lane < len - done) dst[done + lane] = sm[ms + done + lane];
+    const unsigned int sh = pos & 15u;
+    uint4* sv = reinterpret_cast<uint4*>(sm) + (pos >> 4);
+    if (sh != 0 && nvec) {
+        __syncwarp();                                      // the head bytes have been read
+        const int bsh = (int)(sh & 3u) * 8;
+        switch (sh >> 2) {                                 // warp-uniform, once per piece
+        case 0:  realign_body<0>(sv, nvec, bsh, lane); break;
+        case 1:  realign_body<1>(sv, nvec, bsh, lane); break;
+        case 2:  realign_body<2>(sv, nvec, bsh, lane); break;
+        default: realign_body<3>(sv, nvec, bsh, lane); break;
+        }
+        fence_proxy_async_smem();                          // this lane's generic writes -> visible to the TMA store
+    }
+    __syncwarp();
+    bodyDst = dst + hb;
+    bodySmem = smem_u32(sv);
+    bodyBytes = nvec << 4;
+}
+
 #ifdef XDEV_TIMELINE
 enum { TL_ENTER = 0, TL_READY, TL_FIRST_LOAD, TL_FIRST_STORE, TL_LAST_STORE, TL_DRAINED, TL_EXIT, TL_TILES, TL_ENV, TL_CURSOR, TL_ENSURED, TL_COUNT };
 __device__ __forceinline__ unsigned long long tl_now() {
@@ -595,8 +661,9 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
 // [s & ~15, align16(s + len)) -- cp.async.bulk needs 16-byte aligned addresses and sizes, not aligned SEGMENTS;
 // the up-to-15 bytes read on either side share a 16-byte word with valid data, so they lie inside the caller's
 // allocation.  Up to VEC_SLOTS pieces are in flight per engine (bookkeeping in lanes 0..15, as in the bulk engine),
-// also across tile and segment boundaries.  A landed piece is moved to the destination by the whole warp
-// (warp_drain_shifted); its ring bytes are free as soon as the warp has read them.
+// also across tile and segment boundaries.  A landed piece is realigned by the whole warp and stored by the TMA
+// (warp_drain_realign); its ring bytes are released once that store has read them (one store may be outstanding), as in
+// the bulk engine.  (XDEV_VEC_TMA_STORE = 0 builds the earlier drain: aligned 16-byte warp stores from shared memory.)
 // The engine runs on either work list (L): when the bulk list holds only a small part of a mostly unaligned call,
 // the vector engines sweep it up as well (plan_ring: bulkByVec) instead of idling warps as bulk engines.
 // Measured (R = 16, 360 MB each way, odd bf16 counts): the loop is instruction-issue bound, so per-piece work is kept
@@ -611,6 +678,7 @@ __device__ __forceinline__ void vector_engine(Cursor<L, SM>& cur, unsigned char*
     unsigned long long mDst = 0;          // slot registers (lane j <-> slot j, j < VEC_SLOTS)
     unsigned int mPack = 0, mAlloc = 0;   // ring offset >> 7 | len << 11 | source misalignment << 24;  ring bytes to release
     unsigned int used = 0, phys = 0;      // ring bytes held by pieces in flight (incl. wrap padding); allocation offset
+    int freed = pieceSeq; (void)freed;    // (TMA-store drain) pieces [.., freed) have released their ring bytes: freed <= iStore <= iLoad
     int iLoad = pieceSeq, iStore = pieceSeq;   // piece numbers continue across the engine's runs: slot = number mod VEC_SLOTS, and the
                                                // slot's mbarrier has completed number / VEC_SLOTS phases before this piece
     unsigned long long tS = 0, tD = 0;    // the rest of the current tile
@@ -636,7 +704,11 @@ __device__ __forceinline__ void vector_engine(Cursor<L, SM>& cur, unsigned char*
                 const unsigned int ld = (ms + len + 15u) & ~15u;
                 const unsigned int adv = (ld + 127u) & ~127u;
                 const unsigned int pad = phys + ld > ringBytes ? ringBytes - phys : 0u;   // wrap
+#if XDEV_VEC_TMA_STORE
+                if (iLoad - freed >= VEC_SLOTS || used + pad + adv > ringBytes) break;    // drain a landed piece first
+#else
                 if (iLoad - iStore >= VEC_SLOTS || used + pad + adv > ringBytes) break;   // drain a landed piece first
+#endif
                 const unsigned int po = pad ? 0u : phys;
                 const int slot = iLoad & (VEC_SLOTS - 1);
                 if (lane == slot) { mDst = tD; mPack = (po >> 7) | (len << 11) | (ms << 24); mAlloc = pad + adv; }
@@ -658,6 +730,11 @@ __device__ __forceinline__ void vector_engine(Cursor<L, SM>& cur, unsigned char*
         }
         if (iStore == iLoad) {
             if (!more) break;
+#if XDEV_VEC_TMA_STORE
+            if (lane == 0) { bulk_wait_read<0>(); fence_proxy_async_smem(); }   // the stores still reading their ring bytes
+            __syncwarp();
+            freed = iStore; used = 0;
+#endif
             phys = 0;                      // nothing in flight: restart the ring at offset 0 (the piece did not fit behind phys)
             continue;
         }
@@ -666,13 +743,36 @@ __device__ __forceinline__ void vector_engine(Cursor<L, SM>& cur, unsigned char*
         const unsigned int dlo = __shfl_sync(0xffffffffu, (unsigned int)mDst, slot);
         const unsigned int dhi = __shfl_sync(0xffffffffu, (unsigned int)(mDst >> 32), slot);
         const unsigned int pk = __shfl_sync(0xffffffffu, mPack, slot);
+#if XDEV_VEC_TMA_STORE
+        {
+            unsigned char* bDst; uint32_t bSm; unsigned int bBytes;
+            warp_drain_realign(reinterpret_cast<unsigned char*>(((unsigned long long)dhi << 32) | dlo), ring + ((pk & 0x7ffu) << 7),
+                               pk >> 24, (pk >> 11) & 0x1fffu, bDst, bSm, bBytes);
+            if (lane == 0) {
+                if (bBytes) bulk_s2g(bDst, bSm, bBytes PAYLOAD_POL(pol));
+                bulk_commit();                             // one group per piece (possibly empty), so that groups count pieces
+            }
+            ++iStore;
+            if (iStore - freed > 1) {                      // at most ONE store keeps its ring bytes: release the older piece
+                if (lane == 0) { bulk_wait_read<1>(); fence_proxy_async_smem(); }   // (lanes' head / tail byte reads precede the syncwarp of the drain)
+                __syncwarp();
+                used -= __shfl_sync(0xffffffffu, mAlloc, freed & (VEC_SLOTS - 1));
+                ++freed;
+            }
+        }
+#else
         used -= __shfl_sync(0xffffffffu, mAlloc, slot);
         warp_drain_shifted(reinterpret_cast<unsigned char*>(((unsigned long long)dhi << 32) | dlo), ring + ((pk & 0x7ffu) << 7),
                            pk >> 24, (pk >> 11) & 0x1fffu);
         ++iStore;
         __syncwarp();                      // every lane has read its words before the TMA may overwrite them
         if (lane == 0) fence_proxy_async_smem();
+#endif
     }
+#if XDEV_VEC_TMA_STORE
+    if (lane == 0) bulk_wait_all<0>();     // shared memory stays valid until every store has read it (and the run's writes are done)
+    __syncwarp();
+#endif
     pieceSeq = iLoad;
 }
 
@@ -801,8 +901,8 @@ __device__ __forceinline__ bool run_copy_engines(const SegDesc* desc, int* const
     const bool rrV = fusedStatic == 0 && nV > 0 && (long long)totV <= (long long)XDEV_RR_TPE * nV;
     const int stB = fusedStatic > 0 ? fusedStatic : rrB ? clamped_quotient(totB, 32 * nB, 1, totB >= 8 * RR ? COPY_KMAX_LONG : min(kmax, 8))
                                                         : static_first_chunk(totB, nB, kmax, COPY_KMAX_LONG, RR);
-    const int stV = fusedStatic > 0 ? fusedStatic : rrV ? clamped_quotient(totV, 32 * nV, 1, totV >= 8 * RR ? COPY_KMAX_LONG : COPY_KMAX_VEC)
-                                                        : static_first_chunk(totV, nV, COPY_KMAX_VEC, COPY_KMAX_LONG, RR);
+    const int stV = fusedStatic > 0 ? fusedStatic : rrV ? clamped_quotient(totV, 32 * nV, 1, totV >= 8 * RR ? COPY_KMAX_LONG_VEC : COPY_KMAX_VEC)
+                                                        : static_first_chunk(totV, nV, COPY_KMAX_VEC, COPY_KMAX_LONG_VEC, RR);
 #ifdef XDEV_TIMELINE
     if (tl) tl[TL_TILES] = (unsigned long long)totB;
 #endif
@@ -811,7 +911,7 @@ __device__ __forceinline__ bool run_copy_engines(const SegDesc* desc, int* const
                         nB, kmax, COPY_KMAX_LONG, stB, claimDiv, rrB);
     if (threadIdx.x == 32)
         cursor_env_init(&envs[LIST_VEC], LIST_VEC, desc, colBase[LIST_VEC], coarse[LIST_VEC], &ctl->next[LIST_VEC], cls, ncols, colLen,
-                        nV, COPY_KMAX_VEC, COPY_KMAX_LONG, stV, claimDiv, rrV);
+                        nV, COPY_KMAX_VEC, COPY_KMAX_LONG_VEC, stV, claimDiv, rrV);
     __syncthreads();
     TL_STAMP(tl, TL_ENV);
     if (warp < rp.E) {
