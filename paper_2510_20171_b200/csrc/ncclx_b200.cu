@@ -444,7 +444,10 @@ int topkCommon(int R, int T, int k, int width, int es) {
 
 int topkGrid(long long tokens) {
     long long ctas = (tokens + TOPK_THREADS / 32 - 1) / (TOPK_THREADS / 32);
-    const long long cap = (long long)g.smCount * 8;
+#ifndef XDEV_TOPK_CTAS_PER_SM
+#define XDEV_TOPK_CTAS_PER_SM 16
+#endif
+    const long long cap = (long long)g.smCount * XDEV_TOPK_CTAS_PER_SM;
     return (int)(ctas < 1 ? 1 : (ctas > cap ? cap : ctas));
 }
 

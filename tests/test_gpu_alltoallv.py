@@ -288,3 +288,29 @@ def test_every_source_destination_misalignment_pair(fused):
                     assert got[d].tobytes() == exp[d].tobytes(), f"mis_send={ms} mis_recv={md} recv[{d}]"
     finally:
         nx.ncclx_set_param(nx.PARAM_FUSED_MAX_RANKS, 32)
+
+
+@pytest.mark.parametrize("fused", [32, 0])
+def test_vector_pieces_around_the_staging_boundaries(fused):
+    """The vector engines stage a tile in pieces of at most 4 KiB whose ends follow the DESTINATION's 16-byte grid, realign
+    each piece in shared memory and store its body with one bulk copy: segment lengths 0..80 (no body at all, head and
+    tail only) and every length around one and two pieces (tiny trailing piece copied by lanes, body of a single vector),
+    each with source and destination misaligned alike, differently, and not at all.  One call holds all lengths (a
+    segment per (s, d) pair), so the full receive capacity incl. every neighbour's bytes is compared each time."""
+    nx.ncclx_set_param(nx.PARAM_FUSED_MAX_RANKS, fused)
+    try:
+        lens = list(range(0, 81)) + list(range(4060, 4140)) + list(range(8170, 8215)) + [16384, 16385, 16399, 32769]
+        R = 15
+        assert R * R >= len(lens)
+        C = np.zeros((R, R), np.int64)
+        for i, n in enumerate(lens):
+            C[i // R, i % R] = n
+        send = make_send(C, "u8", 91)
+        exp, eRC, *_ = oracle_a2a(send, C, "u8")
+        for ms, md in ((0, 0), (5, 5), (3, 9), (9, 3), (0, 15), (1, 0), (15, 14)):
+            got, RC, _, _ = run_a2a(send, C, "u8", mis_send=ms, mis_recv=md)
+            assert (RC == eRC).all()
+            for d in range(R):
+                assert got[d].tobytes() == exp[d].tobytes(), f"mis_send={ms} mis_recv={md} recv[{d}]"
+    finally:
+        nx.ncclx_set_param(nx.PARAM_FUSED_MAX_RANKS, 32)
