@@ -489,6 +489,29 @@ int launchTopkDispatch(int p, const void* const* tokens, const int32_t* pos, voi
     if (T == 0) return NCCLX_OK;
     TopkArgs ta = topkArgs(p, pos, R, T, k, rowBytes);
     ta.tokens = tokens; ta.packed = recv; ta.out = nullptr;
+#if XDEV_TOPK_TMA
+    // (A/B build) rows that are multiples of 16 bytes and fit a shared-memory slot (at least 4 warps' worth) move by TMA
+    const size_t slotBytes = alignUp((size_t)rowBytes, 128);
+    const size_t room = (size_t)g.maxSmemOptin - 1024;
+    int warps = (int)(room / (2 * slotBytes + 16));                // two slots per warp
+    if (warps > 16) warps = 16;
+    if (rowBytes % 16 == 0 && warps >= 4) {
+        LaunchScope ls(NCCLX_KERNEL_TOPK, s);
+        cudaLaunchConfig_t cfg{};
+        const long long tokens_ = (long long)R * T;
+        long long grid = (tokens_ + warps - 1) / warps;
+        if (grid > g.smCount) grid = g.smCount;
+        cfg.gridDim = dim3((unsigned)(grid < 1 ? 1 : grid));
+        cfg.blockDim = dim3((unsigned)warps * 32);
+        cfg.dynamicSmemBytes = (size_t)warps * (2 * slotBytes + 16);
+        cfg.stream = s;
+        cudaLaunchAttribute attr[1];
+        setPdl(cfg, attr, g.params[NCCLX_PARAM_PDL] != 0);
+        CK(cudaLaunchKernelEx(&cfg, topk_dispatch_tma_kernel, ta, (unsigned int)slotBytes));
+        ls.ok();
+        return NCCLX_OK;
+    }
+#endif
     return launchTopk(topk_dispatch_kernel, ta, s);
 }
 
@@ -636,6 +659,9 @@ static int initLocked(int max_ranks, int device) {
     if ((rc = optInSmem(segment_copy_kernel, g.maxSmemOptin))) return rc;
     if ((rc = optInSmem(counts_kernel, g.maxSmemOptin))) return rc;
     if ((rc = optInSmem(alltoallv_fused_kernel, g.maxSmemOptin))) return rc;
+#if XDEV_TOPK_TMA
+    if ((rc = optInSmem(topk_dispatch_tma_kernel, g.maxSmemOptin))) return rc;
+#endif
     if ((rc = optInSmem(dyn_build_kernel, (int)dyn_smem_bytes(DYN_SMEM_SLOTS)))) return rc;
     if ((rc = optInSmem(reducecopy_tma_kernel<RED_BF16>, RCT_SMEM_BYTES))) return rc;
     if ((rc = optInSmem(reducecopy_tma_kernel<RED_F32>, RCT_SMEM_BYTES))) return rc;
