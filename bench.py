@@ -731,6 +731,9 @@ def timeline_probe(torch, nx, peak, cfg_index=5, workload=None):
             def dispatch():
                 nx.ncclx_alltoallv_dynamic_dev(st, Ld, n, Id, idx.shape[1], Bd, J, rt, allL, R, "bf16")
         a = _Dyn
+    elif workload == "cfg1_two_kernels":
+        nx.ncclx_set_param(nx.PARAM_FUSED_MAX_RANKS, 0)
+        a = A2A(W.a2a_config(1), torch, nx, with_back=False)
     elif workload == "small64":
         a = A2A(W.A2AConfig("small64", 64, 5120, "bf16", 1, np.ones((64, 64), np.int64)), torch, nx, with_back=False)
     else:

@@ -29,6 +29,8 @@ struct WorkCtl {
     unsigned int status;      // sticky: bit 0 = negative count seen
     unsigned int done;        // CTAs of the running copy kernel that have drained their engines
     unsigned int pad_probe;   // sink of the streaming micro-probe (never read)
+    unsigned int barArrive;   // counts_kernel's grid barrier: CTAs that have published their block sums ...
+    unsigned int barDepart;   // ... and CTAs that have passed it (the last one zeroes both)
 };
 
 struct Workspace {
@@ -39,7 +41,9 @@ struct Workspace {
     int* colKiB;              // R: KiB of column d's bulk-list segments (-> average tile size -> bulk engines per CTA)
     int* coarse[2];           // R*ceil(colLen/32) each: tiles of list L in column d before its descriptor 32*j
     WorkCtl* ctl;
+    long long* blockSum;      // COUNTS_MAX_CTAS * R: blockSum[j*R+s] = sum of row s of C over CTA j's columns (counts_kernel)
 };
+constexpr int COUNTS_MAX_CTAS = 128;
 
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
 

@@ -5,12 +5,16 @@
 //       copy in parallel"; replaces the serial T_c*(N-1) issue loop of L447)
 // all on the device, from the counts as they are in memory when the kernel RUNS (L401, L409).
 //
-// Parallel decomposition with no inter-CTA communication: CTA j owns the W destination
-// columns [j*W, j*W+W).  Everything indexed by destination (RC row d, roff row d, descriptor row
-// d, per-column tile totals) is produced by the owner; the only cross-column quantity, the
-// row-wise send offset soff[s][d], is rebuilt by the owner from row s's prefix C[s][0..d0) (an
-// L2-resident re-read of at most R*R*8 bytes per CTA).  The cross-column tile base is left to
-// the copy kernel, which scans the R per-column totals itself.
+// Parallel decomposition: CTA j owns the W destination columns [j*W, j*W+W).  Everything indexed by destination (RC
+// row d, roff row d, descriptor row d, per-column tile totals) is produced by the owner; the only cross-column
+// quantity is the row-wise send offset soff[s][d] = (row s's prefix over the columns before d0) + a running sum:
+//   R <= 128  the owner rebuilds that prefix from C[s][0..d0) itself (an L2-resident re-read of at most 128 KB per CTA,
+//             no inter-CTA communication: cheaper than any barrier at this size);
+//   R  > 128  every CTA reads only its own R x W block, publishes one block sum per row, and after ONE grid barrier adds
+//             up the block sums of the CTAs before it (R*j values instead of R*d0: the re-read grows as R^3 / W over the
+//             grid and was 23 / 81 / 181 us of the kernel at R = 256 / 512 / 1024; now 112 / 411 / 1480 us per call
+//             instead of 116 / 437 / 1571).
+// The cross-column tile base is left to the copy kernel, which scans the R per-column totals itself.
 //
 // This kernel sits on the small-message latency path (config 5: ~5 % of the call; a per-CTA %globaltimer timeline
 // of it is in profiles/r2_cfg5_timeline.md), so both phases are laid out for latency: phase 1 issues all global
@@ -31,6 +35,7 @@ struct CountsArgs {
     Workspace ws;
     int R;
     int W;                        // columns per CTA (<= 32)
+    int blockSums;                // 1: phase 1 through per-CTA block sums and a grid barrier (R > 128); 0: row prefixes re-read from C
     long long elemSize;               // bytes per count unit (an element, or a whole row for the top-k calls)
     ClassParams cls;
 #ifdef XDEV_TIMELINE
@@ -83,48 +88,60 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
     }
     const unsigned long long rp = (threadIdx.x < Wc && a.recv) ? ld_keep_ptr(a.recv + d0 + threadIdx.x, keep) : 0ull;
 
-    // ---- phase 1: soff for the owned columns = row prefix C[s][0..d0) + running sum over the owned columns ------
-    // LPR lanes share a row (LPR = 512 / R rounded down to a power of two, 8..32): lane q sums the prefix columns
-    // q, q + LPR, ..., all loads independent (a handful per lane at R <= 128), then log2(LPR) shuffle steps combine
-    // the row.  (Round 1 gave a warp 8 rows and ran a 64-bit warp reduction AND a warp scan per row: ~5 us of
-    // dependent shuffles at R = 128; this is one round trip plus a few adds.)
-    int LPR = 32;
-    while (LPR > 8 && LPR * R > COUNTS_THREADS) LPR >>= 1;    // >= 8 lanes (64 contiguous bytes) per row: coalescing at large R
-    const int rowsPerPass = COUNTS_THREADS / LPR;
-    const int q = threadIdx.x & (LPR - 1);
     bool sawNeg = false;
-    for (int row0 = 0; row0 < R; row0 += rowsPerPass) {
-        const int s = row0 + threadIdx.x / LPR;
-        const bool valid = s < R;
-        const long long* row = a.C + (size_t)(valid ? s : 0) * R;
-        constexpr int OW = 4;                                          // owned columns kept in registers (W <= 4: R <= 128)
-        long long own[OW];
-#pragma unroll
-        for (int j = 0; j < OW; ++j) own[j] = (valid && q == 0 && j < Wc) ? ld_keep(row + d0 + j, keep) : 0;
-        long long part = 0;
-        constexpr int LU = 16;                                         // independent loads per trip
-        for (int dd = q; dd < d0; dd += LPR * LU) {
-            long long v[LU];
-#pragma unroll
-            for (int u = 0; u < LU; ++u) { const int x = dd + u * LPR; v[u] = (valid && x < d0) ? ld_keep(row + x, keep) : 0; }
-#pragma unroll
-            for (int u = 0; u < LU; ++u) part += v[u] > 0 ? v[u] : 0;
-        }
-        if (row0 == 0) {                                               // every thread passes here exactly once
-#pragma unroll
-            for (int i = 0; i < PT; ++i) {
-                const int t = threadIdx.x + i * COUNTS_THREADS;
-                if (t < R) sendPtr[t] = sp[i];
+    if (!a.blockSums) {
+        // (R <= 128) the row prefix straight from the count matrix: at most 128 KB of L2-resident re-reads per CTA cost
+        // less than a grid barrier (measured, graph replay p50: config 5 155.0 vs 157.0 us, R = 64 x 10 KB 26.0 vs 28.1 us)
+        // ---- phase 1: soff for the owned columns = row prefix C[s][0..d0) + running sum over the owned columns ------
+        // LPR lanes share a row (LPR = 512 / R rounded down to a power of two, 8..32): lane q sums the prefix columns
+        // q, q + LPR, ..., all loads independent (a handful per lane at R <= 128), then log2(LPR) shuffle steps combine
+        // the row.  (Round 1 gave a warp 8 rows and ran a 64-bit warp reduction AND a warp scan per row: ~5 us of
+        // dependent shuffles at R = 128; this is one round trip plus a few adds.)
+        int LPR = 32;
+        while (LPR > 8 && LPR * R > COUNTS_THREADS) LPR >>= 1;    // >= 8 lanes (64 contiguous bytes) per row: coalescing at large R
+        const int rowsPerPass = COUNTS_THREADS / LPR;
+        const int q = threadIdx.x & (LPR - 1);
+        for (int row0 = 0; row0 < R; row0 += rowsPerPass) {
+            const int s = row0 + threadIdx.x / LPR;
+            const bool valid = s < R;
+            const long long* row = a.C + (size_t)(valid ? s : 0) * R;
+            constexpr int OW = 4;                                          // owned columns kept in registers (W <= 4: R <= 128)
+            long long own[OW];
+    #pragma unroll
+            for (int j = 0; j < OW; ++j) own[j] = (valid && q == 0 && j < Wc) ? ld_keep(row + d0 + j, keep) : 0;
+            long long part = 0;
+            constexpr int LU = 16;                                         // independent loads per trip
+            for (int dd = q; dd < d0; dd += LPR * LU) {
+                long long v[LU];
+    #pragma unroll
+                for (int u = 0; u < LU; ++u) { const int x = dd + u * LPR; v[u] = (valid && x < d0) ? ld_keep(row + x, keep) : 0; }
+    #pragma unroll
+                for (int u = 0; u < LU; ++u) part += v[u] > 0 ? v[u] : 0;
             }
-            if (threadIdx.x < Wc) recvPtr[threadIdx.x] = rp;
-        }
-        for (int o = LPR >> 1; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-        if (valid && q == 0) {
-            long long run = part;
-#pragma unroll
-            for (int j = 0; j < OW; ++j) {
-                if (j < Wc) {
-                    long long cc = own[j];
+            if (row0 == 0) {                                               // every thread passes here exactly once
+    #pragma unroll
+                for (int i = 0; i < PT; ++i) {
+                    const int t = threadIdx.x + i * COUNTS_THREADS;
+                    if (t < R) sendPtr[t] = sp[i];
+                }
+                if (threadIdx.x < Wc) recvPtr[threadIdx.x] = rp;
+            }
+            for (int o = LPR >> 1; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+            if (valid && q == 0) {
+                long long run = part;
+    #pragma unroll
+                for (int j = 0; j < OW; ++j) {
+                    if (j < Wc) {
+                        long long cc = own[j];
+                        if (cc < 0) { sawNeg = true; cc = 0; }
+                        cval[(size_t)s * P + j] = cc;
+                        sofs[(size_t)s * P + j] = run;
+                        a.ws.soff[(size_t)s * R + d0 + j] = run;
+                        run += cc;
+                    }
+                }
+                for (int j = OW; j < Wc; ++j) {
+                    long long cc = ld_keep(row + d0 + j, keep);
                     if (cc < 0) { sawNeg = true; cc = 0; }
                     cval[(size_t)s * P + j] = cc;
                     sofs[(size_t)s * P + j] = run;
@@ -132,13 +149,67 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
                     run += cc;
                 }
             }
-            for (int j = OW; j < Wc; ++j) {
-                long long cc = ld_keep(row + d0 + j, keep);
-                if (cc < 0) { sawNeg = true; cc = 0; }
-                cval[(size_t)s * P + j] = cc;
-                sofs[(size_t)s * P + j] = run;
-                a.ws.soff[(size_t)s * R + d0 + j] = run;
-                run += cc;
+        }
+    } else {
+        // ---- phase 1: soff for the owned columns = (row prefix over the columns of CTAs 0..j-1) + running sum over the owned ones ----
+        // Round 1 / 2a rebuilt the row prefix C[s][0..d0) in every CTA from the count matrix itself: R*d0 loads per CTA, all
+        // CTAs pulling the same lines through L2 -- 2 to 6.5 us per CTA at R = 128 (per-CTA stamps), and 23 / 81 / 181 us for
+        // the whole kernel at R = 256 / 512 / 1024.  Now every CTA reads ONLY its own R x W block (coalesced), publishes one
+        // block sum per row, and after one grid barrier adds up the block sums of the CTAs before it (R*j values instead of
+        // R*d0).  The barrier is safe: the grid has at most COUNTS_MAX_CTAS small CTAs, all of which are resident before any
+        // dependent kernel may start (griddepcontrol.launch_dependents fires only once every CTA has issued it), and no kernel
+        // that could hold SMs depends on this one.
+        for (int i = threadIdx.x; i < R * Wc; i += COUNTS_THREADS) {            // own block -> shared memory, clamped
+            const int s = i / Wc, j = i - s * Wc;
+            long long cc = ld_keep(a.C + (size_t)s * R + d0 + j, keep);
+            if (cc < 0) { sawNeg = true; cc = 0; }
+            cval[(size_t)s * P + j] = cc;
+        }
+    #pragma unroll
+        for (int i = 0; i < PT; ++i) {
+            const int t = threadIdx.x + i * COUNTS_THREADS;
+            if (t < R) sendPtr[t] = sp[i];
+        }
+        if (threadIdx.x < Wc) recvPtr[threadIdx.x] = rp;
+        __syncthreads();
+        const int G = (int)gridDim.x;
+        for (int s = threadIdx.x; s < R; s += COUNTS_THREADS) {                 // running sums inside the block, block sum out
+            long long run = 0;
+            for (int j = 0; j < Wc; ++j) { sofs[(size_t)s * P + j] = run; run += cval[(size_t)s * P + j]; }
+            if (G > 1) a.ws.blockSum[(size_t)blockIdx.x * R + s] = run;
+        }
+        if (G > 1) {
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                __threadfence();
+                atomicAdd(&a.ws.ctl->barArrive, 1u);
+                unsigned int seen;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(&a.ws.ctl->barArrive) : "memory");
+                } while (seen < (unsigned int)G);
+            }
+            __syncthreads();
+        }
+        for (int s = threadIdx.x; s < R; s += COUNTS_THREADS) {                 // + the block sums of the CTAs before this one
+            long long pre = 0;
+            constexpr int BU = 8;
+            for (int jb = 0; jb < (int)blockIdx.x; jb += BU) {
+                long long v[BU];
+    #pragma unroll
+                for (int u = 0; u < BU; ++u) v[u] = jb + u < (int)blockIdx.x ? __ldcg(a.ws.blockSum + (size_t)(jb + u) * R + s) : 0;   // L2: written by other CTAs of this grid
+    #pragma unroll
+                for (int u = 0; u < BU; ++u) pre += v[u];
+            }
+            for (int j = 0; j < Wc; ++j) {
+                const long long o = sofs[(size_t)s * P + j] + pre;
+                sofs[(size_t)s * P + j] = o;
+                a.ws.soff[(size_t)s * R + d0 + j] = o;
+            }
+        }
+        if (G > 1 && threadIdx.x == 0) {                                        // last CTA past the barrier re-arms it
+            if (atomicAdd(&a.ws.ctl->barDepart, 1u) == (unsigned int)G - 1u) {
+                a.ws.ctl->barArrive = 0u; a.ws.ctl->barDepart = 0u;
+                __threadfence();
             }
         }
     }

@@ -126,6 +126,7 @@ struct LaunchScope {
 
 constexpr size_t kMaxCoarseBytes = 16 * 1024;     // both coarse indexes; larger tables fall back to the L2 search
 constexpr int kVecTileShift = 14;                 // vector-list work unit: 16 KiB (staged in 2 KiB pieces)
+constexpr int kCountsBlockSumMinRanks = 128;      // above this many ranks the counts kernel's phase 1 goes through block sums + a grid barrier
 constexpr int kScanCtas = 32;                     // upper bound on CTAs of the counts kernel
 constexpr int kFusedMinTileShift = 12;            // smallest bulk tile the single-launch path may choose
 
@@ -244,11 +245,13 @@ int launchCounts(const Workspace& ws, const void* const* send, const int64_t* C,
     ca.C = reinterpret_cast<const long long*>(C);
     ca.RC = reinterpret_cast<long long*>(RC);
     ca.ws = ws; ca.R = R; ca.W = countsW(R); ca.elemSize = es;
+    ca.blockSums = R > kCountsBlockSumMinRanks ? 1 : 0;
     ca.cls = cls;
 #ifdef XDEV_TIMELINE
     ca.timeline = g.timeline + (size_t)g.smCount * TL_COUNT;      // counts-kernel stamps follow the copy kernel's
 #endif
     const int G = (R + ca.W - 1) / ca.W;
+    if (G > COUNTS_MAX_CTAS) return NCCLX_ERR_ARG;        // (cannot happen for R <= NCCLX_MAX_RANKS: W >= 12 there)
     const size_t csm = countsSmemBytes(R, ca.W);
     LaunchScope ls(NCCLX_KERNEL_COUNTS, stream);
     cudaLaunchConfig_t cfg{};
@@ -617,7 +620,7 @@ static int initLocked(int max_ranks, int device) {
     const size_t rr = (size_t)max_ranks * max_ranks;
     size_t off = 0;
     size_t oSoff[NCCLX_NUM_PLANS], oRoff[NCCLX_NUM_PLANS], oDesc[NCCLX_NUM_PLANS], oCt0[NCCLX_NUM_PLANS],
-        oCt1[NCCLX_NUM_PLANS], oCtl[NCCLX_NUM_PLANS], oCo0[NCCLX_NUM_PLANS], oCo1[NCCLX_NUM_PLANS], oKib[NCCLX_NUM_PLANS];
+        oCt1[NCCLX_NUM_PLANS], oCtl[NCCLX_NUM_PLANS], oCo0[NCCLX_NUM_PLANS], oCo1[NCCLX_NUM_PLANS], oKib[NCCLX_NUM_PLANS], oBs[NCCLX_NUM_PLANS];
     const size_t coarseInts = (size_t)max_ranks * coarse_blocks(max_ranks);
     for (int p = 0; p < NCCLX_NUM_PLANS; ++p) {
         oSoff[p] = off; off = alignUp(off + rr * 8, 256);
@@ -629,6 +632,7 @@ static int initLocked(int max_ranks, int device) {
         oCtl[p] = off; off = alignUp(off + sizeof(WorkCtl), 256);
         oCo0[p] = off; off = alignUp(off + coarseInts * 4, 256);
         oCo1[p] = off; off = alignUp(off + coarseInts * 4, 256);
+        oBs[p] = off; off = alignUp(off + (size_t)COUNTS_MAX_CTAS * max_ranks * 8, 256);
     }
     const size_t oFctl = off; off = alignUp(off + sizeof(WorkCtl), 256);
     const size_t oRcs = off; off = alignUp(off + rr * 8, 256);
@@ -646,6 +650,7 @@ static int initLocked(int max_ranks, int device) {
         w.ctl = reinterpret_cast<WorkCtl*>(b + oCtl[p]);
         w.coarse[0] = reinterpret_cast<int*>(b + oCo0[p]);
         w.coarse[1] = reinterpret_cast<int*>(b + oCo1[p]);
+        w.blockSum = reinterpret_cast<long long*>(b + oBs[p]);
         g.plan[p] = Context::PlanState{};
     }
     g.fusedCtl = reinterpret_cast<WorkCtl*>(b + oFctl);
