@@ -222,77 +222,94 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
     // (round 1 ran one warp per COLUMN, serially over the row blocks: with few columns per CTA most warps idled through
     //  the longest dependent chain of the kernel.)  An item needs two column-wise prefixes: the elements before the block
     //  (-> roff, destination addresses) and the tiles before it (-> work-list prefixes).  The first is a masked sum over
-    //  shared memory; the second depends on the first (tile counts depend on the addresses), so: pass 1 computes every
-    //  item's tile totals, pass 2 (after one barrier) recomputes the item with its tile base and writes everything out.
+    //  shared memory; the second depends on the first (tile counts depend on the addresses), so: the front half computes
+    //  every item's tile totals, the back half (after one barrier) adds the tile base and writes everything out.
     const int nb = (R + 31) >> 5;
     const int nItems = Wc * nb;
     long long* tileTot = reinterpret_cast<long long*>(recvPtr + W);      // [W*nb] tiles of the item: bulk << 32 | vector
     long long* rowsBefore = tileTot + (size_t)W * nb;                    // [W*nb] elements of the column before the block
     long long* byteTot = rowsBefore + (size_t)W * nb;                    // [W*nb] bytes of the item's bulk-list segments
-    for (int pass = 0; pass < 2; ++pass) {
-        for (int item = warp; item < nItems; item += nwarps) {
-            const int j = item / nb, b = item - j * nb;
-            const int d = d0 + j;
-            long long run;
-            if (pass == 0) {
-                long long part = 0;
-                for (int sp2 = lane; sp2 < b * 32; sp2 += 32) part += cval[(size_t)sp2 * P + j];
-                run = warp_sum(part);
-                if (lane == 0) rowsBefore[item] = run;
-            } else {
-                run = rowsBefore[item];
-            }
-            const int s = b * 32 + lane;
-            const bool valid = s < R;
-            const long long c = valid ? cval[(size_t)s * P + j] : 0;
-            const long long incl = warp_incl_scan(c);
-            const long long ro = run + incl - c;
-            const long long bytes = c * a.elemSize;
-            unsigned long long src = 0, dst = 0;
-            int tb = 0, tv = 0;
-            if (valid) {
-                src = sendPtr[s] + (unsigned long long)(sofs[(size_t)s * P + j] * a.elemSize);
-                dst = recvPtr[j] + (unsigned long long)(ro * a.elemSize);
-                tb = seg_tiles(LIST_BULK, src, dst, bytes, a.cls);
-                tv = seg_tiles(LIST_VEC, src, dst, bytes, a.cls);
-            }
-            const long long it = warp_incl_scan(((long long)tb << 32) | (long long)(unsigned int)tv);   // both lists at once
-            if (pass == 0) {
-                const long long bb = warp_sum(tb > 0 ? bytes : 0);
-                if (lane == 31) tileTot[item] = it;
-                if (lane == 0) byteTot[item] = bb;
-                continue;
-            }
-            long long base = 0, allT = 0, allB = 0;                        // tiles of the column before this block / in total
-            for (int bp = lane; bp < nb; bp += 32) {
-                const long long t = tileTot[(size_t)j * nb + bp];
-                if (bp < b) base += t;
-                allT += t;
-                allB += byteTot[(size_t)j * nb + bp];
-            }
-            base = warp_sum(base);
-            if (lane < 2) a.ws.coarse[lane][(size_t)d * nb + b] = lane ? (int)(unsigned int)base : (int)(base >> 32);   // coarse index for the copy kernel's search
-            if (valid) {
-                const size_t q = (size_t)d * R + s;
-                const long long pf = base + it;
-                a.RC[q] = c;
-                a.ws.roff[q] = ro;
-                uint4* out = reinterpret_cast<uint4*>(a.ws.desc + q);
-                out[0] = make_uint4((unsigned int)src, (unsigned int)(src >> 32), (unsigned int)dst, (unsigned int)(dst >> 32));
-                out[1] = make_uint4((unsigned int)bytes, (unsigned int)((unsigned long long)bytes >> 32),
-                                    (unsigned int)(pf >> 32), (unsigned int)pf);
-            }
-            if (b == 0) {                                                  // column totals, once per column
-                allT = warp_sum(allT);
-                allB = warp_sum(allB);
-                if (lane == 0) {
-                    a.ws.colTiles[LIST_BULK][d] = (int)(allT >> 32);
-                    a.ws.colTiles[LIST_VEC][d] = (int)(unsigned int)allT;
-                    a.ws.colKiB[d] = (int)(allB >> 10);
-                }
+    struct Item { int j, b, s; bool valid; long long c, ro, bytes, it; unsigned long long src, dst; int tb; };
+    // front half: everything that does not need the other items' tile totals
+    auto front = [&](int item, bool first) {
+        Item x;
+        x.j = item / nb; x.b = item - x.j * nb;
+        long long run;
+        if (first) {
+            long long part = 0;
+            for (int sp2 = lane; sp2 < x.b * 32; sp2 += 32) part += cval[(size_t)sp2 * P + x.j];
+            run = warp_sum(part);
+            if (lane == 0) rowsBefore[item] = run;
+        } else {
+            run = rowsBefore[item];
+        }
+        x.s = x.b * 32 + lane;
+        x.valid = x.s < R;
+        x.c = x.valid ? cval[(size_t)x.s * P + x.j] : 0;
+        const long long incl = warp_incl_scan(x.c);
+        x.ro = run + incl - x.c;
+        x.bytes = x.c * a.elemSize;
+        x.src = 0; x.dst = 0; x.tb = 0;
+        int tv = 0;
+        if (x.valid) {
+            x.src = sendPtr[x.s] + (unsigned long long)(sofs[(size_t)x.s * P + x.j] * a.elemSize);
+            x.dst = recvPtr[x.j] + (unsigned long long)(x.ro * a.elemSize);
+            x.tb = seg_tiles(LIST_BULK, x.src, x.dst, x.bytes, a.cls);
+            tv = seg_tiles(LIST_VEC, x.src, x.dst, x.bytes, a.cls);
+        }
+        x.it = warp_incl_scan(((long long)x.tb << 32) | (long long)(unsigned int)tv);   // both lists at once
+        if (first) {
+            const long long bb = warp_sum(x.tb > 0 ? x.bytes : 0);
+            if (lane == 31) tileTot[item] = x.it;
+            if (lane == 0) byteTot[item] = bb;
+        }
+        return x;
+    };
+    // back half (after the barrier): tile base of the item inside its column, then everything is written out
+    auto back = [&](const Item& x) {
+        const int d = d0 + x.j;
+        long long base = 0, allT = 0, allB = 0;                        // tiles of the column before this block / in total
+        for (int bp = lane; bp < nb; bp += 32) {
+            const long long t = tileTot[(size_t)x.j * nb + bp];
+            if (bp < x.b) base += t;
+            allT += t;
+            allB += byteTot[(size_t)x.j * nb + bp];
+        }
+        base = warp_sum(base);
+        if (lane < 2) a.ws.coarse[lane][(size_t)d * nb + x.b] = lane ? (int)(unsigned int)base : (int)(base >> 32);   // coarse index for the copy kernel's search
+        if (x.valid) {
+            const size_t q = (size_t)d * R + x.s;
+            const long long pf = base + x.it;
+            a.RC[q] = x.c;
+            a.ws.roff[q] = x.ro;
+            uint4* out = reinterpret_cast<uint4*>(a.ws.desc + q);
+            out[0] = make_uint4((unsigned int)x.src, (unsigned int)(x.src >> 32), (unsigned int)x.dst, (unsigned int)(x.dst >> 32));
+            out[1] = make_uint4((unsigned int)x.bytes, (unsigned int)((unsigned long long)x.bytes >> 32),
+                                (unsigned int)(pf >> 32), (unsigned int)pf);
+        }
+        if (x.b == 0) {                                                // column totals, once per column
+            allT = warp_sum(allT);
+            allB = warp_sum(allB);
+            if (lane == 0) {
+                a.ws.colTiles[LIST_BULK][d] = (int)(allT >> 32);
+                a.ws.colTiles[LIST_VEC][d] = (int)(unsigned int)allT;
+                a.ws.colKiB[d] = (int)(allB >> 10);
             }
         }
-        if (pass == 0) { __syncthreads(); CT_STAMP(4); }
+    };
+    if (nItems <= nwarps) {
+        // at most one item per warp (R <= 128 with 32 CTAs): its state stays in registers across the barrier, nothing is
+        // computed twice
+        Item x{};
+        if (warp < nItems) x = front(warp, true);
+        __syncthreads();
+        CT_STAMP(4);
+        if (warp < nItems) back(x);
+    } else {
+        for (int item = warp; item < nItems; item += nwarps) (void)front(item, true);
+        __syncthreads();
+        CT_STAMP(4);
+        for (int item = warp; item < nItems; item += nwarps) back(front(item, false));
     }
     CT_STAMP(5);
 }

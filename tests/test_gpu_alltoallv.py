@@ -204,6 +204,64 @@ def test_large_R(R):
     assert_a2a_matches(send, C, "bf16")
 
 
+@pytest.mark.parametrize("R", [129, 160, 512])
+def test_large_R_metadata_barrier_in_plan_slots_and_graph_replays(R):
+    """Above 128 ranks the metadata kernel's CTAs exchange block sums through a self-resetting grid barrier in the plan
+    slot's control block: a dispatch and its inverse prepared into two slots (the second on a side stream, beside the
+    first one's payload kernel, which holds every SM), captured once and replayed with the counts rewritten between
+    replays -- offsets, receive counts and every byte against the oracle each time."""
+    import oracle
+    rng = np.random.default_rng(R)
+    hi = max(3, 6_000_000 // (R * R))
+    cap = hi * R                                               # elements a rank can send / receive at most
+    send_np = [W.np_values(cap, "bf16", 700 + s) for s in range(R)]
+    send = [to_dev(a) for a in send_np]
+    recv = [sentinel(cap * 2) for _ in range(R)]
+    bk = [sentinel(cap * 2) for _ in range(R)]
+    Cd = torch.zeros((R, R), dtype=torch.int64, device="cuda")
+    RCd, C2d = torch.zeros_like(Cd), torch.zeros_like(Cd)
+    st, rt, bt = nx.device_ptr_table(send), nx.device_ptr_table(recv), nx.device_ptr_table(bk)
+    side = torch.cuda.Stream()
+
+    def pair():
+        main = torch.cuda.current_stream()
+        nx.ncclx_alltoallv_prepare_dev(2, st, Cd, rt, RCd, R, "bf16")
+        side.wait_stream(main)
+        with torch.cuda.stream(side):
+            nx.ncclx_alltoallv_prepare_dev(3, rt, RCd, bt, C2d, R, "bf16")
+        nx.ncclx_alltoallv_execute_dev(2)
+        main.wait_stream(side)
+        nx.ncclx_alltoallv_execute_dev(3)
+    warm = torch.cuda.Stream()
+    warm.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(warm):
+        pair()
+    torch.cuda.current_stream().wait_stream(warm)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        pair()
+    for it in range(3):
+        C = rng.integers(0, hi, (R, R)).astype(np.int64)
+        C[rng.random((R, R)) < 0.4] = 0
+        if it == 1:
+            C[:, R // 2] = 0
+        for r in recv + bk:
+            r.fill_(SENT8)
+        Cd.copy_(torch.from_numpy(C), non_blocking=True)
+        graph.replay()
+        torch.cuda.synchronize()
+        exp = [np.full(cap, 0xA5A5, np.uint16) for _ in range(R)]
+        RC, *_ = oracle.alltoallv(send_np, C, exp, "bf16", nthreads=4)
+        assert (RCd.cpu().numpy() == RC).all() and (C2d.cpu().numpy() == C).all()
+        for d in range(R):
+            assert back(recv[d], "bf16").tobytes() == exp[d].tobytes(), f"replay {it} recv[{d}]"
+        for s in range(R):
+            n = int(C[s].sum())
+            got = back(bk[s], "bf16")
+            assert got[:n].tobytes() == send_np[s][:n].tobytes() and (got[n:] == 0xA5A5).all(), f"replay {it} round trip {s}"
+
+
 def test_graph_capture_counts_by_reference():
     """counts may change until the collective executes.  Capture once with one
     count matrix, rewrite the device-resident counts between replays, outputs must follow."""
