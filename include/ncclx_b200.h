@@ -103,7 +103,8 @@ int ncclx_version(void);
  * sum_s C[s][d] elements; overflow is undefined (as in NCCL).  send and recv buffers must not
  * overlap.  Segment addresses may have any element alignment; full speed is only promised
  * when every segment's source address, destination address and byte length are multiples of
- * 16 (TMA in and out); everything else is loaded by the TMA as aligned spans and stored by warps (vector list).
+ * 16 (bulk list: 32 KiB tiles, TMA in and out); everything else is loaded by the TMA as aligned spans, realigned in
+ * shared memory and stored by the TMA as well, 4 KiB at a time (vector list: ~0.9 of the bulk list's rate).
  * The inverse ("combine") is the same call with send := recv, sendcounts := recvcounts.
  * For R <= 32 (NCCLX_PARAM_FUSED_MAX_RANKS) the call is ONE kernel launch (the small-message fast path,
  * PAPER.md L483): every CTA rebuilds offsets and work list from the <= 8 KB count matrix in shared memory
@@ -274,7 +275,7 @@ int ncclx_reducescatter_sum_host(const void* const* send, void* const* recv, siz
 
 typedef enum {
     NCCLX_PARAM_BULK_MIN_BYTES = 0,     /* 16B-aligned segments >= this many bytes go on the bulk list (32 KiB tiles, TMA in and out);  */
-                                        /* smaller or unaligned ones on the vector list (TMA in, warp stores out). default 1024         */
+                                        /* smaller or unaligned ones on the vector list (4 KiB pieces, realigned in shared memory). default 1024 */
     NCCLX_PARAM_REDUCE_CTAS_PER_SM = 1, /* reduce grid = this * SM count (1..64), default 16 (4x what fits at once: a short call such  */
                                         /* as config 2 becomes one tile per CTA, dealt out by the hardware scheduler)                  */
     NCCLX_PARAM_PROFILE = 2,            /* 1: bracket each kernel with CUDA events (never while capturing)                              */
