@@ -738,9 +738,44 @@ def timeline_probe(torch, nx, peak, cfg_index=5, workload=None):
         a = A2A(W.A2AConfig("small64", 64, 5120, "bf16", 1, np.ones((64, 64), np.int64)), torch, nx, with_back=False)
     else:
         a = A2A(W.a2a_config(cfg_index), torch, nx, with_back=False)
-    for _ in range(5):
-        a.dispatch()
-    torch.cuda.synchronize()
+    graph_mode = None
+    if os.environ.get("NCCLX_TIMELINE_MODE", "eager") == "graph":
+        # the configuration the latency numbers are quoted in: ONE call per CUDA-graph replay, replays separated by a
+        # synchronise (so every replay starts cold and alone); stamps of 300 replays, percentiles over the replays
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            a.dispatch()
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            a.dispatch()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        rows = []
+        for i in range(320):
+            e0.record(); g.replay(); e1.record()
+            torch.cuda.synchronize()
+            tl_, ct_ = nx.ncclx_debug_timeline()
+            tl_, ct_ = tl_.astype(np.int64), ct_.astype(np.int64)
+            ct_ = ct_[ct_[:, 0] > 0]
+            z = int(ct_[:, 0].min())
+            last = ct_.shape[1] - 1 if workload == "dynamic" else 5
+            rows.append([e0.elapsed_time(e1) * 1e3, (tl_[:, 0].min() - z) / 1e3, (ct_[:, 1].max() - z) / 1e3, (ct_[:, last].max() - z) / 1e3,
+                         (np.median(tl_[:, 1]) - z) / 1e3, (np.median(tl_[:, 2]) - z) / 1e3, (np.median(tl_[:, 3]) - z) / 1e3,
+                         (tl_[:, 4].max() - z) / 1e3, (tl_[:, 6].max() - z) / 1e3])
+        r = np.array(rows[20:])
+        gn = ["event_pair_around_the_replay", "copy_kernel_first_cta_enters", "metadata_dependency_wait_over", "metadata_last_cta_exits",
+              "copy_metadata_ready_median", "copy_first_load_median", "copy_first_store_median", "copy_last_store_of_last_cta", "copy_last_cta_exits"]
+        graph_mode = {n: {"p10": round(float(np.percentile(r[:, i], 10)), 2), "p50": round(float(np.percentile(r[:, i], 50)), 2),
+                          "p90": round(float(np.percentile(r[:, i], 90)), 2)} for i, n in enumerate(gn)}
+        d_ = r[:, 0] - r[:, 8]
+        graph_mode["event_pair_minus_gpu_side_span"] = {"p10": round(float(np.percentile(d_, 10)), 2), "p50": round(float(np.percentile(d_, 50)), 2),
+                                                        "p90": round(float(np.percentile(d_, 90)), 2)}
+    else:
+        for _ in range(5):
+            a.dispatch()
+        torch.cuda.synchronize()
     tl, ct = nx.ncclx_debug_timeline()
     tl, ct = tl.astype(np.int64), ct.astype(np.int64)
     ct = ct[ct[:, 0] > 0]                                              # CTAs of the counts kernel that ran
@@ -764,6 +799,8 @@ def timeline_probe(torch, nx, peak, cfg_index=5, workload=None):
     out["kernel_span_us"] = round(span, 2)
     out["median_cta_streaming_window_us"] = round(busy, 2)
     out["at_6.9TBps_us"] = round(2 * a.bytes_one_way / 6.9e12 * 1e6, 2)
+    if graph_mode:
+        out["graph_replay_mode_us_since_first_metadata_cta"] = graph_mode
     out["per_cta"] = [[round(float(cols[nm][i]), 2) for nm in names] for i in range(tl.shape[0])]
     out["metadata_kernel_per_cta"] = [[round(float((ct[c, i] - t0) / 1e3), 2) for i in range(len(cnames))] for c in range(len(ct))]
     return out
