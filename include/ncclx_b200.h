@@ -277,7 +277,8 @@ typedef enum {
     NCCLX_PARAM_BULK_MIN_BYTES = 0,     /* 16B-aligned segments >= this many bytes go on the bulk list (32 KiB tiles, TMA in and out);  */
                                         /* smaller or unaligned ones on the vector list (4 KiB pieces, realigned in shared memory). default 1024 */
     NCCLX_PARAM_REDUCE_CTAS_PER_SM = 1, /* reduce grid = this * SM count (1..64), default 16 (4x what fits at once: a short call such  */
-                                        /* as config 2 becomes one tile per CTA, dealt out by the hardware scheduler)                  */
+                                        /* as config 2 becomes one tile per CTA, dealt out by the hardware scheduler); reductions below */
+                                        /* 256 MiB of input run on 64-thread CTAs and twice this many of them                           */
     NCCLX_PARAM_PROFILE = 2,            /* 1: bracket each kernel with CUDA events (never while capturing)                              */
     NCCLX_PARAM_BULK_TILE_SHIFT = 3,    /* log2 bytes of a bulk tile (12..16), default 15                                               */
     NCCLX_PARAM_PDL = 4,                /* 1 (default): programmatic dependent launch -- a kernel's prologue overlaps the tail of the   */

@@ -334,20 +334,21 @@ int launchAllToAllv(const void* const* send, const int64_t* C, void* const* recv
 
 constexpr size_t kReducePdlMaxBytes = (size_t)1 << 30;   // reductions below this many input bytes launch with PDL
 constexpr size_t kReducePrefetchAllBytes = (size_t)96 << 20;
+constexpr size_t kReduceShortBytes = (size_t)256 << 20;   // reductions below this many input bytes run on 64-thread CTAs
 
-template <int DT>
+template <int DT, int TH>
 int launchReduceDT(const ReduceArgs& ra, int grid, size_t smem, bool pdl, cudaStream_t stream) {
     LaunchScope ls(NCCLX_KERNEL_REDUCE, stream);
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid);
-    cfg.blockDim = dim3(REDUCE_THREADS);
+    cfg.blockDim = dim3(TH);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     setPdl(cfg, attr, pdl);
-    if (ra.R <= 4) CK(cudaLaunchKernelEx(&cfg, reduce_kernel<DT, 4>, ra));
-    else if (ra.R <= 8) CK(cudaLaunchKernelEx(&cfg, reduce_kernel<DT, 8>, ra));
-    else CK(cudaLaunchKernelEx(&cfg, reduce_kernel<DT, 16>, ra));
+    if (ra.R <= 4) CK(cudaLaunchKernelEx(&cfg, reduce_kernel<DT, 4, TH>, ra));
+    else if (ra.R <= 8) CK(cudaLaunchKernelEx(&cfg, reduce_kernel<DT, 8, TH>, ra));
+    else CK(cudaLaunchKernelEx(&cfg, reduce_kernel<DT, 16, TH>, ra));
     ls.ok();
     return NCCLX_OK;
 }
@@ -359,8 +360,11 @@ int launchReduce(const void* const* send, void* const* recv, size_t blockElems, 
     ra.send = send; ra.recv = recv; ra.blockElems = blockElems; ra.R = R; ra.scatter = scatter;
     const int es = elemSizeOf(dtype);
     const unsigned long long totalVec = ((unsigned long long)blockElems * (scatter ? R : 1) * es + 31) / 32;
-    unsigned long long tiles = (totalVec + REDUCE_THREADS - 1) / REDUCE_THREADS + (scatter ? R : 0);
-    unsigned long long grid = (unsigned long long)g.smCount * (unsigned long long)g.params[NCCLX_PARAM_REDUCE_CTAS_PER_SM];
+    const size_t inBytes0 = (size_t)blockElems * (scatter ? R : 1) * es * (size_t)R;
+    const bool shortCall = inBytes0 < kReduceShortBytes;        // short: 64-thread CTAs, twice as many
+    const unsigned long long th = shortCall ? REDUCE_THREADS_SHORT : REDUCE_THREADS;
+    unsigned long long tiles = (totalVec + th - 1) / th + (scatter ? R : 0);
+    unsigned long long grid = (unsigned long long)g.smCount * (unsigned long long)g.params[NCCLX_PARAM_REDUCE_CTAS_PER_SM] * (shortCall ? 2 : 1);
     if (grid > tiles) grid = tiles;
     if (grid < 1) grid = 1;
     const size_t smem = 2 * (size_t)R * sizeof(void*);
@@ -379,9 +383,12 @@ int launchReduce(const void* const* send, void* const* recv, size_t blockElems, 
     ra.prefetchTiles = 0;
 #endif
     switch (dtype) {
-    case NCCLX_BF16: return launchReduceDT<RED_BF16>(ra, (int)grid, smem, pdl, stream);
-    case NCCLX_F32: return launchReduceDT<RED_F32>(ra, (int)grid, smem, pdl, stream);
-    case NCCLX_F16: return launchReduceDT<RED_F16>(ra, (int)grid, smem, pdl, stream);
+    case NCCLX_BF16: return shortCall ? launchReduceDT<RED_BF16, REDUCE_THREADS_SHORT>(ra, (int)grid, smem, pdl, stream)
+                                      : launchReduceDT<RED_BF16, REDUCE_THREADS>(ra, (int)grid, smem, pdl, stream);
+    case NCCLX_F32: return shortCall ? launchReduceDT<RED_F32, REDUCE_THREADS_SHORT>(ra, (int)grid, smem, pdl, stream)
+                                     : launchReduceDT<RED_F32, REDUCE_THREADS>(ra, (int)grid, smem, pdl, stream);
+    case NCCLX_F16: return shortCall ? launchReduceDT<RED_F16, REDUCE_THREADS_SHORT>(ra, (int)grid, smem, pdl, stream)
+                                     : launchReduceDT<RED_F16, REDUCE_THREADS>(ra, (int)grid, smem, pdl, stream);
     default: return NCCLX_ERR_DTYPE;
     }
 }
