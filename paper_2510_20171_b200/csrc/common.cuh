@@ -154,13 +154,6 @@ __device__ __forceinline__ void st_stream256(void* p, const u32x8& v) {
                  : "memory");
 }
 
-// 256-bit store with an L2 eviction policy
-__device__ __forceinline__ void st_stream256(void* p, const u32x8& v, unsigned long long pol) {
-    asm volatile("st.global.L1::no_allocate.L2::cache_hint.v8.u32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8}, %9;"
-                 :: "l"(p), "r"(v.lo.x), "r"(v.lo.y), "r"(v.lo.z), "r"(v.lo.w), "r"(v.hi.x), "r"(v.hi.y), "r"(v.hi.z), "r"(v.hi.w), "l"(pol)
-                 : "memory");
-}
-
 // ---- mbarrier + cp.async.bulk (descriptor-less 1-D TMA) --------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 

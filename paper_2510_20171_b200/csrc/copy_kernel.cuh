@@ -142,10 +142,7 @@ __device__ __forceinline__ void cursor_env_init(CursorEnv* e, int L, const SegDe
     e->rr = rr;
     e->claimDiv = claimDiv;
     // a short list (few tiles per engine) pays per claim, a long one for the imbalance of its last chunks
-#ifndef XDEV_KMIN1
-#define XDEV_KMIN1 0
-#endif
-    e->kmin = (XDEV_KMIN1 || e->total >= 32 * e->nEngines) ? 1 : 2;
+    e->kmin = e->total >= 32 * e->nEngines ? 1 : 2;          // (always 1: R = 64 x 10 KB +2 us, NEXT-1 +2 us)
     e->dynBase = staticK * e->nEngines;
     (void)L;
 }
@@ -919,12 +916,10 @@ __device__ __forceinline__ bool run_copy_engines(const SegDesc* desc, int* const
         cur.init(&envs[LIST_BULK], (int)blockIdx.x * rp.E + warp);
         if (warp == 0) TL_STAMP(tl, TL_CURSOR);
         bulk_engine<SM>(cur, smem + (size_t)warp * rp.bulkShare, mbar + warp * COPY_SLOTS, rp.bulkShare, warp == 0 ? tl : nullptr);
-#ifndef XDEV_EXPERIMENT_NOVEC
     } else if (warp < rp.E + rp.NV) {
         const int v = warp - rp.E;
         vector_role<SM>(envs, (int)blockIdx.x * rp.NV + v, smem + rp.vecBase + (size_t)v * rp.vecShare,
                         mbar + COPY_MAX_ENGINES * COPY_SLOTS + v * VEC_SLOTS, rp.vecShare, rp.bulkByVec);
-#endif
     }
     return (nB > 0 && totB > stB * nB && !rrB) || (nV > 0 && totV > stV * nV && !rrV);
 }

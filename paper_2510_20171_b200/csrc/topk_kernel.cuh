@@ -24,9 +24,6 @@ namespace xdev {
 #ifndef XDEV_TOPK_UNROLL
 #define XDEV_TOPK_UNROLL 2
 #endif
-#ifndef XDEV_TOPK_STORE_POLICY
-#define XDEV_TOPK_STORE_POLICY 0
-#endif
 constexpr int TOPK_THREADS = XDEV_TOPK_THREADS;
 constexpr int TOPK_UNROLL = XDEV_TOPK_UNROLL;             // dispatch: vectors per lane in flight per copy (4 measured 8 % slower)
 constexpr int TOPK_COMBINE_UNROLL = 4;     // combine: 4 measured 1 % faster than 2
