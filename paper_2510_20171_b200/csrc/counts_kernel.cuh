@@ -26,6 +26,7 @@
 namespace xdev {
 
 constexpr int COUNTS_THREADS = 512;
+constexpr int COUNTS_BARRIER_POLLS = 8192;   // ~2-4 ms of polling before a CTA falls back to the barrier-free prefix (see phase 1)
 
 struct CountsArgs {
     const void* const* send;      // device table (null: no descriptors wanted, offsets and RC only)
@@ -178,27 +179,47 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
             for (int j = 0; j < Wc; ++j) { sofs[(size_t)s * P + j] = run; run += cval[(size_t)s * P + j]; }
             if (G > 1) a.ws.blockSum[(size_t)blockIdx.x * R + s] = run;
         }
+        __shared__ int sTimedOut;
         if (G > 1) {
             __syncthreads();
             if (threadIdx.x == 0) {
                 __threadfence();
                 atomicAdd(&a.ws.ctl->barArrive, 1u);
-                unsigned int seen;
-                do {
+                // bounded wait: should the grid ever NOT be resident as a whole (two such metadata kernels of > 700 ranks
+                // dispatched interleaved on two streams would each hold part of the device), a CTA gives up after a few
+                // milliseconds, rebuilds its row prefixes from the count matrix like the R <= 128 path, and leaves --
+                // freeing its SM, so the barrier can never deadlock; results are the same either way
+                unsigned int seen = 0;
+                for (int it = 0; it < COUNTS_BARRIER_POLLS; ++it) {
                     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(&a.ws.ctl->barArrive) : "memory");
-                } while (seen < (unsigned int)G);
+                    if (seen >= (unsigned int)G) break;
+                    if (it > 64) __nanosleep(256);
+                }
+                sTimedOut = seen < (unsigned int)G ? 1 : 0;
+#ifdef XDEV_TEST_FORCE_BARRIER_TIMEOUT
+                if (blockIdx.x & 1) sTimedOut = 1;                 // test builds: odd CTAs take the fallback although everyone arrived
+#endif
             }
             __syncthreads();
+        } else if (threadIdx.x == 0) {
+            sTimedOut = 0;
         }
+        if (G <= 1) __syncthreads();
+        const bool timedOut = sTimedOut != 0;
         for (int s = threadIdx.x; s < R; s += COUNTS_THREADS) {                 // + the block sums of the CTAs before this one
             long long pre = 0;
             constexpr int BU = 8;
-            for (int jb = 0; jb < (int)blockIdx.x; jb += BU) {
-                long long v[BU];
+            if (!timedOut) {
+                for (int jb = 0; jb < (int)blockIdx.x; jb += BU) {
+                    long long v[BU];
     #pragma unroll
-                for (int u = 0; u < BU; ++u) v[u] = jb + u < (int)blockIdx.x ? __ldcg(a.ws.blockSum + (size_t)(jb + u) * R + s) : 0;   // L2: written by other CTAs of this grid
+                    for (int u = 0; u < BU; ++u) v[u] = jb + u < (int)blockIdx.x ? __ldcg(a.ws.blockSum + (size_t)(jb + u) * R + s) : 0;   // L2: written by other CTAs of this grid
     #pragma unroll
-                for (int u = 0; u < BU; ++u) pre += v[u];
+                    for (int u = 0; u < BU; ++u) pre += v[u];
+                }
+            } else {
+                const long long* row = a.C + (size_t)s * R;
+                for (int x = 0; x < d0; ++x) { const long long v = ld_keep(row + x, keep); pre += v > 0 ? v : 0; }
             }
             for (int j = 0; j < Wc; ++j) {
                 const long long o = sofs[(size_t)s * P + j] + pre;
