@@ -301,7 +301,7 @@ typedef enum {
     NCCLX_KERNEL_COUNTS = 0, /* counts transpose + offsets scan + work list   */
     NCCLX_KERNEL_COPY = 1,   /* byte-balanced segment copy                    */
     NCCLX_KERNEL_REDUCE = 2, /* rank-order sum                                */
-    NCCLX_KERNEL_DYN = 3,    /* AllToAllvDynamic metadata kernels (prep + desc) */
+    NCCLX_KERNEL_DYN = 3,    /* AllToAllvDynamic metadata kernel (dyn_build)     */
     NCCLX_KERNEL_TOPK = 4,   /* top-k dispatch / combine kernels               */
     NCCLX_KERNEL_FUSED = 5,  /* single-launch AllToAllv (scan + work list + copy in one kernel) */
     NCCLX_KERNEL_COUNT_
