@@ -264,11 +264,12 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the per-config table (cfg1/cfg5 latency, cfg2 warm/cold)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--latency-replays", type=int, default=10000)
-    ap.add_argument("--probe", type=int, default=0, choices=list(range(0, 15)),
+    ap.add_argument("--probe", type=int, default=0, choices=list(range(0, 16)),
                     help="run ONLY BASELINE.json config N (1-5) eagerly for --steps iterations, or one of the widenings "
                          "(6 = NEXT-4 latency, 7 = NEXT-1 dynamic, 8 = NEXT-3 top-k, 9 = HBM streaming ceilings, 10 = per-SM timeline of a "
                          "config-5 copy [instrumented build], 11 = misaligned segments, 12 = NEXT-2 ReduceCopy variants + per-CTA ceiling, "
-                         "13 = top-k at PAPER.md Table 3's decode shapes, 14 = R > 256 small messages): the commands ncu captures are taken from")
+                         "13 = top-k at PAPER.md Table 3's decode shapes, 14 = R > 256 small messages, 15 = granularity of graph-replay timing): the commands "
+                         "ncu captures are taken from")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -806,6 +807,32 @@ def timeline_probe(torch, nx, peak, cfg_index=5, workload=None):
     return out
 
 
+def quantisation_extra(torch, nx, peak, reps):
+    """How fine is a graph-replay p50?  The R = 64 x 10 KB call (and a 32-element torch add) followed, inside the same graph, by a
+    spin kernel of 0 ... 8000 SM cycles (torch.cuda._sleep): on this pool the event pair around a replay moves in steps of about
+    2.05 us -- a trailing spin of 0.2 ... 1 us adds either nothing or one whole step -- so differences below one step between two
+    builds are invisible in p50 / p99 and show only in total / replays (reported beside them for configs 1 and 5)."""
+    w = A2A(W.A2AConfig("small64", 64, 5120, "bf16", 1, np.ones((64, 64), np.int64)), torch, nx, with_back=False)
+    x = torch.zeros(32, device="cuda")
+    res = {"sm_cycles_of_trailing_spin": [], "small_R64_call_p50_us": [], "tiny_kernel_p50_us": []}
+    for cyc in (0, 400, 800, 1200, 1600, 2000, 2400, 2800, 3200, 3600, 4000, 4800, 5600, 6400, 8000):
+        def enq_call():
+            w.dispatch()
+            if cyc:
+                torch.cuda._sleep(cyc)
+
+        def enq_tiny():
+            x.add_(1)
+            if cyc:
+                torch.cuda._sleep(cyc)
+        res["sm_cycles_of_trailing_spin"].append(cyc)
+        res["small_R64_call_p50_us"].append(graph_p50(torch, enq_call, reps)["p50_us"])
+        res["tiny_kernel_p50_us"].append(graph_p50(torch, enq_tiny, reps)["p50_us"])
+    v = sorted(set(round(t, 1) for t in res["small_R64_call_p50_us"]))
+    res["distinct_p50_levels_us"] = v
+    return res
+
+
 def graph_p50(torch, enqueue, reps, warm=20):
     """Capture `enqueue` once (after one eager run on a side stream), time `reps` replays with CUDA events."""
     side = torch.cuda.Stream()
@@ -887,9 +914,10 @@ def probe(args, torch, nx, peak):
                misaligned_extra(torch, nx, peak) if n == 11 else
                reducecopy_extra(torch, nx, peak) if n == 12 else
                topk_table3_extra(torch, nx, peak, args.steps) if n == 13 else
-               large_r_extra(torch, nx, peak, args.steps))
+               large_r_extra(torch, nx, peak, args.steps) if n == 14 else
+               quantisation_extra(torch, nx, peak, args.steps))
         names = {6: "next4_latency", 7: "next1_dynamic", 8: "next3_topk", 9: "hbm_ceiling", 10: "cfg5_timeline", 11: "misaligned",
-                 12: "next2_reducecopy", 13: "next3_topk_table3", 14: "large_R"}
+                 12: "next2_reducecopy", 13: "next3_topk_table3", 14: "large_R", 15: "graph_replay_timing_granularity"}
         print(json.dumps({"probe": names[n], **res}))
         nx.ncclx_finalize()
         return 0
