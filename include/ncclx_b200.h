@@ -31,7 +31,8 @@
  *   - Entry points may be called from several host threads (one internal mutex); the workspace rule above
  *     still applies to what they enqueue.
  *   - There is no CPU fallback: without a CUDA device ncclx_init fails with
- *     NCCLX_ERR_CUDA and every other call fails with NCCLX_ERR_NOT_INITIALIZED.
+ *     NCCLX_ERR_CUDA and every other call fails with NCCLX_ERR_NOT_INITIALIZED
+ *     (ncclx_alltoallv_static_dev, the one call that needs no init, fails with NCCLX_ERR_CUDA).
  */
 #ifndef NCCLX_B200_H
 #define NCCLX_B200_H
@@ -61,7 +62,8 @@ typedef enum {
     NCCLX_ERR_DTYPE = 2,           /* dtype not supported by this call                         */
     NCCLX_ERR_NOT_INITIALIZED = 3, /* ncclx_init not called, or R > max_ranks given to it      */
     NCCLX_ERR_CUDA = 4,            /* a CUDA runtime call failed (see ncclx_last_cuda_error)   */
-    NCCLX_ERR_CAPTURE = 5          /* a host-synchronous call was made while `stream` captures */
+    NCCLX_ERR_CAPTURE = 5,         /* a host-synchronous call was made while `stream` captures */
+    NCCLX_ERR_TOO_LARGE = 6        /* ncclx_alltoallv_static_dev only: R > NCCLX_STATIC_MAX_RANKS */
 } ncclx_result_t;
 
 /* ---- lifetime ------------------------------------------------------------------------- */
@@ -111,6 +113,60 @@ int ncclx_version(void);
  * and picks the tile size from the byte total; results are identical to the two-kernel path.          */
 int ncclx_alltoallv_dev(const void* const* send, const int64_t* sendcounts_dev, void* const* recv,
                         int64_t* recvcounts_dev, int R, ncclx_dtype_t dtype, ncclx_stream_t stream);
+
+/* ---- AllToAllv for callers that cannot allocate device memory -------------------------------------- *
+ *
+ * Who this is for.  Every other entry point needs ncclx_init, and ncclx_init calls cudaMalloc for the
+ * workspace.  Some callers are not in a position to do that: a plug-in running inside a host application
+ * whose memory pool already owns (nearly) all of HBM, so a late cudaMalloc fails or fragments the pool; code
+ * that runs in a phase where the surrounding framework forbids allocator calls because cudaMalloc / cudaFree
+ * synchronise the whole device and would stall other streams mid-step; or a sandboxed worker that is handed
+ * finished device buffers and is simply not allowed to create new ones.  For them this ONE call performs the
+ * complete AllToAllv of ncclx_alltoallv_dev (same semantics, same argument meaning, byte-identical results)
+ * and never calls cudaMalloc, cudaFree, cudaMallocAsync, cudaEventCreate or any allocating library routine.
+ * It does NOT need ncclx_init and does not touch the ncclx_init workspace; it may be used before, after or
+ * without it.
+ *
+ * Where its scratch memory lives.  The kernel needs a little global memory that is neither input nor output
+ * (the claim counters of its work list, the two R x R offset matrices it derives from the counts, a status
+ * word).  Here that scratch is a fixed array of NCCLX_STATIC_SCRATCH_BYTES (16 896) bytes compiled into the
+ * library's device image.  Consequences a user should know:
+ *   - every GPU on which this library's device code gets loaded carries those 16.5 KiB until the process
+ *     exits, whether or not this call is ever used;
+ *   - the size is fixed, so the call is limited to R <= NCCLX_STATIC_MAX_RANKS (32).  A larger R is refused
+ *     with NCCLX_ERR_TOO_LARGE before anything is enqueued (use ncclx_init + ncclx_alltoallv_dev there).
+ *     The payload size is NOT limited by the scratch: any byte counts the buffers can hold are fine;
+ *   - there is ONE array per GPU and every call on that GPU uses it.  Two calls that can be in flight on the
+ *     same GPU at the same time (different streams without an event between them, or two host threads each
+ *     driving its own stream) race on it and may corrupt each other's transfer.  Keep the calls of one GPU in
+ *     one stream's order.  The array keeps whatever the previous call left; the part that has to start at
+ *     zero (counters, status) is cleared on `stream` ahead of the kernel by every call.
+ *
+ * First call on a GPU.  The call works on the CUDA device that is CURRENT in the calling thread (all pointers
+ * must belong to it; up to 64 devices per process).  The first call on each device looks up the device
+ * address of the scratch array, reads the SM count and shared-memory limit, and raises the kernel's
+ * shared-memory limit; later calls on that device reuse the result.  Make that first call OUTSIDE any stream
+ * capture: if `stream` is capturing when the set-up is still to be done the call returns NCCLX_ERR_CAPTURE
+ * and enqueues nothing.
+ *
+ *   send, sendcounts_dev, recv, recvcounts_dev, dtype, stream: exactly as for ncclx_alltoallv_dev (counts are
+ *       DEVICE-resident and read when the kernel executes; recv bytes outside the packed range are not
+ *       written; a negative count moves nothing).
+ *   status_dev   optional DEVICE uint32 owned by the caller (NULL: not reported).  Bit 0 is OR-ed into it
+ *                when a negative count was seen; the library never clears it.  (ncclx_device_status does not
+ *                see this call.)
+ *   R            1 <= R <= NCCLX_STATIC_MAX_RANKS.
+ * Errors: NCCLX_ERR_ARG (null pointer, R < 1, sendcounts_dev == recvcounts_dev, device index >= 64),
+ * NCCLX_ERR_TOO_LARGE, NCCLX_ERR_DTYPE, NCCLX_ERR_CAPTURE (see above), NCCLX_ERR_CUDA (no usable sm_100
+ * device current, or the runtime refused the memset / launch).  Except for a refused kernel launch, which
+ * leaves the harmless 512-byte clear of the scratch behind, an error means nothing was enqueued.  The call
+ * only enqueues (one 512-byte memset + one kernel): it does not synchronise and is not counted by
+ * ncclx_launch_count / the profiling events. */
+#define NCCLX_STATIC_MAX_RANKS 32
+#define NCCLX_STATIC_SCRATCH_BYTES (512 + 2 * NCCLX_STATIC_MAX_RANKS * NCCLX_STATIC_MAX_RANKS * 8)
+int ncclx_alltoallv_static_dev(const void* const* send, const int64_t* sendcounts_dev, void* const* recv,
+                               int64_t* recvcounts_dev, uint32_t* status_dev, int R, ncclx_dtype_t dtype,
+                               ncclx_stream_t stream);
 
 /* ---- split-phase form and plan slots (section 6.2) ---------- *
  *

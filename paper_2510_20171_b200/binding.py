@@ -29,6 +29,8 @@ PARAM_HOST_ZERO_COPY = 8
 PARAM_REDUCECOPY_TMA = 9
 PARAM_COUNT = 10
 NUM_PLANS = 4
+STATIC_MAX_RANKS = 32            # NCCLX_STATIC_MAX_RANKS
+ERR_TOO_LARGE = 6                # NCCLX_ERR_TOO_LARGE
 
 KERNEL_COUNTS, KERNEL_COPY, KERNEL_REDUCE, KERNEL_DYN, KERNEL_TOPK, KERNEL_FUSED = 0, 1, 2, 3, 4, 5
 
@@ -42,7 +44,7 @@ SYMBOLS = [
     "ncclx_reducecopy_sum", "ncclx_moe_dispatch_topk_dev", "ncclx_moe_combine_topk_sum_dev",
     "ncclx_alltoallv_prepare_dev", "ncclx_alltoallv_execute_dev", "ncclx_stream_probe", "ncclx_stream_probe_ctas",
     "ncclx_alltoallv_dynamic_prepare_dev", "ncclx_moe_topk_prepare_dev", "ncclx_moe_dispatch_topk_execute_dev",
-    "ncclx_moe_combine_topk_sum_execute_dev", "ncclx_debug_timeline",
+    "ncclx_moe_combine_topk_sum_execute_dev", "ncclx_debug_timeline", "ncclx_alltoallv_static_dev",
 ]
 
 
@@ -73,6 +75,7 @@ def lib() -> ctypes.CDLL:
         L.ncclx_strerror.restype = ctypes.c_char_p
         L.ncclx_last_cuda_error_string.restype = ctypes.c_char_p
         L.ncclx_alltoallv_dev.argtypes = [vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, vp]
+        L.ncclx_alltoallv_static_dev.argtypes = [vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, vp]
         L.ncclx_alltoallv_prepare_dev.argtypes = [ctypes.c_int, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, vp]
         L.ncclx_alltoallv_execute_dev.argtypes = [ctypes.c_int, vp]
         L.ncclx_alltoallv_last_offsets.argtypes = [vp, vp, ctypes.c_int, vp]
@@ -160,6 +163,19 @@ def device_ptr_table(tensors: Sequence, device=None):
 def ncclx_alltoallv_dev(send_table, sendcounts_dev, recv_table, recvcounts_dev, R: int, dtype, stream=None) -> None:
     _ck(lib().ncclx_alltoallv_dev(_ptr(send_table), _ptr(sendcounts_dev), _ptr(recv_table), _ptr(recvcounts_dev),
                                   R, _dt(dtype), _stream(stream)), "ncclx_alltoallv_dev")
+
+
+def ncclx_alltoallv_static_dev(send_table, sendcounts_dev, recv_table, recvcounts_dev, R: int, dtype, stream=None,
+                               status_dev=None) -> None:
+    """AllToAllv for callers that may not allocate device memory (a plug-in inside an application whose pool owns
+    all of HBM, a phase in which the framework forbids cudaMalloc because it stalls every stream, a worker that is
+    only handed finished buffers).  Needs no ncclx_init and allocates nothing: its scratch is a fixed 16.5 KiB array
+    built into the library, hence R <= STATIC_MAX_RANKS (NcclxError code ERR_TOO_LARGE above that), one call in
+    flight per GPU at a time, and the first call on a GPU (which does the one-time set-up) made outside stream
+    capture.  Same arguments and results as ncclx_alltoallv_dev; `status_dev`: optional uint32 device tensor that
+    gets bit 0 OR-ed in when a negative count was seen."""
+    _ck(lib().ncclx_alltoallv_static_dev(_ptr(send_table), _ptr(sendcounts_dev), _ptr(recv_table), _ptr(recvcounts_dev),
+                                         _ptr(status_dev), R, _dt(dtype), _stream(stream)), "ncclx_alltoallv_static_dev")
 
 
 def ncclx_alltoallv_prepare_dev(plan: int, send_table, sendcounts_dev, recv_table, recvcounts_dev, R: int, dtype,

@@ -607,6 +607,7 @@ const char* ncclx_strerror(int code) {
     case NCCLX_ERR_NOT_INITIALIZED: return "not initialised, or R / work-list size exceeds what init was given";
     case NCCLX_ERR_CUDA: return "CUDA runtime error";
     case NCCLX_ERR_CAPTURE: return "host-synchronous call while the stream is capturing";
+    case NCCLX_ERR_TOO_LARGE: return "R exceeds NCCLX_STATIC_MAX_RANKS (32), the fixed capacity of ncclx_alltoallv_static_dev's built-in scratch";
     default: return "unknown error code";
     }
 }
@@ -1182,3 +1183,117 @@ int ncclx_debug_timeline(uint64_t* stamps_host, int max_ctas, int* fields) {
 }
 
 }  // extern "C"
+
+// ---- AllToAllv without any allocation: ncclx_alltoallv_static_dev ------------------------------------------
+//
+// For callers that must not (or cannot) call cudaMalloc -- see the header for who they are.  The single-launch
+// kernel (alltoallv_fused_kernel) is launched with its scratch pointers aimed at the file-scope device array
+// below instead of at the ncclx_init workspace.  Nothing here reads or writes the Context `g` apart from the
+// last-CUDA-error slot that the CK macro fills.
+//
+// The array is part of the library's device image: each GPU that loads the image holds these 16.5 KiB until the
+// process ends.  Layout: [0,256) WorkCtl claim counters | [256,512) fallback status word | soff R*R i64 | roff R*R i64.
+// IMPORTANT for anyone editing this: in HOST code the identifier `ncclx_static_scratch` is only a handle for the
+// runtime, not an address a kernel can use.  The device address is fetched once per device with
+// cudaGetSymbolAddress (staticSetup) and only that pointer is handed to the kernel.
+static_assert(sizeof(xdev::WorkCtl) <= 256, "control block must fit its 256-byte slot");
+static_assert(NCCLX_STATIC_MAX_RANKS <= xdev::FUSED_MAX_R, "the static entry point rides on the single-launch kernel");
+static __device__ __align__(256) unsigned char ncclx_static_scratch[NCCLX_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+constexpr size_t kStaticClearBytes = 512;          // counters + status: what has to be zero when the kernel starts
+
+struct StaticDev {
+    bool ready = false;
+    unsigned char* scratch = nullptr;              // DEVICE address of ncclx_static_scratch on this device
+    int smCount = 0;
+    int smemOptin = 0;
+    int smemDynamicMax = 0;                        // what the kernel was opted in to
+};
+StaticDev gStatic[kStaticMaxDevices];
+std::mutex gStaticMu;
+
+// Once per device, with that device current.  Not done under stream capture (symbol look-up may load the module).
+int staticSetup(int dev, StaticDev& sd, cudaStream_t s) {
+    if (isCapturing(s)) return NCCLX_ERR_CAPTURE;
+    int major = 0;
+    CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major < 10) { g.lastCuda = (int)cudaErrorNoKernelImageForDevice; return NCCLX_ERR_CUDA; }
+    CK(cudaDeviceGetAttribute(&sd.smCount, cudaDevAttrMultiProcessorCount, dev));
+    CK(cudaDeviceGetAttribute(&sd.smemOptin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    void* p = nullptr;
+    CK(cudaGetSymbolAddress(&p, ncclx_static_scratch));
+    if (!p) { g.lastCuda = (int)cudaErrorInvalidSymbol; return NCCLX_ERR_CUDA; }
+    cudaFuncAttributes fa{};
+    CK(cudaFuncGetAttributes(&fa, alltoallv_fused_kernel));
+    sd.smemDynamicMax = sd.smemOptin - (int)fa.sharedSizeBytes;
+    CK(cudaFuncSetAttribute(alltoallv_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sd.smemDynamicMax));
+    sd.scratch = static_cast<unsigned char*>(p);
+    sd.ready = true;
+    return NCCLX_OK;
+}
+
+}  // namespace
+
+extern "C" int ncclx_alltoallv_static_dev(const void* const* send, const int64_t* sendcounts_dev, void* const* recv,
+                                          int64_t* recvcounts_dev, uint32_t* status_dev, int R, ncclx_dtype_t dtype,
+                                          ncclx_stream_t stream) {
+    // size and argument checks first: they need no device
+    if (R < 1) return NCCLX_ERR_ARG;
+    if (R > NCCLX_STATIC_MAX_RANKS) return NCCLX_ERR_TOO_LARGE;
+    if (!send || !sendcounts_dev || !recv || !recvcounts_dev) return NCCLX_ERR_ARG;
+    if (sendcounts_dev == recvcounts_dev) return NCCLX_ERR_ARG;
+    const int es = elemSizeOf((int)dtype);
+    if (!es) return NCCLX_ERR_DTYPE;
+
+    std::lock_guard<std::mutex> lk(gStaticMu);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return NCCLX_ERR_ARG;
+    StaticDev& sd = gStatic[dev];
+    if (!sd.ready) {
+        const int rc = staticSetup(dev, sd, s);
+        if (rc) return rc;
+    }
+
+    // launch geometry with the library's default tunables (the result does not depend on them)
+    FusedArgs fa{};
+    fa.cls.bulkMinBytes = 1024;
+    fa.cls.tileShift[LIST_BULK] = 15;
+    fa.cls.tileShift[LIST_VEC] = kVecTileShift;
+    fa.bulkEngines = 0;
+    fa.kmax = 6;
+    const int room = sd.smemOptin - 1024 < sd.smemDynamicMax ? sd.smemOptin - 1024 : sd.smemDynamicMax;   // as planFused: 1 KB kept for static shared memory
+    const size_t budget = room > 0 ? (size_t)room : 0;
+    const size_t aux = fused_aux_bytes(R);
+    if (budget < aux + 64 * 1024) { g.lastCuda = (int)cudaErrorInvalidConfiguration; return NCCLX_ERR_CUDA; }
+    fa.ringBytes = (unsigned int)((budget - aux) & ~(size_t)127);
+    if ((size_t)VEC_SUB_BYTES + 256 > ((fa.ringBytes / COPY_WARPS) & ~127u)) { g.lastCuda = (int)cudaErrorInvalidConfiguration; return NCCLX_ERR_CUDA; }
+    while (fa.cls.tileShift[LIST_BULK] > 10 && !bulkTileFits(fa.cls.tileShift[LIST_BULK], fa.ringBytes, fa.bulkEngines)) --fa.cls.tileShift[LIST_BULK];
+    fa.minTileShift[LIST_BULK] = kFusedMinTileShift < fa.cls.tileShift[LIST_BULK] ? kFusedMinTileShift : fa.cls.tileShift[LIST_BULK];
+    fa.minTileShift[LIST_VEC] = 10 < fa.cls.tileShift[LIST_VEC] ? 10 : fa.cls.tileShift[LIST_VEC];
+
+    fa.send = send; fa.recv = recv;
+    fa.C = reinterpret_cast<const long long*>(sendcounts_dev);
+    fa.RC = reinterpret_cast<long long*>(recvcounts_dev);
+    fa.ctl = reinterpret_cast<WorkCtl*>(sd.scratch);
+    fa.status = status_dev ? status_dev : reinterpret_cast<unsigned int*>(sd.scratch + 256);
+    fa.soff = reinterpret_cast<long long*>(sd.scratch + kStaticClearBytes);
+    fa.roff = fa.soff + (size_t)NCCLX_STATIC_MAX_RANKS * NCCLX_STATIC_MAX_RANKS;
+    fa.R = R; fa.elemSize = es;
+
+    // The array still holds the previous call's state.  The counters normally return to zero by themselves, but a
+    // kernel that was aborted half-way would leave them dirty, so they are cleared in stream order every time.
+    CK(cudaMemsetAsync(sd.scratch, 0, kStaticClearBytes, s));
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)sd.smCount);
+    cfg.blockDim = dim3(COPY_THREADS);
+    cfg.dynamicSmemBytes = (size_t)fa.ringBytes + aux;
+    cfg.stream = s;
+    cfg.attrs = nullptr; cfg.numAttrs = 0;          // plain stream order: the memset above has to be complete first
+    CK(cudaLaunchKernelEx(&cfg, alltoallv_fused_kernel, fa));
+    return NCCLX_OK;
+}

@@ -88,3 +88,20 @@ def test_missing_library_raises(tmp_path, monkeypatch):
     monkeypatch.setattr(binding, "LIB_PATH", str(tmp_path / "nope.so"))
     with pytest.raises(ImportError):
         binding.lib()
+
+
+def test_static_entry_point_checks_sizes_before_touching_cuda(L):
+    """ncclx_alltoallv_static_dev (the call for users who may not allocate) validates on the host first: its fixed
+    built-in scratch stops at R = 32, and the refusal names that limit."""
+    from paper_2510_20171_b200 import binding as b
+    assert b.STATIC_MAX_RANKS == 32 and b.ERR_TOO_LARGE == 6
+    assert L.ncclx_alltoallv_static_dev(1, 1, 1, 2, None, 33, 0, None) == 6
+    assert L.ncclx_alltoallv_static_dev(1, 1, 1, 2, None, 1024, 0, None) == 6
+    assert b"32" in L.ncclx_strerror(6)
+    assert L.ncclx_alltoallv_static_dev(1, 1, 1, 2, None, 0, 0, None) == 1
+    assert L.ncclx_alltoallv_static_dev(1, 1, 1, 1, None, 4, 0, None) == 1     # counts in == counts out
+    assert L.ncclx_alltoallv_static_dev(None, 1, 1, 2, None, 4, 0, None) == 1
+    assert L.ncclx_alltoallv_static_dev(1, 1, 1, 2, None, 4, 9, None) == 2
+    import torch
+    if not torch.cuda.is_available():
+        assert L.ncclx_alltoallv_static_dev(1, 1, 1, 2, None, 4, 0, None) == 4   # no device: loud, no CPU path
