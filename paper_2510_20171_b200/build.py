@@ -29,9 +29,6 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in DEPS)
 
 
-LIB_TIMELINE = os.path.join(HERE, "libncclx_b200_timeline.so")
-
-
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         tmp = LIB + f".tmp{os.getpid()}"
@@ -41,18 +38,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-def build_timeline() -> str:
-    """Instrumented build (-DXDEV_TIMELINE): segment_copy_kernel stamps %globaltimer per CTA.  A measurement aid kept out of
-    the default library; select it with NCCLX_B200_LIB=<path> (bench.py --probe 10 reads the stamps)."""
-    tmp = LIB_TIMELINE + f".tmp{os.getpid()}"
-    subprocess.check_call([nvcc(), *NVCC_FLAGS, "-DXDEV_TIMELINE", "-o", tmp, *SOURCES])
-    os.replace(tmp, LIB_TIMELINE)
-    return LIB_TIMELINE
+def build_variant(defines, out_path: str) -> str:
+    """The same sources compiled with extra -D flags into `out_path` (never the default library).  Used by
+    tests/test_gpu_barrier_fallback.py for the -DXDEV_TEST_FORCE_BARRIER_TIMEOUT build; select the result with
+    NCCLX_B200_LIB=<path>."""
+    assert os.path.abspath(out_path) != LIB
+    tmp = out_path + f".tmp{os.getpid()}"
+    subprocess.check_call([nvcc(), *NVCC_FLAGS, *defines, "-o", tmp, *SOURCES])
+    os.replace(tmp, out_path)
+    return out_path
 
 
 if __name__ == "__main__":
     import sys
-    if "--timeline" in sys.argv:
-        print(build_timeline())
-    else:
-        print(build(force=True, verbose="-v" in sys.argv))
+    print(build(force=True, verbose="-v" in sys.argv))

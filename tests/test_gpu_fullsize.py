@@ -85,6 +85,100 @@ def test_cfg3_full_size_dispatch_and_combine():
         assert bool((back[s][send_n[s]:].view(torch.int16) == -23131).all())
     assert sum(recv_n) == sum(send_n) == 64 * 16384 * width
 
+    # ---- the same dispatch + combine REPLAYED FROM ONE CUDA GRAPH (BASELINE.json configs[2]: "counts device-resident,
+    # call captured in a CUDA graph").  recv was compared with the oracle over 100 % above, so a
+    # device-side equality against a copy of it is an oracle comparison of the replay, byte for byte incl. the tails.
+    recv_ref = [r.clone() for r in recv]
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        nx.ncclx_alltoallv_dev(st, Cd, rt, RCd, R, "bf16")
+        nx.ncclx_alltoallv_dev(rt, RCd, bt, C2d, R, "bf16")
+
+    def refill():
+        for t in recv + back:
+            t.view(torch.int16).fill_(-23131)
+        RCd.fill_(-1); C2d.fill_(-1)
+
+    # replay 1 with the counts rewritten to zero ON THE DEVICE: the kernels read them at replay time, nothing moves
+    refill()
+    Cd.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert int(RCd.abs().sum()) == 0 and int(C2d.abs().sum()) == 0
+    assert all(bool((t.view(torch.int16) == -23131).all()) for t in recv + back), "a replay with zero counts moved bytes"
+    # replay 2 with the real counts restored: everything as verified above
+    Cd.copy_(torch.from_numpy(C))
+    g.replay()
+    torch.cuda.synchronize()
+    assert nx.ncclx_device_status() == 0
+    assert (RCd.cpu().numpy() == eRC).all() and (C2d.cpu().numpy() == C).all()
+    for d in range(R):
+        assert torch.equal(recv[d].view(torch.int16), recv_ref[d].view(torch.int16)), f"graph replay: recv[{d}]"
+    for s in range(R):
+        assert torch.equal(back[s][:send_n[s]].view(torch.int16), send[s].view(torch.int16)), f"graph replay: round trip rank {s}"
+        assert bool((back[s][send_n[s]:].view(torch.int16) == -23131).all())
+    del recv_ref, g
+
+
+def test_topk_bench_shape_sampled_against_the_oracle():
+    """The top-k shape bench.py times (R = 64, T = 4096 tokens per rank, k = 4, hidden 5120 bf16: 262 144 tokens = 27.7
+    trips of the kernels' grid-stride loops, 10 GiB dispatched).  Sampled outputs computed by the oracle one by one:
+    for sampled copies (s, t, j) the oracle's offset matrices place the row (linear walk over destinations, as in
+    alltoallv_source_of) and the dispatched row must equal token t; for sampled tokens the combine's output must equal
+    the oracle's fixed-order sum of the k rows.  Plus the properties that hold at any size: receive counts are the
+    transpose, every packed row is written, every sentinel tail is intact."""
+    R, T, k, width = 64, 4096, 4, 5120
+    pos, C = W.topk_routing(R, T, k, 128, 5)
+    slack = 8
+    X = [W.torch_values(T * width, "bf16", 3000 + s) for s in range(R)]
+    recv_rows = [int(C[:, d].sum()) for d in range(R)]
+    recv = [torch.full(((n + slack) * width,), -23131, dtype=torch.int16, device="cuda") for n in recv_rows]
+    out = [torch.full((T * width + slack,), -23131, dtype=torch.int16, device="cuda") for _ in range(R)]
+    dpos, dC = torch.from_numpy(pos).cuda(), torch.from_numpy(C).cuda()
+    dRC = torch.zeros_like(dC)
+    nx.ncclx_moe_dispatch_topk_dev(nx.device_ptr_table(X), dpos, dC, nx.device_ptr_table(recv), dRC, R, T, k, width, "bf16")
+    torch.cuda.synchronize()
+    assert nx.ncclx_device_status() == 0
+    eRC, esoff, eroff, _ = oracle.alltoallv_offsets(C)
+    assert (dRC.cpu().numpy() == eRC).all()
+
+    def place(s, p):                                            # definition, one by one: which rank's window holds row p
+        for d in range(R):
+            lo = int(esoff[s, d])
+            if lo <= p < lo + int(C[s, d]):
+                return d, int(eroff[d, s]) + (p - lo)
+        raise AssertionError("position outside the send buffer")
+
+    rng = np.random.default_rng(1)
+    for s in range(R):
+        for t, j in zip(rng.integers(0, T, 24), rng.integers(0, k, 24)):
+            d, row = place(s, int(pos[s, t, j]))
+            a = recv[d][row * width:(row + 1) * width]
+            b = X[s].view(torch.int16)[int(t) * width:(int(t) + 1) * width]
+            assert torch.equal(a, b), (s, int(t), int(j), d, row)
+    for d in range(R):
+        body = recv[d][: recv_rows[d] * width].view(recv_rows[d], width)
+        assert int((body == -23131).all(dim=1).sum()) == 0, f"recv[{d}] has unwritten rows"
+        assert bool((recv[d][recv_rows[d] * width:] == -23131).all())
+
+    # combine on scrambled expert outputs (rows rolled by a per-rank amount, so the k copies of a token differ)
+    Y = [torch.roll(recv[d][: recv_rows[d] * width], 3 * d + 1) for d in range(R)]
+    nx.ncclx_moe_combine_topk_sum_dev(nx.device_ptr_table(Y), dpos, dC, nx.device_ptr_table(out), R, T, k, width, "bf16")
+    torch.cuda.synchronize()
+    assert nx.ncclx_device_status() == 0
+    for s in range(R):
+        for t in rng.integers(0, T, 6):
+            rows = []
+            for j in range(k):
+                d, row = place(s, int(pos[s, t, j]))
+                rows.append(Y[d][row * width:(row + 1) * width].cpu().numpy().view(np.uint16))
+            exp = oracle.reduce_samples(np.stack(rows), "bf16")            # (k, width): fp32 sum in router order j, one rounding
+            got = out[s][int(t) * width:(int(t) + 1) * width].cpu().numpy().view(np.uint16)
+            assert got.tobytes() == exp.tobytes(), (s, int(t))
+        assert bool((out[s][T * width:] == -23131).all())
+    del X, recv, out, Y
+    torch.cuda.empty_cache()
+
 
 def test_cfg4_full_size_reducescatter():
     cfg = W.reduce_config(4)

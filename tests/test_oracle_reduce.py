@@ -110,6 +110,25 @@ def test_R2_and_fp32_reduce_to_numpy_float32_adds():
     assert oracle.allreduce_sum([xa, xb], "bf16")[0].tobytes() == bf16_bits(fa + fb).tobytes()
 
 
+def test_R2_f16_reduces_to_numpy_half_widen_add_narrow():
+    """Direct pin of the oracle's f16 -> f32 widening (until now reached only through the 65 536-pattern round trip):
+    numpy's float16 -> float32 cast is exact, float32 add is one IEEE add, float32 -> float16 rounds to nearest even.
+    Includes subnormal halves, both zeros and +-65504; the sum of two finite halves never overflows binary32, and
+    NaN/Inf inputs are excluded because the oracle canonicalises NaN while numpy keeps payloads."""
+    rng = np.random.default_rng(12)
+    xa = rng.integers(0, 1 << 16, 200_000).astype(np.uint16)
+    xb = rng.integers(0, 1 << 16, 200_000).astype(np.uint16)
+    edge = np.array([0x0000, 0x8000, 0x0001, 0x8001, 0x03FF, 0x0400, 0x7BFF, 0xFBFF, 0x3C00, 0xBC00], np.uint16)
+    xa = np.concatenate([xa, np.repeat(edge, edge.size)])
+    xb = np.concatenate([xb, np.tile(edge, edge.size)])
+    finite = ((xa & 0x7C00) != 0x7C00) & ((xb & 0x7C00) != 0x7C00)
+    xa, xb = np.ascontiguousarray(xa[finite]), np.ascontiguousarray(xb[finite])
+    with np.errstate(over="ignore"):
+        want = (xa.view(np.float16).astype(np.float32) + xb.view(np.float16).astype(np.float32)).astype(np.float16)
+    got = oracle.allreduce_sum([xa, xb], "f16")[0]
+    assert got.tobytes() == want.view(np.uint16).tobytes()
+
+
 @pytest.mark.parametrize("R,std", [(8, 1.0), (16, 1e-3)])
 def test_error_bound_against_fp64(R, std):
     n = 50_000
