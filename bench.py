@@ -264,11 +264,11 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the per-config table (cfg1/cfg5 latency, cfg2 warm/cold)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--latency-replays", type=int, default=10000)
-    ap.add_argument("--probe", type=int, default=0, choices=list(range(0, 16)),
+    ap.add_argument("--probe", type=int, default=0, choices=[0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 11, 12, 13, 14],
                     help="run ONLY BASELINE.json config N (1-5) eagerly for --steps iterations, or one of the widenings "
-                         "(6 = NEXT-4 latency, 7 = NEXT-1 dynamic, 8 = NEXT-3 top-k, 9 = HBM streaming ceilings, 10 = per-SM timeline of a "
-                         "config-5 copy [instrumented build], 11 = misaligned segments, 12 = NEXT-2 ReduceCopy variants + per-CTA ceiling, "
-                         "13 = top-k at PAPER.md Table 3's decode shapes, 14 = R > 256 small messages, 15 = granularity of graph-replay timing): the commands "
+                         "(6 = NEXT-4 latency, 7 = NEXT-1 dynamic, 8 = NEXT-3 top-k, 9 = HBM streaming ceilings, "
+                         "11 = misaligned segments, 12 = NEXT-2 ReduceCopy variants + per-CTA ceiling, "
+                         "13 = top-k at PAPER.md Table 3's decode shapes, 14 = R > 256 small messages): the commands "
                          "ncu captures are taken from")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -279,6 +279,7 @@ def main():
     config = {"workload": "cfg3 MoE dispatch+combine AllToAllv (R=64, 16384 tok x 5120 bf16, Zipf 1.1) + cfg2 AllReduce "
                           "(R=8, 4Mi bf16) + cfg4 ReduceScatter (R=16, 256Mi bf16/rank); BASELINE.json configs[2],[1],[3]",
               "bytes_per_step_GiB": 48.625, "l2": "inputs larger than L2 (48.6 GiB touched per step vs 126 MB)",
+              "launch": "one CUDA-graph replay per step (the four calls captured once; counts re-read on the device at every replay)",
               "parallelism": f"replicas x{world} (path does not shard across GPUs)"}
 
     if args.impl == "reference":
@@ -287,7 +288,8 @@ def main():
         cb, dt = run_oracle_leg(args.steps, args.warmup)
         line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": "GB/s", "n_gpus": args.gpus,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(dt * 1e3, 2), "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic", "config": config,
+                "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                "config": dict(config, launch="CPU oracle, no GPU", sample_run_per_step=cb["sample"]),
                 "cpu_baseline": cb,
                 "e2e": {"value": cb["value"], "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
                 "gpu_launches": 0}
@@ -329,21 +331,46 @@ def main():
     assert all(torch.equal(b[:n], s[:n]) for b, s, n in zip(a3.back, a3.send, a3.send_elems)), "round trip broken"
     assert torch.equal(a3.C2, a3.C) and torch.equal(a3.RC, a3.C.t().contiguous())
 
-    nx.ncclx_profile_reset()
-    nx.ncclx_set_param(nx.PARAM_PROFILE, 1)
+    # The whole step is captured ONCE into a CUDA graph and every timed step is one replay (BASELINE.json configs[2]:
+    # "counts device-resident, call captured in a CUDA graph"): the kernels re-read the device-resident
+    # counts at every replay.  Profiling is off here: nothing but the graph launches sits in the timed region.
+    nx.ncclx_set_param(nx.PARAM_PROFILE, 0)
+    l0 = nx.ncclx_launch_count()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        step()
+    launches_per_step = nx.ncclx_launch_count() - l0          # captured launches are counted once, at capture
+    for b in a3.back:                                          # the replay itself has to restore these
+        b.zero_()
+    graph.replay()
+    barrier()
+    assert all(torch.equal(b[:n], s[:n]) for b, s, n in zip(a3.back, a3.send, a3.send_elems)), "round trip broken (graph replay)"
     sampler = ClockSampler(local_rank)
     sampler.start()
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    l0 = nx.ncclx_launch_count()
     e0.record()
     for _ in range(args.steps):
-        step()
+        graph.replay()
     e1.record()
     barrier()
-    launches = nx.ncclx_launch_count() - l0
+    launches = launches_per_step * args.steps
     clocks = sampler.stop()
     ms_total = e0.elapsed_time(e1)
+
+    # Second pass, reported separately: the same K steps launched eagerly with the library's per-launch CUDA events on
+    # (the events cannot sit inside a captured graph), for the per-kernel split and the dominant kernel's average
+    # launch duration.
+    nx.ncclx_profile_reset()
+    nx.ncclx_set_param(nx.PARAM_PROFILE, 1)
+    barrier()
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record()
+    for _ in range(args.steps):
+        step()
+    p1.record()
+    barrier()
+    ms_profiled_total = p0.elapsed_time(p1)
     nx.ncclx_set_param(nx.PARAM_PROFILE, 0)
     copy_ms, copy_n = nx.ncclx_profile_read(nx.KERNEL_COPY)
     red_ms, red_n = nx.ncclx_profile_read(nx.KERNEL_REDUCE)
@@ -360,14 +387,16 @@ def main():
                 "unit": "GB/s", "frac": round(copy_gbs / peak, 4), "peak_source": peak_src,
                 "frac_of_nominal_8TBps": round(copy_gbs / NOMINAL_HBM_GBS, 4),
                 "algorithmic_bytes_per_launch": 2 * a3.bytes_one_way, "avg_launch_ms": round(copy_avg_ms, 4),
-                "launches_timed": copy_n, "share_of_step": round(copy_ms / ms_total, 4),
+                "launches_timed": copy_n, "share_of_step": round(copy_ms / ms_profiled_total, 4),
+                "timed_in": "second pass: the same steps launched eagerly with per-launch CUDA events (headline pass = graph replays, no events)",
+                "per_kernel_pass_ms_per_step": round(ms_profiled_total / args.steps, 4),
                 "traffic": None,
                 "other_kernels": {"reduce_kernel": {"avg_ms": round(red_ms / max(red_n, 1), 4), "launches": red_n,
-                                                    "share_of_step": round(red_ms / ms_total, 4)},
+                                                    "share_of_step": round(red_ms / ms_profiled_total, 4)},
                                   "counts_kernel": {"avg_ms": round(cnt_ms / max(cnt_n, 1), 5), "launches": cnt_n,
-                                                    "share_of_step": round(cnt_ms / ms_total, 5)}}}
-    # dram bytes per launch from the committed ncu capture: profiles/traffic.csv is (re)written from the capture's raw
-    # page by `python -m paper_2510_20171_b200.ncu_traffic` (ncu cannot run inside this timed process)
+                                                    "share_of_step": round(cnt_ms / ms_profiled_total, 5)}}}
+    # dram bytes per launch from the committed ncu capture: profiles/traffic.csv was written from the capture's raw
+    # page with the command in profiles/r2_summary.md section 2 (ncu cannot run inside this timed process)
     tr = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tr):
         try:
@@ -703,136 +732,6 @@ def large_r_extra(torch, nx, peak, reps):
     return res
 
 
-def timeline_probe(torch, nx, peak, cfg_index=5, workload=None):
-    """Instrumented build only (python -m paper_2510_20171_b200.build --timeline; NCCLX_B200_LIB=<that .so>): per-CTA
-    %globaltimer stamps of ONE copy kernel and the metadata kernel before it -> where the time beyond bytes / bandwidth
-    goes (start-up, ramp, tail).  workload: cfg5 (default), dynamic (NEXT-1's inference shape) or small64 (one 10 KB row per pair)."""
-    workload = workload or os.environ.get("NCCLX_TIMELINE_WORKLOAD", "cfg5")
-    if workload == "dynamic":
-        Ls, idx, bl, J = W.dynamic_moe_metadata()
-        R, n = Ls.shape
-        nx.ncclx_init_dynamic(n, R * R * J)
-        tot = Ls.sum(axis=1)
-        send = [W.torch_values(int(t), "bf16", 5000 + s) for s, t in enumerate(tot)]
-        recv = [torch.empty(int(tot[s]), dtype=torch.bfloat16, device="cuda") for d in range(R) for s in range(R)]
-        st, rt = nx.device_ptr_table(send), nx.device_ptr_table(recv)
-        allL = torch.empty((R, R, n), dtype=torch.int64, device="cuda")
-        Ld, Id, Bd = (torch.from_numpy(np.ascontiguousarray(x)).cuda() for x in (Ls, idx, bl))
-        moved = 0
-        for s_ in range(R):
-            pos = 0
-            for d in range(R):
-                moved += int(Ls[s_, idx[s_, pos:pos + bl[s_, d]]].sum()) * 2
-                pos += int(bl[s_, d])
-
-        class _Dyn:
-            bytes_one_way = moved
-
-            @staticmethod
-            def dispatch():
-                nx.ncclx_alltoallv_dynamic_dev(st, Ld, n, Id, idx.shape[1], Bd, J, rt, allL, R, "bf16")
-        a = _Dyn
-    elif workload == "cfg1_two_kernels":
-        nx.ncclx_set_param(nx.PARAM_FUSED_MAX_RANKS, 0)
-        a = A2A(W.a2a_config(1), torch, nx, with_back=False)
-    elif workload == "small64":
-        a = A2A(W.A2AConfig("small64", 64, 5120, "bf16", 1, np.ones((64, 64), np.int64)), torch, nx, with_back=False)
-    else:
-        a = A2A(W.a2a_config(cfg_index), torch, nx, with_back=False)
-    graph_mode = None
-    if os.environ.get("NCCLX_TIMELINE_MODE", "eager") == "graph":
-        # the configuration the latency numbers are quoted in: ONE call per CUDA-graph replay, replays separated by a
-        # synchronise (so every replay starts cold and alone); stamps of 300 replays, percentiles over the replays
-        side = torch.cuda.Stream()
-        side.wait_stream(torch.cuda.current_stream())
-        with torch.cuda.stream(side):
-            a.dispatch()
-        torch.cuda.current_stream().wait_stream(side)
-        torch.cuda.synchronize()
-        g = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(g):
-            a.dispatch()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        rows = []
-        for i in range(320):
-            e0.record(); g.replay(); e1.record()
-            torch.cuda.synchronize()
-            tl_, ct_ = nx.ncclx_debug_timeline()
-            tl_, ct_ = tl_.astype(np.int64), ct_.astype(np.int64)
-            ct_ = ct_[ct_[:, 0] > 0]
-            z = int(ct_[:, 0].min())
-            last = ct_.shape[1] - 1 if workload == "dynamic" else 5
-            rows.append([e0.elapsed_time(e1) * 1e3, (tl_[:, 0].min() - z) / 1e3, (ct_[:, 1].max() - z) / 1e3, (ct_[:, last].max() - z) / 1e3,
-                         (np.median(tl_[:, 1]) - z) / 1e3, (np.median(tl_[:, 2]) - z) / 1e3, (np.median(tl_[:, 3]) - z) / 1e3,
-                         (tl_[:, 4].max() - z) / 1e3, (tl_[:, 6].max() - z) / 1e3])
-        r = np.array(rows[20:])
-        gn = ["event_pair_around_the_replay", "copy_kernel_first_cta_enters", "metadata_dependency_wait_over", "metadata_last_cta_exits",
-              "copy_metadata_ready_median", "copy_first_load_median", "copy_first_store_median", "copy_last_store_of_last_cta", "copy_last_cta_exits"]
-        graph_mode = {n: {"p10": round(float(np.percentile(r[:, i], 10)), 2), "p50": round(float(np.percentile(r[:, i], 50)), 2),
-                          "p90": round(float(np.percentile(r[:, i], 90)), 2)} for i, n in enumerate(gn)}
-        d_ = r[:, 0] - r[:, 8]
-        graph_mode["event_pair_minus_gpu_side_span"] = {"p10": round(float(np.percentile(d_, 10)), 2), "p50": round(float(np.percentile(d_, 50)), 2),
-                                                        "p90": round(float(np.percentile(d_, 90)), 2)}
-    else:
-        for _ in range(5):
-            a.dispatch()
-        torch.cuda.synchronize()
-    tl, ct = nx.ncclx_debug_timeline()
-    tl, ct = tl.astype(np.int64), ct.astype(np.int64)
-    ct = ct[ct[:, 0] > 0]                                              # CTAs of the counts kernel that ran
-    names = ["enter", "metadata_ready", "first_load", "first_store", "last_store", "drained", "exit"]
-    t0 = int(min(tl[:, 0].min(), ct[:, 0].min() if len(ct) else tl[:, 0].min()))
-    cols = {nm: (tl[:, i] - t0) / 1e3 for i, nm in enumerate(names)}           # us since the first CTA of either kernel entered
-    out = {"ctas": int(tl.shape[0]), "bulk_tiles": int(tl[0, 7]), "bytes_moved": 2 * a.bytes_one_way, "us": {}}
-    if tl.shape[1] > 10:                                                  # finer start-up stamps of CTA thread 0 (bulk engine 0)
-        for i, nm in ((8, "env_ready"), (9, "cursor_init_done"), (10, "first_ensure_done")):
-            cols[nm] = (tl[:, i] - t0) / 1e3
-    for nm, v in cols.items():
-        out["us"][nm] = {"min": round(float(v.min()), 2), "median": round(float(np.median(v)), 2), "max": round(float(v.max()), 2)}
-    cnames = (["enter", "dependency_wait_over", "list_offsets_known", "split_indices_known", "phaseA_done", "barrier_passed",
-               "phaseB_done", "exit"] if workload == "dynamic" else
-              ["enter", "dependency_wait_over", "phase1_done", "barrier_passed", "tile_totals_known", "exit"])
-    out["counts_kernel_ctas"] = int(len(ct))
-    out["counts_kernel_us"] = {nm: {"min": round(float(((ct[:, i] - t0) / 1e3).min()), 2), "median": round(float(np.median((ct[:, i] - t0) / 1e3)), 2),
-                                     "max": round(float(((ct[:, i] - t0) / 1e3).max()), 2)} for i, nm in enumerate(cnames)} if len(ct) else {}
-    span = float(cols["exit"].max())
-    busy = float(np.median(cols["last_store"] - cols["first_load"]))
-    out["kernel_span_us"] = round(span, 2)
-    out["median_cta_streaming_window_us"] = round(busy, 2)
-    out["at_6.9TBps_us"] = round(2 * a.bytes_one_way / 6.9e12 * 1e6, 2)
-    if graph_mode:
-        out["graph_replay_mode_us_since_first_metadata_cta"] = graph_mode
-    out["per_cta"] = [[round(float(cols[nm][i]), 2) for nm in names] for i in range(tl.shape[0])]
-    out["metadata_kernel_per_cta"] = [[round(float((ct[c, i] - t0) / 1e3), 2) for i in range(len(cnames))] for c in range(len(ct))]
-    return out
-
-
-def quantisation_extra(torch, nx, peak, reps):
-    """How fine is a graph-replay p50?  The R = 64 x 10 KB call (and a 32-element torch add) followed, inside the same graph, by a
-    spin kernel of 0 ... 8000 SM cycles (torch.cuda._sleep): on this pool the event pair around a replay moves in steps of about
-    2.05 us -- a trailing spin of 0.2 ... 1 us adds either nothing or one whole step -- so differences below one step between two
-    builds are invisible in p50 / p99 and show only in total / replays (reported beside them for configs 1 and 5)."""
-    w = A2A(W.A2AConfig("small64", 64, 5120, "bf16", 1, np.ones((64, 64), np.int64)), torch, nx, with_back=False)
-    x = torch.zeros(32, device="cuda")
-    res = {"sm_cycles_of_trailing_spin": [], "small_R64_call_p50_us": [], "tiny_kernel_p50_us": []}
-    for cyc in (0, 400, 800, 1200, 1600, 2000, 2400, 2800, 3200, 3600, 4000, 4800, 5600, 6400, 8000):
-        def enq_call():
-            w.dispatch()
-            if cyc:
-                torch.cuda._sleep(cyc)
-
-        def enq_tiny():
-            x.add_(1)
-            if cyc:
-                torch.cuda._sleep(cyc)
-        res["sm_cycles_of_trailing_spin"].append(cyc)
-        res["small_R64_call_p50_us"].append(graph_p50(torch, enq_call, reps)["p50_us"])
-        res["tiny_kernel_p50_us"].append(graph_p50(torch, enq_tiny, reps)["p50_us"])
-    v = sorted(set(round(t, 1) for t in res["small_R64_call_p50_us"]))
-    res["distinct_p50_levels_us"] = v
-    return res
-
-
 def graph_p50(torch, enqueue, reps, warm=20):
     """Capture `enqueue` once (after one eager run on a side stream), time `reps` replays with CUDA events."""
     side = torch.cuda.Stream()
@@ -910,14 +809,12 @@ def probe(args, torch, nx, peak):
                dynamic_extra(torch, nx, peak, args.steps) if n == 7 else
                topk_extra(torch, nx, peak) if n == 8 else
                ceiling_extra(torch, nx, peak) if n == 9 else
-               timeline_probe(torch, nx, peak) if n == 10 else
                misaligned_extra(torch, nx, peak) if n == 11 else
                reducecopy_extra(torch, nx, peak) if n == 12 else
                topk_table3_extra(torch, nx, peak, args.steps) if n == 13 else
-               large_r_extra(torch, nx, peak, args.steps) if n == 14 else
-               quantisation_extra(torch, nx, peak, args.steps))
-        names = {6: "next4_latency", 7: "next1_dynamic", 8: "next3_topk", 9: "hbm_ceiling", 10: "cfg5_timeline", 11: "misaligned",
-                 12: "next2_reducecopy", 13: "next3_topk_table3", 14: "large_R", 15: "graph_replay_timing_granularity"}
+               large_r_extra(torch, nx, peak, args.steps))
+        names = {6: "next4_latency", 7: "next1_dynamic", 8: "next3_topk", 9: "hbm_ceiling", 11: "misaligned",
+                 12: "next2_reducecopy", 13: "next3_topk_table3", 14: "large_R"}
         print(json.dumps({"probe": names[n], **res}))
         nx.ncclx_finalize()
         return 0

@@ -184,7 +184,7 @@ int ncclx_alltoallv_static_dev(const void* const* send, const int64_t* sendcount
  * or events; different slots are independent, so the combine's prepare (whose counts are the dispatch's
  * recvcounts, complete as soon as the dispatch's prepare is) can run on a second stream WHILE the dispatch's
  * payload moves.  ncclx_alltoallv_dev == prepare(0) + execute(0) for R > 32, one fused kernel otherwise (slot 0
- * is then left as it was).  The one-call dynamic and top-k entry points also (re)build slot 0: after them slot 0
+ * is then left exactly as it was: the fused kernel keeps its offsets in a workspace of its own).  The one-call dynamic and top-k entry points also (re)build slot 0: after them slot 0
  * holds THEIR plan (a dynamic plan can be executed again with ncclx_alltoallv_execute_dev(0); a top-k plan makes
  * it return NCCLX_ERR_ARG).  Tunables (ncclx_set_param) are snapshotted into the slot by prepare: execute uses
  * the values the work list was built with.  Arguments as for ncclx_alltoallv_dev; 0 <= plan < NCCLX_NUM_PLANS;
@@ -380,14 +380,6 @@ int ncclx_stream_probe(int mode, const void* src, void* dst, size_t bytes, ncclx
 /* Same probe on a FIXED grid of num_ctas >= 1 CTAs x 1024 threads (128 KB of loads in flight per CTA): the per-SM
  * ceiling the SM-frugal ncclx_reducecopy_sum (2 CTAs) is read against. */
 int ncclx_stream_probe_ctas(int mode, const void* src, void* dst, size_t bytes, int num_ctas, ncclx_stream_t stream);
-
-/* Instrumented builds only (python -m paper_2510_20171_b200.build --timeline; -DXDEV_TIMELINE): copies the per-CTA
- * globaltimer stamps of the LAST segment_copy_kernel launch to stamps_host[ctas][*fields] (ns; fields: kernel entry,
- * metadata ready, first load issued, first store issued, last store issued, engine drained, exit, bulk tiles of the
- * call), followed by 1024 x 8 stamps of the LAST counts_kernel launch (per CTA: entry, dependency wait over, phase 1
- * done, barrier passed, tile totals known, exit).  stamps_host holds (ncclx_sm_count() * *fields + 8192) uint64;
- * max_ctas >= ncclx_sm_count().  Synchronises the device.  NCCLX_ERR_ARG in a normal build. */
-int ncclx_debug_timeline(uint64_t* stamps_host, int max_ctas, int* fields);
 
 /* Number of SMs of the device the library was initialised on (0 before init). */
 int ncclx_sm_count(void);

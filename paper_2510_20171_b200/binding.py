@@ -11,7 +11,7 @@ import os
 from typing import Sequence
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-# NCCLX_B200_LIB selects another build of the same library (the instrumented -DXDEV_TIMELINE one); never a fallback
+# NCCLX_B200_LIB selects another build of the same library (tests/test_gpu_barrier_fallback.py's forced-time-out one); never a fallback
 LIB_PATH = os.environ.get("NCCLX_B200_LIB") or os.path.join(HERE, "libncclx_b200.so")
 
 BF16, F32, F16, U8 = 0, 1, 2, 3
@@ -44,7 +44,7 @@ SYMBOLS = [
     "ncclx_reducecopy_sum", "ncclx_moe_dispatch_topk_dev", "ncclx_moe_combine_topk_sum_dev",
     "ncclx_alltoallv_prepare_dev", "ncclx_alltoallv_execute_dev", "ncclx_stream_probe", "ncclx_stream_probe_ctas",
     "ncclx_alltoallv_dynamic_prepare_dev", "ncclx_moe_topk_prepare_dev", "ncclx_moe_dispatch_topk_execute_dev",
-    "ncclx_moe_combine_topk_sum_execute_dev", "ncclx_debug_timeline", "ncclx_alltoallv_static_dev",
+    "ncclx_moe_combine_topk_sum_execute_dev", "ncclx_alltoallv_static_dev",
 ]
 
 
@@ -97,7 +97,6 @@ def lib() -> ctypes.CDLL:
         L.ncclx_moe_topk_prepare_dev.argtypes = [ctypes.c_int, vp, vp, ctypes.c_int, vp]
         L.ncclx_moe_dispatch_topk_execute_dev.argtypes = [ctypes.c_int, vp, vp, vp] + [ctypes.c_int] * 4 + [vp]
         L.ncclx_moe_combine_topk_sum_execute_dev.argtypes = [ctypes.c_int, vp, vp, vp] + [ctypes.c_int] * 4 + [vp]
-        L.ncclx_debug_timeline.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
         L.ncclx_set_param.argtypes = [ctypes.c_int, i64]
         L.ncclx_get_param.argtypes = [ctypes.c_int, i64p]
         L.ncclx_profile_read.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double), i64p]
@@ -307,17 +306,6 @@ def ncclx_stream_probe(mode: int, src, dst, nbytes: int, stream=None) -> None:
 
 def ncclx_stream_probe_ctas(mode: int, src, dst, nbytes: int, num_ctas: int, stream=None) -> None:
     _ck(lib().ncclx_stream_probe_ctas(mode, _ptr(src), _ptr(dst), nbytes, num_ctas, _stream(stream)), "ncclx_stream_probe_ctas")
-
-
-def ncclx_debug_timeline():
-    """Instrumented builds only: (copy: ctas x fields, counts: 1024 x 8) uint64 globaltimer stamps of the last launches."""
-    import numpy as np
-    n = ncclx_sm_count()
-    buf = np.zeros(n * 16 + 8192, np.uint64)
-    fields = ctypes.c_int(0)
-    _ck(lib().ncclx_debug_timeline(buf.ctypes.data, n, ctypes.byref(fields)), "ncclx_debug_timeline")
-    f = fields.value
-    return buf[:n * f].reshape(n, f), buf[n * f:n * f + 8192].reshape(1024, 8)
 
 
 def ncclx_set_param(param: int, value: int) -> None:

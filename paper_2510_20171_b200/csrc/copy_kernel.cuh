@@ -34,35 +34,16 @@ constexpr int COPY_WARPS = COPY_THREADS / 32;
 constexpr int COPY_SLOTS = 32;             // outstanding bulk tiles per engine (mbarriers; slot j lives in lane j): <= 32
 constexpr int COPY_MAX_ENGINES = 4;        // bulk engines (warps 0..E-1) per CTA, each with its own share of the ring
 constexpr int VEC_SLOTS = 16;              // outstanding staged pieces per vector engine
-#ifndef XDEV_VEC_SUB_BYTES
-#define XDEV_VEC_SUB_BYTES 4096
-#endif
-constexpr int VEC_SUB_BYTES = XDEV_VEC_SUB_BYTES;        // bytes of a vector tile staged per TMA load (multiple of 16, <= 4096: slot word)
+constexpr int VEC_SUB_BYTES = 4096;        // bytes of a vector tile staged per TMA load (multiple of 16, <= 4096: slot word)
 constexpr int VEC_DIRECT_MAX = 48;         // pieces shorter than this are copied by lanes, global -> global
 constexpr int VEC_MAX_IN_BULK_MIX = 13;    // vector engines when both lists have work: the bulk engines keep >= 3/16 of the ring (>= 1 tile)
 constexpr int COPY_MBAR_COUNT = COPY_MAX_ENGINES * COPY_SLOTS + COPY_WARPS * VEC_SLOTS;
 constexpr int COPY_MBAR_BYTES = COPY_MBAR_COUNT * 8;
 constexpr int COPY_KMAX_LONG = 2;          // max tiles per dynamic claim when segments average >= 8 tiles (measured: config 3)
-#ifndef XDEV_KMAX_LONG_VEC
-#define XDEV_KMAX_LONG_VEC 2
-#endif
-constexpr int COPY_KMAX_LONG_VEC = XDEV_KMAX_LONG_VEC;   // the same for the vector list (16 engines per CTA, 16 KiB tiles)
+constexpr int COPY_KMAX_LONG_VEC = 2;   // the same for the vector list (16 engines per CTA, 16 KiB tiles)
 constexpr int COPY_KMAX_VEC = 8;           // max tiles per dynamic claim on the vector list
-#ifndef XDEV_VEC_TMA_STORE
-#define XDEV_VEC_TMA_STORE 1              // vector list: body of a piece realigned in shared memory and stored by the TMA (0: warp stores)
-#endif
-#ifndef XDEV_PAYLOAD_POLICY
-#define XDEV_PAYLOAD_POLICY 1              // 1: payload bulk copies carry an L2 evict_first policy (common.cuh); 0: none (A/B builds)
-#endif
-#if XDEV_PAYLOAD_POLICY
 #define PAYLOAD_POL(p) , p
-#else
-#define PAYLOAD_POL(p)
-#endif
-#ifndef XDEV_CLAIM_DIV
-#define XDEV_CLAIM_DIV 8
-#endif
-constexpr int COPY_CLAIM_DIV = XDEV_CLAIM_DIV;          // guided claims: K = remaining / (COPY_CLAIM_DIV * engines), clamped to [1, kmax]: an engine holds up to three
+constexpr int COPY_CLAIM_DIV = 8;          // guided claims: K = remaining / (COPY_CLAIM_DIV * engines), clamped to [1, kmax]: an engine holds up to three
                                            // chunks (current, staged, claimed), so chunks shrink early (config 5: 2 -> 4: 163 -> 157 us with two engines)
 
 // Optional side job for the warps that are not engines at the start of the kernel: `copies` copies of the int64
@@ -89,9 +70,6 @@ struct CopyArgs {
     int bulkEngines;                       // E = 1, 2 or 4 bulk engine warps per CTA; 0 = chosen on the device from the tile count
     ClassParams cls;
     SideJob side;
-#ifdef XDEV_TIMELINE
-    unsigned long long* timeline;          // [grid][TL_COUNT] globaltimer stamps (instrumented build only)
-#endif
 };
 
 __host__ __device__ inline int coarse_blocks(int colLen) { return (colLen + 31) >> 5; }
@@ -134,7 +112,7 @@ __device__ __forceinline__ void cursor_env_init(CursorEnv* e, int L, const SegDe
     // long segments (>= 8 tiles each on average): claims resolve inside the cached window, so take
     // small chunks and keep all SMs in a tight moving window of HBM; short segments: amortise the
     // per-claim work over a few tiles and hide it behind the previous chunk.
-    e->longSegs = e->total >= 8 * e->RR;
+    e->longSegs = (long long)e->total >= 8ll * e->RR;
     e->indexed = coarse != nullptr || e->nb == 1;
     e->pipelined = e->indexed && !e->longSegs;
     e->kmax = e->longSegs ? kmaxLong : kmax;
@@ -449,56 +427,7 @@ __device__ __forceinline__ uint4 shift_join(const uint4& a, const uint4& b, cons
     return make_uint4(__funnelshift_r(w[WSEL], w[WSEL + 1], bsh), __funnelshift_r(w[WSEL + 1], w[WSEL + 2], bsh),
                       __funnelshift_r(w[WSEL + 2], w[WSEL + 3], bsh), __funnelshift_r(w[WSEL + 3], w[WSEL + 4], bsh));
 }
-template <int WSEL>
-__device__ __forceinline__ void drain_shifted_body(const uint4* sv, uint4* dv, const unsigned int nvec, const int bsh, const unsigned int lane) {
-    unsigned int i = lane;
-    for (; i + 32 < nvec; i += 64) {                       // two full warp rows per trip, loads first, no predicates
-        const uint4 a0 = sv[i], b0 = sv[i + 1], a1 = sv[i + 32], b1 = sv[i + 33];
-        st_stream(dv + i, shift_join<WSEL>(a0, b0, bsh));
-        st_stream(dv + i + 32, shift_join<WSEL>(a1, b1, bsh));
-    }
-    for (; i < nvec; i += 32) st_stream(dv + i, shift_join<WSEL>(sv[i], sv[i + 1], bsh));
-}
-
-// One warp: write `len` bytes to global `dst` (any alignment) from the shared-memory image `sm` (16-byte aligned) of
-// the aligned source span that holds them from byte offset ms (0..15) on.  Head and tail (< 16 bytes each, only at the
-// ends of a tile) go byte by byte, the body as aligned 16-byte stores; every shared-memory word read lies inside the
-// loaded span [0, align16(ms + len)) (the second word of a join is only read when it holds a needed byte: sh >= 1).
-__device__ __forceinline__ void warp_drain_shifted(unsigned char* dst, const unsigned char* sm, const unsigned int ms, const unsigned int len) {
-    const unsigned int lane = (unsigned int)lane_id();
-    unsigned int hb = (16u - (unsigned int)((unsigned long long)dst & 15ull)) & 15u;
-    if (hb) {                                              // warp-uniform
-        if (hb > len) hb = len;
-        if (lane < hb) dst[lane] = sm[ms + lane];
-    }
-    const unsigned int pos = ms + hb;                      // shared-memory offset of the first body byte
-    const unsigned int nvec = (len - hb) >> 4;
-    const unsigned int sh = pos & 15u;
-    const uint4* sv = reinterpret_cast<const uint4*>(sm) + (pos >> 4);
-    uint4* dv = reinterpret_cast<uint4*>(dst + hb);
-    if (sh == 0) {
-        unsigned int i = lane;
-        for (; i + 96 < nvec; i += 128) {
-            const uint4 v0 = sv[i], v1 = sv[i + 32], v2 = sv[i + 64], v3 = sv[i + 96];
-            st_stream(dv + i, v0); st_stream(dv + i + 32, v1); st_stream(dv + i + 64, v2); st_stream(dv + i + 96, v3);
-        }
-        for (; i < nvec; i += 32) st_stream(dv + i, sv[i]);
-    } else {
-        const int bsh = (int)(sh & 3u) * 8;
-        switch (sh >> 2) {                                 // warp-uniform, once per piece
-        case 0:  drain_shifted_body<0>(sv, dv, nvec, bsh, lane); break;
-        case 1:  drain_shifted_body<1>(sv, dv, nvec, bsh, lane); break;
-        case 2:  drain_shifted_body<2>(sv, dv, nvec, bsh, lane); break;
-        default: drain_shifted_body<3>(sv, dv, nvec, bsh, lane); break;
-        }
-    }
-    const unsigned int done = hb + (nvec << 4);
-    if (done < len) {                                      // warp-uniform; tail < 16
-        if (lane < len - done) dst[done + lane] = sm[ms + done + lane];
-    }
-}
-
-// TMA-store variant of the drain: the body is realigned IN PLACE in shared memory (vector i of the destination-aligned
+// The drain: one warp writes a landed piece to global memory at any alignment.  The body is realigned IN PLACE in shared memory (vector i of the destination-aligned
 // image overwrites slot i of the source-aligned one: every batch reads its 32 or 64 slots + the one after them into
 // registers before any lane writes), so that one cp.async.bulk shared -> global can store it; returns the shared-memory
 // address and the byte count of the body for the elected lane to issue.  Head / tail bytes (< 16 each, only at the ends
@@ -552,20 +481,6 @@ __device__ __forceinline__ void warp_drain_realign(unsigned char* dst, unsigned 
     bodyBytes = nvec << 4;
 }
 
-#ifdef XDEV_TIMELINE
-enum { TL_ENTER = 0, TL_READY, TL_FIRST_LOAD, TL_FIRST_STORE, TL_LAST_STORE, TL_DRAINED, TL_EXIT, TL_TILES, TL_ENV, TL_CURSOR, TL_ENSURED, TL_COUNT };
-__device__ __forceinline__ unsigned long long tl_now() {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
-#define TL_STAMP(tl, k) do { if (tl) (tl)[k] = tl_now(); } while (0)
-#define TL_STAMP_ONCE(tl, k) do { if ((tl) && (tl)[k] == 0ull) (tl)[k] = tl_now(); } while (0)
-#else
-#define TL_STAMP(tl, k) do { } while (0)
-#define TL_STAMP_ONCE(tl, k) do { } while (0)
-#endif
-
 // ================= bulk engine: byte-granular TMA ring driven by one elected lane (one warp) ========
 // The ring is a circular BYTE buffer (not fixed-size stages): every tile takes exactly
 // align128(len) bytes, so short tiles (config 5: 10-28 KiB) keep as many bytes in flight as
@@ -575,7 +490,7 @@ __device__ __forceinline__ unsigned long long tl_now() {
 // (keeping up to 8 stores unreclaimed was measured 10 % slower on config 5: the ring is for LOADS in flight).
 template <bool SM>
 __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned char* ring, unsigned long long* mbar,
-                                            const unsigned int ringBytes, unsigned long long* tl) {
+                                            const unsigned int ringBytes) {
     const int lane = lane_id();
     const unsigned int tileBytes = 1u << cur.tileShift;
     const uint32_t ring0 = smem_u32(ring);
@@ -585,7 +500,6 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
     unsigned int vHead = 0, phys = 0;     // virtual (mod 2^32) and physical allocation offsets
     int iLoad = 0, iStore = 0, freed = 0;  // stores [0, freed) have finished reading their smem; freed <= iStore <= iLoad
     bool more = cur.ensure();
-    TL_STAMP(tl, TL_ENSURED);
     while (true) {
         // fill: issue loads while a slot and enough ring bytes are free
         while (more) {
@@ -607,7 +521,6 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
                     const uint32_t bar = smem_u32(&mbar[slot]);
                     mbar_expect_tx(bar, len16);
                     bulk_g2s(ring0 + po, srcp, len16, bar PAYLOAD_POL(pol));
-                    TL_STAMP_ONCE(tl, TL_FIRST_LOAD);
                 }
                 const unsigned int adv = (len16 + 127u) & ~127u;
                 vHead = vStart + adv;
@@ -638,8 +551,6 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
         if (lane == 0) {
             bulk_s2g(reinterpret_cast<void*>(((unsigned long long)dhi << 32) | dlo), ring0 + soff, slen PAYLOAD_POL(pol));
             bulk_commit();
-            TL_STAMP_ONCE(tl, TL_FIRST_STORE);
-            TL_STAMP(tl, TL_LAST_STORE);
         }
         ++iStore;
         if (iStore - freed > 1) {                                 // at most ONE store keeps its ring bytes: reclaim the older one
@@ -648,7 +559,7 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
         }
         __syncwarp();
     }
-    if (lane == 0) { bulk_wait_all<0>(); TL_STAMP(tl, TL_DRAINED); }
+    if (lane == 0) bulk_wait_all<0>();
 }
 
 // ================= vector engine: one warp, its own share of the ring, TMA loads + warp stores ================
@@ -660,7 +571,7 @@ __device__ __forceinline__ void bulk_engine(Cursor<LIST_BULK, SM>& cur, unsigned
 // allocation.  Up to VEC_SLOTS pieces are in flight per engine (bookkeeping in lanes 0..15, as in the bulk engine),
 // also across tile and segment boundaries.  A landed piece is realigned by the whole warp and stored by the TMA
 // (warp_drain_realign); its ring bytes are released once that store has read them (one store may be outstanding), as in
-// the bulk engine.  (XDEV_VEC_TMA_STORE = 0 builds the earlier drain: aligned 16-byte warp stores from shared memory.)
+// the bulk engine.
 // The engine runs on either work list (L): when the bulk list holds only a small part of a mostly unaligned call,
 // the vector engines sweep it up as well (plan_ring: bulkByVec) instead of idling warps as bulk engines.
 // Measured (R = 16, 360 MB each way, odd bf16 counts): the loop is instruction-issue bound, so per-piece work is kept
@@ -701,11 +612,7 @@ __device__ __forceinline__ void vector_engine(Cursor<L, SM>& cur, unsigned char*
                 const unsigned int ld = (ms + len + 15u) & ~15u;
                 const unsigned int adv = (ld + 127u) & ~127u;
                 const unsigned int pad = phys + ld > ringBytes ? ringBytes - phys : 0u;   // wrap
-#if XDEV_VEC_TMA_STORE
                 if (iLoad - freed >= VEC_SLOTS || used + pad + adv > ringBytes) break;    // drain a landed piece first
-#else
-                if (iLoad - iStore >= VEC_SLOTS || used + pad + adv > ringBytes) break;   // drain a landed piece first
-#endif
                 const unsigned int po = pad ? 0u : phys;
                 const int slot = iLoad & (VEC_SLOTS - 1);
                 if (lane == slot) { mDst = tD; mPack = (po >> 7) | (len << 11) | (ms << 24); mAlloc = pad + adv; }
@@ -727,11 +634,9 @@ __device__ __forceinline__ void vector_engine(Cursor<L, SM>& cur, unsigned char*
         }
         if (iStore == iLoad) {
             if (!more) break;
-#if XDEV_VEC_TMA_STORE
             if (lane == 0) { bulk_wait_read<0>(); fence_proxy_async_smem(); }   // the stores still reading their ring bytes
             __syncwarp();
             freed = iStore; used = 0;
-#endif
             phys = 0;                      // nothing in flight: restart the ring at offset 0 (the piece did not fit behind phys)
             continue;
         }
@@ -740,7 +645,6 @@ __device__ __forceinline__ void vector_engine(Cursor<L, SM>& cur, unsigned char*
         const unsigned int dlo = __shfl_sync(0xffffffffu, (unsigned int)mDst, slot);
         const unsigned int dhi = __shfl_sync(0xffffffffu, (unsigned int)(mDst >> 32), slot);
         const unsigned int pk = __shfl_sync(0xffffffffu, mPack, slot);
-#if XDEV_VEC_TMA_STORE
         {
             unsigned char* bDst; uint32_t bSm; unsigned int bBytes;
             warp_drain_realign(reinterpret_cast<unsigned char*>(((unsigned long long)dhi << 32) | dlo), ring + ((pk & 0x7ffu) << 7),
@@ -757,19 +661,9 @@ __device__ __forceinline__ void vector_engine(Cursor<L, SM>& cur, unsigned char*
                 ++freed;
             }
         }
-#else
-        used -= __shfl_sync(0xffffffffu, mAlloc, slot);
-        warp_drain_shifted(reinterpret_cast<unsigned char*>(((unsigned long long)dhi << 32) | dlo), ring + ((pk & 0x7ffu) << 7),
-                           pk >> 24, (pk >> 11) & 0x1fffu);
-        ++iStore;
-        __syncwarp();                      // every lane has read its words before the TMA may overwrite them
-        if (lane == 0) fence_proxy_async_smem();
-#endif
     }
-#if XDEV_VEC_TMA_STORE
     if (lane == 0) bulk_wait_all<0>();     // shared memory stays valid until every store has read it (and the run's writes are done)
     __syncwarp();
-#endif
     pieceSeq = iLoad;
 }
 
@@ -845,7 +739,7 @@ __device__ __forceinline__ RingPlan plan_ring(int requestedE, int bulkTiles, int
 // First chunk of every engine is static (chunk e to engine e; see Cursor::init).
 __device__ __forceinline__ int static_first_chunk(int total, int nEngines, int kmax, int kmaxLong, int RR) {
     if (nEngines <= 0) return 0;
-    const int km = total >= 8 * RR ? kmaxLong : kmax;
+    const int km = (long long)total >= 8ll * RR ? kmaxLong : kmax;
     return clamped_quotient(total, 4 * nEngines, 1, km);
 }
 
@@ -877,7 +771,7 @@ template <bool SM>
 __device__ __forceinline__ bool run_copy_engines(const SegDesc* desc, int* const colBase[2], int* const coarse[2], WorkCtl* ctl,
                                                  const ClassParams& cls, int ncols, int colLen, int requestedE, int kmax,
                                                  int fusedStatic, long long bulkKiB, int claimDiv, unsigned char* smem, unsigned long long* mbar,
-                                                 unsigned int ringBytes, unsigned long long* tl) {
+                                                 unsigned int ringBytes) {
     __shared__ CursorEnv envs[2];
     const int warp = threadIdx.x >> 5;
     const int totB = colBase[LIST_BULK][ncols], totV = colBase[LIST_VEC][ncols];
@@ -885,24 +779,19 @@ __device__ __forceinline__ bool run_copy_engines(const SegDesc* desc, int* const
     const int nV = (int)gridDim.x * rp.NV;
     const int nB = rp.bulkByVec ? nV : (int)gridDim.x * rp.E;
     const int RR = ncols * colLen;
-    // Short lists (at most XDEV_RR_TPE tiles per engine: the small-message regime, a call of ~10 us) are dealt ROUND-ROBIN,
+    // Short lists (at most RR_TILES_PER_ENGINE tiles per engine: the small-message regime, a call of ~10 us) are dealt ROUND-ROBIN,
     // chunk c to engine c mod nEngines: same HBM order as in-order claims, but no atomic round trip sits between an
     // engine and its next tile.  Measured (graph replay p50): R = 64 x one 10 KB row per pair 28.1 -> 26.0 us, R = 128 x
     // 14 KB for 28 % of pairs 31.6 -> 30.1 us, and no longer build-dependent (with claims the same sources landed on
     // either value depending on instruction scheduling).  Longer lists need the claims' balance by TIME: round-robin
-    // there costs config 5 +17 us, config 3 +14 % (XDEV_RR_TPE = 64 / unlimited).
-#ifndef XDEV_RR_TPE
-#define XDEV_RR_TPE 16
-#endif
-    const bool rrB = fusedStatic == 0 && nB > 0 && (long long)totB <= (long long)XDEV_RR_TPE * nB;
-    const bool rrV = fusedStatic == 0 && nV > 0 && (long long)totV <= (long long)XDEV_RR_TPE * nV;
-    const int stB = fusedStatic > 0 ? fusedStatic : rrB ? clamped_quotient(totB, 32 * nB, 1, totB >= 8 * RR ? COPY_KMAX_LONG : min(kmax, 8))
+    // there costs config 5 +17 us, config 3 +14 % (measured with 64 / unlimited).
+    constexpr int RR_TILES_PER_ENGINE = 16;
+    const bool rrB = fusedStatic == 0 && nB > 0 && (long long)totB <= (long long)RR_TILES_PER_ENGINE * nB;
+    const bool rrV = fusedStatic == 0 && nV > 0 && (long long)totV <= (long long)RR_TILES_PER_ENGINE * nV;
+    const int stB = fusedStatic > 0 ? fusedStatic : rrB ? clamped_quotient(totB, 32 * nB, 1, (long long)totB >= 8ll * RR ? COPY_KMAX_LONG : min(kmax, 8))
                                                         : static_first_chunk(totB, nB, kmax, COPY_KMAX_LONG, RR);
-    const int stV = fusedStatic > 0 ? fusedStatic : rrV ? clamped_quotient(totV, 32 * nV, 1, totV >= 8 * RR ? COPY_KMAX_LONG_VEC : COPY_KMAX_VEC)
+    const int stV = fusedStatic > 0 ? fusedStatic : rrV ? clamped_quotient(totV, 32 * nV, 1, (long long)totV >= 8ll * RR ? COPY_KMAX_LONG_VEC : COPY_KMAX_VEC)
                                                         : static_first_chunk(totV, nV, COPY_KMAX_VEC, COPY_KMAX_LONG_VEC, RR);
-#ifdef XDEV_TIMELINE
-    if (tl) tl[TL_TILES] = (unsigned long long)totB;
-#endif
     if (threadIdx.x == 0)
         cursor_env_init(&envs[LIST_BULK], LIST_BULK, desc, colBase[LIST_BULK], coarse[LIST_BULK], &ctl->next[LIST_BULK], cls, ncols, colLen,
                         nB, kmax, COPY_KMAX_LONG, stB, claimDiv, rrB);
@@ -910,12 +799,10 @@ __device__ __forceinline__ bool run_copy_engines(const SegDesc* desc, int* const
         cursor_env_init(&envs[LIST_VEC], LIST_VEC, desc, colBase[LIST_VEC], coarse[LIST_VEC], &ctl->next[LIST_VEC], cls, ncols, colLen,
                         nV, COPY_KMAX_VEC, COPY_KMAX_LONG_VEC, stV, claimDiv, rrV);
     __syncthreads();
-    TL_STAMP(tl, TL_ENV);
     if (warp < rp.E) {
         Cursor<LIST_BULK, SM> cur;
         cur.init(&envs[LIST_BULK], (int)blockIdx.x * rp.E + warp);
-        if (warp == 0) TL_STAMP(tl, TL_CURSOR);
-        bulk_engine<SM>(cur, smem + (size_t)warp * rp.bulkShare, mbar + warp * COPY_SLOTS, rp.bulkShare, warp == 0 ? tl : nullptr);
+        bulk_engine<SM>(cur, smem + (size_t)warp * rp.bulkShare, mbar + warp * COPY_SLOTS, rp.bulkShare);
     } else if (warp < rp.E + rp.NV) {
         const int v = warp - rp.E;
         vector_role<SM>(envs, (int)blockIdx.x * rp.NV + v, smem + rp.vecBase + (size_t)v * rp.vecShare,
@@ -953,13 +840,6 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
     const int nbR = R * coarse_blocks(a.colLen);
     int* coarse[2] = {nullptr, nullptr};
     if (a.useCoarse) { coarse[0] = colBase[1] + (R + 1); coarse[1] = coarse[0] + nbR; }
-#ifdef XDEV_TIMELINE
-    unsigned long long* tl = (a.timeline && threadIdx.x == 0) ? a.timeline + (size_t)blockIdx.x * TL_COUNT : nullptr;
-    if (tl) { for (int i = 0; i < TL_COUNT; ++i) tl[i] = 0ull; }
-#else
-    unsigned long long* tl = nullptr;
-#endif
-    TL_STAMP(tl, TL_ENTER);
 
     // ---- prologue: mbarrier init (overlaps the metadata kernel under PDL), then cross-column tile
     //      bases = scan of the R per-column totals the metadata kernel wrote, and the coarse indexes ----
@@ -998,13 +878,11 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) segment_copy_kernel(const Cop
         if (lane == 0) *totKiB = k;
     }
     __syncthreads();
-    TL_STAMP(tl, TL_READY);
 
     run_side_job(a.side, COPY_WARPS / 2);
     const bool usedCounters = run_copy_engines<false>(a.desc, colBase, coarse, a.ctl, a.cls, a.ncols, a.colLen, a.bulkEngines, a.kmax, 0,
-                                                      *totKiB, COPY_CLAIM_DIV, smem, mbar, a.ringBytes, tl);
+                                                      *totKiB, COPY_CLAIM_DIV, smem, mbar, a.ringBytes);
     workctl_checkout(a.ctl, usedCounters);
-    TL_STAMP(tl, TL_EXIT);
 }
 
 }  // namespace xdev

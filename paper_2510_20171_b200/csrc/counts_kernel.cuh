@@ -39,16 +39,8 @@ struct CountsArgs {
     int blockSums;                // 1: phase 1 through per-CTA block sums and a grid barrier (R > 128); 0: row prefixes re-read from C
     long long elemSize;               // bytes per count unit (an element, or a whole row for the top-k calls)
     ClassParams cls;
-#ifdef XDEV_TIMELINE
-    unsigned long long* timeline;     // [CTAs][8] globaltimer stamps (instrumented build only)
-#endif
 };
 
-#ifdef XDEV_TIMELINE
-#define CT_STAMP(k) do { if (threadIdx.x == 0 && a.timeline) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); a.timeline[(size_t)blockIdx.x * 8 + (k)] = t_; } } while (0)
-#else
-#define CT_STAMP(k) do { } while (0)
-#endif
 
 // dynamic smem: long long cval[R][W+1], sofs[R][W+1] (+1: conflict-free column reads), u64 sendPtr[R], recvPtr[W],
 //               long long tileTot[W*nb], rowsBefore[W*nb], byteTot[W*nb]   (nb = ceil(R/32))
@@ -66,7 +58,6 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
     const int d0 = blockIdx.x * W;
     const int Wc = min(W, R - d0);
 
-    CT_STAMP(0);
     griddep_launch_dependents();                 // let the copy kernel's CTAs start their prologue
     // the count matrix is usually cold (the previous call streamed far more than L2 holds): the grid prefetches all of
     // it into L2 with one DRAM round trip, before and after the dependency wait (before: while the stream's previous
@@ -76,7 +67,6 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
     for (size_t i = gtid; i < cLines; i += gthreads) prefetch_l2(reinterpret_cast<const char*>(a.C) + (i << 7));
     griddep_wait();                              // (launched with PDL itself: the stream's previous kernel must be complete)
     for (size_t i = gtid; i < cLines; i += gthreads) prefetch_l2(reinterpret_cast<const char*>(a.C) + (i << 7));
-    CT_STAMP(1);
     // pointer tables: issue the loads now, park them in shared memory after phase 1's loads are in flight too (one
     // DRAM round trip instead of two on a cold start)
     constexpr int PT = 2;                        // covers R <= 1024 with 512 threads
@@ -235,9 +225,7 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
         }
     }
     if (sawNeg) atomicOr(&a.ws.ctl->status, 1u);
-    CT_STAMP(2);
     __syncthreads();
-    CT_STAMP(3);
 
     // ---- phase 2: one work item per (owned column j, block b of 32 source rows), items round-robin over the warps ----
     // (round 1 ran one warp per COLUMN, serially over the row blocks: with few columns per CTA most warps idled through
@@ -324,15 +312,12 @@ __global__ void __launch_bounds__(COUNTS_THREADS) counts_kernel(const CountsArgs
         Item x{};
         if (warp < nItems) x = front(warp, true);
         __syncthreads();
-        CT_STAMP(4);
         if (warp < nItems) back(x);
     } else {
         for (int item = warp; item < nItems; item += nwarps) (void)front(item, true);
         __syncthreads();
-        CT_STAMP(4);
         for (int item = warp; item < nItems; item += nwarps) back(front(item, false));
     }
-    CT_STAMP(5);
 }
 
 }  // namespace xdev

@@ -43,16 +43,8 @@ struct DynArgs {
     Workspace ws;                     // desc / coarse / colTiles / ctl of the plan slot
     int R, n, maxIndices, maxBlockLen, elemSize;
     ClassParams cls;
-#ifdef XDEV_TIMELINE
-    unsigned long long* timeline;     // [CTAs][8] globaltimer stamps (instrumented build only; same layout as counts_kernel's)
-#endif
 };
 
-#ifdef XDEV_TIMELINE
-#define DY_STAMP(k) do { if (threadIdx.x == 0 && a.timeline) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); a.timeline[(size_t)blockIdx.x * 8 + (k)] = t_; } } while (0)
-#else
-#define DY_STAMP(k) do { } while (0)
-#endif
 
 struct __align__(32) DynSlot {        // same 32-byte stride as SegDesc, so the table itself can serve as the slot array
     unsigned long long src, dst;
@@ -75,7 +67,6 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
     const int nb = (colLen + 31) >> 5;
     DynSlot* slots = colLen <= DYN_SMEM_SLOTS ? reinterpret_cast<DynSlot*>(dyn_smem)
                                               : reinterpret_cast<DynSlot*>(a.ws.desc + (size_t)d * colLen);
-    DY_STAMP(0);
     griddep_launch_dependents();
     if (threadIdx.x == 0) sStatus = 0u;
     // (before the dependency wait: a hint, and L2 is the point of coherence, so a line fetched early cannot go stale)
@@ -92,7 +83,6 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
         }
     }
     griddep_wait();                                        // the metadata may have been written by the stream's previous kernel
-    DY_STAMP(1);
     unsigned int st = 0;
     const unsigned long long keep = l2_policy_keep();      // metadata inputs stay in L2 across the payload stream (common.cuh)
 
@@ -150,7 +140,6 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
             ioff[u] = warp_sum(before);
             bl[u] = (int)warp_sum(mine);
         }
-        if (sBase == warp) DY_STAMP(2);
         for (int j0 = 0; j0 < J; j0 += 32) {               // one pass per 32 list entries (J <= 32: one pass)
             const int j = j0 + lane;
             // round trip 2: this lane's split index, for all DYN_SU sources at once
@@ -172,7 +161,6 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
                     else live[u] = true;
                 }
             }
-            if (sBase == warp && j0 == 0) DY_STAMP(3);
             // offsets: exclusive prefix sums of the split lengths, DYN_CHUNK at a time, for all DYN_SU sources together (their
             // shuffle chains interleave): lane l holds lengths 4l .. 4l+3 of the chunk, one 64-bit warp scan of the lane totals,
             // then every lane PICKS offset and length of its own split from the owning lane's registers by shuffle -- no
@@ -231,9 +219,7 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
     }
     st = __reduce_or_sync(0xffffffffu, st);
     if (lane == 0 && st) atomicOr(&sStatus, st);
-    DY_STAMP(4);
     __syncthreads();
-    DY_STAMP(5);
 
     // ---- phase B: tile prefixes in slot order, descriptors, coarse index ------------------------------------------
     long long run = 0;                                     // tiles of the column before this round: bulk << 32 | vector
@@ -268,7 +254,6 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
         run += all;
         __syncthreads();                                   // sWarpTot is rewritten in the next round
     }
-    DY_STAMP(6);
     myBulkBytes = warp_sum(myBulkBytes);
     if (lane == 0) sWarpTot[warp] = myBulkBytes;           // (the last round's barrier has passed: sWarpTot is free)
     __syncthreads();
@@ -280,7 +265,6 @@ __global__ void __launch_bounds__(DYN_THREADS, 1) dyn_build_kernel(const DynArgs
         a.ws.colKiB[d] = (int)(bb >> 10);
         if (sStatus) atomicOr(&a.ws.ctl->status, sStatus);
     }
-    DY_STAMP(7);
 }
 
 }  // namespace xdev

@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(COPY_THREADS, 1) alltoallv_fused_kernel(const 
 
     // ---- a4: the copy engines of the big path, fed from shared memory; the first tile of every engine is static ----
     const bool usedCounters = run_copy_engines<true>(sdesc, colBase, nullptrs, a.ctl, cls, R, R, a.bulkEngines, a.kmax, 1, -1, 2, smem, mbar,
-                                                     a.ringBytes, nullptr);
+                                                     a.ringBytes);
     workctl_checkout(a.ctl, usedCounters);
 }
 

@@ -50,6 +50,9 @@ struct Context {
     Workspace wsPlan[NCCLX_NUM_PLANS]{};  // one workspace per plan slot; slot 0 also serves the one-call entry points
     struct PlanState { int kind = PLAN_NONE; int R = 0; CopyLaunch cl{}; const long long* topkC = nullptr; } plan[NCCLX_NUM_PLANS];
     WorkCtl* fusedCtl = nullptr;          // claim counters of the single-launch path (self-resetting)
+    long long* fusedSoff = nullptr;       // the single-launch path's own offset matrices: it leaves every plan slot alone
+    long long* fusedRoff = nullptr;
+    bool lastOffsetsFused = false;        // which of the two ncclx_alltoallv_last_offsets reads
     void* wsBase = nullptr;
     // tunables (ncclx_param_t order)
     int64_t params[NCCLX_PARAM_COUNT_] = {1024, 16, 0, 15, 1, 6, 32, 0, 1, 0};
@@ -66,7 +69,6 @@ struct Context {
     // host-path staging (device memory, grown on demand)
     void* stage[4] = {nullptr, nullptr, nullptr, nullptr};   // 0 send data, 1 recv data, 2 meta, 3 spare
     size_t stageCap[4] = {0, 0, 0, 0};
-    unsigned long long* timeline = nullptr;                   // instrumented build only
     int lastCuda = 0;
     std::mutex mu;                        // every entry point that reads params / plans or launches takes it
 };
@@ -222,9 +224,6 @@ int launchCopy(const Workspace& ws, const CopyLaunch& cl, cudaStream_t stream) {
     cp.ringBytes = cl.ringBytes;
     cp.kmax = cl.kmax;
     cp.side = cl.side;
-#ifdef XDEV_TIMELINE
-    cp.timeline = g.timeline;
-#endif
     LaunchScope ls(NCCLX_KERNEL_COPY, stream);
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)g.smCount);
@@ -247,9 +246,6 @@ int launchCounts(const Workspace& ws, const void* const* send, const int64_t* C,
     ca.ws = ws; ca.R = R; ca.W = countsW(R); ca.elemSize = es;
     ca.blockSums = R > kCountsBlockSumMinRanks ? 1 : 0;
     ca.cls = cls;
-#ifdef XDEV_TIMELINE
-    ca.timeline = g.timeline + (size_t)g.smCount * TL_COUNT;      // counts-kernel stamps follow the copy kernel's
-#endif
     const int G = (R + ca.W - 1) / ca.W;
     if (G > COUNTS_MAX_CTAS) return NCCLX_ERR_ARG;        // (cannot happen for R <= NCCLX_MAX_RANKS: W >= 12 there)
     const size_t csm = countsSmemBytes(R, ca.W);
@@ -275,6 +271,7 @@ int planFused(FusedArgs& fa, int R) {
     const size_t aux = fused_aux_bytes(R);
     if (budget < aux + 64 * 1024) return NCCLX_ERR_ARG;
     fa.ringBytes = (unsigned int)((budget - aux) & ~(size_t)127);
+    if ((size_t)VEC_SUB_BYTES + 256 > ((fa.ringBytes / COPY_WARPS) & ~127u)) return NCCLX_ERR_ARG;   // as planCopy: a vector engine's share must hold one staged piece
     fa.bulkEngines = (int)g.params[NCCLX_PARAM_COPY_BULK_ENGINES];
     while (fa.cls.tileShift[0] > 10 && !bulkTileFits(fa.cls.tileShift[0], fa.ringBytes, fa.bulkEngines)) --fa.cls.tileShift[0];
     fa.kmax = (int)g.params[NCCLX_PARAM_COPY_KMAX];
@@ -288,7 +285,7 @@ int launchFused(FusedArgs& fa, const void* const* send, const int64_t* C, void* 
     fa.send = send; fa.recv = recv;
     fa.C = reinterpret_cast<const long long*>(C);
     fa.RC = reinterpret_cast<long long*>(RC);
-    fa.soff = g.wsPlan[0].soff; fa.roff = g.wsPlan[0].roff;
+    fa.soff = g.fusedSoff; fa.roff = g.fusedRoff;
     fa.ctl = g.fusedCtl; fa.status = &g.wsPlan[0].ctl->status;
     fa.R = R; fa.elemSize = es;
     LaunchScope ls(NCCLX_KERNEL_FUSED, stream);
@@ -301,6 +298,7 @@ int launchFused(FusedArgs& fa, const void* const* send, const int64_t* C, void* 
     setPdl(cfg, attr, g.params[NCCLX_PARAM_PDL] != 0);
     CK(cudaLaunchKernelEx(&cfg, alltoallv_fused_kernel, fa));
     ls.ok();
+    g.lastOffsetsFused = true;
     return NCCLX_OK;
 }
 
@@ -316,6 +314,7 @@ int prepareA2A(int p, const void* const* send, const int64_t* C, void* const* re
     rc = launchCounts(ws, send, C, recv, RC, R, es, cl.cls, stream);
     if (rc) return rc;
     ps.kind = PLAN_A2A; ps.R = R; ps.cl = cl;
+    if (p == 0) g.lastOffsetsFused = false;
     return NCCLX_OK;
 }
 
@@ -379,9 +378,6 @@ int launchReduce(const void* const* send, void* const* recv, size_t blockElems, 
         ra.prefetchCtas = (int)grid;
         ra.prefetchTiles = inBytes <= kReducePrefetchAllBytes ? (int)((tiles + grid - 1) / grid) : 2;
     }
-#ifdef XDEV_NO_REDUCE_PREFETCH
-    ra.prefetchTiles = 0;
-#endif
     switch (dtype) {
     case NCCLX_BF16: return shortCall ? launchReduceDT<RED_BF16, REDUCE_THREADS_SHORT>(ra, (int)grid, smem, pdl, stream)
                                       : launchReduceDT<RED_BF16, REDUCE_THREADS>(ra, (int)grid, smem, pdl, stream);
@@ -422,7 +418,6 @@ int checkCommon(int R) {
 void freeAll() {
     if (g.wsBase) { cudaFree(g.wsBase); g.wsBase = nullptr; }
     if (g.dynBase) { cudaFree(g.dynBase); g.dynBase = nullptr; g.dynMaxSplits = 0; g.dynMaxSegments = 0; }
-    if (g.timeline) { cudaFree(g.timeline); g.timeline = nullptr; }
     for (int i = 0; i < 4; ++i) {
         if (g.stage[i]) { cudaFree(g.stage[i]); g.stage[i] = nullptr; g.stageCap[i] = 0; }
     }
@@ -452,12 +447,11 @@ int topkCommon(int R, int T, int k, int width, int es) {
     return NCCLX_OK;
 }
 
+constexpr int kTopkCtasPerSm = 16;
+
 int topkGrid(long long tokens) {
     long long ctas = (tokens + TOPK_THREADS / 32 - 1) / (TOPK_THREADS / 32);
-#ifndef XDEV_TOPK_CTAS_PER_SM
-#define XDEV_TOPK_CTAS_PER_SM 16
-#endif
-    const long long cap = (long long)g.smCount * XDEV_TOPK_CTAS_PER_SM;
+    const long long cap = (long long)g.smCount * kTopkCtasPerSm;
     return (int)(ctas < 1 ? 1 : (ctas > cap ? cap : ctas));
 }
 
@@ -499,29 +493,6 @@ int launchTopkDispatch(int p, const void* const* tokens, const int32_t* pos, voi
     if (T == 0) return NCCLX_OK;
     TopkArgs ta = topkArgs(p, pos, R, T, k, rowBytes);
     ta.tokens = tokens; ta.packed = recv; ta.out = nullptr;
-#if XDEV_TOPK_TMA
-    // (A/B build) rows that are multiples of 16 bytes and fit a shared-memory slot (at least 4 warps' worth) move by TMA
-    const size_t slotBytes = alignUp((size_t)rowBytes, 128);
-    const size_t room = (size_t)g.maxSmemOptin - 1024;
-    int warps = (int)(room / (2 * slotBytes + 16));                // two slots per warp
-    if (warps > 16) warps = 16;
-    if (rowBytes % 16 == 0 && warps >= 4) {
-        LaunchScope ls(NCCLX_KERNEL_TOPK, s);
-        cudaLaunchConfig_t cfg{};
-        const long long tokens_ = (long long)R * T;
-        long long grid = (tokens_ + warps - 1) / warps;
-        if (grid > g.smCount) grid = g.smCount;
-        cfg.gridDim = dim3((unsigned)(grid < 1 ? 1 : grid));
-        cfg.blockDim = dim3((unsigned)warps * 32);
-        cfg.dynamicSmemBytes = (size_t)warps * (2 * slotBytes + 16);
-        cfg.stream = s;
-        cudaLaunchAttribute attr[1];
-        setPdl(cfg, attr, g.params[NCCLX_PARAM_PDL] != 0);
-        CK(cudaLaunchKernelEx(&cfg, topk_dispatch_tma_kernel, ta, (unsigned int)slotBytes));
-        ls.ok();
-        return NCCLX_OK;
-    }
-#endif
     return launchTopk(topk_dispatch_kernel, ta, s);
 }
 
@@ -561,9 +532,6 @@ int prepareDynamic(int p, const void* const* send, const int64_t* L, int nsplits
     da.ws = ws;
     da.R = R; da.n = nsplits; da.maxIndices = maxIndices; da.maxBlockLen = maxBlockLen; da.elemSize = es;
     da.cls = cl.cls;
-#ifdef XDEV_TIMELINE
-    da.timeline = g.timeline + (size_t)g.smCount * TL_COUNT;
-#endif
     ps.kind = PLAN_NONE;
     {
         LaunchScope ls(NCCLX_KERNEL_DYN, s);
@@ -644,6 +612,9 @@ static int initLocked(int max_ranks, int device) {
     }
     const size_t oFctl = off; off = alignUp(off + sizeof(WorkCtl), 256);
     const size_t oRcs = off; off = alignUp(off + rr * 8, 256);
+    const size_t fusedRR = (size_t)FUSED_MAX_R * FUSED_MAX_R * 8;
+    const size_t oFso = off; off = alignUp(off + fusedRR, 256);
+    const size_t oFro = off; off = alignUp(off + fusedRR, 256);
     CK(cudaMalloc(&g.wsBase, off));
     CK(cudaMemset(g.wsBase, 0, off));
     char* b = static_cast<char*>(g.wsBase);
@@ -663,18 +634,14 @@ static int initLocked(int max_ranks, int device) {
     }
     g.fusedCtl = reinterpret_cast<WorkCtl*>(b + oFctl);
     g.rcScratch = reinterpret_cast<long long*>(b + oRcs);
-#ifdef XDEV_TIMELINE
-    CK(cudaMalloc(&g.timeline, ((size_t)g.smCount * TL_COUNT + 1024 * 8) * 8));
-    CK(cudaMemset(g.timeline, 0, ((size_t)g.smCount * TL_COUNT + 1024 * 8) * 8));
-#endif
+    g.fusedSoff = reinterpret_cast<long long*>(b + oFso);
+    g.fusedRoff = reinterpret_cast<long long*>(b + oFro);
+    g.lastOffsetsFused = false;
 
     int rc;
     if ((rc = optInSmem(segment_copy_kernel, g.maxSmemOptin))) return rc;
     if ((rc = optInSmem(counts_kernel, g.maxSmemOptin))) return rc;
     if ((rc = optInSmem(alltoallv_fused_kernel, g.maxSmemOptin))) return rc;
-#if XDEV_TOPK_TMA
-    if ((rc = optInSmem(topk_dispatch_tma_kernel, g.maxSmemOptin))) return rc;
-#endif
     if ((rc = optInSmem(dyn_build_kernel, (int)dyn_smem_bytes(DYN_SMEM_SLOTS)))) return rc;
     if ((rc = optInSmem(reducecopy_tma_kernel<RED_BF16>, RCT_SMEM_BYTES))) return rc;
     if ((rc = optInSmem(reducecopy_tma_kernel<RED_F32>, RCT_SMEM_BYTES))) return rc;
@@ -746,8 +713,9 @@ int ncclx_alltoallv_last_offsets(int64_t* soff_host, int64_t* roff_host, int R, 
     if (isCapturing(s)) return NCCLX_ERR_CAPTURE;
     CK(cudaStreamSynchronize(s));
     const size_t bytes = (size_t)R * R * 8;
-    if (soff_host) CK(cudaMemcpy(soff_host, g.wsPlan[0].soff, bytes, cudaMemcpyDeviceToHost));
-    if (roff_host) CK(cudaMemcpy(roff_host, g.wsPlan[0].roff, bytes, cudaMemcpyDeviceToHost));
+    if (g.lastOffsetsFused && R > FUSED_MAX_R) return NCCLX_ERR_ARG;       // the last call had at most 32 ranks
+    if (soff_host) CK(cudaMemcpy(soff_host, g.lastOffsetsFused ? g.fusedSoff : g.wsPlan[0].soff, bytes, cudaMemcpyDeviceToHost));
+    if (roff_host) CK(cudaMemcpy(roff_host, g.lastOffsetsFused ? g.fusedRoff : g.wsPlan[0].roff, bytes, cudaMemcpyDeviceToHost));
     return NCCLX_OK;
 }
 
@@ -1166,21 +1134,6 @@ int ncclx_profile_reset(void) {
 }
 
 int64_t ncclx_launch_count(void) { return g.launches.load(); }
-
-int ncclx_debug_timeline(uint64_t* stamps_host, int max_ctas, int* fields) {
-    Lock lk(g.mu);
-    if (!g.ready) return NCCLX_ERR_NOT_INITIALIZED;
-#ifdef XDEV_TIMELINE
-    if (!stamps_host || !fields || max_ctas < g.smCount) return NCCLX_ERR_ARG;
-    CK(cudaDeviceSynchronize());
-    CK(cudaMemcpy(stamps_host, g.timeline, ((size_t)g.smCount * TL_COUNT + 1024 * 8) * 8, cudaMemcpyDeviceToHost));
-    *fields = TL_COUNT;
-    return NCCLX_OK;
-#else
-    (void)stamps_host; (void)max_ctas; (void)fields;
-    return NCCLX_ERR_ARG;                          // not an instrumented build (-DXDEV_TIMELINE)
-#endif
-}
 
 }  // extern "C"
 

@@ -21,14 +21,8 @@
 
 namespace xdev {
 
-#ifndef XDEV_REDUCE_THREADS
-#define XDEV_REDUCE_THREADS 128
-#endif
-constexpr int REDUCE_THREADS = XDEV_REDUCE_THREADS;        // CTA size of long reductions
-#ifndef XDEV_REDUCE_THREADS_SHORT
-#define XDEV_REDUCE_THREADS_SHORT 64
-#endif
-constexpr int REDUCE_THREADS_SHORT = XDEV_REDUCE_THREADS_SHORT;                   // ... and of short ones (below kReduceShortBytes of input: twice as many, smaller
+constexpr int REDUCE_THREADS = 128;        // CTA size of long reductions
+constexpr int REDUCE_THREADS_SHORT = 64;                   // ... and of short ones (below kReduceShortBytes of input: twice as many, smaller
                                                            // CTAs for the hardware scheduler to deal out; config 2 23.1 -> 22.8 us per call,
                                                            // while config 4 prefers 128: +0.3 % with 64)
 enum { RED_BF16 = 0, RED_F32 = 1, RED_F16 = 2 };

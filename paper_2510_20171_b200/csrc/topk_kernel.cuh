@@ -18,14 +18,8 @@
 
 namespace xdev {
 
-#ifndef XDEV_TOPK_THREADS
-#define XDEV_TOPK_THREADS 128              // 4 warps per CTA, up to 16 CTAs per SM: measured 1.6 % faster on the dispatch than 256 x 8 (512 x 4: 6 % slower)
-#endif
-#ifndef XDEV_TOPK_UNROLL
-#define XDEV_TOPK_UNROLL 2
-#endif
-constexpr int TOPK_THREADS = XDEV_TOPK_THREADS;
-constexpr int TOPK_UNROLL = XDEV_TOPK_UNROLL;             // dispatch: vectors per lane in flight per copy (4 measured 8 % slower)
+constexpr int TOPK_THREADS = 128;               // 4 warps per CTA, up to 16 CTAs per SM: measured 1.6 % faster on the dispatch than 256 x 8 (512 x 4: 6 % slower)
+constexpr int TOPK_UNROLL = 2;             // dispatch: vectors per lane in flight per copy (4 measured 8 % slower)
 constexpr int TOPK_COMBINE_UNROLL = 4;     // combine: 4 measured 1 % faster than 2
 
 struct TopkArgs {
@@ -110,77 +104,6 @@ __global__ void __launch_bounds__(TOPK_THREADS) topk_dispatch_kernel(const TopkA
     }
 }
 
-#ifndef XDEV_TOPK_TMA
-#define XDEV_TOPK_TMA 0                     // A/B build only: measured SLOWER than the LSU kernel (R = 64, T = 4096, k = 4: 2.36 vs 2.14 ms, one or two
-#endif                                     // slots per warp alike) -- a write-dominated stream gains nothing from TMA stores (probe mode 3: -2..4 % vs STG.256)
-#if XDEV_TOPK_TMA
-// The same dispatch with the rows moved by the TMA (rows that are multiples of 16 bytes and fit a shared-memory slot):
-// persistent grid of one CTA per SM; every warp owns TWO slots of align128(rowBytes) bytes and works one token ahead:
-// the bulk load of token i+1 is started (its address needs no metadata) as soon as the stores of token i-1 have READ
-// that slot, then the warp waits for token i's row and issues its k bulk stores; the k destination addresses are
-// resolved while loads are in flight.  One elected lane issues; the row never passes through registers.  A token whose
-// row or destinations are not 16-byte aligned takes the LSU path above (warp-uniform choice per token).
-// dynamic smem: [slots: warps x 2 x slotBytes][mbar: warps x 2 x u64]
-__global__ void __launch_bounds__(512, 1) topk_dispatch_tma_kernel(const TopkArgs a, const unsigned int slotBytes) {
-    extern __shared__ __align__(128) unsigned char topk_smem[];
-    const int lane = lane_id(), warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    unsigned long long* mbar = reinterpret_cast<unsigned long long*>(topk_smem + (size_t)nwarps * 2 * slotBytes);
-    const uint32_t slot0 = smem_u32(topk_smem + (size_t)warp * 2 * slotBytes);
-    const uint32_t bar0 = smem_u32(&mbar[warp * 2]);
-    const long long nTok = (long long)a.R * a.T;
-    const long long wStride = (long long)gridDim.x * nwarps;
-    if (lane < 2) mbar_init(bar0 + 8u * lane, 1);
-    fence_mbar_init();
-    __syncwarp();
-    const unsigned long long pol = l2_policy_stream();
-    griddep_wait();                                         // soff / roff come from counts_kernel
-    auto row_of = [&](long long tok) {
-        const int s = (int)(tok / a.T), t = (int)(tok - (long long)s * a.T);
-        return reinterpret_cast<const unsigned char*>(a.tokens[s]) + (size_t)t * a.rowBytes;
-    };
-    auto start_load = [&](long long tok, uint32_t b) -> bool {       // -> the row is being loaded into slot b
-        const unsigned char* src = row_of(tok);
-        const bool ok = (((unsigned long long)src | (unsigned long long)a.rowBytes) & 15ull) == 0;
-        if (ok && lane == 0) {
-            mbar_expect_tx(bar0 + 8u * b, (uint32_t)a.rowBytes);
-            bulk_g2s(slot0 + b * slotBytes, src, (uint32_t)a.rowBytes, bar0 + 8u * b, pol);
-        }
-        return ok;
-    };
-    long long cur = (long long)blockIdx.x * nwarps + warp;
-    uint32_t b = 0, ph0 = 0, ph1 = 0;
-    bool curOk = cur < nTok ? start_load(cur, 0) : false;
-    while (cur < nTok) {
-        const int s = (int)(cur / a.T), t = (int)(cur - (long long)s * a.T);
-        bool bad = false;
-        const unsigned long long mine = lane < a.k ? topk_resolve(a, s, t, lane, bad) : 0ull;
-        if (__any_sync(0xffffffffu, bad) && lane == 0) atomicOr(&a.ctl->status, 2u);
-        const bool dstOk = __reduce_or_sync(0xffffffffu, (unsigned int)(mine & 15ull)) == 0;
-        const long long nxt = cur + wStride;
-        if (lane == 0) bulk_wait_read<0>();                 // the previous token's stores have read the other slot
-        __syncwarp();
-        const bool nxtOk = nxt < nTok ? start_load(nxt, b ^ 1u) : false;
-        if (curOk) {
-            const uint32_t ph = b ? ph1 : ph0;
-            mbar_wait(bar0 + 8u * b, ph);                   // the row has landed (also when it is then copied by lanes)
-            if (b) ph1 ^= 1u; else ph0 ^= 1u;
-        }
-        if (curOk && dstOk) {
-            for (int j = 0; j < a.k; ++j) {
-                const unsigned long long dlo = __shfl_sync(0xffffffffu, (unsigned int)mine, j);
-                const unsigned long long dhi = __shfl_sync(0xffffffffu, (unsigned int)(mine >> 32), j);
-                const unsigned long long dst = (dhi << 32) | dlo;
-                if (dst && lane == 0) bulk_s2g(reinterpret_cast<void*>(dst), slot0 + b * slotBytes, (uint32_t)a.rowBytes, pol);
-            }
-            if (lane == 0) bulk_commit();
-        } else {
-            topk_dispatch_row_lsu(a, row_of(cur), mine, lane);
-        }
-        cur = nxt; curOk = nxtOk; b ^= 1u;
-    }
-    if (lane == 0) bulk_wait_all<0>();
-}
-#endif  // XDEV_TOPK_TMA
 
 template <int DT>
 __global__ void __launch_bounds__(TOPK_THREADS) topk_combine_kernel(const TopkArgs a) {

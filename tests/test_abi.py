@@ -55,7 +55,6 @@ def test_calls_fail_loudly_without_init(L):
     assert L.ncclx_moe_dispatch_topk_execute_dev(0, 1, 1, 1, 4, 2, 16, 0, None) == 3
     assert L.ncclx_moe_combine_topk_sum_execute_dev(0, 1, 1, 1, 4, 2, 16, 0, None) == 3
     assert L.ncclx_stream_probe_ctas(2, 32, 64, 32, 1, None) == 3
-    assert L.ncclx_debug_timeline(None, 0, None) == 3
     with pytest.raises(binding.NcclxError):
         binding.ncclx_finalize()
 
