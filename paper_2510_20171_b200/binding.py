@@ -11,7 +11,7 @@ import os
 from typing import Sequence
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-# NCCLX_B200_LIB selects another build of the same library (tests/test_gpu_barrier_fallback.py's forced-time-out one); never a fallback
+# NCCLX_B200_LIB selects another build of the same library (tests/test_zy_barrier_fallback.py's forced-time-out one); never a fallback
 LIB_PATH = os.environ.get("NCCLX_B200_LIB") or os.path.join(HERE, "libncclx_b200.so")
 
 BF16, F32, F16, U8 = 0, 1, 2, 3

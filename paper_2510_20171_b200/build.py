@@ -40,7 +40,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 def build_variant(defines, out_path: str) -> str:
     """The same sources compiled with extra -D flags into `out_path` (never the default library).  Used by
-    tests/test_gpu_barrier_fallback.py for the -DXDEV_TEST_FORCE_BARRIER_TIMEOUT build; select the result with
+    tests/test_zy_barrier_fallback.py for the -DXDEV_TEST_FORCE_BARRIER_TIMEOUT build; select the result with
     NCCLX_B200_LIB=<path>."""
     assert os.path.abspath(out_path) != LIB
     tmp = out_path + f".tmp{os.getpid()}"
