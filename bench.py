@@ -395,8 +395,8 @@ def main():
                                                     "share_of_step": round(red_ms / ms_profiled_total, 4)},
                                   "counts_kernel": {"avg_ms": round(cnt_ms / max(cnt_n, 1), 5), "launches": cnt_n,
                                                     "share_of_step": round(cnt_ms / ms_profiled_total, 5)}}}
-    # dram bytes per launch from the committed ncu capture: profiles/traffic.csv was written from the capture's raw
-    # page with the command in profiles/r2_summary.md section 2 (ncu cannot run inside this timed process)
+    # dram bytes per launch from the committed ncu capture: profiles/traffic.csv is written from the capture's raw page
+    # by `python -m paper_2510_20171_b200.ncu_traffic` (profiles/r3_summary.md section 2; ncu cannot run in this process)
     tr = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tr):
         try:

@@ -46,3 +46,20 @@ def test_reference_arm_nonzero_rank_exits_quietly():
     p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
                         "--steps", "1", "--warmup", "0"], env=env, capture_output=True, text=True, timeout=300)
     assert p.returncode == 0 and p.stdout.strip() == ""
+
+
+def test_ncu_traffic_reads_a_raw_page_and_rewrites_one_row(tmp_path, golden_dir):
+    """paper_2510_20171_b200.ncu_traffic: the committed tool behind bench.py's `roofline.traffic` (tests/golden/
+    ncu_raw_page_sample.csv = the round-3 capture's raw page trimmed to the columns it reads)."""
+    import csv
+    import os
+    from paper_2510_20171_b200 import ncu_traffic as T
+    rd, wr = T.dram_bytes(os.path.join(golden_dir, "ncu_raw_page_sample.csv"), "segment_copy_kernel")
+    assert (rd, wr) == (10737655000, 10683552000)
+    assert abs((rd + wr) / (2 * 10 * 2**30) - 1) < 0.01          # within 1 % of config 3's algorithmic bytes
+    p = tmp_path / "traffic.csv"
+    T.update(str(p), "k", "w", 1, 2, "first")
+    T.update(str(p), "k2", "w", 5, 6, "other")
+    T.update(str(p), "k", "w", 3, 4, "second")                   # replaces the first row
+    rows = list(csv.DictReader(open(p)))
+    assert [(r["kernel"], r["bytes_per_launch"], r["source"]) for r in rows] == [("k2", "11", "other"), ("k", "7", "second")]
